@@ -1,0 +1,428 @@
+/*
+ * ris_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, CPU-only oracle for the TDDFT-ris derivative-integral contractions
+ *   G_J [A,x] = sum_{mu nu} sum_P D_{mu nu} c_P  d(mu nu|P)/dR_{A,x}
+ *   G_K [A,x] = sum_P sum_{mu nu} Gamma^P_{mu nu} d(mu nu|P)/dR_{A,x}
+ *   G_PQ[A,x] = sum_{PQ} c_P d_Q d(P|Q)/dR_{A,x}
+ * i.e. the integral-derivative factors of the first two terms and of the third term of
+ * Eq. 27, for the three-centre integrals (pq|A) and metric M_AB=(A|B) of
+ * Eqs. 21-22, with the minimal auxiliary basis of one s-type Gaussian
+ * per atom.  (pq|sr) is in charge-cloud notation, Eq. 7.
+ * The derivative is the TOTAL nuclear derivative (xi is a nuclear coordinate, Eq. 8,
+ * PAPER.md:62-65): every centre that sits on atom A moves.
+ *
+ * The paper does not describe the integral evaluation ("We will not discuss the details of
+ * these integral evaluation algorithms"), so the oracle writes out the
+ * textbook McMurchie-Davidson definition, step by step, with no
+ * blocking, screening (except the documented opt-in primitive cutoff), symmetry or
+ * translational-invariance shortcuts: all ORDERED (mu,nu) pairs are visited and the three
+ * centre derivatives are computed explicitly.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+ * may call this file.  It shares no code with paper_2511_18233_b200/csrc.
+ *
+ * Pins (tests/test_oracle_pins.py): closed-form sss value and gradient, Boys reference
+ * values / erf / incomplete gamma / quadrature, the worked example of SURVEY.md 8(c) P4-P5,
+ * finite differences, translational invariance, brute-force quadrature, far-aux limit.
+ * Nothing in this file is "parity unpinned".
+ *
+ * Conventions: atomic units; row-major double arrays; Cartesian component order inside a
+ * shell: lx descending, then ly descending (xx,xy,xz,yy,yz,zz; ...).  prim_coef is applied
+ * as-is to UNnormalised primitives; the aux function carries N_P = (2 alpha/pi)^(3/4).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define LMAX 3                 /* shells up to f */
+#define EMAX (LMAX + 1)        /* one raised by the derivative */
+#define TMAX (2 * EMAX + 2)    /* Hermite order bound (+1 for the aux derivative) */
+#define MMAX (TMAX + 1)
+
+static const double PI = 3.14159265358979323846264338327950288;
+
+/* ---------------------------------------------------------------- O1: Boys function
+ * F_m(T) = int_0^1 t^(2m) exp(-T t^2) dt.
+ * T < 35: F_M = e^-T sum_k (2T)^k / [(2M+1)(2M+3)...(2M+2k+1)] at M = mmax, then downward
+ *         F_m = (2T F_{m+1} + e^-T)/(2m+1).
+ * T >= 35: F_0 = 1/2 sqrt(pi/T) erf(sqrt T), upward F_{m+1} = ((2m+1)F_m - e^-T)/(2T).
+ */
+void ris_oracle_boys(int mmax, double T, double *F)
+{
+    if (T < 35.0) {
+        long double t = (long double)T;
+        long double et = expl(-t);
+        long double term = 1.0L / (2 * mmax + 1);
+        long double sum = term;
+        for (int k = 1; k < 2000; ++k) {
+            term *= 2.0L * t / (2 * mmax + 2 * k + 1);
+            sum += term;
+            if (term < 1e-22L * sum) break;
+        }
+        long double f = et * sum;
+        F[mmax] = (double)f;
+        for (int m = mmax - 1; m >= 0; --m) {
+            f = (2.0L * t * f + et) / (2 * m + 1);
+            F[m] = (double)f;
+        }
+    } else {
+        long double t = (long double)T;
+        long double et = expl(-t);
+        long double f = 0.5L * sqrtl((long double)PI / t) * erfl(sqrtl(t));
+        F[0] = (double)f;
+        for (int m = 0; m < mmax; ++m) {
+            f = ((2 * m + 1) * f - et) / (2.0L * t);
+            F[m + 1] = (double)f;
+        }
+    }
+}
+
+/* ---------------------------------------------------------------- O2: Hermite expansion
+ * E[i][j][t], 0<=i<=imax, 0<=j<=jmax, one Cartesian direction.  Q = A_x - B_x.
+ *   E^{00}_0 = exp(-q Q^2),  q = ab/p
+ *   E^{i+1,j}_t = E^{ij}_{t-1}/(2p) - (q Q/a) E^{ij}_t + (t+1) E^{ij}_{t+1}
+ *   E^{i,j+1}_t = E^{ij}_{t-1}/(2p) + (q Q/b) E^{ij}_t + (t+1) E^{ij}_{t+1}
+ */
+typedef double Etab[EMAX + 1][EMAX + 1][2 * EMAX + 2];
+
+static void hermite_E(int imax, int jmax, double a, double b, double Q, Etab E)
+{
+    double p = a + b, q = a * b / p;
+    memset(E, 0, sizeof(Etab));
+    E[0][0][0] = exp(-q * Q * Q);
+    for (int i = 0; i <= imax; ++i) {
+        for (int j = 0; j <= jmax; ++j) {
+            if (i == 0 && j == 0) continue;
+            for (int t = 0; t <= i + j; ++t) {
+                double lo, mid, hi;
+                if (j == 0) {           /* raise i from (i-1, 0) */
+                    lo = (t > 0) ? E[i - 1][j][t - 1] : 0.0;
+                    mid = E[i - 1][j][t];
+                    hi = (t + 1 <= i - 1 + j) ? E[i - 1][j][t + 1] : 0.0;
+                    E[i][j][t] = lo / (2 * p) - (q * Q / a) * mid + (t + 1) * hi;
+                } else {                /* raise j from (i, j-1) */
+                    lo = (t > 0) ? E[i][j - 1][t - 1] : 0.0;
+                    mid = E[i][j - 1][t];
+                    hi = (t + 1 <= i + j - 1) ? E[i][j - 1][t + 1] : 0.0;
+                    E[i][j][t] = lo / (2 * p) + (q * Q / b) * mid + (t + 1) * hi;
+                }
+            }
+        }
+    }
+}
+
+/* ---------------------------------------------------------------- O3: Hermite Coulomb
+ * R^n_{000} = (-2 rho)^n F_n(T);  R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X_x R^{n+1}_{t,u,v}
+ * (same in y and z).  Output R[t][u][v] = R^0_{tuv} for t+u+v <= nmax.
+ */
+typedef double Rtab[TMAX + 1][TMAX + 1][TMAX + 1];
+
+static void hermite_R(int nmax, double rho, const double X[3], Rtab R0)
+{
+    double F[MMAX + 1];
+    double T = rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
+    ris_oracle_boys(nmax, T, F);
+    /* Rn[n][t][u][v]; every entry read below has been written before it is read */
+    int N = nmax + 1;
+    double Rn[N][N][N][N];
+    double pw = 1.0;
+    for (int n = 0; n <= nmax; ++n) { Rn[n][0][0][0] = pw * F[n]; pw *= -2.0 * rho; }
+    for (int tot = 1; tot <= nmax; ++tot)
+        for (int t = 0; t <= tot; ++t)
+            for (int u = 0; u <= tot - t; ++u) {
+                int v = tot - t - u;
+                for (int n = 0; n <= nmax - tot; ++n) {
+                    double val;
+                    if (t > 0)
+                        val = ((t > 1) ? (t - 1) * Rn[n + 1][t - 2][u][v] : 0.0) + X[0] * Rn[n + 1][t - 1][u][v];
+                    else if (u > 0)
+                        val = ((u > 1) ? (u - 1) * Rn[n + 1][t][u - 2][v] : 0.0) + X[1] * Rn[n + 1][t][u - 1][v];
+                    else
+                        val = ((v > 1) ? (v - 1) * Rn[n + 1][t][u][v - 2] : 0.0) + X[2] * Rn[n + 1][t][u][v - 1];
+                    Rn[n][t][u][v] = val;
+                }
+            }
+    for (int t = 0; t <= nmax; ++t)
+        for (int u = 0; u <= nmax - t; ++u)
+            for (int v = 0; v <= nmax - t - u; ++v) R0[t][u][v] = Rn[0][t][u][v];
+}
+
+/* sum_{tuv} Ex[t] Ey[u] Ez[v] R[t+dt][u+du][v+dv] */
+static double hsum(const double *Ex, int nx, const double *Ey, int ny, const double *Ez, int nz,
+                   Rtab R, int dt, int du, int dv)
+{
+    long double s = 0.0L;
+    for (int t = 0; t <= nx; ++t)
+        for (int u = 0; u <= ny; ++u)
+            for (int v = 0; v <= nz; ++v) s += (long double)(Ex[t] * Ey[u] * Ez[v]) * R[t + dt][u + du][v + dv];
+    return (double)s;
+}
+
+/* ---------------------------------------------------------------- O4/O5: one primitive integral
+ * Unnormalised Cartesian primitives la=(lax,lay,laz) at A (exponent a), lb at B (exponent b);
+ * s-type aux exp(-alpha |r-C|^2) WITHOUT N_P.
+ *   [ab|P]       = 2 pi^{5/2}/(p alpha sqrt(p+alpha)) sum_{tuv} E_t E_u E_v R^0_{tuv}
+ *   d/dA_x[ab|P] = 2a [a+1_x,b|P] - a_x [a-1_x,b|P]          (same for B with b)
+ *   d/dC_x[ab|P] = -pref sum E_tuv R^0_{t+1,u,v}              (explicit aux derivative)
+ * out[0] = value, out[1..3] = d/dA, out[4..6] = d/dB, out[7..9] = d/dC.
+ */
+void ris_oracle_prim3c(const int la[3], const int lb[3], double a, double b, double alpha,
+                       const double A[3], const double B[3], const double C[3], double out[10])
+{
+    double p = a + b, rho = p * alpha / (p + alpha);
+    double P[3], X[3];
+    Etab E[3];
+    for (int d = 0; d < 3; ++d) {
+        P[d] = (a * A[d] + b * B[d]) / p;
+        X[d] = P[d] - C[d];
+        hermite_E(la[d] + 1, lb[d] + 1, a, b, A[d] - B[d], E[d]);
+    }
+    int L = la[0] + la[1] + la[2] + lb[0] + lb[1] + lb[2];
+    Rtab *R = malloc(sizeof(Rtab));
+    hermite_R(L + 2, rho, X, *R);
+    double pref = 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+#define EE(d, i, j) E[d][i][j], (i) + (j)
+    out[0] = pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R, 0, 0, 0);
+    for (int d = 0; d < 3; ++d) {
+        int ia[3] = {la[0], la[1], la[2]}, ib[3] = {lb[0], lb[1], lb[2]};
+        double up, dn;
+        /* bra centre A */
+        ia[d] = la[d] + 1;
+        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        dn = 0.0;
+        if (la[d] > 0) {
+            ia[d] = la[d] - 1;
+            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        }
+        out[1 + d] = pref * (2.0 * a * up - la[d] * dn);
+        ia[d] = la[d];
+        /* ket-side bra centre B */
+        ib[d] = lb[d] + 1;
+        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        dn = 0.0;
+        if (lb[d] > 0) {
+            ib[d] = lb[d] - 1;
+            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        }
+        out[4 + d] = pref * (2.0 * b * up - lb[d] * dn);
+        ib[d] = lb[d];
+        /* aux centre C, explicitly */
+        out[7 + d] = -pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R,
+                                  d == 0, d == 1, d == 2);
+    }
+#undef EE
+    free(R);
+}
+
+/* ---------------------------------------------------------------- O7: two-centre term
+ * (P|Q) = 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)) F_0(rho R^2), rho = alpha beta/(alpha+beta)
+ * d/dR_P = -2 rho (R_P-R_Q) * 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)) * F_1(rho R^2) = -d/dR_Q.
+ * WITHOUT N_P N_Q.  out[0]=value, out[1..3] = d/dR_P.
+ */
+void ris_oracle_prim2c(double alpha, double beta, const double RP[3], const double RQ[3], double out[4])
+{
+    double rho = alpha * beta / (alpha + beta);
+    double X[3] = {RP[0] - RQ[0], RP[1] - RQ[1], RP[2] - RQ[2]};
+    double F[2];
+    ris_oracle_boys(1, rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]), F);
+    double pref = 2.0 * pow(PI, 2.5) / (alpha * beta * sqrt(alpha + beta));
+    out[0] = pref * F[0];
+    for (int d = 0; d < 3; ++d) out[1 + d] = -2.0 * rho * X[d] * pref * F[1];
+}
+
+/* ---------------------------------------------------------------- molecule description */
+typedef struct {
+    int natoms;
+    const double *coords;          /* [natoms][3] */
+    int nshells;
+    const int32_t *shell_atom, *shell_l, *shell_nprim, *shell_prim_off;
+    const double *prim_exp, *prim_coef;
+    const double *aux_exponents;   /* [natoms] */
+} ris_oracle_mol;
+
+static int ncart(int l) { return (l + 1) * (l + 2) / 2; }
+
+static void cart_components(int l, int comp[][3])
+{
+    int n = 0;
+    for (int lx = l; lx >= 0; --lx)
+        for (int ly = l - lx; ly >= 0; --ly) {
+            comp[n][0] = lx; comp[n][1] = ly; comp[n][2] = l - lx - ly; ++n;
+        }
+}
+
+static double aux_norm(double alpha) { return pow(2.0 * alpha / PI, 0.75); }
+
+/* ---------------------------------------------------------------- O6: contraction for one aux P
+ * For aux function P (on atom P) and nmat dense matrices G_s[nao][nao] with scale factors
+ * scale[s]:
+ *   eacc[s]        += scale[s] sum_{mu nu} G_s[mu,nu] (mu nu|P)
+ *   gacc[s][A][x]  += scale[s] sum_{mu nu} G_s[mu,nu] d(mu nu|P)/dR_{A,x}
+ * over ALL ordered (mu,nu).  J-type: G = D, scale = c_P.  K-type: G = Gamma^P, scale = 1.
+ * atom_mask (nullable): when given, only triplets that touch a masked atom are visited and
+ * only masked atoms' rows of gacc are meaningful (used to sample outputs at full size).
+ * prim_cutoff: a primitive pair is skipped when |d_a d_b| K_ab (pi/p)^{3/2} < prim_cutoff
+ * (0 = no cutoff; 1e-22 for the 300-atom config only).
+ * Accumulation in long double.
+ */
+int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const double *G,
+                          const double *scale, const uint8_t *atom_mask, double prim_cutoff,
+                          long double *gacc, long double *eacc)
+{
+    int natoms = mol->natoms, nsh = mol->nshells;
+    int *ao_off = malloc(sizeof(int) * (size_t)(nsh + 1));
+    ao_off[0] = 0;
+    for (int s = 0; s < nsh; ++s) {
+        if (mol->shell_l[s] < 0 || mol->shell_l[s] > LMAX) { free(ao_off); return -1; }
+        ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
+    }
+    int nao = ao_off[nsh];
+    double alpha = mol->aux_exponents[P];
+    double NP = aux_norm(alpha);
+    const double *C = mol->coords + 3 * P;
+    int Pmasked = atom_mask ? atom_mask[P] : 1;
+    size_t ng = (size_t)nmat * natoms * 3;
+
+#pragma omp parallel
+    {
+        long double *gl = calloc(ng, sizeof(long double));
+        long double *el = calloc((size_t)nmat, sizeof(long double));
+        double *buf = malloc(sizeof(double) * 10 * 10 * 10);   /* [ca][cb][10] */
+#pragma omp for schedule(dynamic, 1)
+        for (int sa = 0; sa < nsh; ++sa) {
+            int la = mol->shell_l[sa], at_a = mol->shell_atom[sa];
+            int na = ncart(la);
+            int compa[10][3];
+            cart_components(la, compa);
+            const double *A = mol->coords + 3 * at_a;
+            for (int sb = 0; sb < nsh; ++sb) {
+                int lb = mol->shell_l[sb], at_b = mol->shell_atom[sb];
+                if (atom_mask && !Pmasked && !atom_mask[at_a] && !atom_mask[at_b]) continue;
+                int nb = ncart(lb);
+                int compb[10][3];
+                cart_components(lb, compb);
+                const double *Bc = mol->coords + 3 * at_b;
+                memset(buf, 0, sizeof(double) * 1000);
+                double AB2 = 0.0;
+                for (int d = 0; d < 3; ++d) AB2 += (A[d] - Bc[d]) * (A[d] - Bc[d]);
+                for (int ka = 0; ka < mol->shell_nprim[sa]; ++ka) {
+                    double a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
+                    double da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
+                    for (int kb = 0; kb < mol->shell_nprim[sb]; ++kb) {
+                        double b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
+                        double db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
+                        double p = a + b;
+                        if (prim_cutoff > 0.0 &&
+                            fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, 1.5) < prim_cutoff)
+                            continue;
+                        /* O2-O5 for every Cartesian component pair of this primitive pair */
+                        double rho = p * alpha / (p + alpha);
+                        double Pc[3], X[3];
+                        Etab E[3];
+                        for (int d = 0; d < 3; ++d) {
+                            Pc[d] = (a * A[d] + b * Bc[d]) / p;
+                            X[d] = Pc[d] - C[d];
+                            hermite_E(la + 1, lb + 1, a, b, A[d] - Bc[d], E[d]);
+                        }
+                        Rtab R;
+                        hermite_R(la + lb + 2, rho, X, R);
+                        double pref = NP * da * db * 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+                        for (int ca = 0; ca < na; ++ca)
+                            for (int cb = 0; cb < nb; ++cb) {
+                                const int *ia = compa[ca], *ib = compb[cb];
+                                double *o = buf + (ca * 10 + cb) * 10;
+#define EE(d, i, j) E[d][i][j], (i) + (j)
+                                o[0] += pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R, 0, 0, 0);
+                                for (int d = 0; d < 3; ++d) {
+                                    int ja[3] = {ia[0], ia[1], ia[2]}, jb[3] = {ib[0], ib[1], ib[2]};
+                                    double up, dn = 0.0;
+                                    ja[d] = ia[d] + 1;
+                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    if (ia[d] > 0) {
+                                        ja[d] = ia[d] - 1;
+                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    }
+                                    o[1 + d] += pref * (2.0 * a * up - ia[d] * dn);
+                                    ja[d] = ia[d];
+                                    jb[d] = ib[d] + 1;
+                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    dn = 0.0;
+                                    if (ib[d] > 0) {
+                                        jb[d] = ib[d] - 1;
+                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    }
+                                    o[4 + d] += pref * (2.0 * b * up - ib[d] * dn);
+                                    o[7 + d] += -pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R,
+                                                             d == 0, d == 1, d == 2);
+                                }
+#undef EE
+                            }
+                    }
+                }
+                /* O6: multiply by G and scale, add to the three atoms */
+                for (int s = 0; s < nmat; ++s) {
+                    const double *Gs = G + (size_t)s * nao * nao;
+                    long double *g = gl + (size_t)s * natoms * 3;
+                    for (int ca = 0; ca < na; ++ca)
+                        for (int cb = 0; cb < nb; ++cb) {
+                            long double w = (long double)scale[s] * Gs[(size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb];
+                            const double *o = buf + (ca * 10 + cb) * 10;
+                            el[s] += w * o[0];
+                            for (int d = 0; d < 3; ++d) {
+                                g[at_a * 3 + d] += w * o[1 + d];
+                                g[at_b * 3 + d] += w * o[4 + d];
+                                g[P * 3 + d] += w * o[7 + d];
+                            }
+                        }
+                }
+            }
+        }
+#pragma omp critical
+        {
+            for (size_t i = 0; i < ng; ++i) gacc[i] += gl[i];
+            for (int s = 0; s < nmat; ++s) eacc[s] += el[s];
+        }
+        free(gl); free(el); free(buf);
+    }
+    free(ao_off);
+    return 0;
+}
+
+/* ---------------------------------------------------------------- O7: G_PQ and E_PQ
+ * gacc[s][A][x] += sum_{PQ} c^s_P d^s_Q d(P|Q)/dR_{A,x};  eacc[s] += sum_{PQ} c_P d_Q (P|Q),
+ * with N_P N_Q included.  P and Q run over all ordered pairs; P = Q contributes no gradient.
+ */
+int ris_oracle_grad_PQ(const ris_oracle_mol *mol, int nbatch, const double *c, const double *dq,
+                       long double *gacc, long double *eacc)
+{
+    int n = mol->natoms;
+    for (int s = 0; s < nbatch; ++s)
+        for (int P = 0; P < n; ++P)
+            for (int Q = 0; Q < n; ++Q) {
+                double o[4];
+                double aP = mol->aux_exponents[P], aQ = mol->aux_exponents[Q];
+                ris_oracle_prim2c(aP, aQ, mol->coords + 3 * P, mol->coords + 3 * Q, o);
+                long double w = (long double)c[s * n + P] * dq[s * n + Q] * aux_norm(aP) * aux_norm(aQ);
+                eacc[s] += w * o[0];
+                if (P == Q) continue;
+                for (int d = 0; d < 3; ++d) {
+                    gacc[((size_t)s * n + P) * 3 + d] += w * o[1 + d];
+                    gacc[((size_t)s * n + Q) * 3 + d] -= w * o[1 + d];
+                }
+            }
+    return 0;
+}
+
+int ris_oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

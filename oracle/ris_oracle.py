@@ -1,0 +1,198 @@
+"""ctypes front end of the CPU oracle (oracle/ris_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+import this module.  It imports nothing from paper_2511_18233_b200 except that callers hand
+it a `synth.Molecule`-shaped object (duck-typed: coords, shell_*, prim_*, aux_exponents).
+
+What it computes (Eq. 27 terms 1-3 with everything that is not an integral
+derivative folded into the inputs; Eqs. 21-22 for the integrals):
+
+    grad_J (mol, D, c)              -> G_J[s,A,x] = sum_{mu nu P} D^s_{mu nu} c^s_P d(mu nu|P)/dR_A
+    grad_K (mol, C_occ, C_vir, B)   -> G_K[s,A,x] = sum_P sum_{mu nu} Gamma^{s,P}_{mu nu} d(mu nu|P)/dR_A
+                                       Gamma^{s,P} = C_occ B[s,P] C_vir^T   (numpy float64 matmul,
+                                       i.e. the host BLAS that numpy links; stated in DESIGN.md)
+    grad_PQ(mol, c, d)              -> G_PQ[s,A,x] = sum_{PQ} c_P d_Q d(P|Q)/dR_A
+
+Each also returns the undifferentiated scalar (E_J, E_K, E_PQ) used by the finite-difference pin.
+`atoms=` samples the output: only rows of the listed atoms are computed (and returned; the other
+rows are NaN), visiting only triplets that touch them -- the definition restricted to those
+outputs, used for full-size parity.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libris_oracle.so")
+_SRC = os.path.join(_HERE, "ris_oracle.c")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp -shared.  No -ffast-math: IEEE semantics, long double accumulators."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-fopenmp", "-fPIC", "-shared",
+                               "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+class _Mol(C.Structure):
+    _fields_ = [("natoms", C.c_int), ("coords", C.c_void_p), ("nshells", C.c_int),
+                ("shell_atom", C.c_void_p), ("shell_l", C.c_void_p), ("shell_nprim", C.c_void_p),
+                ("shell_prim_off", C.c_void_p), ("prim_exp", C.c_void_p), ("prim_coef", C.c_void_p),
+                ("aux_exponents", C.c_void_p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+        _lib.ris_oracle_boys.argtypes = [C.c_int, C.c_double, C.c_void_p]
+        _lib.ris_oracle_prim3c.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double,
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_prim2c.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_contract_P.argtypes = [C.POINTER(_Mol), C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                               C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_contract_P.restype = C.c_int
+        _lib.ris_oracle_grad_PQ.argtypes = [C.POINTER(_Mol), C.c_int, C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().ris_oracle_num_threads())
+
+
+def _f64(x):
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _i32(x):
+    return np.ascontiguousarray(x, dtype=np.int32)
+
+
+class _Held:
+    """Keeps the numpy buffers alive next to the C struct."""
+
+    def __init__(self, mol):
+        self.arrs = dict(coords=_f64(mol.coords), shell_atom=_i32(mol.shell_atom), shell_l=_i32(mol.shell_l),
+                         shell_nprim=_i32(mol.shell_nprim), shell_prim_off=_i32(mol.shell_prim_off),
+                         prim_exp=_f64(mol.prim_exp), prim_coef=_f64(mol.prim_coef),
+                         aux_exponents=_f64(mol.aux_exponents))
+        a = self.arrs
+        self.natoms = a["coords"].shape[0]
+        self.nao = int(sum((l + 1) * (l + 2) // 2 for l in a["shell_l"]))
+        self.ao_atom = np.concatenate([[int(at)] * ((l + 1) * (l + 2) // 2)
+                                       for at, l in zip(a["shell_atom"], a["shell_l"])]).astype(np.int64)
+        self.c = _Mol(self.natoms, a["coords"].ctypes.data, a["shell_l"].shape[0], a["shell_atom"].ctypes.data,
+                      a["shell_l"].ctypes.data, a["shell_nprim"].ctypes.data, a["shell_prim_off"].ctypes.data,
+                      a["prim_exp"].ctypes.data, a["prim_coef"].ctypes.data, a["aux_exponents"].ctypes.data)
+
+
+def boys(mmax: int, T: float) -> np.ndarray:
+    out = np.zeros(mmax + 1)
+    lib().ris_oracle_boys(mmax, float(T), out.ctypes.data)
+    return out
+
+
+def prim3c(la, lb, a, b, alpha, A, B, Cc) -> np.ndarray:
+    """[value, dA(3), dB(3), dC(3)] of the unnormalised primitive integral, no N_P."""
+    la, lb = _i32(la), _i32(lb)
+    A, B, Cc = _f64(A), _f64(B), _f64(Cc)
+    out = np.zeros(10)
+    lib().ris_oracle_prim3c(la.ctypes.data, lb.ctypes.data, a, b, alpha, A.ctypes.data, B.ctypes.data,
+                            Cc.ctypes.data, out.ctypes.data)
+    return out
+
+
+def prim2c(alpha, beta, RP, RQ) -> np.ndarray:
+    """[value, d/dR_P(3)] of (P|Q) without N_P N_Q."""
+    RP, RQ = _f64(RP), _f64(RQ)
+    out = np.zeros(4)
+    lib().ris_oracle_prim2c(alpha, beta, RP.ctypes.data, RQ.ctypes.data, out.ctypes.data)
+    return out
+
+
+def _mask(natoms, atoms):
+    if atoms is None:
+        return None
+    m = np.zeros(natoms, dtype=np.uint8)
+    m[np.asarray(atoms, dtype=np.int64)] = 1
+    return m
+
+
+def _finish(g, e, mask):
+    g = g.astype(np.float64)
+    if mask is not None:
+        g[:, mask == 0, :] = np.nan
+        return g, None       # the scalar is not defined on a sampled run
+    return g, e.astype(np.float64)
+
+
+def grad_J(mol, D, c_aux, *, atoms=None, prim_cutoff=0.0):
+    """G_J and E_J = sum D_{mu nu} c_P (mu nu|P).  D [nbatch][nao][nao] (any symmetry), c [nbatch][naux]."""
+    h = _Held(mol)
+    D = _f64(D).reshape(-1, h.nao, h.nao)
+    c_aux = _f64(c_aux).reshape(D.shape[0], h.natoms)
+    nb = D.shape[0]
+    mask = _mask(h.natoms, atoms)
+    g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
+    e = np.zeros(nb, dtype=np.longdouble)
+    for P in range(h.natoms):
+        sc = _f64(c_aux[:, P])
+        rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, sc.ctypes.data,
+                                         mask.ctypes.data if mask is not None else None, prim_cutoff,
+                                         g.ctypes.data, e.ctypes.data)
+        assert rc == 0
+    return _finish(g, e, mask)
+
+
+def gamma_P(C_occ, C_vir, B_sP, rows=None):
+    """Gamma^P = C_occ B^P C_vir^T (Eqs. 32-34, 39: AO back-transform).
+    `rows`: AO indices on sampled atoms; only Gamma[rows,:] and Gamma[:,rows] are filled."""
+    if rows is None:
+        return C_occ @ B_sP @ C_vir.T
+    nao = C_occ.shape[0]
+    G = np.zeros((nao, nao))
+    G[rows, :] = (C_occ[rows, :] @ B_sP) @ C_vir.T
+    G[:, rows] = C_occ @ (B_sP @ C_vir[rows, :].T)
+    return G
+
+
+def grad_K(mol, C_occ, C_vir, B, *, atoms=None, prim_cutoff=0.0):
+    """G_K and E_K = sum_P sum Gamma^P_{mu nu} (mu nu|P).  B [nbatch][naux][nocc][nvir]."""
+    h = _Held(mol)
+    C_occ, C_vir = _f64(C_occ), _f64(C_vir)
+    B = _f64(B).reshape(-1, h.natoms, C_occ.shape[1], C_vir.shape[1])
+    nb = B.shape[0]
+    mask = _mask(h.natoms, atoms)
+    g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
+    e = np.zeros(nb, dtype=np.longdouble)
+    one = np.ones(nb)
+    rows_sampled = None if mask is None else np.nonzero(mask[h.ao_atom])[0]
+    for P in range(h.natoms):
+        rows = None if (mask is None or mask[P]) else rows_sampled
+        G = _f64(np.stack([gamma_P(C_occ, C_vir, B[s, P], rows) for s in range(nb)]))
+        rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, G.ctypes.data, one.ctypes.data,
+                                         mask.ctypes.data if mask is not None else None, prim_cutoff,
+                                         g.ctypes.data, e.ctypes.data)
+        assert rc == 0
+    return _finish(g, e, mask)
+
+
+def grad_PQ(mol, c_aux, d_aux):
+    """G_PQ and E_PQ = sum_{PQ} c_P d_Q (P|Q) (positive sign; Eq. 27's minus is the caller's)."""
+    h = _Held(mol)
+    c_aux = _f64(c_aux).reshape(-1, h.natoms)
+    d_aux = _f64(d_aux).reshape(-1, h.natoms)
+    nb = c_aux.shape[0]
+    g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
+    e = np.zeros(nb, dtype=np.longdouble)
+    lib().ris_oracle_grad_PQ(C.byref(h.c), nb, c_aux.ctypes.data, d_aux.ctypes.data, g.ctypes.data, e.ctypes.data)
+    return g.astype(np.float64), e.astype(np.float64)
