@@ -1,0 +1,129 @@
+/*
+ * ris.h -- C ABI of the B200-native TDDFT-ris derivative-integral library (libris_b200.so).
+ *
+ * The library evaluates, on one NVIDIA B200 (sm_100a), the integral-derivative contractions of the
+ * TDDFT-ris analytical excited-state gradient / derivative coupling (arxiv 2511.18233):
+ *
+ *   the derivative of the RI-factorised two-electron integral, Eq. 27,
+ *       [sum_AB (pq|A) M^-1_AB (B|sr)]^xi = sum (pq|A)^xi M^-1 (B|sr) + sum (pq|A) M^-1 (B|sr)^xi
+ *                                           - sum (pq|A) M^-1 M^xi M^-1 (B|sr),
+ *   with the three-centre integrals (pq|A) and the metric M_AB = (A|B) of Eqs. 21-22
+ *   over the minimal auxiliary basis of ONE s-type Gaussian per atom, contracted
+ *   with everything that is not an integral derivative:
+ *
+ *   ris_grad_J :  G[s][A][x] = sum_{mu nu} sum_P D^s_{mu nu} c^s_P  d(mu nu|P)/dR_{A,x}       (terms 1-2, Coulomb)
+ *   ris_grad_K :  G[s][A][x] = sum_P sum_{mu nu} Gamma^{s,P}_{mu nu} d(mu nu|P)/dR_{A,x},
+ *                 Gamma^{s,P} = C_occ B[s][P] C_vir^T   (terms 1-2, exchange; AO back-transform of
+ *                 Eqs. 32-34, 39)
+ *   ris_grad_PQ:  G[s][A][x] = sum_{PQ} c^s_P d^s_Q d(P|Q)/dR_{A,x}                          (term 3, POSITIVE sign)
+ *
+ * d/dR_A is the total nuclear derivative (xi is a nuclear coordinate, Eq. 8): every
+ * centre sitting on atom A moves.  Physical prefactors (c_x of Eq. 21, closed-shell factors,
+ * (E_J - E_I)^-1 of Eq. 26, the minus sign of term 3) are the caller's.
+ *
+ * Conventions
+ *   - atomic units (bohr, Hartree/bohr); all arrays row-major, FP64 / int32; no hidden normalisation:
+ *     prim_coef is applied as-is to UNnormalised Cartesian primitives
+ *         phi(r) = sum_k d_k (x-A_x)^lx (y-A_y)^ly (z-A_z)^lz exp(-a_k |r-A|^2);
+ *     the auxiliary function on atom P is N_P exp(-alpha_P |r-R_P|^2), N_P = (2 alpha_P/pi)^(3/4).
+ *   - Cartesian component order inside a shell: lx descending, then ly descending
+ *     (p: x,y,z; d: xx,xy,xz,yy,yz,zz; f: xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz).
+ *     AO index = shells in input order, components in that order.
+ *   - Pointers are HOST pointers in ris_setup and in the *_host entry points, DEVICE pointers (on the
+ *     device current at ris_setup) in ris_grad_J / ris_grad_K / ris_grad_PQ.
+ *   - Ownership: the caller owns every input and output buffer; the context owns its packed pair data
+ *     and scratch and frees them in ris_destroy.  Outputs are OVERWRITTEN, not accumulated.
+ *   - Asynchrony: device-pointer calls enqueue work on the stream given at ris_setup and return; the
+ *     caller synchronises that stream.  *_host calls return after the result is in host memory.
+ *   - Errors: 0 on success, a negative ris_status otherwise; nothing aborts or throws across the ABI.
+ *     There is no CPU fallback: without a usable CUDA device every call fails with RIS_ECUDA.
+ */
+#ifndef RIS_H
+#define RIS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ris_ctx ris_ctx;
+
+enum ris_status {
+    RIS_OK = 0,
+    RIS_EINVAL = -1,  /* bad argument: null pointer, l > 3, nprim < 1, index out of range, non-finite input */
+    RIS_ENOMEM = -2,  /* host or device allocation failed */
+    RIS_ECUDA = -3    /* CUDA runtime error; text via ris_strerror(RIS_ECUDA) */
+};
+
+typedef struct ris_options {
+    double schwarz_tol;   /* primitive-pair screening threshold, default 1e-13; <= 0 disables screening.
+                             A primitive pair (a,b) of shell pair (mu,nu) is dropped when
+                             |d_a d_b| K_ab (pi/p)^(3/2) max_P(N_P 2 pi/alpha_P) (1 + 2 max(a,b)) < tol;
+                             a shell pair is dropped when all its primitive pairs are. */
+    int deterministic;    /* nonzero: bitwise run-to-run reproducible reduction (slower) */
+    int p_batch;          /* aux functions per Gamma^P batch in ris_grad_K; 0 = choose from free memory */
+    int profile;          /* nonzero: record CUDA events around every kernel (see ris_profile_*) */
+} ris_options;
+
+/* Build the context: copies the molecule to the device and runs shell-pair screening, sorting by
+ * (l_mu,l_nu) class and SoA packing ON THE DEVICE (north_star; the paper is silent).
+ *   coords[natoms][3] bohr; shell s sits on atom shell_atom[s], has angular momentum shell_l[s] in 0..3 and
+ *   shell_nprim[s] >= 1 primitives at prim_exp/prim_coef[shell_prim_off[s] ...]; aux P sits on atom P with
+ *   exponent aux_exponents[P] (bohr^-2).  opt may be NULL (defaults).  cuda_stream is a cudaStream_t
+ *   (NULL = default stream) on which every later call of this context is enqueued. */
+int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
+              const int32_t* shell_l, const int32_t* shell_nprim, const int32_t* shell_prim_off,
+              const double* prim_exp, const double* prim_coef, const double* aux_exponents,
+              const ris_options* opt, void* cuda_stream);
+
+/* J-type contraction.  D device [nbatch][nao][nao] (symmetric or not: only D + D^T contributes),
+ * c_aux device [nbatch][naux], grad device [nbatch][natoms][3]. */
+int ris_grad_J(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, double* grad);
+
+/* K-type contraction.  C_occ device [nao][nocc], C_vir device [nao][nvir] ("occ"/"vir" are just the
+ * left / right coefficient matrices), B device [nbatch][naux][nocc][nvir], grad device [nbatch][natoms][3]. */
+int ris_grad_K(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+               const double* B, double* grad);
+
+/* Two-centre term.  c_aux, d_aux device [nbatch][naux], grad device [nbatch][natoms][3]. */
+int ris_grad_PQ(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
+
+/* The same three calls on HOST buffers: host->device copies, the kernels, and the device->host copy of
+ * the gradient all happen inside the call, which returns when grad (host) is complete. */
+int ris_grad_J_host(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, double* grad);
+int ris_grad_K_host(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                    const double* B, double* grad);
+int ris_grad_PQ_host(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
+
+int ris_destroy(ris_ctx* ctx);
+const char* ris_strerror(int status);
+
+/* Queries (host values, valid after ris_setup). */
+int ris_nao(const ris_ctx* ctx);
+int ris_naux(const ris_ctx* ctx);
+int ris_natoms(const ris_ctx* ctx);
+long long ris_npairs(const ris_ctx* ctx, int la, int lb);      /* surviving unique shell pairs of class (la>=lb) */
+long long ris_npairs_total(const ris_ctx* ctx);                /* unique shell pairs before screening */
+long long ris_nprimpairs(const ris_ctx* ctx, int la, int lb);  /* surviving primitive pairs of the class */
+long long ris_ntriplets(const ris_ctx* ctx);                   /* surviving primitive pairs x naux */
+long long ris_ntriplets_unscreened(const ris_ctx* ctx);
+long long ris_npair_elements(const ris_ctx* ctx);              /* packed Cartesian pair elements (no padding) */
+int ris_p_batch(const ris_ctx* ctx);                           /* Gamma^P batch size chosen by the last ris_grad_K */
+
+/* Profiling (opt.profile != 0): after synchronising the stream, ris_profile_count returns the number of
+ * kernel launches recorded since the last ris_profile_reset; ris_profile_get returns launch i's kernel
+ * name (static string) and device time in milliseconds. */
+int ris_profile_reset(ris_ctx* ctx);
+int ris_profile_count(ris_ctx* ctx);
+int ris_profile_get(ris_ctx* ctx, int i, const char** name, float* ms);
+
+/* Measurement helper: runs an independent-DFMA-chain kernel on every SM and returns the achieved
+ * FP64 rate in TFLOP/s (the denominator of the "% FP64 peak" metric; MEASURED_PEAKS.json has none). */
+int ris_probe_fp64_peak(double* tflops, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RIS_H */

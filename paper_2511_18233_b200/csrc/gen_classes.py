@@ -1,0 +1,283 @@
+#!/usr/bin/env python3
+"""Code generator for the per-(l_mu,l_nu)-class derivative-integral device functions.
+
+Emits `generated/ris_classes.cuh`: for every class (la >= lb, la <= 3) straight-line CUDA for
+
+  ris_vrr_<la><lb>    one primitive triplet: Obara-Saika vertical recurrence on the bra with the
+                      s-type auxiliary function folded in (no ket recurrence),
+                        [e+1_i]^(m) = PA_i [e]^(m) + WP_i [e]^(m+1)
+                                      + e_i/(2p) ( [e-1_i]^(m) - (rho/p) [e-1_i]^(m+1) ),
+                        WP = -(rho/p)(P-C),  [0]^(m) = kappa F_m(T),
+                      for e <= E = la+lb+1, followed by the exponent-scaled accumulation of the
+                      [e0|s]^(0) classes into the contracted targets
+                        acc2a[e] += 2a [e],  e = la+1 .. E      (-> (a+1_i, b|)
+                        acc2b[e] += 2b [e],  e = la   .. E      (-> (a, b+1_i|)
+                        acc1 [e] +=    [e],  e = max(la-1,0) .. E-2   (-> (a-1_i,b|, (a,b-1_i|)
+  ris_hrrc_<la><lb>   one contracted triplet: horizontal recurrence
+                        (a, b+1_i| = (a+1_i, b| + (A-B)_i (a, b|
+                      on the contracted targets, then
+                        d/dA_i (ab|P) = (a+1_i,b|_{2a} - a_i (a-1_i,b|_1
+                        d/dB_i (ab|P) = (a,b+1_i|_{2b} - b_i (a,b-1_i|_1
+                      contracted on the fly with the D / Gamma^P tile of each state.
+
+What is computed is Eq. 27 terms 1-2 of the paper for the integrals of Eq. 21
+(PAPER.md:119); the evaluation scheme is ours (the paper is silent).  The aux-centre
+derivative is NOT generated: the kernels use translational invariance, dC = -(dA + dB).
+
+Numerical stability: the HRR expands (x-B)^k in powers of (x-A); for a primitive pair whose product
+centre P sits next to B (b >> a) that expansion cancels by a factor (1 + b/a) per transferred unit.
+Every function is therefore generated for BOTH host centres -- "host" (h) carries the VRR, "other" (o)
+receives angular momentum through the HRR -- i.e. for all 16 ordered pairs (lh, lo), and the kernels
+run the primitive pairs with a >= b hosted on A and those with b > a hosted on B (cancellation <= 2).
+In the generated code "a" always means the host: a2 = 2 x host exponent, PA = P - host centre,
+AB = host centre - other centre, ga = d/d(host centre), gb = d/d(other centre).  TR selects the tile
+element order: false -> (c_host*n_other + c_other), true -> (c_other*n_host + c_host).
+
+Component order inside a shell of degree l: lx descending, then ly descending.
+"""
+from __future__ import annotations
+
+import os
+import sys
+
+LMAX = 3
+
+
+def comps(l):
+    return [(lx, ly, l - lx - ly) for lx in range(l, -1, -1) for ly in range(l - lx, -1, -1)]
+
+
+_CIDX = {}
+for _l in range(0, 2 * LMAX + 3):
+    for _k, _c in enumerate(comps(_l)):
+        _CIDX[_c] = _k
+
+
+def cidx(c):
+    return _CIDX[tuple(c)]
+
+
+def nc(l):
+    return (l + 1) * (l + 2) // 2
+
+
+def lower(c, i, k=1):
+    c = list(c)
+    c[i] -= k
+    return tuple(c)
+
+
+def raise_(c, i):
+    c = list(c)
+    c[i] += 1
+    return tuple(c)
+
+
+class ClassPlan:
+    """Static description of one class: accumulator layout shared by VRR and HRR."""
+
+    def __init__(self, la, lb):
+        self.la, self.lb = la, lb
+        self.E = la + lb + 1
+        self.r2a = list(range(la + 1, self.E + 1))
+        self.r2b = list(range(la, self.E + 1))
+        lo = la - 1 if la >= 1 else la
+        self.r1 = list(range(lo, self.E - 1)) if (la >= 1 or lb >= 1) else []
+        self.off = {}
+        n = 0
+        for tag, rng in (("2a", self.r2a), ("2b", self.r2b), ("1", self.r1)):
+            for e in rng:
+                self.off[(tag, e)] = n
+                n += nc(e)
+        self.nacc = n
+
+    def acc(self, tag, e, c):
+        return f"acc[{self.off[(tag, e)] + cidx(c)}]"
+
+
+# --------------------------------------------------------------------------- VRR
+
+def gen_vrr(pl: ClassPlan) -> str:
+    la, lb, E = pl.la, pl.lb, pl.E
+    out = []
+    w = out.append
+    w(f"// class ({la},{lb}): E={E}, {pl.nacc} contracted targets")
+    w(f"RIS_DEV void ris_vrr_{la}{lb}(const double (&F)[{E + 1}], double PA0, double PA1, double PA2,")
+    w("    double WP0, double WP1, double WP2, double oo2p, double q, double a2, double b2,")
+    w(f"    double (&acc)[{pl.nacc}])")
+    w("{")
+    PA = ["PA0", "PA1", "PA2"]
+    WP = ["WP0", "WP1", "WP2"]
+    emin_target = min([pl.r2b[0]] + (pl.r1[:1] if pl.r1 else []))
+    # needed set by backward closure
+    need = set()
+
+    def want(e, c, m):
+        if (e, c, m) in need:
+            return
+        need.add((e, c, m))
+        if e == 0:
+            return
+        i = pick_dir(c)
+        c1 = lower(c, i)
+        want(e - 1, c1, m)
+        want(e - 1, c1, m + 1)
+        if c[i] >= 2:
+            c2 = lower(c, i, 2)
+            want(e - 2, c2, m)
+            want(e - 2, c2, m + 1)
+
+    def pick_dir(c):
+        ones = [i for i in range(3) if c[i] == 1]
+        if ones:
+            return ones[0]
+        nz = [i for i in range(3) if c[i] > 0]
+        return min(nz, key=lambda i: c[i])
+
+    for e in range(emin_target, E + 1):
+        for c in comps(e):
+            want(e, c, 0)
+
+    def v(e, c, m):
+        return "F[%d]" % m if e == 0 else f"v{e}_{cidx(c)}_{m}"
+
+    brackets = set()
+    kk = sorted({c[i] - 1 for (e, c, m) in need if e >= 2 for i in [pick_dir(c)] if c[i] >= 2})
+    for k in kk:
+        w(f"    const double k{k} = {float(k)} * oo2p;")
+    for e in range(1, E + 1):
+        for m in range(E - e, -1, -1):
+            for c in comps(e):
+                if (e, c, m) not in need:
+                    continue
+                i = pick_dir(c)
+                c1 = lower(c, i)
+                expr = f"fma({PA[i]}, {v(e - 1, c1, m)}, {WP[i]} * {v(e - 1, c1, m + 1)})"
+                if c[i] >= 2:
+                    c2 = lower(c, i, 2)
+                    bn = f"b{e - 2}_{cidx(c2)}_{m}"
+                    if bn not in brackets:
+                        brackets.add(bn)
+                        w(f"    const double {bn} = fma(-q, {v(e - 2, c2, m + 1)}, {v(e - 2, c2, m)});")
+                    expr = f"fma(k{c[i] - 1}, {bn}, {expr})"
+                w(f"    const double {v(e, c, m)} = {expr};")
+        # accumulate level e as soon as it is complete
+    for e in range(0, E + 1):
+        for c in comps(e):
+            val = v(e, c, 0)
+            if e in pl.r2a:
+                w(f"    {pl.acc('2a', e, c)} = fma(a2, {val}, {pl.acc('2a', e, c)});")
+            if e in pl.r2b:
+                w(f"    {pl.acc('2b', e, c)} = fma(b2, {val}, {pl.acc('2b', e, c)});")
+            if e in pl.r1:
+                w(f"    {pl.acc('1', e, c)} += {val};")
+    w("}")
+    return "\n".join(out)
+
+
+# --------------------------------------------------------------------------- HRR + contraction
+
+def gen_hrr_chain(w, pl, tag, la_t, lb_t, prefix, done):
+    """Emit (la_t, lb_t| built from acc[tag][e], e = la_t .. la_t+lb_t.  Returns name(ca, cb) for the
+    target block; `done` caches emitted intermediates (prefix, e, k, ia, ib)."""
+
+    def name(e, k, a, b):
+        if k == 0:
+            return pl.acc(tag, e, a)
+        return f"{prefix}{e}{k}_{cidx(a)}_{cidx(b)}"
+
+    def build(e, k):
+        if k == 0 or (prefix, e, k) in done:
+            return
+        build(e + 1, k - 1)
+        build(e, k - 1)
+        done.add((prefix, e, k))
+        for a in comps(e):
+            for b in comps(k):
+                i = max(range(3), key=lambda d: b[d])       # any direction with b_i > 0
+                b1 = lower(b, i)
+                a1 = raise_(a, i)
+                w(f"    const double {name(e, k, a, b)} = fma(AB{i}, {name(e, k - 1, a, b1)}, {name(e + 1, k - 1, a1, b1)});")
+
+    build(la_t, lb_t)
+    return lambda a, b: name(la_t, lb_t, a, b)
+
+
+def gen_hrrc(pl: ClassPlan) -> str:
+    la, lb = pl.la, pl.lb
+    out = []
+    w = out.append
+    w(f"// contracted triplet of class ({la},{lb}): HRR, derivative assembly, contraction with the tile.")
+    w("// tile element (c_host,c_other) of state s sits at tile[s*sstride + el*estride], el by TR (see gen_classes.py).")
+    w("template <bool TR, class Sink>")
+    w(f"RIS_DEV void ris_hrrc_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
+    w("    const double* __restrict__ tile, size_t estride, size_t sstride, int nb, Sink&& sink)")
+    w("{")
+    done = set()
+    X2a = gen_hrr_chain(w, pl, "2a", la + 1, lb, "xa", done)
+    Y2b = gen_hrr_chain(w, pl, "2b", la, lb + 1, "yb", done)
+    X1m = gen_hrr_chain(w, pl, "1", la - 1, lb, "xm", done) if la >= 1 else None
+    Y1m = gen_hrr_chain(w, pl, "1", la, lb - 1, "xm", done) if lb >= 1 else None
+    nca, ncb = nc(la), nc(lb)
+    w("    for (int s = 0; s < nb; ++s) {")
+    w("        const double* __restrict__ t = tile + (size_t)s * sstride;")
+    w("        double ga0 = 0.0, ga1 = 0.0, ga2 = 0.0, gb0 = 0.0, gb1 = 0.0, gb2 = 0.0;")
+    for ia, a in enumerate(comps(la)):
+        for ib, b in enumerate(comps(lb)):
+            w(f"        {{ const double w = t[(TR ? {ib * nca + ia} : {ia * ncb + ib}) * estride];")
+            for i in range(3):
+                w(f"          ga{i} = fma(w, {X2a(raise_(a, i), b)}, ga{i});")
+                if a[i] >= 1:
+                    w(f"          ga{i} = fma(-{float(a[i])} * w, {X1m(lower(a, i), b)}, ga{i});")
+                w(f"          gb{i} = fma(w, {Y2b(a, raise_(b, i))}, gb{i});")
+                if b[i] >= 1:
+                    w(f"          gb{i} = fma(-{float(b[i])} * w, {Y1m(a, lower(b, i))}, gb{i});")
+            w("        }")
+    w("        sink(s, ga0, ga1, ga2, gb0, gb1, gb2);")
+    w("    }")
+    w("}")
+    return "\n".join(out)
+
+
+def generate() -> str:
+    parts = ["// GENERATED by gen_classes.py -- do not edit.  See that file for the recurrences.",
+             "#pragma once", ""]
+    classes = [(la, lb) for la in range(LMAX + 1) for lb in range(LMAX + 1)]
+    for la, lb in classes:
+        pl = ClassPlan(la, lb)
+        parts.append(f"template <> struct RisClass<{la},{lb}> {{ static constexpr int E = {pl.E}; "
+                     f"static constexpr int NACC = {pl.nacc}; static constexpr int NCA = {nc(la)}; "
+                     f"static constexpr int NCB = {nc(lb)}; }};")
+    parts.append("")
+    for la, lb in classes:
+        pl = ClassPlan(la, lb)
+        parts.append(gen_vrr(pl))
+        parts.append("")
+        parts.append(gen_hrrc(pl))
+        parts.append("")
+    # dispatch helpers
+    parts.append("template <int LA, int LB, class... A> RIS_DEV void ris_vrr(A&&... a) {")
+    for la, lb in classes:
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_vrr_{la}{lb}(static_cast<A&&>(a)...);")
+    parts.append("}")
+    parts.append("template <int LA, int LB, bool TR, class... A> RIS_DEV void ris_hrrc(A&&... a) {")
+    for la, lb in classes:
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrrc_{la}{lb}<TR>(static_cast<A&&>(a)...);")
+    parts.append("}")
+    return "\n".join(parts) + "\n"
+
+
+def main():
+    here = os.path.dirname(os.path.abspath(__file__))
+    outdir = os.path.join(here, "generated")
+    os.makedirs(outdir, exist_ok=True)
+    path = os.path.join(outdir, "ris_classes.cuh")
+    text = generate()
+    if not os.path.exists(path) or open(path).read() != text:
+        with open(path, "w") as f:
+            f.write(text)
+    return path
+
+
+if __name__ == "__main__":
+    print(main())

@@ -1,0 +1,593 @@
+// ris_api.cu -- C ABI (include/ris.h), context, host-side orchestration, and the small kernels:
+// tile packing, two-centre term (S5), FP64 probe.  The class kernels live in ris_grad_kernel.cuh
+// (one translation unit per class under generated/), the Gamma^P GEMMs in ris_gemm.cuh.
+#include "../../include/ris.h"
+#include "ris_boys_table.h"
+#include "ris_core.cuh"
+#include "ris_gemm.cuh"
+#include "ris_internal.h"
+#include "ris_setup.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+// --------------------------------------------------------------------------------------- errors
+static thread_local std::string g_cuda_err = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char* what, int line)
+{
+    char buf[512];
+    snprintf(buf, sizeof buf, "CUDA error at %s (ris_api.cu:%d): %s", what, line, cudaGetErrorString(e));
+    g_cuda_err = buf;
+    return RIS_ECUDA;
+}
+#define CU(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cuda_fail(e__, #x, __LINE__); } while (0)
+
+extern "C" const char* ris_strerror(int status)
+{
+    switch (status) {
+    case RIS_OK: return "success";
+    case RIS_EINVAL: return "invalid argument";
+    case RIS_ENOMEM: return "out of memory";
+    case RIS_ECUDA: return g_cuda_err.c_str();
+    default: return "unknown status";
+    }
+}
+
+// --------------------------------------------------------------------------------------- context
+struct ProfRec { const char* name; cudaEvent_t e0, e1; };
+
+struct ris_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    ris_options opt{};
+    int natoms = 0, nshells = 0, nao = 0, naux = 0;
+    double* d_coords = nullptr;
+    double* d_aux = nullptr;           // [naux][5]
+    int *d_shell_atom = nullptr, *d_shell_l = nullptr, *d_shell_nprim = nullptr, *d_shell_poff = nullptr, *d_shell_ao = nullptr;
+    double *d_pexp = nullptr, *d_pcoef = nullptr;
+    RisClassPack cls[RIS_NCLASS]{};
+    std::vector<void*> owned;          // every device allocation of the packed data
+    long long nelem_slab = 0, nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
+    double* d_boys[8] = {nullptr};
+    // grow-only scratch
+    void* ws[8] = {nullptr};
+    size_t ws_bytes[8] = {0};
+    int last_pbatch = 0;
+    std::vector<ProfRec> prof;
+    std::vector<cudaEvent_t> ev_pool;
+};
+
+enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6 };
+
+static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
+{
+    if (c->ws_bytes[slot] < bytes) {
+        if (c->ws[slot]) { CU(cudaStreamSynchronize(c->stream)); CU(cudaFree(c->ws[slot])); c->ws[slot] = nullptr; c->ws_bytes[slot] = 0; }
+        cudaError_t e = cudaMalloc(&c->ws[slot], bytes);
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return RIS_ENOMEM; }
+        CU(e);
+        c->ws_bytes[slot] = bytes;
+    }
+    *out = c->ws[slot];
+    return RIS_OK;
+}
+
+template <class T> static int dev_alloc(ris_ctx* c, T** p, size_t n, bool zero)
+{
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, std::max<size_t>(n, 1) * sizeof(T));
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return RIS_ENOMEM; }
+    CU(e);
+    c->owned.push_back(q);
+    if (zero) CU(cudaMemsetAsync(q, 0, std::max<size_t>(n, 1) * sizeof(T), c->stream));
+    *p = (T*)q;
+    return RIS_OK;
+}
+
+template <class T> static int dev_upload(ris_ctx* c, T** p, const T* h, size_t n)
+{
+    int rc = dev_alloc(c, p, n, false);
+    if (rc) return rc;
+    if (n) CU(cudaMemcpyAsync(*p, h, n * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    return RIS_OK;
+}
+
+// profiling: events around a launch when opt.profile is set
+struct ProfScope {
+    ris_ctx* c; int idx = -1;
+    ProfScope(ris_ctx* c_, const char* name) : c(c_)
+    {
+        if (!c->opt.profile) return;
+        ProfRec r; r.name = name;
+        if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) return;
+        cudaEventRecord(r.e0, c->stream);
+        c->prof.push_back(r);
+        idx = (int)c->prof.size() - 1;
+    }
+    ~ProfScope() { if (idx >= 0) cudaEventRecord(c->prof[idx].e1, c->stream); }
+};
+
+extern "C" int ris_profile_reset(ris_ctx* c)
+{
+    if (!c) return RIS_EINVAL;
+    for (auto& r : c->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    c->prof.clear();
+    return RIS_OK;
+}
+extern "C" int ris_profile_count(ris_ctx* c) { return c ? (int)c->prof.size() : RIS_EINVAL; }
+extern "C" int ris_profile_get(ris_ctx* c, int i, const char** name, float* ms)
+{
+    if (!c || i < 0 || i >= (int)c->prof.size()) return RIS_EINVAL;
+    CU(cudaEventSynchronize(c->prof[i].e1));
+    CU(cudaEventElapsedTime(ms, c->prof[i].e0, c->prof[i].e1));
+    *name = c->prof[i].name;
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- class launchers
+#define DECL(la, lb) void ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
+DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
+#undef DECL
+ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
+    ris_launch_grad_00, ris_launch_grad_10, ris_launch_grad_11, ris_launch_grad_20, ris_launch_grad_21,
+    ris_launch_grad_22, ris_launch_grad_30, ris_launch_grad_31, ris_launch_grad_32, ris_launch_grad_33};
+static const char* const kGradNames[RIS_NCLASS] = {
+    "ris_grad_kernel<0,0>", "ris_grad_kernel<1,0>", "ris_grad_kernel<1,1>", "ris_grad_kernel<2,0>", "ris_grad_kernel<2,1>",
+    "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
+// heaviest class first (flops per primitive triplet), so the tail is made of light kernels
+static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
+
+// --------------------------------------------------------------------------------------- setup
+extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
+                         const int32_t* shell_l, const int32_t* shell_nprim, const int32_t* shell_prim_off,
+                         const double* prim_exp, const double* prim_coef, const double* aux_exponents,
+                         const ris_options* opt, void* cuda_stream)
+{
+    if (!out) return RIS_EINVAL;
+    *out = nullptr;
+    if (natoms < 1 || nshells < 1 || !coords || !shell_atom || !shell_l || !shell_nprim || !shell_prim_off || !prim_exp ||
+        !prim_coef || !aux_exponents)
+        return RIS_EINVAL;
+    int nprim_tot = 0;
+    std::vector<int> shell_ao(nshells);
+    int nao = 0;
+    for (int s = 0; s < nshells; ++s) {
+        if (shell_l[s] < 0 || shell_l[s] > RIS_LMAX || shell_nprim[s] < 1 || shell_atom[s] < 0 || shell_atom[s] >= natoms ||
+            shell_prim_off[s] < 0)
+            return RIS_EINVAL;
+        nprim_tot = std::max(nprim_tot, shell_prim_off[s] + shell_nprim[s]);
+        shell_ao[s] = nao;
+        nao += ris_ncart(shell_l[s]);
+    }
+    for (int i = 0; i < 3 * natoms; ++i) if (!std::isfinite(coords[i])) return RIS_EINVAL;
+    for (int i = 0; i < nprim_tot; ++i)
+        if (!std::isfinite(prim_exp[i]) || !(prim_exp[i] > 0.0) || !std::isfinite(prim_coef[i])) return RIS_EINVAL;
+    for (int i = 0; i < natoms; ++i) if (!std::isfinite(aux_exponents[i]) || !(aux_exponents[i] > 0.0)) return RIS_EINVAL;
+
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) { g_cuda_err = "no CUDA device (this library has no CPU fallback)"; return RIS_ECUDA; }
+
+    ris_ctx* c = new (std::nothrow) ris_ctx;
+    if (!c) return RIS_ENOMEM;
+    struct Guard { ris_ctx* c; bool ok = false; ~Guard() { if (!ok) ris_destroy(c); } } guard{c};
+    CU(cudaGetDevice(&c->device));
+    c->stream = (cudaStream_t)cuda_stream;
+    c->opt.schwarz_tol = 1e-13;
+    if (opt) c->opt = *opt;
+    c->natoms = natoms; c->nshells = nshells; c->nao = nao; c->naux = natoms;
+
+    int rc;
+    if ((rc = dev_upload(c, &c->d_coords, coords, (size_t)3 * natoms))) return rc;
+    if ((rc = dev_upload(c, &c->d_shell_atom, shell_atom, (size_t)nshells))) return rc;
+    if ((rc = dev_upload(c, &c->d_shell_l, shell_l, (size_t)nshells))) return rc;
+    if ((rc = dev_upload(c, &c->d_shell_nprim, shell_nprim, (size_t)nshells))) return rc;
+    if ((rc = dev_upload(c, &c->d_shell_poff, shell_prim_off, (size_t)nshells))) return rc;
+    if ((rc = dev_upload(c, &c->d_shell_ao, shell_ao.data(), (size_t)nshells))) return rc;
+    if ((rc = dev_upload(c, &c->d_pexp, prim_exp, (size_t)nprim_tot))) return rc;
+    if ((rc = dev_upload(c, &c->d_pcoef, prim_coef, (size_t)nprim_tot))) return rc;
+
+    // aux records {Cx,Cy,Cz,alpha,N_P/alpha} and the potential maximum used by the screening bound
+    std::vector<double> aux((size_t)5 * natoms);
+    double vmax = 0.0;
+    for (int P = 0; P < natoms; ++P) {
+        const double al = aux_exponents[P], N = std::pow(2.0 * al / M_PI, 0.75);
+        aux[5 * P + 0] = coords[3 * P]; aux[5 * P + 1] = coords[3 * P + 1]; aux[5 * P + 2] = coords[3 * P + 2];
+        aux[5 * P + 3] = al; aux[5 * P + 4] = N / al;
+        vmax = std::max(vmax, N * 2.0 * M_PI / al);
+    }
+    if ((rc = dev_upload(c, &c->d_aux, aux.data(), aux.size()))) return rc;
+
+    // Boys tables, one per top order M = 1..7
+    for (int M = 1; M <= 7; ++M) {
+        std::vector<double> t;
+        ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, t);
+        if ((rc = dev_upload(c, &c->d_boys[M], t.data(), t.size()))) return rc;
+        CU(cudaStreamSynchronize(c->stream));      // t goes out of scope
+    }
+
+    // ---- S0 on device: survey -> scan -> scatter -> pack
+    RisMolDev m{natoms, nshells, c->d_coords, c->d_shell_atom, c->d_shell_l, c->d_shell_nprim, c->d_shell_poff,
+                c->d_shell_ao, c->d_pexp, c->d_pcoef, vmax, c->opt.schwarz_tol};
+    const long long ntot = (long long)nshells * (nshells + 1) / 2;
+    c->npairs_total = ntot;
+    for (int i = 0; i <= nshells - 1; ++i)
+        for (int j = 0; j <= i; ++j) c->nprim_total += (long long)shell_nprim[i] * shell_nprim[j];
+    const int nblk = (int)((ntot + RIS_SCAN_BLOCK - 1) / RIS_SCAN_BLOCK);
+    unsigned* d_packed;
+    int *d_hist, *d_base, *d_meta;   // d_meta: totals[16], start[16], kmax[16]
+    unsigned long long* d_nprim;
+    long long* d_list[2];
+    if ((rc = dev_alloc(c, &d_packed, (size_t)ntot, false))) return rc;
+    if ((rc = dev_alloc(c, &d_hist, (size_t)nblk * RIS_NBIN, false))) return rc;
+    if ((rc = dev_alloc(c, &d_base, (size_t)nblk * RIS_NBIN, false))) return rc;
+    if ((rc = dev_alloc(c, &d_meta, (size_t)3 * RIS_NBIN, true))) return rc;
+    if ((rc = dev_alloc(c, &d_nprim, (size_t)RIS_NBIN, true))) return rc;
+    if ((rc = dev_alloc(c, &d_list[0], (size_t)ntot, false))) return rc;
+    if ((rc = dev_alloc(c, &d_list[1], (size_t)ntot, false))) return rc;
+    {
+        ProfScope ps(c, "ris_k_pair_survey");
+        ris_k_pair_survey<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(m, ntot, d_packed, d_meta + 2 * RIS_NBIN, d_nprim);
+    }
+    const long long* lin = nullptr;
+    for (int pass = 0; pass < 3; ++pass) {
+        ProfScope ps(c, "ris_k_radix_pass");
+        long long* lout = d_list[pass & 1];
+        ris_k_radix_hist<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_packed, pass, d_hist);
+        ris_k_radix_scan<<<1, 32, 0, c->stream>>>(nblk, d_hist, d_base, d_meta, d_meta + RIS_NBIN);
+        ris_k_radix_scatter<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_packed, pass, d_base, d_meta + RIS_NBIN, lout);
+        lin = lout;
+    }
+    const long long* d_sorted = lin;
+    CU(cudaGetLastError());
+    int meta[3 * RIS_NBIN];
+    unsigned long long nprim_c[RIS_NBIN];
+    CU(cudaMemcpyAsync(meta, d_meta, sizeof meta, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(nprim_c, d_nprim, sizeof nprim_c, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+
+    long long off = 0;
+    for (int la = 0; la <= RIS_LMAX; ++la)
+        for (int lb = 0; lb <= la; ++lb) {
+            const int k = ris_class_id(la, lb);
+            RisClassPack& pk = c->cls[k];
+            pk.la = la; pk.lb = lb;
+            pk.npairs = meta[k];
+            pk.npad = (pk.npairs + RIS_PAIR_PAD - 1) / RIS_PAIR_PAD * RIS_PAIR_PAD;
+            pk.kmax = meta[2 * RIS_NBIN + k];
+            pk.nprim = (long long)nprim_c[k];
+            pk.elem_off = off;
+            off += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npad;
+            c->nelem_real += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npairs;
+            c->nprim_surv += pk.nprim;
+            if (pk.npairs == 0) continue;
+            const size_t n = (size_t)pk.npad;
+            if ((rc = dev_alloc(c, &pk.geom, 6 * n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.atoms, 2 * n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.ao, 2 * n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.nkA, n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.nkB, n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.symf, n, true))) return rc;
+            if ((rc = dev_alloc(c, &pk.prim, (size_t)pk.kmax * RIS_PRIM_FIELDS * n, true))) return rc;
+            ProfScope ps(c, "ris_k_pair_pack");
+            ris_k_pair_pack<<<(pk.npairs + 127) / 128, 128, 0, c->stream>>>(m, pk, d_sorted + meta[RIS_NBIN + k]);
+        }
+    c->nelem_slab = off;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(c->stream));
+    guard.ok = true;
+    *out = c;
+    return RIS_OK;
+}
+
+extern "C" int ris_destroy(ris_ctx* c)
+{
+    if (!c) return RIS_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    for (void* p : c->owned) cudaFree(p);
+    for (int i = 0; i < 8; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
+    ris_profile_reset(c);
+    delete c;
+    return RIS_OK;
+}
+
+extern "C" int ris_nao(const ris_ctx* c) { return c ? c->nao : RIS_EINVAL; }
+extern "C" int ris_naux(const ris_ctx* c) { return c ? c->naux : RIS_EINVAL; }
+extern "C" int ris_natoms(const ris_ctx* c) { return c ? c->natoms : RIS_EINVAL; }
+extern "C" long long ris_npairs(const ris_ctx* c, int la, int lb)
+{
+    if (!c || la < lb || la > RIS_LMAX || lb < 0) return RIS_EINVAL;
+    return c->cls[ris_class_id(la, lb)].npairs;
+}
+extern "C" long long ris_nprimpairs(const ris_ctx* c, int la, int lb)
+{
+    if (!c || la < lb || la > RIS_LMAX || lb < 0) return RIS_EINVAL;
+    return c->cls[ris_class_id(la, lb)].nprim;
+}
+extern "C" long long ris_npairs_total(const ris_ctx* c) { return c ? c->npairs_total : RIS_EINVAL; }
+extern "C" long long ris_ntriplets(const ris_ctx* c) { return c ? c->nprim_surv * c->naux : RIS_EINVAL; }
+extern "C" long long ris_ntriplets_unscreened(const ris_ctx* c) { return c ? c->nprim_total * c->naux : RIS_EINVAL; }
+extern "C" long long ris_npair_elements(const ris_ctx* c) { return c ? c->nelem_real : RIS_EINVAL; }
+extern "C" int ris_p_batch(const ris_ctx* c) { return c ? c->last_pbatch : RIS_EINVAL; }
+
+// --------------------------------------------------------------------------------------- tile packing
+// out[slab][elem_off + e*npad + ip] = symf[ip] * (G[slab][mu0+ca][nu0+cb] + G[slab][nu0+cb][mu0+ca]),  e = ca*ncb + cb.
+// Folds D + D^T (or Gamma + Gamma^T) onto the unique shell pairs.
+__global__ void ris_k_pack_tiles(RisClassPack pk, int nao, const double* __restrict__ G, long long gstride,
+                                 double* __restrict__ out, long long ostride)
+{
+    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ip >= pk.npairs) return;
+    const int ncb = ris_ncart(pk.lb);
+    const int e = blockIdx.y, ca = e / ncb, cb = e - ca * ncb;
+    const size_t r = (size_t)pk.ao[ip] + ca, q = (size_t)pk.ao[(size_t)pk.npad + ip] + cb;
+    const double* g = G + (size_t)blockIdx.z * gstride;
+    out[(size_t)blockIdx.z * ostride + pk.elem_off + (size_t)e * pk.npad + ip] =
+        (double)pk.symf[ip] * (g[r * nao + q] + g[q * nao + r]);
+}
+
+static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab, double* out, long long ostride)
+{
+    for (int k = 0; k < RIS_NCLASS; ++k) {
+        const RisClassPack& pk = c->cls[k];
+        if (pk.npairs == 0) continue;
+        ProfScope ps(c, "ris_k_pack_tiles");
+        dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), nslab);
+        ris_k_pack_tiles<<<grid, 128, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
+    }
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+constexpr int RIS_NB_MAX = 8;      // states per class-kernel launch (shared-memory slots)
+
+static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long pstride, const double* cscale,
+                          int nb, int p0, int p1, double* grad)
+{
+    for (int oi = 0; oi < RIS_NCLASS; ++oi) {
+        const int k = kClassOrder[oi];
+        const RisClassPack& pk = c->cls[k];
+        if (pk.npairs == 0) continue;
+        RisGradParams p{};
+        p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
+        p.tile = tile; p.sstride = sstride; p.pstride = pstride; p.cscale = cscale; p.nb = nb; p.p0 = p0; p.p1 = p1;
+        p.grad = grad;
+        // enough blocks for >= 4 per SM, at least 4 aux per block, at most 64 (shared-memory accumulators)
+        const int bx = pk.npad / RIS_GRAD_THREADS, np = p1 - p0;
+        int ny = std::max(1, (4 * 148 + bx - 1) / bx);
+        int pch = std::max(4, (np + ny - 1) / ny);
+        p.pchunk = std::min(std::min(pch, np), 64);
+        ProfScope ps(c, kGradNames[k]);
+        ris_grad_launchers[k](p, c->stream);
+    }
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- J
+extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad)
+{
+    if (!c || nbatch < 1 || !D || !c_aux || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
+    const long long nao2 = (long long)c->nao * c->nao;
+    for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
+        const int nb = std::min(RIS_NB_MAX, nbatch - s0);
+        double* tile;
+        int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_slab, (void**)&tile);
+        if (rc) return rc;
+        if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_slab))) return rc;
+        if ((rc = launch_classes(c, tile, c->nelem_slab, 0, c_aux + (size_t)s0 * c->naux, nb, 0, c->naux,
+                                 grad + (size_t)s0 * c->natoms * 3)))
+            return rc;
+    }
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- K
+extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                          const double* B, double* grad)
+{
+    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
+    const int nao = c->nao, naux = c->naux;
+    const long long nao2 = (long long)nao * nao;
+    const int nbmax = std::min(nbatch, RIS_NB_MAX);
+    // Gamma^P batch: H [pb][nocc][nao], dense Gamma [pb][nao][nao], packed tiles [nb][pb][slab]
+    int pb = c->opt.p_batch;
+    if (pb <= 0) {
+        size_t fr = 0, tot = 0;
+        CU(cudaMemGetInfo(&fr, &tot));
+        fr += c->ws_bytes[WS_TILE] + c->ws_bytes[WS_H] + c->ws_bytes[WS_G];
+        const double per = 8.0 * ((double)nocc * nao + (double)nao2 + (double)nbmax * c->nelem_slab);
+        const double budget = std::min(0.5 * (double)fr, 16.0e9);
+        pb = (int)std::max(1.0, std::min((double)naux, budget / per));
+    }
+    pb = std::min(pb, naux);
+    c->last_pbatch = pb;
+    double *tile, *H, *G;
+    int rc;
+    if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pb * c->nelem_slab, (void**)&tile))) return rc;
+    if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)pb * nocc * nao, (void**)&H))) return rc;
+    if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * nao2, (void**)&G))) return rc;
+    for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
+        const int nb = std::min(RIS_NB_MAX, nbatch - s0);
+        for (int p0 = 0; p0 < naux; p0 += pb) {
+            const int np = std::min(pb, naux - p0);
+            for (int s = 0; s < nb; ++s) {
+                // S3-K1: H^P = B^P C_vir^T  ([np*nocc x nvir] x [nao x nvir]^T), Gamma^P = C_occ H^P
+                const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
+                {
+                    ProfScope ps(c, "ris_gemm_nt(H=B*Cvir^T)");
+                    ris_gemm<true>(c->stream, np * nocc, nao, nvir, Bs, nvir, 0, C_vir, nvir, 0, H, nao, 0, 1);
+                }
+                {
+                    ProfScope ps(c, "ris_gemm_nn(Gamma=Cocc*H)");
+                    ris_gemm<false>(c->stream, nao, nao, nocc, C_occ, nocc, 0, H, nao, (long long)nocc * nao, G, nao, nao2, np);
+                }
+                CU(cudaGetLastError());
+                if ((rc = pack_tiles(c, G, nao2, np, tile + (size_t)s * pb * c->nelem_slab, c->nelem_slab))) return rc;
+            }
+            if ((rc = launch_classes(c, tile, (long long)pb * c->nelem_slab, c->nelem_slab, nullptr, nb, p0, p0 + np,
+                                     grad + (size_t)s0 * c->natoms * 3)))
+                return rc;
+        }
+    }
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- PQ (S5)
+// g[s][P] = sum_{Q != P} (c_P d_Q + c_Q d_P) N_P N_Q d(P|Q)/dR_P,
+// d(P|Q)/dR_P = -2 rho (R_P - R_Q) 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)) F_1(rho R^2)   (Eq. 22).
+// One block per aux P, threads over Q, fixed-order block reduction: deterministic, no atomics.
+__global__ void __launch_bounds__(128) ris_k_grad_pq(int naux, int nb, const double* __restrict__ aux,
+                                                     const double* __restrict__ boys1, const double* __restrict__ cv,
+                                                     const double* __restrict__ dv, double* __restrict__ grad)
+{
+    const int P = blockIdx.x, s = blockIdx.y;
+    const double Px = aux[5 * P], Py = aux[5 * P + 1], Pz = aux[5 * P + 2], al = aux[5 * P + 3], fP = aux[5 * P + 4];
+    const double cP = cv[(size_t)s * naux + P], dP = dv[(size_t)s * naux + P];
+    double g0 = 0.0, g1 = 0.0, g2 = 0.0;
+    for (int Q = threadIdx.x; Q < naux; Q += blockDim.x) {
+        if (Q == P) continue;
+        const double X0 = Px - aux[5 * Q], X1 = Py - aux[5 * Q + 1], X2 = Pz - aux[5 * Q + 2];
+        const double be = aux[5 * Q + 3], fQ = aux[5 * Q + 4];
+        const double sI = ris_rsqrt(al + be);
+        const double rho = al * be * sI * sI;
+        double F[2];
+        ris_boys<1>(rho * (X0 * X0 + X1 * X1 + X2 * X2), boys1, F);
+        // N_P N_Q/(alpha beta) = fP fQ
+        const double w = (cP * dv[(size_t)s * naux + Q] + cv[(size_t)s * naux + Q] * dP) * fP * fQ *
+                         (2.0 * 17.493418327624862846) * sI * (-2.0 * rho) * F[1];
+        g0 = fma(w, X0, g0); g1 = fma(w, X1, g1); g2 = fma(w, X2, g2);
+    }
+    __shared__ double red[3][128];
+    red[0][threadIdx.x] = g0; red[1][threadIdx.x] = g1; red[2][threadIdx.x] = g2;
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if (threadIdx.x < o)
+            for (int x = 0; x < 3; ++x) red[x][threadIdx.x] += red[x][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) grad[((size_t)s * naux + P) * 3 + threadIdx.x] = red[threadIdx.x][0];
+}
+
+extern "C" int ris_grad_PQ(ris_ctx* c, int nbatch, const double* c_aux, const double* d_aux, double* grad)
+{
+    if (!c || nbatch < 1 || !c_aux || !d_aux || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    ProfScope ps(c, "ris_k_grad_pq");
+    ris_k_grad_pq<<<dim3(c->naux, nbatch), 128, 0, c->stream>>>(c->naux, nbatch, c->d_aux, c->d_boys[1], c_aux, d_aux, grad);
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- host-buffer entry points
+static int h2d(ris_ctx* c, int slot, const double* h, size_t n, double** d)
+{
+    int rc = ws_get(c, slot, n * sizeof(double), (void**)d);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(*d, h, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    return RIS_OK;
+}
+
+static int d2h_grad(ris_ctx* c, const double* d, double* h, size_t n)
+{
+    CU(cudaMemcpyAsync(h, d, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return RIS_OK;
+}
+
+extern "C" int ris_grad_J_host(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad)
+{
+    if (!c || nbatch < 1 || !D || !c_aux || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    double *dD, *dc, *dg;
+    int rc;
+    const size_t ng = (size_t)nbatch * c->natoms * 3;
+    if ((rc = h2d(c, WS_IN0, D, (size_t)nbatch * c->nao * c->nao, &dD))) return rc;
+    if ((rc = h2d(c, WS_IN1, c_aux, (size_t)nbatch * c->naux, &dc))) return rc;
+    if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
+    if ((rc = ris_grad_J(c, nbatch, dD, dc, dg))) return rc;
+    return d2h_grad(c, dg, grad, ng);
+}
+
+extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                               const double* B, double* grad)
+{
+    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    double *dCo, *dCv, *dB, *dg;
+    int rc;
+    const size_t ng = (size_t)nbatch * c->natoms * 3;
+    if ((rc = h2d(c, WS_IN0, B, (size_t)nbatch * c->naux * nocc * nvir, &dB))) return rc;
+    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
+    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
+    if ((rc = ris_grad_K(c, nbatch, nocc, nvir, dCo, dCv, dB, dg))) return rc;
+    return d2h_grad(c, dg, grad, ng);
+}
+
+extern "C" int ris_grad_PQ_host(ris_ctx* c, int nbatch, const double* c_aux, const double* d_aux, double* grad)
+{
+    if (!c || nbatch < 1 || !c_aux || !d_aux || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    double *dc, *dd, *dg;
+    int rc;
+    const size_t ng = (size_t)nbatch * c->natoms * 3;
+    if ((rc = h2d(c, WS_IN0, c_aux, (size_t)nbatch * c->naux, &dc))) return rc;
+    if ((rc = h2d(c, WS_IN1, d_aux, (size_t)nbatch * c->naux, &dd))) return rc;
+    if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
+    if ((rc = ris_grad_PQ(c, nbatch, dc, dd, dg))) return rc;
+    return d2h_grad(c, dg, grad, ng);
+}
+
+// --------------------------------------------------------------------------------------- FP64 probe
+__global__ void ris_k_dfma_probe(double* out, int iters, double a, double b)
+{
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    if (s == 12345.678) out[0] = s;
+}
+
+extern "C" int ris_probe_fp64_peak(double* tflops, void* cuda_stream)
+{
+    if (!tflops) return RIS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    double* d;
+    CU(cudaMalloc(&d, 8));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int iters = 40000, thr = 512;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CU(cudaEventRecord(e0, st));
+        ris_k_dfma_probe<<<nsm, thr, 0, st>>>(d, iters, 1.0000001, 1e-9);
+        CU(cudaEventRecord(e1, st));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep) best = std::max(best, 2.0 * 8 * iters * (double)nsm * thr / (ms * 1e-3) * 1e-12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *tflops = best;
+    return RIS_OK;
+}

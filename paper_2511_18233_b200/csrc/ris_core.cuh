@@ -1,0 +1,116 @@
+// ris_core.cuh -- device-side arithmetic shared by the class kernels:
+//   S1  Boys function F_m(T), m = 0..E
+//   S2  one primitive triplet: prefactor, Boys, OS recurrence
+// The integrals are (pq|A) of Eq. 21 and their nuclear derivatives, Eq. 27 terms 1-2
+// (PAPER.md:119, 150); the paper does not describe their evaluation.
+#pragma once
+#include <math.h>
+#include <stddef.h>
+
+#ifndef RIS_DEV
+#define RIS_DEV __device__ __forceinline__
+#endif
+
+template <int LA, int LB> struct RisClass;
+#include "generated/ris_classes.cuh"
+
+// ---------------------------------------------------------------------------------------------
+// Boys function.
+//   T < RIS_BOYS_TMAX: nearest grid point T0 = i/32, x = T - T0 in [-1/64, 1/64];
+//       F_M(T)  = sum_{k=0..6} F_{M+k}(T0) (-x)^k / k!      (Taylor; d/dT F_m = -F_{m+1})
+//       e^{-T}  = e^{-T0} sum_{k=0..6} (-x)^k / k!
+//       F_m     = (2T F_{m+1} + e^{-T}) / (2m+1)             (downward, stable)
+//     truncation < (1/64)^7/7! = 4.4e-17 relative.  One table row per grid point and per top
+//     order M: {e^{-T0}, c_0..c_6}, c_k = (-1)^k F_{M+k}(T0)/k!  (64 bytes, one 2-sector gather).
+//   T >= RIS_BOYS_TMAX (=40): erfc(sqrt T) < 4e-19, so F_0 = sqrt(pi/T)/2, and upward
+//       F_{m+1} = ((2m+1) F_m - e^{-T}) / (2T)
+//     where e^{-T} is at most a 6e-11 relative correction (m = 7, T = 40): single precision is enough.
+constexpr double RIS_BOYS_TMAX = 40.0;
+constexpr int RIS_BOYS_PER_UNIT = 32;
+constexpr int RIS_BOYS_NGRID = 40 * 32 + 1;
+constexpr int RIS_BOYS_ROW = 8;
+
+RIS_DEV double ris_rsqrt(double x)
+{
+#ifdef __CUDA_ARCH__
+    return rsqrt(x);
+#else
+    return 1.0 / sqrt(x);
+#endif
+}
+
+template <int M>
+RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 1])
+{
+    if (T < RIS_BOYS_TMAX) {
+        const int i = (int)(T * RIS_BOYS_PER_UNIT + 0.5);
+        const double x = T - (double)i * (1.0 / RIS_BOYS_PER_UNIT);
+        const double* __restrict__ r = tab + (size_t)i * RIS_BOYS_ROW;
+#ifdef __CUDA_ARCH__
+        const double2 r0 = __ldg(reinterpret_cast<const double2*>(r));
+        const double2 r1 = __ldg(reinterpret_cast<const double2*>(r) + 1);
+        const double2 r2 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+        const double2 r3 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+        const double e0 = r0.x, c0 = r0.y, c1 = r1.x, c2 = r1.y, c3 = r2.x, c4 = r2.y, c5 = r3.x, c6 = r3.y;
+#else
+        const double e0 = r[0], c0 = r[1], c1 = r[2], c2 = r[3], c3 = r[4], c4 = r[5], c5 = r[6], c6 = r[7];
+#endif
+        double f = fma(c6, x, c5);
+        f = fma(f, x, c4);
+        f = fma(f, x, c3);
+        f = fma(f, x, c2);
+        f = fma(f, x, c1);
+        f = fma(f, x, c0);
+        double ex = fma(x, 1.0 / 720.0, -1.0 / 120.0);
+        ex = fma(ex, x, 1.0 / 24.0);
+        ex = fma(ex, x, -1.0 / 6.0);
+        ex = fma(ex, x, 0.5);
+        ex = fma(ex, x, -1.0);
+        ex = fma(ex, x, 1.0);
+        ex *= e0;
+        F[M] = f;
+        const double t2 = T + T;
+#pragma unroll
+        for (int m = M - 1; m >= 0; --m) {
+            f = fma(t2, f, ex) * (1.0 / (2 * m + 1));
+            F[m] = f;
+        }
+    } else {
+        const double rt = ris_rsqrt(T);
+        const double i2t = 0.5 * rt * rt;
+        const double ex = (double)expf(-(float)T);
+        double f = 0.88622692545275801365 * rt;     // sqrt(pi)/2 / sqrt(T)
+        F[0] = f;
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+            f = fma((double)(2 * m + 1), f, -ex) * i2t;
+            F[m + 1] = f;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// One primitive triplet (primitive of mu, primitive of nu, aux P), hosted on centre Z (see gen_classes.py:
+// Z = A for primitive pairs with a >= b, Z = B otherwise; LH/LO are the host's / the other shell's l):
+//   rho = p alpha/(p+alpha), T = rho |P-C|^2, [0]^(m) = kappa F_m(T) with
+//   kappa = coef * auxfac / sqrt(p+alpha),  coef = d_a d_b K_ab 2 pi^{5/2}/p,  auxfac = N_P/alpha,
+// then the class recurrence + exponent-scaled accumulation (generated code); h2 / o2 = 2 x exponent of the
+// host / other primitive.
+template <int LH, int LO>
+RIS_DEV void ris_prim_triplet(double p, double Px, double Py, double Pz, double oo2p, double h2, double o2,
+                              double coef, double Zx, double Zy, double Zz, double Cx, double Cy, double Cz,
+                              double alpha, double auxfac, const double* __restrict__ boys_tab,
+                              double (&acc)[RisClass<LH, LO>::NACC])
+{
+    constexpr int E = RisClass<LH, LO>::E;
+    const double s = ris_rsqrt(p + alpha);
+    const double q = alpha * s * s;          // rho/p
+    const double X0 = Px - Cx, X1 = Py - Cy, X2 = Pz - Cz;
+    const double T = (p * q) * fma(X0, X0, fma(X1, X1, X2 * X2));
+    double F[E + 1];
+    ris_boys<E>(T, boys_tab, F);
+    const double kappa = coef * auxfac * s;
+#pragma unroll
+    for (int m = 0; m <= E; ++m) F[m] *= kappa;
+    ris_vrr<LH, LO>(F, Px - Zx, Py - Zy, Pz - Zz, -q * X0, -q * X1, -q * X2, oo2p, q, h2, o2, acc);
+}

@@ -1,0 +1,178 @@
+// ris_setup.cuh -- S0: shell-pair screening, sorting by (l_mu,l_nu) class and SoA
+// packing, all on the device.  The paper is silent on screening / ordering; the bound
+// is the one documented in include/ris.h (ris_options.schwarz_tol).
+#pragma once
+#include "ris_internal.h"
+
+struct RisMolDev {
+    int natoms, nshells;
+    const double* coords;
+    const int *shell_atom, *shell_l, *shell_nprim, *shell_poff, *shell_ao;
+    const double *pexp, *pcoef;
+    double vmax;     // max_P N_P 2 pi / alpha_P
+    double tol;      // <= 0: keep everything
+};
+
+constexpr int RIS_SCAN_BLOCK = 1024;
+
+__device__ __forceinline__ void ris_decode_pair(long long t, int& i, int& j)
+{
+    long long r = (long long)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while (r * (r + 1) / 2 > t) --r;
+    while ((r + 1) * (r + 2) / 2 <= t) ++r;
+    i = (int)r;
+    j = (int)(t - r * (r + 1) / 2);
+}
+
+// mu carries the larger l (ties: the larger shell index), so la >= lb in every class.
+__device__ __forceinline__ void ris_order_pair(const RisMolDev& m, int i, int j, int& mu, int& nu)
+{
+    if (m.shell_l[i] >= m.shell_l[j]) { mu = i; nu = j; } else { mu = j; nu = i; }
+}
+
+__device__ __forceinline__ bool ris_prim_survives(const RisMolDev& m, double a, double b, double da, double db, double AB2)
+{
+    if (!(m.tol > 0.0)) return true;
+    const double p = a + b;
+    const double s = 3.14159265358979323846 / p;
+    const double bound = fabs(da * db) * exp(-a * b / p * AB2) * s * sqrt(s) * m.vmax * (1.0 + 2.0 * fmax(a, b));
+    return bound >= m.tol;
+}
+
+// Survey: packed[t] = cls | nkA << 8 | nkB << 16 with cls = 15 for a dropped pair; nkA / nkB = surviving
+// primitive pairs hosted on A (a >= b) / on B (b > a).  Per-class max / total of surviving primitive pairs.
+constexpr int RIS_NBIN = 16;
+constexpr int RIS_DROPPED = 15;
+
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m, long long ntot, unsigned* packed, int* kmax,
+                                                                    unsigned long long* nprim)
+{
+    const long long t = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
+    if (t >= ntot) return;
+    int i, j, mu, nu;
+    ris_decode_pair(t, i, j);
+    ris_order_pair(m, i, j, mu, nu);
+    const double* A = m.coords + 3 * m.shell_atom[mu];
+    const double* B = m.coords + 3 * m.shell_atom[nu];
+    const double dx = A[0] - B[0], dy = A[1] - B[1], dz = A[2] - B[2];
+    const double AB2 = dx * dx + dy * dy + dz * dz;
+    int nA = 0, nB = 0;
+    for (int ka = 0; ka < m.shell_nprim[mu]; ++ka)
+        for (int kb = 0; kb < m.shell_nprim[nu]; ++kb) {
+            const double a = m.pexp[m.shell_poff[mu] + ka], b = m.pexp[m.shell_poff[nu] + kb];
+            if (!ris_prim_survives(m, a, b, m.pcoef[m.shell_poff[mu] + ka], m.pcoef[m.shell_poff[nu] + kb], AB2)) continue;
+            if (a >= b) ++nA; else ++nB;
+        }
+    unsigned k = RIS_DROPPED;
+    if (nA + nB > 0) {
+        k = (unsigned)ris_class_id(m.shell_l[mu], m.shell_l[nu]);
+        atomicMax(&kmax[k], nA + nB);
+        atomicAdd(&nprim[k], (unsigned long long)(nA + nB));
+    }
+    packed[t] = k | ((unsigned)min(nA, 255) << 8) | ((unsigned)min(nB, 255) << 16);
+}
+
+// Stable LSD radix sort of the pair list in three 16-bin passes: nkB, nkA, class.  After it, the pairs of a
+// class are contiguous and ordered by (nkA, nkB), so the lanes of a warp run equally long primitive loops.
+__device__ __forceinline__ int ris_digit(unsigned packed, int pass)
+{
+    if (pass == 0) return min((int)((packed >> 16) & 255u), 15);
+    if (pass == 1) return min((int)((packed >> 8) & 255u), 15);
+    return (int)(packed & 255u);
+}
+
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_hist(long long n, const long long* list_in, const unsigned* packed,
+                                                                   int pass, int* hist)
+{
+    __shared__ int sh[RIS_NBIN];
+    if (threadIdx.x < RIS_NBIN) sh[threadIdx.x] = 0;
+    __syncthreads();
+    const long long i = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
+    if (i < n) atomicAdd(&sh[ris_digit(packed[list_in ? list_in[i] : i], pass)], 1);
+    __syncthreads();
+    if (threadIdx.x < RIS_NBIN) hist[blockIdx.x * RIS_NBIN + threadIdx.x] = sh[threadIdx.x];
+}
+
+// Exclusive scan over blocks for each bin -> base[blk][bin]; totals[bin]; start[bin] (bin-major order).
+__global__ void ris_k_radix_scan(int nblk, const int* hist, int* base, int* totals, int* start)
+{
+    const int c = threadIdx.x;
+    if (c < RIS_NBIN) {
+        int run = 0;
+        for (int b = 0; b < nblk; ++b) { base[b * RIS_NBIN + c] = run; run += hist[b * RIS_NBIN + c]; }
+        totals[c] = run;
+    }
+    __syncthreads();
+    if (c == 0) {
+        int run = 0;
+        for (int k = 0; k < RIS_NBIN; ++k) { start[k] = run; run += totals[k]; }
+    }
+}
+
+// Stable scatter: list_out[start[d] + base[blk][d] + rank-in-block] = element.
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_scatter(long long n, const long long* list_in, const unsigned* packed,
+                                                                      int pass, const int* base, const int* start, long long* list_out)
+{
+    __shared__ int wtot[RIS_SCAN_BLOCK / 32];
+    const long long i = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
+    const long long el = (i < n) ? (list_in ? list_in[i] : i) : -1;
+    const int k = (i < n) ? ris_digit(packed[el], pass) : -1;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int c = 0; c < RIS_NBIN; ++c) {
+        const unsigned bal = __ballot_sync(0xffffffffu, k == c);
+        if (lane == 0) wtot[w] = __popc(bal);
+        __syncthreads();
+        if (k == c) {
+            int rank = __popc(bal & ((1u << lane) - 1u));
+            for (int ww = 0; ww < w; ++ww) rank += wtot[ww];
+            list_out[start[c] + base[blockIdx.x * RIS_NBIN + c] + rank] = el;
+        }
+        __syncthreads();
+    }
+}
+
+// Pack one class: geometry, atoms, AO offsets, symmetry factor, surviving primitive pairs -- those hosted on
+// A (a >= b) first, then those hosted on B.
+__global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* list)
+{
+    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ip >= pk.npairs) return;
+    int i, j, mu, nu;
+    ris_decode_pair(list[ip], i, j);
+    ris_order_pair(m, i, j, mu, nu);
+    const int atA = m.shell_atom[mu], atB = m.shell_atom[nu];
+    const double* A = m.coords + 3 * atA;
+    const double* B = m.coords + 3 * atB;
+    const double dx = A[0] - B[0], dy = A[1] - B[1], dz = A[2] - B[2];
+    const double AB2 = dx * dx + dy * dy + dz * dz;
+    const size_t n = (size_t)pk.npad;
+    pk.geom[0 * n + ip] = A[0]; pk.geom[1 * n + ip] = A[1]; pk.geom[2 * n + ip] = A[2];
+    pk.geom[3 * n + ip] = dx;   pk.geom[4 * n + ip] = dy;   pk.geom[5 * n + ip] = dz;
+    pk.atoms[ip] = atA; pk.atoms[n + ip] = atB;
+    pk.ao[ip] = m.shell_ao[mu]; pk.ao[n + ip] = m.shell_ao[nu];
+    pk.symf[ip] = (mu == nu) ? 0.5f : 1.0f;
+    int k = 0;
+    for (int host = 0; host < 2; ++host) {
+        for (int ka = 0; ka < m.shell_nprim[mu]; ++ka)
+            for (int kb = 0; kb < m.shell_nprim[nu]; ++kb) {
+                const double a = m.pexp[m.shell_poff[mu] + ka], b = m.pexp[m.shell_poff[nu] + kb];
+                if ((a >= b) != (host == 0)) continue;
+                const double da = m.pcoef[m.shell_poff[mu] + ka], db = m.pcoef[m.shell_poff[nu] + kb];
+                if (!ris_prim_survives(m, a, b, da, db, AB2)) continue;
+                const double p = a + b, ip_ = 1.0 / p;
+                double* q = pk.prim + (size_t)k * RIS_PRIM_FIELDS * n + ip;
+                q[0 * n] = p;
+                q[1 * n] = (a * A[0] + b * B[0]) * ip_;
+                q[2 * n] = (a * A[1] + b * B[1]) * ip_;
+                q[3 * n] = (a * A[2] + b * B[2]) * ip_;
+                q[4 * n] = 0.5 * ip_;
+                q[5 * n] = 2.0 * a;
+                q[6 * n] = 2.0 * b;
+                // d_a d_b K_ab 2 pi^{5/2} / p
+                q[7 * n] = da * db * exp(-a * b * ip_ * AB2) * (2.0 * 17.493418327624862846) * ip_;
+                ++k;
+            }
+        if (host == 0) pk.nkA[ip] = k;
+    }
+    pk.nkB[ip] = k - pk.nkA[ip];
+}

@@ -1,0 +1,236 @@
+"""Thin Python binding of the C ABI in include/ris.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of libris_b200.so; PyTorch is used for device
+memory and streams.  There is no CPU path: if the shared library is missing or no CUDA device is
+usable, calls raise RisError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libris_b200.so")
+_lib = None
+
+EXPORTS = [
+    "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host",
+    "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
+    "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
+    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_probe_fp64_peak",
+]
+
+
+class RisError(RuntimeError):
+    pass
+
+
+class RisOptions(C.Structure):
+    _fields_ = [("schwarz_tol", C.c_double), ("deterministic", C.c_int), ("p_batch", C.c_int), ("profile", C.c_int)]
+
+
+def load_library():
+    """dlopen libris_b200.so (built in-tree by paper_2511_18233_b200.build).  Fails loudly when absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RisError(f"{LIB_PATH} not found: build it with `python -m paper_2511_18233_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, ci, cd = C.c_void_p, C.c_int, C.c_double
+    lib.ris_setup.argtypes = [C.POINTER(vp), ci, vp, ci, vp, vp, vp, vp, vp, vp, vp, C.POINTER(RisOptions), vp]
+    lib.ris_grad_J.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_grad_K.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
+    lib.ris_grad_PQ.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_grad_K_host.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
+    lib.ris_grad_PQ_host.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_destroy.argtypes = [vp]
+    lib.ris_strerror.argtypes = [ci]
+    lib.ris_strerror.restype = C.c_char_p
+    for name in ("ris_nao", "ris_naux", "ris_natoms", "ris_p_batch", "ris_profile_reset", "ris_profile_count"):
+        getattr(lib, name).argtypes = [vp]
+    for name in ("ris_npairs", "ris_nprimpairs"):
+        getattr(lib, name).argtypes = [vp, ci, ci]
+        getattr(lib, name).restype = C.c_longlong
+    for name in ("ris_npairs_total", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements"):
+        getattr(lib, name).argtypes = [vp]
+        getattr(lib, name).restype = C.c_longlong
+    lib.ris_profile_get.argtypes = [vp, ci, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    lib.ris_probe_fp64_peak.argtypes = [C.POINTER(cd), vp]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise RisError(f"ris error {rc}: {load_library().ris_strerror(rc).decode()}")
+
+
+def _np(x, dt):
+    return np.ascontiguousarray(x, dtype=dt)
+
+
+def probe_fp64_peak() -> float:
+    """Achieved TFLOP/s of an independent-DFMA-chain kernel on the current device."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RisError("no CUDA device")
+    out = C.c_double()
+    _check(load_library().ris_probe_fp64_peak(C.byref(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return out.value
+
+
+class RisContext:
+    """ris_setup(coords, shells, aux_exponents) -> context with ris_grad_J / ris_grad_K / ris_grad_PQ."""
+
+    def __init__(self, mol, *, schwarz_tol: float = 1e-13, deterministic: bool = False, p_batch: int = 0,
+                 profile: bool = False, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RisError("no CUDA device: the ris library has no CPU fallback")
+        self._lib = load_library()
+        self._torch = torch
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        arrs = (_np(mol.coords, np.float64), _np(mol.shell_atom, np.int32), _np(mol.shell_l, np.int32),
+                _np(mol.shell_nprim, np.int32), _np(mol.shell_prim_off, np.int32), _np(mol.prim_exp, np.float64),
+                _np(mol.prim_coef, np.float64), _np(mol.aux_exponents, np.float64))
+        opt = RisOptions(schwarz_tol, int(deterministic), int(p_batch), int(profile))
+        h = C.c_void_p()
+        _check(self._lib.ris_setup(C.byref(h), arrs[0].shape[0], arrs[0].ctypes.data, arrs[1].shape[0],
+                                   arrs[1].ctypes.data, arrs[2].ctypes.data, arrs[3].ctypes.data, arrs[4].ctypes.data,
+                                   arrs[5].ctypes.data, arrs[6].ctypes.data, arrs[7].ctypes.data, C.byref(opt),
+                                   C.c_void_p(self.stream.cuda_stream)))
+        self._h = h
+        self.nao = self._lib.ris_nao(h)
+        self.naux = self._lib.ris_naux(h)
+        self.natoms = self._lib.ris_natoms(h)
+
+    # ---- queries
+    def npairs(self, la, lb):
+        return int(self._lib.ris_npairs(self._h, la, lb))
+
+    def nprimpairs(self, la, lb):
+        return int(self._lib.ris_nprimpairs(self._h, la, lb))
+
+    @property
+    def npairs_total(self):
+        return int(self._lib.ris_npairs_total(self._h))
+
+    @property
+    def ntriplets(self):
+        return int(self._lib.ris_ntriplets(self._h))
+
+    @property
+    def ntriplets_unscreened(self):
+        return int(self._lib.ris_ntriplets_unscreened(self._h))
+
+    @property
+    def npair_elements(self):
+        return int(self._lib.ris_npair_elements(self._h))
+
+    @property
+    def p_batch(self):
+        return int(self._lib.ris_p_batch(self._h))
+
+    # ---- device-pointer calls (torch CUDA tensors, float64, contiguous)
+    def _dev(self, t, shape):
+        torch = self._torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise RisError("expected a contiguous float64 CUDA tensor")
+        if tuple(t.shape) != tuple(shape):
+            raise RisError(f"shape {tuple(t.shape)} != expected {tuple(shape)}")
+        return C.c_void_p(t.data_ptr())
+
+    def grad_J(self, D, c_aux, out=None):
+        nb = D.shape[0]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_grad_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)),
+                                    self._dev(c_aux, (nb, self.naux)), self._dev(out, (nb, self.natoms, 3))))
+        return out
+
+    def grad_K(self, C_occ, C_vir, B, out=None):
+        nb, nocc, nvir = B.shape[0], C_occ.shape[1], C_vir.shape[1]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_grad_K(self._h, nb, nocc, nvir, self._dev(C_occ, (self.nao, nocc)),
+                                    self._dev(C_vir, (self.nao, nvir)), self._dev(B, (nb, self.naux, nocc, nvir)),
+                                    self._dev(out, (nb, self.natoms, 3))))
+        return out
+
+    def grad_PQ(self, c_aux, d_aux, out=None):
+        nb = c_aux.shape[0]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux)), self._dev(d_aux, (nb, self.naux)),
+                                     self._dev(out, (nb, self.natoms, 3))))
+        return out
+
+    # ---- host-buffer calls (numpy arrays or pinned CPU tensors; copies happen inside the C call)
+    @staticmethod
+    def _host(x):
+        if hasattr(x, "data_ptr"):
+            if x.is_cuda or not x.is_contiguous():
+                raise RisError("expected a contiguous CPU tensor")
+            return C.c_void_p(x.data_ptr()), tuple(x.shape)
+        a = _np(x, np.float64)
+        return C.c_void_p(a.ctypes.data), a.shape, a
+
+    def grad_J_host(self, D, c_aux, out=None):
+        pD, pc = self._host(D), self._host(c_aux)
+        nb = pD[1][0]
+        if out is None:
+            out = np.empty((nb, self.natoms, 3))
+        _check(self._lib.ris_grad_J_host(self._h, nb, pD[0], pc[0], self._host(out)[0]))
+        return out
+
+    def grad_K_host(self, C_occ, C_vir, B, out=None):
+        po, pv, pB = self._host(C_occ), self._host(C_vir), self._host(B)
+        nb, nocc, nvir = pB[1][0], po[1][1], pv[1][1]
+        if out is None:
+            out = np.empty((nb, self.natoms, 3))
+        _check(self._lib.ris_grad_K_host(self._h, nb, nocc, nvir, po[0], pv[0], pB[0], self._host(out)[0]))
+        return out
+
+    def grad_PQ_host(self, c_aux, d_aux, out=None):
+        pc, pd = self._host(c_aux), self._host(d_aux)
+        nb = pc[1][0]
+        if out is None:
+            out = np.empty((nb, self.natoms, 3))
+        _check(self._lib.ris_grad_PQ_host(self._h, nb, pc[0], pd[0], self._host(out)[0]))
+        return out
+
+    # ---- profiling
+    def profile_reset(self):
+        _check(self._lib.ris_profile_reset(self._h))
+
+    def profile(self):
+        """[(kernel name, ms)] for every launch since the last reset (needs profile=True)."""
+        self.stream.synchronize()
+        n = self._lib.ris_profile_count(self._h)
+        out = []
+        for i in range(n):
+            name, ms = C.c_char_p(), C.c_float()
+            _check(self._lib.ris_profile_get(self._h, i, C.byref(name), C.byref(ms)))
+            out.append((name.value.decode(), ms.value))
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.ris_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def ris_setup(mol, **kw) -> RisContext:
+    return RisContext(mol, **kw)

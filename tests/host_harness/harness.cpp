@@ -1,0 +1,83 @@
+// Host-side test harness (tests only, never part of the product path): compiles the generated class
+// recurrences and the Boys interpolation of paper_2511_18233_b200/csrc as plain C++ so that the CPU
+// test-suite can check their arithmetic against the oracle without a GPU.
+#define RIS_DEV inline
+#include "ris_core.cuh"
+#include "ris_boys_table.h"
+#include <cstring>
+#include <map>
+
+static std::map<int, std::vector<double>> g_tabs;
+static const double* tab(int M)
+{
+    auto it = g_tabs.find(M);
+    if (it == g_tabs.end()) {
+        std::vector<double> t;
+        ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, t);
+        it = g_tabs.emplace(M, std::move(t)).first;
+    }
+    return it->second.data();
+}
+
+template <int M> static void boys_t(double T, double* F)
+{
+    double f[M + 1];
+    ris_boys<M>(T, tab(M), f);
+    for (int m = 0; m <= M; ++m) F[m] = f[m];
+}
+
+extern "C" int harness_boys(int M, double T, double* F)
+{
+    switch (M) {
+    case 1: boys_t<1>(T, F); break; case 2: boys_t<2>(T, F); break; case 3: boys_t<3>(T, F); break;
+    case 4: boys_t<4>(T, F); break; case 5: boys_t<5>(T, F); break; case 6: boys_t<6>(T, F); break;
+    case 7: boys_t<7>(T, F); break; default: return -1;
+    }
+    return 0;
+}
+
+// One contracted triplet: nk primitive pairs (prim[k][8] = p,Px,Py,Pz,oo2p,a2,b2,coef), aux (C, alpha,
+// auxfac); tile[nb][nca*ncb]; out[nb][6] = (dA, dB) contracted with the tile.  Primitive pairs with a >= b
+// are hosted on A, the others on B, exactly as the class kernel does.
+template <int LH, int LO, bool TR>
+static void phase_t(int nk, const double* prim, bool hostA, const double* Z, const double* ZO, const double* C,
+                    double alpha, double auxfac, const double* tile, int nb, double* out)
+{
+    using K = RisClass<LH, LO>;
+    double acc[K::NACC];
+    for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
+    int used = 0;
+    for (int k = 0; k < nk; ++k) {
+        const double* q = prim + 8 * k;
+        if ((q[5] >= q[6]) != hostA) continue;
+        ++used;
+        ris_prim_triplet<LH, LO>(q[0], q[1], q[2], q[3], q[4], hostA ? q[5] : q[6], hostA ? q[6] : q[5], q[7], Z[0], Z[1],
+                                 Z[2], C[0], C[1], C[2], alpha, auxfac, tab(K::E), acc);
+    }
+    if (!used) return;
+    ris_hrrc<LH, LO, TR>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)(K::NCA * K::NCB), nb,
+                         [&](int s, double h0, double h1, double h2, double o0, double o1, double o2) {
+                             double* o = out + 6 * s + (hostA ? 0 : 3);
+                             double* oo = out + 6 * s + (hostA ? 3 : 0);
+                             o[0] += h0; o[1] += h1; o[2] += h2; oo[0] += o0; oo[1] += o1; oo[2] += o2;
+                         });
+}
+
+template <int LA, int LB>
+static void triplet_t(int nk, const double* prim, const double* A, const double* AB, const double* C, double alpha,
+                      double auxfac, const double* tile, int nb, double* out)
+{
+    const double B[3] = {A[0] - AB[0], A[1] - AB[1], A[2] - AB[2]};
+    for (int i = 0; i < 6 * nb; ++i) out[i] = 0.0;
+    phase_t<LA, LB, false>(nk, prim, true, A, B, C, alpha, auxfac, tile, nb, out);
+    phase_t<LB, LA, true>(nk, prim, false, B, A, C, alpha, auxfac, tile, nb, out);
+}
+
+extern "C" int harness_triplet(int la, int lb, int nk, const double* prim, const double* A, const double* AB,
+                               const double* C, double alpha, double auxfac, const double* tile, int nb, double* out)
+{
+#define CASE(a, b) if (la == a && lb == b) { triplet_t<a, b>(nk, prim, A, AB, C, alpha, auxfac, tile, nb, out); return 0; }
+    CASE(0, 0) CASE(1, 0) CASE(1, 1) CASE(2, 0) CASE(2, 1) CASE(2, 2) CASE(3, 0) CASE(3, 1) CASE(3, 2) CASE(3, 3)
+#undef CASE
+    return -1;
+}
