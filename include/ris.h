@@ -58,10 +58,16 @@ enum ris_status {
 };
 
 typedef struct ris_options {
-    double schwarz_tol;   /* primitive-pair screening threshold, default 1e-13; <= 0 disables screening.
-                             A primitive pair (a,b) of shell pair (mu,nu) is dropped when
-                             |d_a d_b| K_ab (pi/p)^(3/2) max_P(N_P 2 pi/alpha_P) (1 + 2 max(a,b)) < tol;
-                             a shell pair is dropped when all its primitive pairs are. */
+    double schwarz_tol;   /* screening threshold tau, default 1e-13; <= 0 disables screening.  tau bounds the
+                             ACCUMULATED neglected contribution to a gradient component per unit |D c| / |Gamma|:
+                             a primitive pair (a,b) of shell pair (mu,nu) is dropped when
+                               |d_a d_b| K_ab (pi/p)^(3/2) max_P(N_P 2 pi/alpha_P) (1 + 2 max(a,b))
+                                   < tau / (naux sqrt(n_unique_shell_pairs)),
+                             (the bound on |(ab|P)| for s-type primitives -- the aux potential peaks at
+                             N_P 2 pi/alpha_P -- times a factor for polynomial / derivative growth, with the
+                             random-sign accumulation over naux x pairs folded into the threshold);
+                             a shell pair is dropped when all its primitive pairs are.  There is no screening on
+                             the aux index (the Coulomb tail is 1/R). */
     int deterministic;    /* nonzero: bitwise run-to-run reproducible reduction (slower) */
     int p_batch;          /* aux functions per Gamma^P batch in ris_grad_K; 0 = choose from free memory */
     int profile;          /* nonzero: record CUDA events around every kernel (see ris_profile_*) */

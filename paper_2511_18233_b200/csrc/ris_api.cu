@@ -212,9 +212,12 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     }
 
     // ---- S0 on device: survey -> scan -> scatter -> pack
-    RisMolDev m{natoms, nshells, c->d_coords, c->d_shell_atom, c->d_shell_l, c->d_shell_nprim, c->d_shell_poff,
-                c->d_shell_ao, c->d_pexp, c->d_pcoef, vmax, c->opt.schwarz_tol};
+    // schwarz_tol bounds the ACCUMULATED neglected contribution per unit |D c| or |Gamma| (include/ris.h): the
+    // per-primitive-pair threshold is tol / (naux sqrt(number of unique shell pairs)).
     const long long ntot = (long long)nshells * (nshells + 1) / 2;
+    const double tol_prim = c->opt.schwarz_tol > 0.0 ? c->opt.schwarz_tol / ((double)natoms * std::sqrt((double)ntot)) : 0.0;
+    RisMolDev m{natoms, nshells, c->d_coords, c->d_shell_atom, c->d_shell_l, c->d_shell_nprim, c->d_shell_poff,
+                c->d_shell_ao, c->d_pexp, c->d_pcoef, vmax, tol_prim};
     c->npairs_total = ntot;
     for (int i = 0; i <= nshells - 1; ++i)
         for (int j = 0; j <= i; ++j) c->nprim_total += (long long)shell_nprim[i] * shell_nprim[j];

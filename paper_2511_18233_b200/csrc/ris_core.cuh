@@ -96,21 +96,23 @@ RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 
 //   kappa = coef * auxfac / sqrt(p+alpha),  coef = d_a d_b K_ab 2 pi^{5/2}/p,  auxfac = N_P/alpha,
 // then the class recurrence + exponent-scaled accumulation (generated code); h2 / o2 = 2 x exponent of the
 // host / other primitive.
+// Accuracy: the packed record carries PZ = P - Z = -(o/p)(Z - O) computed from the centre difference, never
+// as a difference of absolute coordinates: for a tight pair on one atom the whole derivative is the small
+// WP term, and a rounding residue of size eps*|coords| in P - Z would swamp it.  P - C = (Z - C) + PZ.
 template <int LH, int LO>
-RIS_DEV void ris_prim_triplet(double p, double Px, double Py, double Pz, double oo2p, double h2, double o2,
-                              double coef, double Zx, double Zy, double Zz, double Cx, double Cy, double Cz,
-                              double alpha, double auxfac, const double* __restrict__ boys_tab,
-                              double (&acc)[RisClass<LH, LO>::NACC])
+RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, double oo2p, double h2, double o2,
+                              double coef, double ZCx, double ZCy, double ZCz, double alpha, double auxfac,
+                              const double* __restrict__ boys_tab, double (&acc)[RisClass<LH, LO>::NACC])
 {
     constexpr int E = RisClass<LH, LO>::E;
     const double s = ris_rsqrt(p + alpha);
     const double q = alpha * s * s;          // rho/p
-    const double X0 = Px - Cx, X1 = Py - Cy, X2 = Pz - Cz;
+    const double X0 = ZCx + PZx, X1 = ZCy + PZy, X2 = ZCz + PZz;
     const double T = (p * q) * fma(X0, X0, fma(X1, X1, X2 * X2));
     double F[E + 1];
     ris_boys<E>(T, boys_tab, F);
     const double kappa = coef * auxfac * s;
 #pragma unroll
     for (int m = 0; m <= E; ++m) F[m] *= kappa;
-    ris_vrr<LH, LO>(F, Px - Zx, Py - Zy, Pz - Zz, -q * X0, -q * X1, -q * X2, oo2p, q, h2, o2, acc);
+    ris_vrr<LH, LO>(F, PZx, PZy, PZz, -q * X0, -q * X1, -q * X2, oo2p, q, h2, o2, acc);
 }

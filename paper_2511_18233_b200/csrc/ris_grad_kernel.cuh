@@ -31,11 +31,12 @@ RIS_DEV void ris_phase(int k0, int k1, const double* __restrict__ prim, size_t f
     double acc[K::NACC];
 #pragma unroll
     for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
+    const double ZCx = Zx - Cx, ZCy = Zy - Cy, ZCz = Zz - Cz;
     for (int k = k0; k < k1; ++k) {
         const double* __restrict__ q = prim + (size_t)k * RIS_PRIM_FIELDS * fs;
         const double a2 = q[5 * fs], b2 = q[6 * fs];
         ris_prim_triplet<LH, LO>(q[0], q[fs], q[2 * fs], q[3 * fs], q[4 * fs], TR ? b2 : a2, TR ? a2 : b2, q[7 * fs],
-                                 Zx, Zy, Zz, Cx, Cy, Cz, alpha, auxfac, boys, acc);
+                                 ZCx, ZCy, ZCz, alpha, auxfac, boys, acc);
     }
     ris_hrrc<LH, LO, TR>(acc, Zx - ZOx, Zy - ZOy, Zz - ZOz, tile, fs, sstride, nb, sink);
 }

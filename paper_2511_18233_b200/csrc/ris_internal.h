@@ -5,7 +5,7 @@
 
 constexpr int RIS_LMAX = 3;
 constexpr int RIS_NCLASS = 10;          // (la,lb), la >= lb, la <= 3
-constexpr int RIS_PRIM_FIELDS = 8;      // p, Px, Py, Pz, 1/(2p), 2a, 2b, coef
+constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a, 2b, coef   (Z = host centre)
 constexpr int RIS_PAIR_PAD = 128;       // pairs per class padded to a multiple of this
 constexpr int RIS_GRAD_THREADS = 128;
 

@@ -162,9 +162,11 @@ __global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* l
                 const double p = a + b, ip_ = 1.0 / p;
                 double* q = pk.prim + (size_t)k * RIS_PRIM_FIELDS * n + ip;
                 q[0 * n] = p;
-                q[1 * n] = (a * A[0] + b * B[0]) * ip_;
-                q[2 * n] = (a * A[1] + b * B[1]) * ip_;
-                q[3 * n] = (a * A[2] + b * B[2]) * ip_;
+                // P - Z (Z = host centre) from the centre difference: host A: -(b/p)(A-B); host B: (a/p)(A-B)
+                const double fz = (host == 0) ? -b * ip_ : a * ip_;
+                q[1 * n] = fz * dx;
+                q[2 * n] = fz * dy;
+                q[3 * n] = fz * dz;
                 q[4 * n] = 0.5 * ip_;
                 q[5 * n] = 2.0 * a;
                 q[6 * n] = 2.0 * b;

@@ -36,7 +36,7 @@ extern "C" int harness_boys(int M, double T, double* F)
     return 0;
 }
 
-// One contracted triplet: nk primitive pairs (prim[k][8] = p,Px,Py,Pz,oo2p,a2,b2,coef), aux (C, alpha,
+// One contracted triplet: nk primitive pairs (prim[k][8] = p,(P-Z)x,(P-Z)y,(P-Z)z,oo2p,a2,b2,coef; Z = host centre), aux (C, alpha,
 // auxfac); tile[nb][nca*ncb]; out[nb][6] = (dA, dB) contracted with the tile.  Primitive pairs with a >= b
 // are hosted on A, the others on B, exactly as the class kernel does.
 template <int LH, int LO, bool TR>
@@ -51,8 +51,8 @@ static void phase_t(int nk, const double* prim, bool hostA, const double* Z, con
         const double* q = prim + 8 * k;
         if ((q[5] >= q[6]) != hostA) continue;
         ++used;
-        ris_prim_triplet<LH, LO>(q[0], q[1], q[2], q[3], q[4], hostA ? q[5] : q[6], hostA ? q[6] : q[5], q[7], Z[0], Z[1],
-                                 Z[2], C[0], C[1], C[2], alpha, auxfac, tab(K::E), acc);
+        ris_prim_triplet<LH, LO>(q[0], q[1], q[2], q[3], q[4], hostA ? q[5] : q[6], hostA ? q[6] : q[5], q[7],
+                                 Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac, tab(K::E), acc);
     }
     if (!used) return;
     ris_hrrc<LH, LO, TR>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)(K::NCA * K::NCB), nb,

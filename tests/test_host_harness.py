@@ -79,10 +79,10 @@ def test_class_recurrence_vs_oracle(harness, la, lb):
             for kb in range(3):
                 a, b = mol.prim_exp[ka], mol.prim_exp[3 + kb]
                 p = a + b
-                Pc = (a * A + b * B) / p
+                PZ = -(b / p) * (A - B) if a >= b else (a / p) * (A - B)     # P - host centre
                 Kab = math.exp(-a * b / p * np.dot(A - B, A - B))
                 coef = mol.prim_coef[ka] * mol.prim_coef[3 + kb] * Kab * 2 * math.pi ** 2.5 / p
-                prim.append([p, Pc[0], Pc[1], Pc[2], 0.5 / p, 2 * a, 2 * b, coef])
+                prim.append([p, PZ[0], PZ[1], PZ[2], 0.5 / p, 2 * a, 2 * b, coef])
         prim = np.ascontiguousarray(prim)
         alpha = mol.aux_exponents[P]
         auxfac = (2 * alpha / math.pi) ** 0.75 / alpha
