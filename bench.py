@@ -1,0 +1,320 @@
+#!/usr/bin/env python3
+"""bench.py -- the TDDFT-ris derivative-integral hot path on B200 (contract: task prompt "Measurement").
+
+One "step" = one pass of the whole hot path over one batch of synthetic input:
+    ris_grad_J(D, c_aux) + ris_grad_K(C_occ, C_vir, B) + ris_grad_PQ(c_aux, d_aux)      (Eq. 27)
+for all `nbatch` states of the workload, on a context built once by ris_setup (one-off per geometry, reported
+separately as `setup_ms`).  Metric (BASELINE.json): TDDFT-ris gradient ms/state -- with the two other figures of
+the metric string (3c2e-derivative primitive triplets/s, % FP64 peak) in the same JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+N > 1 (torchrun): the path shards over independent states: every rank runs the same
+molecule with its own batch of states, no data-path collective; value = time / (N * nbatch)  ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "TDDFT-ris gradient ms/state"
+UNIT = "ms/state"
+ORACLE_CUTOFF = {4: 1e-22}      # the oracle's documented primitive cutoff on config 4
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = the largest")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--oracle-aux", type=int, default=0, help="aux functions in the oracle's timed sample (0 = auto)")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ oracle leg
+def oracle_sample_time(wl, cfg: int, n_aux: int, nstate: int = 1):
+    """Time the oracle AS IT STANDS on a bounded sample of the workload: aux functions P in [0, n_aux) (of naux),
+    `nstate` state(s): J + K (incl. its Gamma^P assembly, numpy matmul) for the sample, PQ in full.  Returns
+    (seconds for the sample, extrapolated ms/state for the whole workload, threads, description)."""
+    from oracle import ris_oracle as orc
+    mol = wl.mol
+    cut = ORACLE_CUTOFF.get(cfg, 0.0)
+    aux = list(range(min(n_aux, mol.natoms)))
+    t0 = time.perf_counter()
+    orc.grad_J(mol, wl.D[:nstate], wl.c_aux[:nstate], prim_cutoff=cut, aux=aux)
+    tJ = time.perf_counter()
+    orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B[:nstate], prim_cutoff=cut, aux=aux)
+    tK = time.perf_counter()
+    orc.grad_PQ(mol, wl.c_aux[:nstate], wl.d_aux[:nstate])
+    tQ = time.perf_counter()
+    frac = len(aux) / mol.natoms
+    ms_state = ((tK - t0) / frac + (tQ - tK)) / nstate * 1e3
+    desc = (f"aux P in [0,{len(aux)}) of {mol.natoms}, {nstate} state of the batch: oracle grad_J {tJ - t0:.2f}s + grad_K "
+            f"(numpy Gamma^P + integrals) {tK - tJ:.2f}s, PQ in full {tQ - tK:.3f}s; ms/state extrapolated x{1 / frac:.1f}"
+            + (f"; oracle primitive cutoff {cut:g}" if cut else ""))
+    return tQ - t0, ms_state, orc.num_threads(), desc
+
+
+def auto_oracle_aux(wl) -> int:
+    # about 10-30 s of CPU work: cost per aux ~ ordered primitive pairs + Gamma^P matmul
+    est = {1: 3, 2: 30, 3: 12, 4: 6, 5: 4}
+    return est.get(wl.meta.get("config", 0), 4)
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2511_18233_b200 import probe_fp64_peak, ris_setup, synth
+    from paper_2511_18233_b200.ris import probe_fp64_mma_peak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the ris library has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    wl = synth.make_workload(args.config)
+    mol = wl.mol
+    nbJ, nbK = wl.D.shape[0], wl.B.shape[0]
+    nstates = max(nbJ, nbK)
+
+    t0 = time.perf_counter()
+    ctx = ris_setup(mol, schwarz_tol=wl.schwarz_tol, profile=True)
+    torch.cuda.synchronize()
+    setup_ms = (time.perf_counter() - t0) * 1e3
+
+    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k))).pin_memory()
+            for k in ("D", "c_aux", "d_aux", "C_occ", "C_vir", "B")}
+    d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+    gJ = torch.empty((nbJ, mol.natoms, 3), dtype=torch.float64, device=dev)
+    gK = torch.empty((nbK, mol.natoms, 3), dtype=torch.float64, device=dev)
+    gQ = torch.empty((nbJ, mol.natoms, 3), dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+
+    def step():
+        ctx.grad_J(d["D"], d["c_aux"], out=gJ)
+        ctx.grad_K(d["C_occ"], d["C_vir"], d["B"], out=gK)
+        ctx.grad_PQ(d["c_aux"], d["d_aux"], out=gQ)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    fp64_peak = probe_fp64_peak()            # DFMA chains, TFLOP/s (MEASURED_PEAKS.json has no FP64 figure)
+    mma_peak = probe_fp64_mma_peak()         # mma.sync f64 chains, TFLOP/s
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    ctx.profile_reset()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    prof = ctx.profile()
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = ms_step / (world * nstates)
+
+    # ---- per-kernel accounting from the CUDA events the library records around every launch (same stream)
+    groups = {}
+    for name, ms, fl, by in prof:
+        g = groups.setdefault(name, {"launches": 0, "ms": 0.0, "flops": 0.0, "bytes": 0.0})
+        g["launches"] += 1; g["ms"] += ms; g["flops"] += fl; g["bytes"] += by
+    ksum = sum(g["ms"] for g in groups.values())
+    dom_name = max(groups, key=lambda k: groups[k]["ms"])
+    dom = groups[dom_name]
+    is_gemm = dom_name.startswith("ris_gemm")
+    peak = mma_peak if is_gemm else fp64_peak
+    achieved = dom["flops"] / (dom["ms"] * 1e-3) * 1e-12 if dom["ms"] > 0 else 0.0
+    roofline = {"kernel": dom_name, "bound": "tensor" if is_gemm else "alu", "achieved": round(achieved, 3),
+                "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4) if peak else None,
+                "traffic": None, "launches": dom["launches"], "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
+                "share_of_kernel_time": round(dom["ms"] / ksum, 4),
+                "peak_source": ("measured in this run by ris_probe_fp64_mma_peak (mma.sync f64 chains)" if is_gemm else
+                                "measured in this run by ris_probe_fp64_peak (independent DFMA chains)")
+                               + "; MEASURED_PEAKS.json carries no FP64 figure"}
+    cls = [g for n, g in groups.items() if n.startswith("ris_grad_kernel")]
+    cls_ms = sum(g["ms"] for g in cls)
+    cls_fl = sum(g["flops"] for g in cls)
+    ncalls = 2 * args.steps                      # J and K each run the class kernels over all triplets
+    integrals = {"tflops_model": round(cls_fl / (cls_ms * 1e-3) * 1e-12, 3) if cls_ms else None,
+                 "frac_of_fp64_peak": round(cls_fl / (cls_ms * 1e-3) * 1e-12 / fp64_peak, 4) if cls_ms else None,
+                 "fp64_peak_tflops": round(fp64_peak, 2), "ms_per_step": round(cls_ms / args.steps, 4),
+                 "triplets_per_s": round(ctx.ntriplets * ncalls / (cls_ms * 1e-3), 1) if cls_ms else None,
+                 "ntriplets": ctx.ntriplets, "ntriplets_unscreened": ctx.ntriplets_unscreened}
+    gemm_ms = sum(g["ms"] for n, g in groups.items() if n.startswith("ris_gemm"))
+    gemm_fl = sum(g["flops"] for n, g in groups.items() if n.startswith("ris_gemm"))
+    kernels = {n: {"launches": g["launches"], "ms_per_step": round(g["ms"] / args.steps, 4),
+                   "tflops": round(g["flops"] / (g["ms"] * 1e-3) * 1e-12, 3) if g["ms"] > 0 else None,
+                   "gbs": round(g["bytes"] / (g["ms"] * 1e-3) * 1e-9, 1) if g["ms"] > 0 else None}
+               for n, g in sorted(groups.items(), key=lambda kv: -kv[1]["ms"])}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D + kernels + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hJ = np.empty((nbJ, mol.natoms, 3)); hK = np.empty((nbK, mol.natoms, 3)); hQ = np.empty((nbJ, mol.natoms, 3))
+
+        def step_host():
+            ctx.grad_J_host(host["D"], host["c_aux"], out=hJ)
+            ctx.grad_K_host(host["C_occ"], host["C_vir"], host["B"], out=hK)
+            ctx.grad_PQ_host(host["c_aux"], host["d_aux"], out=hQ)
+
+        step_host()
+        barrier()
+        n_e2e = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            step_host()
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) * 1e3 / n_e2e
+        if world > 1:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        h2d = 8 * (host["D"].numel() + 2 * host["c_aux"].numel() + host["C_occ"].numel() + host["C_vir"].numel()
+                   + host["B"].numel() + host["c_aux"].numel() + host["d_aux"].numel())
+        d2h = 8 * (hJ.size + hK.size + hQ.size)
+        e2e = {"value": round(t_e2e / (world * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
+               "how": "ris_grad_{J,K,PQ}_host on pinned host buffers; host wall clock around the calls (they return "
+                      "after the D2H copy of the gradient)"}
+
+    line = {
+        "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "natoms": mol.natoms, "nao": mol.nao, "naux": mol.natoms, "nocc": wl.nocc,
+                   "nvir": wl.nvir, "nbatch_J": nbJ, "nbatch_K": nbK, "schwarz_tol": wl.schwarz_tol,
+                   "p_batch": ctx.p_batch, "l2": "inputs larger than L2 (B alone is %.2f GB)" % (host["B"].numel() * 8e-9)
+                   if host["B"].numel() * 8 > 200e6 else "inputs smaller than L2; no flush (latency-bound case)",
+                   "step": "ris_grad_J + ris_grad_K + ris_grad_PQ, all states; ris_setup excluded (one-off per geometry)"},
+        "setup_ms": round(setup_ms, 2), "e2e": e2e, "gpu_launches": len(prof),
+        "roofline": roofline, "integral_kernels": integrals,
+        "gamma_gemm": {"ms_per_step": round(gemm_ms / args.steps, 4),
+                       "tflops": round(gemm_fl / (gemm_ms * 1e-3) * 1e-12, 3) if gemm_ms else None,
+                       "fp64_mma_peak_tflops": round(mma_peak, 2)},
+        "kernels": kernels, "clocks": clocks,
+    }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            n_aux = args.oracle_aux or auto_oracle_aux(wl)
+            secs, ms_state, thr, desc = oracle_sample_time(wl, args.config, n_aux)
+            line["cpu_baseline"] = {"value": round(ms_state, 2), "unit": UNIT, "cores": thr, "kind": "oracle",
+                                    "sample": desc, "sample_seconds": round(secs, 2)}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def run_reference(args):
+    """The oracle, as it stands, on the host cores (rank 0 only); each step = the bounded sample."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2511_18233_b200 import synth        # input generator only (no arithmetic of the method)
+    wl = synth.make_workload(args.config)
+    n_aux = args.oracle_aux or auto_oracle_aux(wl)
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle_sample_time(wl, args.config, 1)
+    vals, secs = [], 0.0
+    steps = max(1, min(args.steps, 3))
+    for _ in range(steps):
+        s, ms_state, thr, desc = oracle_sample_time(wl, args.config, n_aux)
+        vals.append(ms_state); secs += s
+    v = float(np.mean(vals))
+    nstates = max(wl.D.shape[0], wl.B.shape[0])
+    line = {"impl": "reference", "metric": METRIC, "value": round(v, 2), "unit": UNIT,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": steps, "warmup": min(args.warmup, 1),
+            "ms_per_step": round(v * nstates, 2), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "natoms": wl.mol.natoms, "nao": wl.mol.nao, "nocc": wl.nocc, "nvir": wl.nvir},
+            "cpu_baseline": {"value": round(v, 2), "unit": UNIT, "cores": thr, "kind": "oracle", "sample": desc,
+                             "sample_seconds": round(secs / steps, 2)},
+            "e2e": {"value": round(v, 2), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -16,7 +16,8 @@ derivative folded into the inputs; Eqs. 21-22 for the integrals
 Each also returns the undifferentiated scalar (E_J, E_K, E_PQ) used by the finite-difference pin.
 `atoms=` samples the output: only rows of the listed atoms are computed (and returned; the other
 rows are NaN), visiting only triplets that touch them -- the definition restricted to those
-outputs, used for full-size parity.
+outputs, used for full-size parity.  `aux=` restricts the sum over P to the listed auxiliary
+functions (a bounded sample of the same workload, used only for timing the oracle in bench.py).
 """
 from __future__ import annotations
 
@@ -135,7 +136,7 @@ def _finish(g, e, mask):
     return g, e.astype(np.float64)
 
 
-def grad_J(mol, D, c_aux, *, atoms=None, prim_cutoff=0.0):
+def grad_J(mol, D, c_aux, *, atoms=None, prim_cutoff=0.0, aux=None):
     """G_J and E_J = sum D_{mu nu} c_P (mu nu|P).  D [nbatch][nao][nao] (any symmetry), c [nbatch][naux]."""
     h = _Held(mol)
     D = _f64(D).reshape(-1, h.nao, h.nao)
@@ -144,7 +145,7 @@ def grad_J(mol, D, c_aux, *, atoms=None, prim_cutoff=0.0):
     mask = _mask(h.natoms, atoms)
     g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
     e = np.zeros(nb, dtype=np.longdouble)
-    for P in range(h.natoms):
+    for P in (range(h.natoms) if aux is None else aux):
         sc = _f64(c_aux[:, P])
         rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, sc.ctypes.data,
                                          mask.ctypes.data if mask is not None else None, prim_cutoff,
@@ -165,7 +166,7 @@ def gamma_P(C_occ, C_vir, B_sP, rows=None):
     return G
 
 
-def grad_K(mol, C_occ, C_vir, B, *, atoms=None, prim_cutoff=0.0):
+def grad_K(mol, C_occ, C_vir, B, *, atoms=None, prim_cutoff=0.0, aux=None):
     """G_K and E_K = sum_P sum Gamma^P_{mu nu} (mu nu|P).  B [nbatch][naux][nocc][nvir]."""
     h = _Held(mol)
     C_occ, C_vir = _f64(C_occ), _f64(C_vir)
@@ -176,7 +177,7 @@ def grad_K(mol, C_occ, C_vir, B, *, atoms=None, prim_cutoff=0.0):
     e = np.zeros(nb, dtype=np.longdouble)
     one = np.ones(nb)
     rows_sampled = None if mask is None else np.nonzero(mask[h.ao_atom])[0]
-    for P in range(h.natoms):
+    for P in (range(h.natoms) if aux is None else aux):
         rows = None if (mask is None or mask[P]) else rows_sampled
         G = _f64(np.stack([gamma_P(C_occ, C_vir, B[s, P], rows) for s in range(nb)]))
         rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, G.ctypes.data, one.ctypes.data,

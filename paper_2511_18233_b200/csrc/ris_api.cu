@@ -39,7 +39,7 @@ extern "C" const char* ris_strerror(int status)
 }
 
 // --------------------------------------------------------------------------------------- context
-struct ProfRec { const char* name; cudaEvent_t e0, e1; };
+struct ProfRec { const char* name; cudaEvent_t e0, e1; double flops, bytes; };
 
 struct ris_ctx {
     int device = 0;
@@ -100,10 +100,11 @@ template <class T> static int dev_upload(ris_ctx* c, T** p, const T* h, size_t n
 // profiling: events around a launch when opt.profile is set
 struct ProfScope {
     ris_ctx* c; int idx = -1;
-    ProfScope(ris_ctx* c_, const char* name) : c(c_)
+    // flops / bytes: ALGORITHMIC work of the launch
+    ProfScope(ris_ctx* c_, const char* name, double flops = 0.0, double bytes = 0.0) : c(c_)
     {
         if (!c->opt.profile) return;
-        ProfRec r; r.name = name;
+        ProfRec r; r.name = name; r.flops = flops; r.bytes = bytes;
         if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) return;
         cudaEventRecord(r.e0, c->stream);
         c->prof.push_back(r);
@@ -129,6 +130,14 @@ extern "C" int ris_profile_get(ris_ctx* c, int i, const char** name, float* ms)
     return RIS_OK;
 }
 
+extern "C" int ris_profile_get_work(ris_ctx* c, int i, double* flops, double* bytes)
+{
+    if (!c || i < 0 || i >= (int)c->prof.size() || !flops || !bytes) return RIS_EINVAL;
+    *flops = c->prof[i].flops;
+    *bytes = c->prof[i].bytes;
+    return RIS_OK;
+}
+
 // --------------------------------------------------------------------------------------- class launchers
 #define DECL(la, lb) void ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
@@ -139,6 +148,9 @@ ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
 static const char* const kGradNames[RIS_NCLASS] = {
     "ris_grad_kernel<0,0>", "ris_grad_kernel<1,0>", "ris_grad_kernel<1,1>", "ris_grad_kernel<2,0>", "ris_grad_kernel<2,1>",
     "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
+// Algorithmic FP64 flops per primitive triplet by E = la + lb + 1 (SURVEY.md 8(d) model: setup ~45, Boys ~30 + 4E,
+// 7 flops per OS-VRR intermediate, scaled accumulation), plus 12 nca ncb flops per contracted triplet and state.
+static const double kModelFlopsByE[8] = {0.0, 140.0, 250.0, 450.0, 750.0, 1250.0, 2000.0, 3100.0};
 // heaviest class first (flops per primitive triplet), so the tail is made of light kernels
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
@@ -339,7 +351,8 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
     for (int k = 0; k < RIS_NCLASS; ++k) {
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
-        ProfScope ps(c, "ris_k_pack_tiles");
+        const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs * nslab;
+        ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel, 24.0 * nel);
         dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), nslab);
         ris_k_pack_tiles<<<grid, 128, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
     }
@@ -365,7 +378,10 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         int ny = std::max(1, (4 * 148 + bx - 1) / bx);
         int pch = std::max(4, (np + ny - 1) / ny);
         p.pchunk = std::min(std::min(pch, np), 64);
-        ProfScope ps(c, kGradNames[k]);
+        const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
+        ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
+                     8.0 * (np_ * (pstride ? 1.0 : 0.0) + (pstride ? 0.0 : 1.0)) * nel * pk.npairs * nb +
+                         8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
         ris_grad_launchers[k](p, c->stream);
     }
     CU(cudaGetLastError());
@@ -427,11 +443,13 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                 // S3-K1: H^P = B^P C_vir^T  ([np*nocc x nvir] x [nao x nvir]^T), Gamma^P = C_occ H^P
                 const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
                 {
-                    ProfScope ps(c, "ris_gemm_nt(H=B*Cvir^T)");
+                    ProfScope ps(c, "ris_gemm_nt(H=B*Cvir^T)", 2.0 * np * nocc * (double)nao * nvir,
+                                 8.0 * ((double)np * nocc * nvir + (double)nao * nvir + (double)np * nocc * nao));
                     ris_gemm<true>(c->stream, np * nocc, nao, nvir, Bs, nvir, 0, C_vir, nvir, 0, H, nao, 0, 1);
                 }
                 {
-                    ProfScope ps(c, "ris_gemm_nn(Gamma=Cocc*H)");
+                    ProfScope ps(c, "ris_gemm_nn(Gamma=Cocc*H)", 2.0 * np * nocc * (double)nao * nao,
+                                 8.0 * np * ((double)nocc * nao + (double)nao * nao) + 8.0 * nao * nocc);
                     ris_gemm<false>(c->stream, nao, nao, nocc, C_occ, nocc, 0, H, nao, (long long)nocc * nao, G, nao, nao2, np);
                 }
                 CU(cudaGetLastError());
@@ -485,7 +503,7 @@ extern "C" int ris_grad_PQ(ris_ctx* c, int nbatch, const double* c_aux, const do
 {
     if (!c || nbatch < 1 || !c_aux || !d_aux || !grad) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
-    ProfScope ps(c, "ris_k_grad_pq");
+    ProfScope ps(c, "ris_k_grad_pq", 60.0 * c->naux * (double)c->naux * nbatch, 0.0);
     ris_k_grad_pq<<<dim3(c->naux, nbatch), 128, 0, c->stream>>>(c->naux, nbatch, c->d_aux, c->d_boys[1], c_aux, d_aux, grad);
     CU(cudaGetLastError());
     return RIS_OK;
@@ -567,7 +585,22 @@ __global__ void ris_k_dfma_probe(double* out, int iters, double a, double b)
     if (s == 12345.678) out[0] = s;
 }
 
-extern "C" int ris_probe_fp64_peak(double* tflops, void* cuda_stream)
+__global__ void ris_k_dmma_probe(double* out, int iters)
+{
+    double c0[2] = {0, 0}, c1[2] = {0, 0}, c2[2] = {0, 0}, c3[2] = {0, 0};
+    const double a = threadIdx.x * 1e-3, b = 1.0 + threadIdx.x * 1e-4;
+    for (int it = 0; it < iters; ++it) {
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c0[0]), "+d"(c0[1]) : "d"(a), "d"(b));
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c1[0]), "+d"(c1[1]) : "d"(a), "d"(b));
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c2[0]), "+d"(c2[1]) : "d"(a), "d"(b));
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c3[0]), "+d"(c3[1]) : "d"(a), "d"(b));
+    }
+    const double s = c0[0] + c0[1] + c1[0] + c1[1] + c2[0] + c2[1] + c3[0] + c3[1];
+    if (s == 12345.678) out[0] = s;
+}
+
+// kind 0: independent DFMA chains (FP64 FMA pipe); kind 1: mma.sync m8n8k4 f64 chains (FP64 tensor path)
+static int probe_fp64(int kind, double* tflops, void* cuda_stream)
 {
     if (!tflops) return RIS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -583,14 +616,19 @@ extern "C" int ris_probe_fp64_peak(double* tflops, void* cuda_stream)
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {
         CU(cudaEventRecord(e0, st));
-        ris_k_dfma_probe<<<nsm, thr, 0, st>>>(d, iters, 1.0000001, 1e-9);
+        if (kind == 0) ris_k_dfma_probe<<<nsm, thr, 0, st>>>(d, iters, 1.0000001, 1e-9);
+        else ris_k_dmma_probe<<<nsm, thr, 0, st>>>(d, iters);
         CU(cudaEventRecord(e1, st));
         CU(cudaEventSynchronize(e1));
         float ms = 0.f;
         CU(cudaEventElapsedTime(&ms, e0, e1));
-        if (rep) best = std::max(best, 2.0 * 8 * iters * (double)nsm * thr / (ms * 1e-3) * 1e-12);
+        const double fl = kind == 0 ? 2.0 * 8 * iters * (double)nsm * thr : 2.0 * 8 * 8 * 4 * 4 * iters * (double)nsm * (thr / 32);
+        if (rep) best = std::max(best, fl / (ms * 1e-3) * 1e-12);
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     *tflops = best;
     return RIS_OK;
 }
+
+extern "C" int ris_probe_fp64_peak(double* tflops, void* cuda_stream) { return probe_fp64(0, tflops, cuda_stream); }
+extern "C" int ris_probe_fp64_mma_peak(double* tflops, void* cuda_stream) { return probe_fp64(1, tflops, cuda_stream); }

@@ -19,7 +19,7 @@ EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
-    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_probe_fp64_peak",
+    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work", "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak",
 ]
 
 
@@ -60,7 +60,9 @@ def load_library():
         getattr(lib, name).argtypes = [vp]
         getattr(lib, name).restype = C.c_longlong
     lib.ris_profile_get.argtypes = [vp, ci, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    lib.ris_profile_get_work.argtypes = [vp, ci, C.POINTER(cd), C.POINTER(cd)]
     lib.ris_probe_fp64_peak.argtypes = [C.POINTER(cd), vp]
+    lib.ris_probe_fp64_mma_peak.argtypes = [C.POINTER(cd), vp]
     _lib = lib
     return lib
 
@@ -81,6 +83,16 @@ def probe_fp64_peak() -> float:
         raise RisError("no CUDA device")
     out = C.c_double()
     _check(load_library().ris_probe_fp64_peak(C.byref(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return out.value
+
+
+def probe_fp64_mma_peak() -> float:
+    """Achieved TFLOP/s of independent mma.sync f64 chains on the current device."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RisError("no CUDA device")
+    out = C.c_double()
+    _check(load_library().ris_probe_fp64_mma_peak(C.byref(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
     return out.value
 
 
@@ -210,14 +222,16 @@ class RisContext:
         _check(self._lib.ris_profile_reset(self._h))
 
     def profile(self):
-        """[(kernel name, ms)] for every launch since the last reset (needs profile=True)."""
+        """[(kernel name, ms, algorithmic flops, algorithmic bytes)] for every launch since the last reset
+        (needs profile=True)."""
         self.stream.synchronize()
         n = self._lib.ris_profile_count(self._h)
         out = []
         for i in range(n):
-            name, ms = C.c_char_p(), C.c_float()
+            name, ms, fl, by = C.c_char_p(), C.c_float(), C.c_double(), C.c_double()
             _check(self._lib.ris_profile_get(self._h, i, C.byref(name), C.byref(ms)))
-            out.append((name.value.decode(), ms.value))
+            _check(self._lib.ris_profile_get_work(self._h, i, C.byref(fl), C.byref(by)))
+            out.append((name.value.decode(), ms.value, fl.value, by.value))
         return out
 
     def close(self):
