@@ -54,6 +54,10 @@ struct ris_ctx {
     std::vector<void*> owned;          // every device allocation of the packed data
     long long nelem_slab = 0, nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[8] = {nullptr};
+    // Gamma^P GEMM-2 block list: 128x128 AO blocks (I >= J) that contain a surviving shell pair
+    int nblk = 0, ntiles = 0;
+    int2* d_tiles = nullptr;           // [ntiles] (I, J)
+    int* d_tmap = nullptr;             // [nblk][nblk] tile index of (I >= J), -1 if absent
     // grow-only scratch
     void* ws[8] = {nullptr};
     size_t ws_bytes[8] = {0};
@@ -62,7 +66,7 @@ struct ris_ctx {
     std::vector<cudaEvent_t> ev_pool;
 };
 
-enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6 };
+enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -155,6 +159,17 @@ static const double kModelFlopsByE[8] = {0.0, 140.0, 250.0, 450.0, 750.0, 1250.0
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
 // --------------------------------------------------------------------------------------- setup
+// Marks the 128x128 AO blocks (I >= J) touched by the surviving shell pairs of one class.
+__global__ void ris_k_mark_blocks(RisClassPack pk, int nblk, int* mark)
+{
+    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ip >= pk.npairs) return;
+    const int r0 = pk.ao[ip], q0 = pk.ao[(size_t)pk.npad + ip];
+    const int r1 = r0 + ris_ncart(pk.la) - 1, q1 = q0 + ris_ncart(pk.lb) - 1;
+    for (int I = r0 / RIS_GBM; I <= r1 / RIS_GBM; ++I)
+        for (int J = q0 / RIS_GBM; J <= q1 / RIS_GBM; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
+}
+
 extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
                          const int32_t* shell_l, const int32_t* shell_nprim, const int32_t* shell_prim_off,
                          const double* prim_exp, const double* prim_coef, const double* aux_exponents,
@@ -294,6 +309,29 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         }
     c->nelem_slab = off;
     CU(cudaGetLastError());
+    // block list for the pair-restricted Gamma^P GEMM-2
+    c->nblk = (nao + RIS_GBM - 1) / RIS_GBM;
+    {
+        int* d_mark;
+        if ((rc = dev_alloc(c, &d_mark, (size_t)c->nblk * c->nblk, true))) return rc;
+        for (int k = 0; k < RIS_NCLASS; ++k)
+            if (c->cls[k].npairs > 0)
+                ris_k_mark_blocks<<<(c->cls[k].npairs + 127) / 128, 128, 0, c->stream>>>(c->cls[k], c->nblk, d_mark);
+        CU(cudaGetLastError());
+        std::vector<int> mark((size_t)c->nblk * c->nblk);
+        CU(cudaMemcpyAsync(mark.data(), d_mark, mark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        std::vector<int2> tiles;
+        for (int I = 0; I < c->nblk; ++I)
+            for (int J = 0; J <= I; ++J) {
+                int& m_ = mark[(size_t)I * c->nblk + J];
+                if (m_) { m_ = (int)tiles.size(); tiles.push_back(make_int2(I, J)); } else m_ = -1;
+            }
+        c->ntiles = (int)tiles.size();
+        if ((rc = dev_upload(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
+        if ((rc = dev_upload(c, &c->d_tmap, mark.data(), mark.size()))) return rc;
+        CU(cudaStreamSynchronize(c->stream));      // host vectors go out of scope
+    }
     CU(cudaStreamSynchronize(c->stream));
     guard.ok = true;
     *out = c;
@@ -409,6 +447,30 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
 }
 
 // --------------------------------------------------------------------------------------- K
+// out[z][elem_off + e*npad + ip] = symf[ip] * S^P[mu0+ca][nu0+cb] read from the 128x128 block buffer of GEMM-2
+// (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
+__global__ void ris_k_pack_sym(RisClassPack pk, const double* __restrict__ S, long long sstrideP, const int* __restrict__ tmap,
+                               int nblk, double* __restrict__ out, long long ostride)
+{
+    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ip >= pk.npairs) return;
+    const int ncb = ris_ncart(pk.lb);
+    const int e = blockIdx.y, ca = e / ncb, cb = e - ca * ncb;
+    int r = pk.ao[ip] + ca, q = pk.ao[(size_t)pk.npad + ip] + cb;
+    if ((r >> 7) < (q >> 7)) { const int t = r; r = q; q = t; }
+    const int tile = tmap[(r >> 7) * nblk + (q >> 7)];
+    const double v = S[(size_t)blockIdx.z * sstrideP + (size_t)tile * (RIS_GBM * RIS_GBN) + (r & 127) * RIS_GBN + (q & 127)];
+    out[(size_t)blockIdx.z * ostride + pk.elem_off + (size_t)e * pk.npad + ip] = (double)pk.symf[ip] * v;
+}
+
+__global__ void ris_k_pad_rows(int rows, int cols, int ld, const double* __restrict__ in, double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)rows * ld) return;
+    const int r = (int)(i / ld), cidx = (int)(i - (long long)r * ld);
+    out[i] = cidx < cols ? in[(size_t)r * cols + cidx] : 0.0;
+}
+
 extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                           const double* B, double* grad)
 {
@@ -416,44 +478,68 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     const int nao = c->nao, naux = c->naux;
-    const long long nao2 = (long long)nao * nao;
     const int nbmax = std::min(nbatch, RIS_NB_MAX);
-    // Gamma^P batch: H [pb][nocc][nao], dense Gamma [pb][nao][nao], packed tiles [nb][pb][slab]
+    const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
+    const long long blk = (long long)RIS_GBM * RIS_GBN;
+    // per aux function: HT [nao][noccp], S blocks [ntiles][128*128], packed tiles [nb][slab]
     int pb = c->opt.p_batch;
     if (pb <= 0) {
         size_t fr = 0, tot = 0;
         CU(cudaMemGetInfo(&fr, &tot));
         fr += c->ws_bytes[WS_TILE] + c->ws_bytes[WS_H] + c->ws_bytes[WS_G];
-        const double per = 8.0 * ((double)nocc * nao + (double)nao2 + (double)nbmax * c->nelem_slab);
-        const double budget = std::min(0.5 * (double)fr, 16.0e9);
+        const double per = 8.0 * ((double)noccp * nao + (double)c->ntiles * blk + (double)nbmax * c->nelem_slab);
+        const double budget = std::min(0.5 * (double)fr, 24.0e9);
         pb = (int)std::max(1.0, std::min((double)naux, budget / per));
     }
     pb = std::min(pb, naux);
     c->last_pbatch = pb;
-    double *tile, *H, *G;
+    double *tile, *HT, *S, *Cop;
     int rc;
     if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pb * c->nelem_slab, (void**)&tile))) return rc;
-    if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)pb * nocc * nao, (void**)&H))) return rc;
-    if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * nao2, (void**)&G))) return rc;
+    if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)nao * pb * noccp, (void**)&HT))) return rc;
+    if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * c->ntiles * blk, (void**)&S))) return rc;
+    if ((rc = ws_get(c, WS_COCC, sizeof(double) * (size_t)nao * noccp, (void**)&Cop))) return rc;
+    {
+        ProfScope ps(c, "ris_k_pad_rows", 0.0, 16.0 * nao * (double)noccp);
+        const long long n = (long long)nao * noccp;
+        ris_k_pad_rows<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(nao, nocc, noccp, C_occ, Cop);
+    }
     for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
         const int nb = std::min(RIS_NB_MAX, nbatch - s0);
         for (int p0 = 0; p0 < naux; p0 += pb) {
             const int np = std::min(pb, naux - p0);
+            const long long ldh = (long long)pb * noccp;
             for (int s = 0; s < nb; ++s) {
-                // S3-K1: H^P = B^P C_vir^T  ([np*nocc x nvir] x [nao x nvir]^T), Gamma^P = C_occ H^P
                 const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
-                {
-                    ProfScope ps(c, "ris_gemm_nt(H=B*Cvir^T)", 2.0 * np * nocc * (double)nao * nvir,
+                {   // GEMM-1: HT[nu][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]
+                    RisGemmParams g{};
+                    g.seg[0] = RisGemmSeg{C_vir, nvir, 0, Bs, nvir, 0, nvir};
+                    g.nseg = 1; g.M = nao; g.N = np * nocc; g.C = HT; g.ldc = ldh; g.bsC = 0;
+                    g.cdiv = (noccp != nocc) ? nocc : 0; g.cpad = noccp;
+                    ProfScope ps(c, "ris_gemm_dmma(HT=Cvir*B^T)", 2.0 * np * nocc * (double)nao * nvir,
                                  8.0 * ((double)np * nocc * nvir + (double)nao * nvir + (double)np * nocc * nao));
-                    ris_gemm<true>(c->stream, np * nocc, nao, nvir, Bs, nvir, 0, C_vir, nvir, 0, H, nao, 0, 1);
+                    CU(ris_gemm_launch(c->stream, g, 1, 0));
                 }
-                {
-                    ProfScope ps(c, "ris_gemm_nn(Gamma=Cocc*H)", 2.0 * np * nocc * (double)nao * nao,
-                                 8.0 * np * ((double)nocc * nao + (double)nao * nao) + 8.0 * nao * nocc);
-                    ris_gemm<false>(c->stream, nao, nao, nocc, C_occ, nocc, 0, H, nao, (long long)nocc * nao, G, nao, nao2, np);
+                {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 128x128 blocks
+                    RisGemmParams g{};
+                    g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, ldh, noccp, nocc};
+                    g.seg[1] = RisGemmSeg{HT, ldh, noccp, Cop, noccp, 0, nocc};
+                    g.nseg = 2; g.M = nao; g.N = nao; g.C = S; g.ldc = RIS_GBN; g.bsC = (long long)c->ntiles * blk;
+                    g.tiles = c->d_tiles; g.tile_stride = blk;
+                    ProfScope ps(c, "ris_gemm_dmma(S=Cocc*HT^T+HT*Cocc^T,blocks)", 4.0 * np * nocc * (double)c->ntiles * blk,
+                                 8.0 * np * ((double)noccp * nao + (double)c->ntiles * blk) + 8.0 * nao * noccp);
+                    CU(ris_gemm_launch(c->stream, g, np, c->ntiles));
+                }
+                double* out = tile + (size_t)s * pb * c->nelem_slab;
+                for (int k = 0; k < RIS_NCLASS; ++k) {
+                    const RisClassPack& pk = c->cls[k];
+                    if (pk.npairs == 0) continue;
+                    const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs * np;
+                    ProfScope ps(c, "ris_k_pack_sym", nel, 16.0 * nel);
+                    dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), np);
+                    ris_k_pack_sym<<<grid, 128, 0, c->stream>>>(pk, S, (long long)c->ntiles * blk, c->d_tmap, c->nblk, out, c->nelem_slab);
                 }
                 CU(cudaGetLastError());
-                if ((rc = pack_tiles(c, G, nao2, np, tile + (size_t)s * pb * c->nelem_slab, c->nelem_slab))) return rc;
             }
             if ((rc = launch_classes(c, tile, (long long)pb * c->nelem_slab, c->nelem_slab, nullptr, nb, p0, p0 + np,
                                      grad + (size_t)s0 * c->natoms * 3)))
