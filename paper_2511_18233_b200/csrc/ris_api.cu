@@ -9,6 +9,7 @@
 #include "ris_setup.cuh"
 
 #include <algorithm>
+#include <utility>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -54,7 +55,10 @@ struct ris_ctx {
     std::vector<void*> owned;          // every device allocation of the packed data
     long long nelem_slab = 0, nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[8] = {nullptr};
-    // Gamma^P GEMM-2 block list: 128x128 AO blocks (I >= J) that contain a surviving shell pair
+    // Gamma^P GEMM-2 block list: RIS_GTILE2^2 blocks (I >= J) of the spatially (Morton) ordered AO index that
+    // contain a surviving shell pair
+    int* d_ao_pos = nullptr;           // [nao] spatial position of AO
+    int* d_ao_order = nullptr;         // [nao] AO at spatial position
     int nblk = 0, ntiles = 0;
     int2* d_tiles = nullptr;           // [ntiles] (I, J)
     int* d_tmap = nullptr;             // [nblk][nblk] tile index of (I >= J), -1 if absent
@@ -159,15 +163,27 @@ static const double kModelFlopsByE[8] = {0.0, 140.0, 250.0, 450.0, 750.0, 1250.0
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
 // --------------------------------------------------------------------------------------- setup
-// Marks the 128x128 AO blocks (I >= J) touched by the surviving shell pairs of one class.
-__global__ void ris_k_mark_blocks(RisClassPack pk, int nblk, int* mark)
+// Marks the blocks (I >= J) of the spatially ordered AO index touched by the surviving shell pairs of one class.
+__global__ void ris_k_mark_blocks(RisClassPack pk, const int* __restrict__ ao_pos, int nblk, int* mark)
 {
     const int ip = blockIdx.x * blockDim.x + threadIdx.x;
     if (ip >= pk.npairs) return;
-    const int r0 = pk.ao[ip], q0 = pk.ao[(size_t)pk.npad + ip];
+    const int r0 = ao_pos[pk.ao[ip]], q0 = ao_pos[pk.ao[(size_t)pk.npad + ip]];     // shells stay contiguous
     const int r1 = r0 + ris_ncart(pk.la) - 1, q1 = q0 + ris_ncart(pk.lb) - 1;
-    for (int I = r0 / RIS_GBM; I <= r1 / RIS_GBM; ++I)
-        for (int J = q0 / RIS_GBM; J <= q1 / RIS_GBM; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
+    for (int I = r0 / RIS_GTILE2; I <= r1 / RIS_GTILE2; ++I)
+        for (int J = q0 / RIS_GTILE2; J <= q1 / RIS_GTILE2; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
+}
+
+// Morton (Z-order) code of a point on a 3-bohr grid: the spatial AO order that keeps the surviving pairs of an
+// extended molecule in a narrow band of blocks.
+static unsigned long long morton3(const double* r, const double* lo)
+{
+    unsigned long long code = 0;
+    for (int d = 0; d < 3; ++d) {
+        const unsigned long long q = (unsigned long long)std::max(0.0, std::floor((r[d] - lo[d]) / 3.0));
+        for (int b = 0; b < 20; ++b) code |= ((q >> b) & 1ull) << (3 * b + d);
+    }
+    return code;
 }
 
 extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
@@ -309,14 +325,31 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         }
     c->nelem_slab = off;
     CU(cudaGetLastError());
-    // block list for the pair-restricted Gamma^P GEMM-2
-    c->nblk = (nao + RIS_GBM - 1) / RIS_GBM;
+    // spatial AO order + block list for the pair-restricted Gamma^P GEMM-2
     {
+        double lo[3] = {coords[0], coords[1], coords[2]};
+        for (int a = 0; a < natoms; ++a)
+            for (int d = 0; d < 3; ++d) lo[d] = std::min(lo[d], coords[3 * a + d]);
+        std::vector<std::pair<unsigned long long, int>> key(natoms);
+        for (int a = 0; a < natoms; ++a) key[a] = {morton3(coords + 3 * a, lo), a};
+        std::sort(key.begin(), key.end());
+        std::vector<int> arank(natoms);
+        for (int i = 0; i < natoms; ++i) arank[key[i].second] = i;
+        std::vector<int> sh(nshells);
+        for (int i = 0; i < nshells; ++i) sh[i] = i;
+        std::stable_sort(sh.begin(), sh.end(), [&](int x, int y) { return arank[shell_atom[x]] < arank[shell_atom[y]]; });
+        std::vector<int> ao_pos(nao), ao_order(nao);
+        int pos = 0;
+        for (int i = 0; i < nshells; ++i)
+            for (int k = 0; k < ris_ncart(shell_l[sh[i]]); ++k) { ao_pos[shell_ao[sh[i]] + k] = pos; ao_order[pos] = shell_ao[sh[i]] + k; ++pos; }
+        if ((rc = dev_upload(c, &c->d_ao_pos, ao_pos.data(), ao_pos.size()))) return rc;
+        if ((rc = dev_upload(c, &c->d_ao_order, ao_order.data(), ao_order.size()))) return rc;
+        c->nblk = (nao + RIS_GTILE2 - 1) / RIS_GTILE2;
         int* d_mark;
         if ((rc = dev_alloc(c, &d_mark, (size_t)c->nblk * c->nblk, true))) return rc;
         for (int k = 0; k < RIS_NCLASS; ++k)
             if (c->cls[k].npairs > 0)
-                ris_k_mark_blocks<<<(c->cls[k].npairs + 127) / 128, 128, 0, c->stream>>>(c->cls[k], c->nblk, d_mark);
+                ris_k_mark_blocks<<<(c->cls[k].npairs + 127) / 128, 128, 0, c->stream>>>(c->cls[k], c->d_ao_pos, c->nblk, d_mark);
         CU(cudaGetLastError());
         std::vector<int> mark((size_t)c->nblk * c->nblk);
         CU(cudaMemcpyAsync(mark.data(), d_mark, mark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -447,28 +480,31 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
 }
 
 // --------------------------------------------------------------------------------------- K
-// out[z][elem_off + e*npad + ip] = symf[ip] * S^P[mu0+ca][nu0+cb] read from the 128x128 block buffer of GEMM-2
+// out[z][elem_off + e*npad + ip] = symf[ip] * S^P[pos(mu0+ca)][pos(nu0+cb)] read from the block buffer of GEMM-2
 // (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
-__global__ void ris_k_pack_sym(RisClassPack pk, const double* __restrict__ S, long long sstrideP, const int* __restrict__ tmap,
-                               int nblk, double* __restrict__ out, long long ostride)
+__global__ void ris_k_pack_sym(RisClassPack pk, const double* __restrict__ S, long long sstrideP, const int* __restrict__ ao_pos,
+                               const int* __restrict__ tmap, int nblk, double* __restrict__ out, long long ostride)
 {
+    constexpr int T = RIS_GTILE2;
     const int ip = blockIdx.x * blockDim.x + threadIdx.x;
     if (ip >= pk.npairs) return;
     const int ncb = ris_ncart(pk.lb);
     const int e = blockIdx.y, ca = e / ncb, cb = e - ca * ncb;
-    int r = pk.ao[ip] + ca, q = pk.ao[(size_t)pk.npad + ip] + cb;
-    if ((r >> 7) < (q >> 7)) { const int t = r; r = q; q = t; }
-    const int tile = tmap[(r >> 7) * nblk + (q >> 7)];
-    const double v = S[(size_t)blockIdx.z * sstrideP + (size_t)tile * (RIS_GBM * RIS_GBN) + (r & 127) * RIS_GBN + (q & 127)];
+    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npad + ip]] + cb;
+    if (r / T < q / T) { const int t = r; r = q; q = t; }
+    const int tile = tmap[(r / T) * nblk + (q / T)];
+    const double v = S[(size_t)blockIdx.z * sstrideP + (size_t)tile * (T * T) + (r % T) * T + (q % T)];
     out[(size_t)blockIdx.z * ostride + pk.elem_off + (size_t)e * pk.npad + ip] = (double)pk.symf[ip] * v;
 }
 
-__global__ void ris_k_pad_rows(int rows, int cols, int ld, const double* __restrict__ in, double* __restrict__ out)
+// out[pos][0..ld) = in[order[pos]][0..cols) zero padded: C_occ in spatial row order with an even leading dimension
+__global__ void ris_k_pad_rows(int rows, int cols, int ld, const int* __restrict__ order, const double* __restrict__ in,
+                               double* __restrict__ out)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= (long long)rows * ld) return;
     const int r = (int)(i / ld), cidx = (int)(i - (long long)r * ld);
-    out[i] = cidx < cols ? in[(size_t)r * cols + cidx] : 0.0;
+    out[i] = cidx < cols ? in[(size_t)order[r] * cols + cidx] : 0.0;
 }
 
 extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
@@ -480,8 +516,8 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
     const int nao = c->nao, naux = c->naux;
     const int nbmax = std::min(nbatch, RIS_NB_MAX);
     const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
-    const long long blk = (long long)RIS_GBM * RIS_GBN;
-    // per aux function: HT [nao][noccp], S blocks [ntiles][128*128], packed tiles [nb][slab]
+    const long long blk = (long long)RIS_GTILE2 * RIS_GTILE2;
+    // per aux function: HT [nao][noccp], S blocks [ntiles][64*64], packed tiles [nb][slab]
     int pb = c->opt.p_batch;
     if (pb <= 0) {
         size_t fr = 0, tot = 0;
@@ -502,7 +538,7 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
     {
         ProfScope ps(c, "ris_k_pad_rows", 0.0, 16.0 * nao * (double)noccp);
         const long long n = (long long)nao * noccp;
-        ris_k_pad_rows<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(nao, nocc, noccp, C_occ, Cop);
+        ris_k_pad_rows<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(nao, nocc, noccp, c->d_ao_order, C_occ, Cop);
     }
     for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
         const int nb = std::min(RIS_NB_MAX, nbatch - s0);
@@ -515,20 +551,22 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                     RisGemmParams g{};
                     g.seg[0] = RisGemmSeg{C_vir, nvir, 0, Bs, nvir, 0, nvir};
                     g.nseg = 1; g.M = nao; g.N = np * nocc; g.C = HT; g.ldc = ldh; g.bsC = 0;
+                    g.rowsA = c->d_ao_order;                  // HT rows in spatial order
                     g.cdiv = (noccp != nocc) ? nocc : 0; g.cpad = noccp;
                     ProfScope ps(c, "ris_gemm_dmma(HT=Cvir*B^T)", 2.0 * np * nocc * (double)nao * nvir,
                                  8.0 * ((double)np * nocc * nvir + (double)nao * nvir + (double)np * nocc * nao));
-                    CU(ris_gemm_launch(c->stream, g, 1, 0));
+                    CU(ris_gemm_dense(c->stream, g, 1));
                 }
                 {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 128x128 blocks
                     RisGemmParams g{};
                     g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, ldh, noccp, nocc};
                     g.seg[1] = RisGemmSeg{HT, ldh, noccp, Cop, noccp, 0, nocc};
-                    g.nseg = 2; g.M = nao; g.N = nao; g.C = S; g.ldc = RIS_GBN; g.bsC = (long long)c->ntiles * blk;
+                    g.nseg = 2; g.M = nao; g.N = nao; g.C = S; g.ldc = RIS_GTILE2; g.bsC = (long long)c->ntiles * blk;
                     g.tiles = c->d_tiles; g.tile_stride = blk;
-                    ProfScope ps(c, "ris_gemm_dmma(S=Cocc*HT^T+HT*Cocc^T,blocks)", 4.0 * np * nocc * (double)c->ntiles * blk,
+                    // algorithmic flops: two length-nocc dot products per unique surviving pair element
+                    ProfScope ps(c, "ris_gemm_dmma(S=Cocc*HT^T+HT*Cocc^T,blocks)", 4.0 * np * nocc * (double)c->nelem_real,
                                  8.0 * np * ((double)noccp * nao + (double)c->ntiles * blk) + 8.0 * nao * noccp);
-                    CU(ris_gemm_launch(c->stream, g, np, c->ntiles));
+                    CU(ris_gemm_blocks(c->stream, g, np, c->ntiles));
                 }
                 double* out = tile + (size_t)s * pb * c->nelem_slab;
                 for (int k = 0; k < RIS_NCLASS; ++k) {
@@ -537,7 +575,7 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                     const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs * np;
                     ProfScope ps(c, "ris_k_pack_sym", nel, 16.0 * nel);
                     dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), np);
-                    ris_k_pack_sym<<<grid, 128, 0, c->stream>>>(pk, S, (long long)c->ntiles * blk, c->d_tmap, c->nblk, out, c->nelem_slab);
+                    ris_k_pack_sym<<<grid, 128, 0, c->stream>>>(pk, S, (long long)c->ntiles * blk, c->d_ao_pos, c->d_tmap, c->nblk, out, c->nelem_slab);
                 }
                 CU(cudaGetLastError());
             }
