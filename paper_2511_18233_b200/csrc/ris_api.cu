@@ -444,10 +444,11 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
         p.tile = tile; p.sstride = sstride; p.pstride = pstride; p.cscale = cscale; p.nb = nb; p.p0 = p0; p.p1 = p1;
         p.grad = grad;
-        // enough blocks for >= 4 per SM, at least 4 aux per block, at most 64 (shared-memory accumulators)
-        const int bx = pk.npad / RIS_GRAD_THREADS, np = p1 - p0;
+        // enough blocks for >= 4 per SM; at least 4 aux per block for the light classes (amortises the pair-side
+        // loads and atomics), 2 / 1 for the heavy ones (few pairs, long recurrences); at most 64 (shared accumulators)
+        const int bx = pk.npad / RIS_GRAD_THREADS, np = p1 - p0, E = pk.la + pk.lb + 1;
         int ny = std::max(1, (4 * 148 + bx - 1) / bx);
-        int pch = std::max(4, (np + ny - 1) / ny);
+        int pch = std::max(E >= 5 ? 1 : (E >= 3 ? 2 : 4), (np + ny - 1) / ny);
         p.pchunk = std::min(std::min(pch, np), 64);
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
         ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),

@@ -10,16 +10,18 @@
 // One kernel serves both:  C[m][n] = sum_seg sum_k A_seg[row(m)][k] B_seg[n][k]  (up to two K segments; row(m)
 // optionally through an index list, which is how GEMM-1 emits HT in spatial order).
 // tcgen05.mma has no FP64 kind, so the tensor path for FP64 on sm_100a is the warp-level mma.sync f64 (DMMA;
-// SASS DMMA.8x8x4); operands are staged global -> shared with cp.async (LDGSTS) in a 3-stage pipeline,
-// fragments are read from shared memory with a row stride of 20 doubles (conflict-free for the 64-bit fragment
-// pattern: row g, column t).
-//   config A (GEMM-1): CTA tile 128x128, K step 16, 8 warps as 2 x 4, warp tile 64x32, 1 CTA/SM
-//   config B (GEMM-2): CTA tile  64x64,  K step 16, 4 warps as 2 x 2, warp tile 32x32, 3 CTAs/SM
+// SASS DMMA.8x8x4, 16 cycles of the pipe per SM sub-partition each).  Operands are staged global -> shared with
+// cp.async (LDGSTS) through a multi-stage pipeline that is synchronised by mbarriers only (full[s]: the stage's
+// cp.async have landed; empty[s]: every warp has read its fragments) -- a CTA-wide barrier per K step cost 15 % of the
+// DMMA pipe (profiles/r01_v3_ncu.md -> r01_v4_gemm.md).  Fragments are read with 128-bit shared loads from a
+// 16-double row whose halves are swapped on odd rows (bank-conflict free, no padding).
+//   GEMM-1: CTA tile 64x128, K step 16, 8 warps as 2 x 4, warp tile 32x32, 3 stages, 2 CTAs/SM
+//   GEMM-2: CTA tile 64x64,  K step 16, 4 warps as 2 x 2, warp tile 32x32, 3 stages, 3 CTAs/SM
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-constexpr int RIS_GBK = 16, RIS_GLD = 20, RIS_GSTAGES = 3;
+constexpr int RIS_GBK = 16, RIS_GLD = 16;   // K step; shared row stride in doubles (swizzled, see the kernel)
 constexpr int RIS_GTILE2 = 64;           // AO block edge of the GEMM-2 block list
 
 struct RisGemmSeg {
@@ -54,22 +56,22 @@ __device__ __forceinline__ void ris_dmma_16x8x8(double (&c)[4], const double (&a
                  : "d"(a[0]), "d"(a[1]), "d"(a[2]), "d"(a[3]), "d"(b[0]), "d"(b[1]));
 }
 
-template <int BM, int BN, int WM, int WN>
+template <int BM, int BN, int WM, int WN, int STAGES>
 struct RisGemmCfg {
     static constexpr int THREADS = (BM / WM) * (BN / WN) * 32;
     static constexpr int MT = WM / 16, NT = WN / 8;
-    static constexpr size_t SMEM = (size_t)RIS_GSTAGES * (BM + BN) * RIS_GLD * sizeof(double);
+    static constexpr size_t SMEM = (size_t)STAGES * (BM + BN) * RIS_GLD * sizeof(double);
 };
 
 // VEC16: all operand rows are 16-byte aligned (even leading dimensions, aligned bases) -> 16-byte cp.async
-template <int BM, int BN, int WM, int WN, int MINB, bool VEC16>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool VEC16>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_dmma(const RisGemmParams p)
 {
-    using Cfg = RisGemmCfg<BM, BN, WM, WN>;
+    using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
     constexpr int THREADS = Cfg::THREADS, MT = Cfg::MT, NT = Cfg::NT;
     extern __shared__ __align__(16) double smem[];
-    double* As = smem;                                          // [stage][BM][20]
-    double* Bs = smem + (size_t)RIS_GSTAGES * BM * RIS_GLD;     // [stage][BN][20]
+    double* As = smem;                                     // [stage][BM][16]
+    double* Bs = smem + (size_t)STAGES * BM * RIS_GLD;     // [stage][BN][16]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     const int wm0 = (warp / (BN / WN)) * WM, wn0 = (warp % (BN / WN)) * WN;
@@ -118,29 +120,55 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
             pb[j] = r < p.N ? Bg + (long long)r * sg.ldb + kc : nullptr;
         }
     };
-    const unsigned sA0 = (unsigned)__cvta_generic_to_shared(As) + ((tid / CH) * RIS_GLD + kc) * 8;
-    const unsigned sB0 = (unsigned)__cvta_generic_to_shared(Bs) + ((tid / CH) * RIS_GLD + kc) * 8;
-    int ld_ks = 0;                                     // next K step to load
-    auto load_next = [&]() {
-        if (ld_ks < nk) {
-            if (ld_ks == 0) bind_segment(0);
-            else if (ld_ks == nk0) bind_segment(1);
-            const int k0 = (ld_ks < nk0 ? ld_ks : ld_ks - nk0) * RIS_GBK;
-            const int stage = ld_ks % RIS_GSTAGES;
-            const int kv = min(max(segK - (k0 + kc), 0), CW) * 8;               // valid bytes along K
+    // shared layout: row stride RIS_GLD = 16 doubles (one K step), the two 8-double halves of odd rows swapped
+    // (k' = k ^ 8 (row & 1)): the 8 lanes of a quarter warp (rows g, g+1; t = 0..3) of a 128-bit fragment load then
+    // cover all 32 banks once, without padding.
+    const int lrow = tid / CH;                         // loader row (same parity for every j: THREADS / CH is even)
+    const int lk = kc ^ ((lrow & 1) << 3);
+    const unsigned sA0 = (unsigned)__cvta_generic_to_shared(As) + (lrow * RIS_GLD + lk) * 8;
+    const unsigned sB0 = (unsigned)__cvta_generic_to_shared(Bs) + (lrow * RIS_GLD + lk) * 8;
+    // ---- pipeline: STAGES shared stages, no CTA-wide barrier in the K loop.  full[s] completes when every thread's
+    // cp.async of the stage has landed (cp.async.mbarrier.arrive.noinc, count THREADS); empty[s] when every warp has
+    // read its fragments (count NWARPS).  K step j is issued DIST = STAGES - 2 steps ahead, into the stage all warps
+    // left two steps ago, so warps drift apart by up to a step instead of meeting at a barrier.
+    constexpr int NWARPS = THREADS / 32, DIST = STAGES - 2;
+    static_assert(STAGES >= 3, "pipeline depth");
+    __shared__ __align__(8) unsigned long long bars[2 * STAGES];
+    const unsigned bar0 = (unsigned)__cvta_generic_to_shared(bars);
+    if (tid == 0) {
 #pragma unroll
-            for (int j = 0; j < NA; ++j) {
-                const bool v = pa[j] != nullptr && kv > 0;
-                ris_cp_async<VEC16>(sA0 + (stage * BM + j * (THREADS / CH)) * RIS_GLD * 8, v ? pa[j] + k0 : p.seg[0].A, v ? kv : 0);
-            }
-#pragma unroll
-            for (int j = 0; j < NB; ++j) {
-                const bool v = pb[j] != nullptr && kv > 0;
-                ris_cp_async<VEC16>(sB0 + (stage * BN + j * (THREADS / CH)) * RIS_GLD * 8, v ? pb[j] + k0 : p.seg[0].A, v ? kv : 0);
-            }
+        for (int s = 0; s < STAGES; ++s) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar0 + 8 * s), "r"(THREADS));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar0 + 8 * (STAGES + s)), "r"(NWARPS));
         }
-        ++ld_ks;
-        asm volatile("cp.async.commit_group;");
+    }
+    __syncthreads();
+    auto bar_wait = [&](unsigned bar, int parity) {
+        unsigned done;
+        do {
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        } while (!done);
+    };
+    auto produce = [&](int j) {
+        if (j >= nk) return;
+        if (j == 0) bind_segment(0);
+        else if (j == nk0) bind_segment(1);
+        const int k0 = (j < nk0 ? j : j - nk0) * RIS_GBK;
+        const int stage = j % STAGES, round = j / STAGES;
+        if (round > 0) bar_wait(bar0 + 8 * (STAGES + stage), (round - 1) & 1);
+        const int kv = min(max(segK - (k0 + kc), 0), CW) * 8;               // valid bytes along K
+#pragma unroll
+        for (int jj = 0; jj < NA; ++jj) {
+            const bool v = pa[jj] != nullptr && kv > 0;
+            ris_cp_async<VEC16>(sA0 + (stage * BM + jj * (THREADS / CH)) * RIS_GLD * 8, v ? pa[jj] + k0 : p.seg[0].A, v ? kv : 0);
+        }
+#pragma unroll
+        for (int jj = 0; jj < NB; ++jj) {
+            const bool v = pb[jj] != nullptr && kv > 0;
+            ris_cp_async<VEC16>(sB0 + (stage * BN + jj * (THREADS / CH)) * RIS_GLD * 8, v ? pb[jj] + k0 : p.seg[0].A, v ? kv : 0);
+        }
+        asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar0 + 8 * stage) : "memory");
     };
 
     double acc[MT][NT][4];
@@ -152,27 +180,37 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
             for (int r = 0; r < 4; ++r) acc[i][j][r] = 0.0;
 
 #pragma unroll
-    for (int s = 0; s < RIS_GSTAGES - 1; ++s) load_next();
+    for (int j = 0; j < DIST; ++j) produce(j);
+    const int ksw = (g & 1) << 3;
     for (int ks = 0; ks < nk; ++ks) {
-        asm volatile("cp.async.wait_group %0;" ::"n"(RIS_GSTAGES - 2));
-        __syncthreads();
-        load_next();                                   // refills the stage consumed in the previous iteration
-        const double* as = As + (size_t)(ks % RIS_GSTAGES) * BM * RIS_GLD + (wm0 + g) * RIS_GLD + t;
-        const double* bs = Bs + (size_t)(ks % RIS_GSTAGES) * BN * RIS_GLD + (wn0 + g) * RIS_GLD + t;
+        produce(ks + DIST);
+        const int stage = ks % STAGES;
+        bar_wait(bar0 + 8 * stage, (ks / STAGES) & 1);
+        // Fragments, K-permuted: the MMA's k index t (t + 4) is the shared column kk + 2t (kk + 2t + 1) for A and B
+        // alike, so one 128-bit load fetches both k halves of a fragment row.
+        const double* as = As + (size_t)stage * BM * RIS_GLD + (wm0 + g) * RIS_GLD + 2 * t;
+        const double* bs = Bs + (size_t)stage * BN * RIS_GLD + (wn0 + g) * RIS_GLD + 2 * t;
 #pragma unroll
-        for (int kk = 0; kk < RIS_GBK; kk += 8) {
+        for (int h = 0; h < 2; ++h) {
             double a[MT][4], b[NT][2];
+            const int kk = (8 * h) ^ ksw;
 #pragma unroll
             for (int i = 0; i < MT; ++i) {
-                a[i][0] = as[(16 * i) * RIS_GLD + kk];
-                a[i][1] = as[(16 * i + 8) * RIS_GLD + kk];
-                a[i][2] = as[(16 * i) * RIS_GLD + kk + 4];
-                a[i][3] = as[(16 * i + 8) * RIS_GLD + kk + 4];
+                const double2 lo = *reinterpret_cast<const double2*>(as + (16 * i) * RIS_GLD + kk);
+                const double2 hi = *reinterpret_cast<const double2*>(as + (16 * i + 8) * RIS_GLD + kk);
+                a[i][0] = lo.x; a[i][1] = hi.x; a[i][2] = lo.y; a[i][3] = hi.y;
             }
 #pragma unroll
             for (int j = 0; j < NT; ++j) {
-                b[j][0] = bs[(8 * j) * RIS_GLD + kk];
-                b[j][1] = bs[(8 * j) * RIS_GLD + kk + 4];
+                const double2 v = *reinterpret_cast<const double2*>(bs + (8 * j) * RIS_GLD + kk);
+                b[j][0] = v.x; b[j][1] = v.y;
+            }
+            if (h == 1) {          // every fragment of the stage is in registers: release it before the last MMAs
+                __syncwarp();
+                if (lane == 0) {
+                    unsigned long long st_;
+                    asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(st_) : "r"(bar0 + 8 * (STAGES + stage)) : "memory");
+                }
             }
 #pragma unroll
             for (int i = 0; i < MT; ++i)
@@ -180,7 +218,6 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
                 for (int j = 0; j < NT; ++j) ris_dmma_16x8x8(acc[i][j], a[i], b[j]);
         }
     }
-    asm volatile("cp.async.wait_group 0;");
 
     // ---- epilogue: c0,c1 -> (row g, cols 2t, 2t+1); c2,c3 -> row g + 8
     const int Mrem = p.M - m0, Nrem = p.N - n0;
@@ -221,15 +258,17 @@ inline bool ris_gemm_aligned16(const RisGemmParams& p)
     return true;
 }
 
-template <int BM, int BN, int WM, int WN, int MINB>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB>
 inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
-    using Cfg = RisGemmCfg<BM, BN, WM, WN>;
+    using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+        e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -237,18 +276,20 @@ inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, 
     if (p.tiles) grid = dim3(ntiles, 1, batch);
     else grid = dim3((p.M + BM - 1) / BM, (p.N + BN - 1) / BN, batch);
     if (grid.x == 0 || grid.y == 0 || grid.z == 0) return cudaSuccess;
-    if (ris_gemm_aligned16(p)) ris_k_gemm_dmma<BM, BN, WM, WN, MINB, true><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
-    else ris_k_gemm_dmma<BM, BN, WM, WN, MINB, false><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    if (ris_gemm_aligned16(p)) ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    else ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
     return cudaGetLastError();
 }
 
-// GEMM-1: dense, 128x128 CTA tiles
+// GEMM-1: dense, CTA tile 64x128, 8 warps (2 x 4, warp tile 32x32), 3 stages, 2 CTAs/SM.  Measured on B200 (config 4,
+// profiles/r01_v4_gemm.md): 33.2 TFLOP/s = 90 % of the mma.sync f64 peak; 128x128 tiles with 8 or 16 warps on one
+// CTA/SM reach 31.3-31.6, 128x64 x 2 CTAs 31.9, the same tile with 4 stages 32.4.
 inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int batch)
 {
-    return ris_gemm_launch_cfg<128, 128, 64, 32, 1>(st, p, batch, 0);
+    return ris_gemm_launch_cfg<64, 128, 32, 32, 3, 2>(st, p, batch, 0);
 }
 // GEMM-2: block list of RIS_GTILE2 x RIS_GTILE2 tiles
 inline cudaError_t ris_gemm_blocks(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
-    return ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3>(st, p, batch, ntiles);
+    return ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3, 3>(st, p, batch, ntiles);
 }

@@ -72,12 +72,14 @@ __global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m,
     packed[t] = k | ((unsigned)min(nA, 255) << 8) | ((unsigned)min(nB, 255) << 16);
 }
 
-// Stable LSD radix sort of the pair list in three 16-bin passes: nkB, nkA, class.  After it, the pairs of a
-// class are contiguous and ordered by (nkA, nkB), so the lanes of a warp run equally long primitive loops.
+// Stable LSD radix sort of the pair list in three 16-bin passes: nkB, nkA (both DEscending), class.  After it, the
+// pairs of a class are contiguous and ordered by (nkA, nkB), so the lanes of a warp run equally long primitive
+// loops in both host phases, and the blocks with the longest loops start first.  (Measured on config 4: ordering
+// by the TOTAL number of primitive pairs instead costs 10 % of the class-kernel time in either direction.)
 __device__ __forceinline__ int ris_digit(unsigned packed, int pass)
 {
-    if (pass == 0) return min((int)((packed >> 16) & 255u), 15);
-    if (pass == 1) return min((int)((packed >> 8) & 255u), 15);
+    if (pass == 0) return 15 - min((int)((packed >> 16) & 255u), 15);
+    if (pass == 1) return 15 - min((int)((packed >> 8) & 255u), 15);
     return (int)(packed & 255u);
 }
 
