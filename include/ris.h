@@ -68,7 +68,12 @@ typedef struct ris_options {
                              random-sign accumulation over naux x pairs folded into the threshold);
                              a shell pair is dropped when all its primitive pairs are.  There is no screening on
                              the aux index (the Coulomb tail is 1/R). */
-    int deterministic;    /* nonzero: bitwise run-to-run reproducible reduction (slower) */
+    int deterministic;    /* nonzero: bitwise run-to-run reproducible results.  Every in-block sum already has a fixed
+                             order; the cross-block sums then use 64-bit INTEGER atomics on a fixed-point split of
+                             each contribution (value = hi 2^-28 + lo 2^-60; resolution 8.7e-19, contributions
+                             |x| < 2^34, sums < 2^35 Hartree/bohr) instead of FP64 atomics.  A contribution outside
+                             that range turns the whole output into NaN.  Default 0: FP64 atomics, run-to-run
+                             differences at the 1e-16 relative level of the summation order. */
     int p_batch;          /* aux functions per Gamma^P batch in ris_grad_K; 0 = choose from free memory */
     int profile;          /* nonzero: record CUDA events around every kernel (see ris_profile_*) */
 } ris_options;

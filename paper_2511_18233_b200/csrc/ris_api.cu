@@ -63,14 +63,14 @@ struct ris_ctx {
     int2* d_tiles = nullptr;           // [ntiles] (I, J)
     int* d_tmap = nullptr;             // [nblk][nblk] tile index of (I >= J), -1 if absent
     // grow-only scratch
-    void* ws[8] = {nullptr};
-    size_t ws_bytes[8] = {0};
+    void* ws[10] = {nullptr};
+    size_t ws_bytes[10] = {0};
     int last_pbatch = 0;
     std::vector<ProfRec> prof;
     std::vector<cudaEvent_t> ev_pool;
 };
 
-enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7 };
+enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_N = 10 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -376,7 +376,7 @@ extern "C" int ris_destroy(ris_ctx* c)
     if (!c) return RIS_EINVAL;
     cudaStreamSynchronize(c->stream);
     for (void* p : c->owned) cudaFree(p);
-    for (int i = 0; i < 8; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
+    for (int i = 0; i < WS_N; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
     ris_profile_reset(c);
     delete c;
     return RIS_OK;
@@ -434,7 +434,7 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
 constexpr int RIS_NB_MAX = 8;      // states per class-kernel launch (shared-memory slots)
 
 static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long pstride, const double* cscale,
-                          int nb, int p0, int p1, double* grad)
+                          int nb, int p0, int p1, double* grad, unsigned long long* det)
 {
     for (int oi = 0; oi < RIS_NCLASS; ++oi) {
         const int k = kClassOrder[oi];
@@ -443,19 +443,54 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         RisGradParams p{};
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
         p.tile = tile; p.sstride = sstride; p.pstride = pstride; p.cscale = cscale; p.nb = nb; p.p0 = p0; p.p1 = p1;
-        p.grad = grad;
+        p.grad = grad; p.det = det; p.det_flag = det ? (int*)c->ws[WS_DET] : nullptr;
         // enough blocks for >= 4 per SM; at least 4 aux per block for the light classes (amortises the pair-side
         // loads and atomics), 2 / 1 for the heavy ones (few pairs, long recurrences); at most 64 (shared accumulators)
         const int bx = pk.npad / RIS_GRAD_THREADS, np = p1 - p0, E = pk.la + pk.lb + 1;
         int ny = std::max(1, (4 * 148 + bx - 1) / bx);
         int pch = std::max(E >= 5 ? 1 : (E >= 3 ? 2 : 4), (np + ny - 1) / ny);
-        p.pchunk = std::min(std::min(pch, np), 64);
+        p.pchunk = std::min(std::min(pch, np), std::max(8, std::min(64, 192 / nb)));
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
         ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
                      8.0 * (np_ * (pstride ? 1.0 : 0.0) + (pstride ? 0.0 : 1.0)) * nel * pk.npairs * nb +
                          8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
         ris_grad_launchers[k](p, c->stream);
     }
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- deterministic reduction
+// grad[i] = hi[i] 2^-28 + lo[i] 2^-60 (ris_internal.h: ris_grad_add); NaN everywhere when a contribution left the range.
+__global__ void ris_k_det_finish(long long n, const unsigned long long* __restrict__ acc, const int* __restrict__ flag,
+                                 double* __restrict__ grad)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = (double)(long long)acc[2 * i] * (1.0 / 268435456.0) + (double)(long long)acc[2 * i + 1] * (1.0 / 1152921504606846976.0);
+    grad[i] = *flag ? nan("") : v;
+}
+
+// Layout of WS_DET: int flag (16 bytes reserved), then [nbatch][natoms][3][2] accumulators.
+static int det_begin(ris_ctx* c, int nbatch, unsigned long long** acc)
+{
+    *acc = nullptr;
+    if (!c->opt.deterministic) return RIS_OK;
+    void* w;
+    const size_t bytes = 16 + sizeof(unsigned long long) * 2 * (size_t)nbatch * c->natoms * 3;
+    int rc = ws_get(c, WS_DET, bytes, &w);
+    if (rc) return rc;
+    CU(cudaMemsetAsync(w, 0, bytes, c->stream));
+    *acc = (unsigned long long*)((char*)w + 16);
+    return RIS_OK;
+}
+
+static int det_end(ris_ctx* c, int nbatch, const unsigned long long* acc, double* grad)
+{
+    if (!acc) return RIS_OK;
+    const long long n = (long long)nbatch * c->natoms * 3;
+    ProfScope ps(c, "ris_k_det_finish", 2.0 * n, 24.0 * n);
+    ris_k_det_finish<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, acc, (const int*)c->ws[WS_DET], grad);
     CU(cudaGetLastError());
     return RIS_OK;
 }
@@ -467,6 +502,8 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     const long long nao2 = (long long)c->nao * c->nao;
+    unsigned long long* det;
+    { int rc = det_begin(c, nbatch, &det); if (rc) return rc; }
     for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
         const int nb = std::min(RIS_NB_MAX, nbatch - s0);
         double* tile;
@@ -474,10 +511,10 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
         if (rc) return rc;
         if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_slab))) return rc;
         if ((rc = launch_classes(c, tile, c->nelem_slab, 0, c_aux + (size_t)s0 * c->naux, nb, 0, c->naux,
-                                 grad + (size_t)s0 * c->natoms * 3)))
+                                 grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
             return rc;
     }
-    return RIS_OK;
+    return det_end(c, nbatch, det, grad);
 }
 
 // --------------------------------------------------------------------------------------- K
@@ -532,6 +569,8 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
     c->last_pbatch = pb;
     double *tile, *HT, *S, *Cop;
     int rc;
+    unsigned long long* det;
+    if ((rc = det_begin(c, nbatch, &det))) return rc;
     if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pb * c->nelem_slab, (void**)&tile))) return rc;
     if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)nao * pb * noccp, (void**)&HT))) return rc;
     if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * c->ntiles * blk, (void**)&S))) return rc;
@@ -581,11 +620,11 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                 CU(cudaGetLastError());
             }
             if ((rc = launch_classes(c, tile, (long long)pb * c->nelem_slab, c->nelem_slab, nullptr, nb, p0, p0 + np,
-                                     grad + (size_t)s0 * c->natoms * 3)))
+                                     grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
                 return rc;
         }
     }
-    return RIS_OK;
+    return det_end(c, nbatch, det, grad);
 }
 
 // --------------------------------------------------------------------------------------- PQ (S5)

@@ -8,7 +8,10 @@
 //   pair-side gradients g[A_mu], g[A_nu]: per-thread shared-memory slots across the whole P loop,
 //       one global atomic per (thread, state, component) at the end;
 //   aux-side gradient g[A_P] = -(g_mu + g_nu) (translational invariance): warp-shuffle reduction per
-//       (P, state), one shared-memory atomic per warp, one global atomic per (block, P, state, x).
+//       (P, state) into a per-warp shared-memory slot (no shared atomics), the warps' slots summed in fixed order
+//       at the end, one global atomic per (block, P, state, x).
+// Every in-block sum has a fixed order; the global atomics are FP64 adds, or -- deterministic mode -- 64-bit integer
+// adds of a fixed-point split (ris_grad_add), which makes the result bitwise reproducible.
 #pragma once
 #include "ris_core.cuh"
 #include "ris_internal.h"
@@ -51,11 +54,12 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
     const int pc0 = prm.p0 + blockIdx.y * prm.pchunk;
     const int npc = min(pc0 + prm.pchunk, prm.p1) - pc0;
     double* s_aux = sm;                              // [pchunk][5]
-    double* s_gaux = s_aux + 5 * prm.pchunk;         // [pchunk][nb][3]
-    double* s_slot = s_gaux + 3 * nb * prm.pchunk;   // [nb][6][NT]  pair-side accumulators (A: 0..2, B: 3..5)
+    constexpr int NW = NT / 32;
+    double* s_gaux = s_aux + 5 * prm.pchunk;         // [NW][pchunk][nb][3]   per-warp aux-side accumulators
+    double* s_slot = s_gaux + 3 * nb * prm.pchunk * NW;   // [nb][6][NT]  pair-side accumulators (A: 0..2, B: 3..5)
     double* s_stash = s_slot + 6 * nb * NT;          // [nb][3][NT]  dA+dB of the current contracted triplet
     for (int i = tid; i < 5 * npc; i += NT) s_aux[i] = prm.aux[5 * (size_t)pc0 + i];
-    for (int i = tid; i < 3 * nb * npc; i += NT) s_gaux[i] = 0.0;
+    for (int i = tid; i < 3 * nb * prm.pchunk * NW; i += NT) s_gaux[i] = 0.0;
     for (int i = 0; i < 6 * nb; ++i) s_slot[i * NT + tid] = 0.0;
     __syncthreads();
 
@@ -106,8 +110,8 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
             const double* st = s_stash + (size_t)s * 3 * NT + tid;
             const double t0 = ris_warp_sum(st[0 * NT]), t1 = ris_warp_sum(st[1 * NT]), t2 = ris_warp_sum(st[2 * NT]);
             if ((tid & 31) == 0) {
-                double* g = s_gaux + ((size_t)pl * nb + s) * 3;
-                atomicAdd(g + 0, -t0); atomicAdd(g + 1, -t1); atomicAdd(g + 2, -t2);
+                double* g = s_gaux + (((size_t)(tid >> 5) * prm.pchunk + pl) * nb + s) * 3;
+                g[0] -= t0; g[1] -= t1; g[2] -= t2;
             }
         }
     }
@@ -116,21 +120,22 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
         const int atA = pk.atoms[ip], atB = pk.atoms[(size_t)npad + ip];
         for (int s = 0; s < nb; ++s) {
             const double* sl = s_slot + (size_t)s * 6 * NT + tid;
-            double* gA = prm.grad + ((size_t)s * prm.natoms + atA) * 3;
-            double* gB = prm.grad + ((size_t)s * prm.natoms + atB) * 3;
-            atomicAdd(gA + 0, sl[0 * NT]); atomicAdd(gA + 1, sl[1 * NT]); atomicAdd(gA + 2, sl[2 * NT]);
-            atomicAdd(gB + 0, sl[3 * NT]); atomicAdd(gB + 1, sl[4 * NT]); atomicAdd(gB + 2, sl[5 * NT]);
+            const size_t iA = ((size_t)s * prm.natoms + atA) * 3, iB = ((size_t)s * prm.natoms + atB) * 3;
+            ris_grad_add(prm, iA + 0, sl[0 * NT]); ris_grad_add(prm, iA + 1, sl[1 * NT]); ris_grad_add(prm, iA + 2, sl[2 * NT]);
+            ris_grad_add(prm, iB + 0, sl[3 * NT]); ris_grad_add(prm, iB + 1, sl[4 * NT]); ris_grad_add(prm, iB + 2, sl[5 * NT]);
         }
     }
     for (int i = tid; i < 3 * nb * npc; i += NT) {
         const int pl = i / (3 * nb), r = i - pl * 3 * nb, s = r / 3, x = r - 3 * s;
-        atomicAdd(prm.grad + ((size_t)s * prm.natoms + (pc0 + pl)) * 3 + x, s_gaux[i]);
+        double v = 0.0;
+        for (int w = 0; w < NW; ++w) v += s_gaux[(size_t)w * 3 * nb * prm.pchunk + i];
+        ris_grad_add(prm, ((size_t)s * prm.natoms + (pc0 + pl)) * 3 + x, v);
     }
 }
 
 inline size_t ris_grad_smem_bytes(const RisGradParams& p)
 {
-    return sizeof(double) * ((size_t)5 * p.pchunk + (size_t)3 * p.nb * p.pchunk + (size_t)9 * p.nb * RIS_GRAD_THREADS);
+    return sizeof(double) * ((size_t)5 * p.pchunk + (size_t)3 * p.nb * p.pchunk * (RIS_GRAD_THREADS / 32) + (size_t)9 * p.nb * RIS_GRAD_THREADS);
 }
 
 template <int LA, int LB>

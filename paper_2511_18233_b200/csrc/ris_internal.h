@@ -42,7 +42,24 @@ struct RisGradParams {
     int p0, p1;              // aux range of this launch
     int pchunk;              // aux functions per blockIdx.y
     double* grad;            // [nb][natoms][3], accumulated with atomics
+    unsigned long long* det; // deterministic mode: [nb][natoms][3][2] fixed-point accumulators (hi, lo), else nullptr
+    int* det_flag;           // set to 1 when a contribution leaves the fixed-point range
 };
+
+// Deterministic reduction (ris_options.deterministic): a contribution x is added as the integer pair
+//   hi = floor(x 2^28),  lo = floor((x 2^28 - hi) 2^32)        value = hi 2^-28 + lo 2^-60
+// with two 64-bit INTEGER atomics; integer addition is associative, so the result does not depend on the order in
+// which blocks arrive (resolution 2^-60 ~ 8.7e-19 per contribution, range |x| < 2^34, |sum| < 2^35).
+__device__ __forceinline__ void ris_grad_add(const RisGradParams& prm, size_t idx, double x)
+{
+    if (prm.det == nullptr) { atomicAdd(prm.grad + idx, x); return; }
+    if (!(fabs(x) < 17179869184.0)) { *prm.det_flag = 1; return; }
+    const double y = x * 268435456.0;
+    const long long hi = __double2ll_rd(y);
+    const long long lo = __double2ll_rd((y - (double)hi) * 4294967296.0);
+    atomicAdd(prm.det + 2 * idx, (unsigned long long)hi);
+    atomicAdd(prm.det + 2 * idx + 1, (unsigned long long)lo);
+}
 
 typedef void (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
 extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];

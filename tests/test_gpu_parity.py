@@ -183,3 +183,34 @@ def test_full_size_sampled_atoms(cfg, atoms):
     assert_parity(gQ, orc.grad_PQ(wl.mol, wl.c_aux, wl.d_aux)[0], f"config {cfg} PQ")
     for g in (gJ, gK, gQ):      # property that holds at any size: each term is translationally invariant
         assert np.all(np.abs(g.sum(axis=1)) < 1e-10 * np.abs(g).sum())
+
+
+def test_deterministic_mode_is_bitwise_reproducible_and_at_parity():
+    """ris_options.deterministic (S4): fixed-order sums inside a block, 64-bit integer atomics of a
+    fixed-point split across blocks -> two runs agree bit for bit, and the result still matches the oracle."""
+    wl = synth.make_workload(2)
+    runs = []
+    for _ in range(2):
+        ctx, gJ, gK, gQ = run_all(wl, deterministic=True)
+        ctx.close()
+        runs.append((gJ, gK, gQ))
+    for a, b in zip(*runs):
+        assert np.array_equal(a.view(np.uint64), b.view(np.uint64))
+    assert_parity(runs[0][0], orc.grad_J(wl.mol, wl.D, wl.c_aux)[0], "deterministic J")
+    assert_parity(runs[0][1], orc.grad_K(wl.mol, wl.C_occ, wl.C_vir, wl.B)[0], "deterministic K")
+    # the default mode (FP64 atomics) agrees with it to summation-order noise
+    ctx, gJ, gK, gQ = run_all(wl)
+    ctx.close()
+    assert np.abs(gJ - runs[0][0]).max() <= 1e-13 * np.abs(gJ).max()
+    assert np.abs(gK - runs[0][1]).max() <= 1e-13 * np.abs(gK).max()
+
+
+def test_deterministic_mode_flags_out_of_range_contributions():
+    """A contribution beyond the fixed-point range (|x| >= 2^34) must not be silently wrapped: the output is NaN."""
+    wl = synth.make_workload(1)
+    ctx = ris_setup(wl.mol, deterministic=True)
+    g = ctx.grad_J(dev(wl.D * 1e12), dev(wl.c_aux)).cpu().numpy()
+    assert np.isnan(g).all()
+    g = ctx.grad_J(dev(wl.D), dev(wl.c_aux)).cpu().numpy()       # the flag does not stick
+    assert_parity(g, orc.grad_J(wl.mol, wl.D, wl.c_aux)[0], "deterministic J after overflow")
+    ctx.close()
