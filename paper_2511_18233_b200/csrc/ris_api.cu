@@ -8,6 +8,8 @@
 #include "ris_internal.h"
 #include "ris_setup.cuh"
 
+constexpr int RIS_NPRIM_MAX = 24;        // primitives per shell (kmax <= 576: the class-kernel task fits in shared memory)
+
 #include <algorithm>
 #include <utility>
 #include <cmath>
@@ -53,7 +55,7 @@ struct ris_ctx {
     double *d_pexp = nullptr, *d_pcoef = nullptr;
     RisClassPack cls[RIS_NCLASS]{};
     std::vector<void*> owned;          // every device allocation of the packed data
-    long long nelem_slab = 0, nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
+    long long nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[8] = {nullptr};
     // Gamma^P GEMM-2 block list: RIS_GTILE2^2 blocks (I >= J) of the spatially (Morton) ordered AO index that
     // contain a surviving shell pair
@@ -147,12 +149,14 @@ extern "C" int ris_profile_get_work(ris_ctx* c, int i, double* flops, double* by
 }
 
 // --------------------------------------------------------------------------------------- class launchers
-#define DECL(la, lb) void ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
+#define DECL(la, lb) void ris_launch_grad_##la##lb##_1(const RisGradParams&, cudaStream_t); void ris_launch_grad_##la##lb##_2(const RisGradParams&, cudaStream_t); \
+    void ris_launch_grad_##la##lb##_3(const RisGradParams&, cudaStream_t); void ris_launch_grad_##la##lb##_4(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
 #undef DECL
-ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
-    ris_launch_grad_00, ris_launch_grad_10, ris_launch_grad_11, ris_launch_grad_20, ris_launch_grad_21,
-    ris_launch_grad_22, ris_launch_grad_30, ris_launch_grad_31, ris_launch_grad_32, ris_launch_grad_33};
+#define ROW(la, lb) {ris_launch_grad_##la##lb##_1, ris_launch_grad_##la##lb##_2, ris_launch_grad_##la##lb##_3, ris_launch_grad_##la##lb##_4}
+ris_grad_launcher ris_grad_launchers[RIS_NCLASS][RIS_NB_MAX] = {
+    ROW(0, 0), ROW(1, 0), ROW(1, 1), ROW(2, 0), ROW(2, 1), ROW(2, 2), ROW(3, 0), ROW(3, 1), ROW(3, 2), ROW(3, 3)};
+#undef ROW
 static const char* const kGradNames[RIS_NCLASS] = {
     "ris_grad_kernel<0,0>", "ris_grad_kernel<1,0>", "ris_grad_kernel<1,1>", "ris_grad_kernel<2,0>", "ris_grad_kernel<2,1>",
     "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
@@ -168,7 +172,7 @@ __global__ void ris_k_mark_blocks(RisClassPack pk, const int* __restrict__ ao_po
 {
     const int ip = blockIdx.x * blockDim.x + threadIdx.x;
     if (ip >= pk.npairs) return;
-    const int r0 = ao_pos[pk.ao[ip]], q0 = ao_pos[pk.ao[(size_t)pk.npad + ip]];     // shells stay contiguous
+    const int r0 = ao_pos[pk.ao[ip]], q0 = ao_pos[pk.ao[(size_t)pk.npairs + ip]];   // shells stay contiguous
     const int r1 = r0 + ris_ncart(pk.la) - 1, q1 = q0 + ris_ncart(pk.lb) - 1;
     for (int I = r0 / RIS_GTILE2; I <= r1 / RIS_GTILE2; ++I)
         for (int J = q0 / RIS_GTILE2; J <= q1 / RIS_GTILE2; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
@@ -193,15 +197,15 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
 {
     if (!out) return RIS_EINVAL;
     *out = nullptr;
-    if (natoms < 1 || nshells < 1 || !coords || !shell_atom || !shell_l || !shell_nprim || !shell_prim_off || !prim_exp ||
+    if (natoms < 1 || natoms >= (1 << 20) || nshells < 1 || !coords || !shell_atom || !shell_l || !shell_nprim || !shell_prim_off || !prim_exp ||
         !prim_coef || !aux_exponents)
         return RIS_EINVAL;
     int nprim_tot = 0;
     std::vector<int> shell_ao(nshells);
     int nao = 0;
     for (int s = 0; s < nshells; ++s) {
-        if (shell_l[s] < 0 || shell_l[s] > RIS_LMAX || shell_nprim[s] < 1 || shell_atom[s] < 0 || shell_atom[s] >= natoms ||
-            shell_prim_off[s] < 0)
+        if (shell_l[s] < 0 || shell_l[s] > RIS_LMAX || shell_nprim[s] < 1 || shell_nprim[s] > RIS_NPRIM_MAX || shell_atom[s] < 0 ||
+            shell_atom[s] >= natoms || shell_prim_off[s] < 0)
             return RIS_EINVAL;
         nprim_tot = std::max(nprim_tot, shell_prim_off[s] + shell_nprim[s]);
         shell_ao[s] = nao;
@@ -266,10 +270,12 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         for (int j = 0; j <= i; ++j) c->nprim_total += (long long)shell_nprim[i] * shell_nprim[j];
     const int nblk = (int)((ntot + RIS_SCAN_BLOCK - 1) / RIS_SCAN_BLOCK);
     unsigned* d_packed;
+    unsigned long long* d_key;
     int *d_hist, *d_base, *d_meta;   // d_meta: totals[16], start[16], kmax[16]
     unsigned long long* d_nprim;
     long long* d_list[2];
     if ((rc = dev_alloc(c, &d_packed, (size_t)ntot, false))) return rc;
+    if ((rc = dev_alloc(c, &d_key, (size_t)ntot, false))) return rc;
     if ((rc = dev_alloc(c, &d_hist, (size_t)nblk * RIS_NBIN, false))) return rc;
     if ((rc = dev_alloc(c, &d_base, (size_t)nblk * RIS_NBIN, false))) return rc;
     if ((rc = dev_alloc(c, &d_meta, (size_t)3 * RIS_NBIN, true))) return rc;
@@ -278,15 +284,22 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     if ((rc = dev_alloc(c, &d_list[1], (size_t)ntot, false))) return rc;
     {
         ProfScope ps(c, "ris_k_pair_survey");
-        ris_k_pair_survey<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(m, ntot, d_packed, d_meta + 2 * RIS_NBIN, d_nprim);
+        ris_k_pair_survey<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(m, ntot, d_packed, d_key, d_meta + 2 * RIS_NBIN, d_nprim);
     }
+    // LSD radix sort on (class, atom of mu, atom of nu): 4-bit digits of the atom indices, then the class
+    int abits = 1;
+    while ((1 << abits) < natoms) ++abits;
+    std::vector<int> shifts;
+    for (int b = 0; b < abits; b += 4) shifts.push_back(b);
+    for (int b = 0; b < abits; b += 4) shifts.push_back(20 + b);
+    shifts.push_back(40);
     const long long* lin = nullptr;
-    for (int pass = 0; pass < 3; ++pass) {
+    for (size_t pass = 0; pass < shifts.size(); ++pass) {
         ProfScope ps(c, "ris_k_radix_pass");
         long long* lout = d_list[pass & 1];
-        ris_k_radix_hist<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_packed, pass, d_hist);
+        ris_k_radix_hist<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_key, shifts[pass], d_hist);
         ris_k_radix_scan<<<1, 32, 0, c->stream>>>(nblk, d_hist, d_base, d_meta, d_meta + RIS_NBIN);
-        ris_k_radix_scatter<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_packed, pass, d_base, d_meta + RIS_NBIN, lout);
+        ris_k_radix_scatter<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_key, shifts[pass], d_base, d_meta + RIS_NBIN, lout);
         lin = lout;
     }
     const long long* d_sorted = lin;
@@ -304,26 +317,26 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             RisClassPack& pk = c->cls[k];
             pk.la = la; pk.lb = lb;
             pk.npairs = meta[k];
-            pk.npad = (pk.npairs + RIS_PAIR_PAD - 1) / RIS_PAIR_PAD * RIS_PAIR_PAD;
             pk.kmax = meta[2 * RIS_NBIN + k];
             pk.nprim = (long long)nprim_c[k];
+            pk.ntasks = (int)((pk.nprim + RIS_TASK_PRIMS - 1) / RIS_TASK_PRIMS);
             pk.elem_off = off;
-            off += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npad;
-            c->nelem_real += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npairs;
+            off += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npairs;
             c->nprim_surv += pk.nprim;
             if (pk.npairs == 0) continue;
-            const size_t n = (size_t)pk.npad;
-            if ((rc = dev_alloc(c, &pk.geom, 6 * n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.atoms, 2 * n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.ao, 2 * n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.nkA, n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.nkB, n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.symf, n, true))) return rc;
-            if ((rc = dev_alloc(c, &pk.prim, (size_t)pk.kmax * RIS_PRIM_FIELDS * n, true))) return rc;
+            const size_t n = (size_t)pk.npairs;
+            if ((rc = dev_alloc(c, &pk.pairs, n, false))) return rc;
+            if ((rc = dev_alloc(c, &pk.ao, 2 * n, false))) return rc;
+            if ((rc = dev_alloc(c, &pk.symf, n, false))) return rc;
+            if ((rc = dev_alloc(c, &pk.prim_off, n + 1, false))) return rc;
+            if ((rc = dev_alloc(c, &pk.prim, (size_t)pk.nprim * RIS_PRIM_FIELDS, false))) return rc;
+            if ((rc = dev_alloc(c, &pk.task_begin, (size_t)pk.ntasks + 1, false))) return rc;
             ProfScope ps(c, "ris_k_pair_pack");
+            ris_k_scan_nk<<<1, 1024, 0, c->stream>>>(pk.npairs, d_sorted + meta[RIS_NBIN + k], d_packed, pk.prim_off);
+            ris_k_task_bounds<<<(pk.ntasks + 1 + 127) / 128, 128, 0, c->stream>>>(pk.npairs, pk.ntasks, pk.prim_off, pk.task_begin);
             ris_k_pair_pack<<<(pk.npairs + 127) / 128, 128, 0, c->stream>>>(m, pk, d_sorted + meta[RIS_NBIN + k]);
         }
-    c->nelem_slab = off;
+    c->nelem_real = off;
     CU(cudaGetLastError());
     // spatial AO order + block list for the pair-restricted Gamma^P GEMM-2
     {
@@ -402,19 +415,18 @@ extern "C" long long ris_npair_elements(const ris_ctx* c) { return c ? c->nelem_
 extern "C" int ris_p_batch(const ris_ctx* c) { return c ? c->last_pbatch : RIS_EINVAL; }
 
 // --------------------------------------------------------------------------------------- tile packing
-// out[slab][elem_off + e*npad + ip] = symf[ip] * (G[slab][mu0+ca][nu0+cb] + G[slab][nu0+cb][mu0+ca]),  e = ca*ncb + cb.
-// Folds D + D^T (or Gamma + Gamma^T) onto the unique shell pairs.
+// J tiles: out[slab][elem_off + ip*nel + e] = symf[ip] * (G[slab][mu0+ca][nu0+cb] + G[slab][nu0+cb][mu0+ca]),  e = ca*ncb + cb.
+// Folds D + D^T onto the unique shell pairs.
 __global__ void ris_k_pack_tiles(RisClassPack pk, int nao, const double* __restrict__ G, long long gstride,
                                  double* __restrict__ out, long long ostride)
 {
-    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ip >= pk.npairs) return;
-    const int ncb = ris_ncart(pk.lb);
-    const int e = blockIdx.y, ca = e / ncb, cb = e - ca * ncb;
-    const size_t r = (size_t)pk.ao[ip] + ca, q = (size_t)pk.ao[(size_t)pk.npad + ip] + cb;
+    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)pk.npairs * nel) return;
+    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
+    const size_t r = (size_t)pk.ao[ip] + ca, q = (size_t)pk.ao[(size_t)pk.npairs + ip] + cb;
     const double* g = G + (size_t)blockIdx.z * gstride;
-    out[(size_t)blockIdx.z * ostride + pk.elem_off + (size_t)e * pk.npad + ip] =
-        (double)pk.symf[ip] * (g[r * nao + q] + g[q * nao + r]);
+    out[(size_t)blockIdx.z * ostride + pk.elem_off + idx] = (double)pk.symf[ip] * (g[r * nao + q] + g[q * nao + r]);
 }
 
 static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab, double* out, long long ostride)
@@ -422,19 +434,18 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
     for (int k = 0; k < RIS_NCLASS; ++k) {
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
-        const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs * nslab;
-        ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel, 24.0 * nel);
-        dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), nslab);
-        ris_k_pack_tiles<<<grid, 128, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
+        const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+        ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel * nslab, 24.0 * nel * nslab);
+        dim3 grid((unsigned)(((long long)nel + 255) / 256), 1, nslab);
+        ris_k_pack_tiles<<<grid, 256, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
     }
     CU(cudaGetLastError());
     return RIS_OK;
 }
 
-constexpr int RIS_NB_MAX = 8;      // states per class-kernel launch (shared-memory slots)
-
-static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long pstride, const double* cscale,
-                          int nb, int p0, int p1, double* grad, unsigned long long* det)
+// One launch per class, heaviest class first.  tile / sstride / estride / lstride: see RisGradParams.
+static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long estride, int lstride,
+                          const double* cscale, int nb, int p0, int p1, double* grad, unsigned long long* det)
 {
     for (int oi = 0; oi < RIS_NCLASS; ++oi) {
         const int k = kClassOrder[oi];
@@ -442,22 +453,23 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         if (pk.npairs == 0) continue;
         RisGradParams p{};
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
-        p.tile = tile; p.sstride = sstride; p.pstride = pstride; p.cscale = cscale; p.nb = nb; p.p0 = p0; p.p1 = p1;
+        p.tile = tile; p.sstride = sstride; p.estride = estride; p.lstride = lstride; p.cscale = cscale; p.nb = nb;
+        p.p0 = p0; p.p1 = p1;
         p.grad = grad; p.det = det; p.det_flag = det ? (int*)c->ws[WS_DET] : nullptr;
-        // enough blocks for >= 4 per SM; at least 4 aux per block for the light classes (amortises the pair-side
-        // loads and atomics), 2 / 1 for the heavy ones (few pairs, long recurrences); at most 64 (shared accumulators)
-        const int bx = pk.npad / RIS_GRAD_THREADS, np = p1 - p0, E = pk.la + pk.lb + 1;
-        int ny = std::max(1, (4 * 148 + bx - 1) / bx);
-        int pch = std::max(E >= 5 ? 1 : (E >= 3 ? 2 : 4), (np + ny - 1) / ny);
-        p.pchunk = std::min(std::min(pch, np), std::max(8, std::min(64, 192 / nb)));
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
         ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
-                     8.0 * (np_ * (pstride ? 1.0 : 0.0) + (pstride ? 0.0 : 1.0)) * nel * pk.npairs * nb +
-                         8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-        ris_grad_launchers[k](p, c->stream);
+                     8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
+        ris_grad_launchers[k][nb - 1](p, c->stream);
     }
     CU(cudaGetLastError());
     return RIS_OK;
+}
+
+// states per class-kernel launch: as even as possible, at most RIS_NB_MAX
+static int next_nb(int remaining)
+{
+    const int launches = (remaining + RIS_NB_MAX - 1) / RIS_NB_MAX;
+    return (remaining + launches - 1) / launches;
 }
 
 // --------------------------------------------------------------------------------------- deterministic reduction
@@ -504,13 +516,13 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
     const long long nao2 = (long long)c->nao * c->nao;
     unsigned long long* det;
     { int rc = det_begin(c, nbatch, &det); if (rc) return rc; }
-    for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
-        const int nb = std::min(RIS_NB_MAX, nbatch - s0);
+    for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
+        nb = next_nb(nbatch - s0);
         double* tile;
-        int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_slab, (void**)&tile);
+        int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile);
         if (rc) return rc;
-        if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_slab))) return rc;
-        if ((rc = launch_classes(c, tile, c->nelem_slab, 0, c_aux + (size_t)s0 * c->naux, nb, 0, c->naux,
+        if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
+        if ((rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux, nb, 0, c->naux,
                                  grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
             return rc;
     }
@@ -518,21 +530,25 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
 }
 
 // --------------------------------------------------------------------------------------- K
-// out[z][elem_off + e*npad + ip] = symf[ip] * S^P[pos(mu0+ca)][pos(nu0+cb)] read from the block buffer of GEMM-2
-// (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
-__global__ void ris_k_pack_sym(RisClassPack pk, const double* __restrict__ S, long long sstrideP, const int* __restrict__ ao_pos,
-                               const int* __restrict__ tmap, int nblk, double* __restrict__ out, long long ostride)
+// K tiles, P-minor: out[(elem_off + ip*nel + e) * pbp + P] = symf[ip] * S^P[pos(mu0+ca)][pos(nu0+cb)] read from the block
+// buffer of GEMM-2 (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).  threadIdx.x runs over P (the
+// contiguous output index: a warp writes 256 bytes), threadIdx.y over 8 consecutive elements (neighbours in S).
+__global__ void __launch_bounds__(256) ris_k_pack_sym(RisClassPack pk, int np, int pbp, const double* __restrict__ S, long long sstrideP,
+                                                      const int* __restrict__ ao_pos, const int* __restrict__ tmap, int nblk,
+                                                      double* __restrict__ out)
 {
     constexpr int T = RIS_GTILE2;
-    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ip >= pk.npairs) return;
-    const int ncb = ris_ncart(pk.lb);
-    const int e = blockIdx.y, ca = e / ncb, cb = e - ca * ncb;
-    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npad + ip]] + cb;
+    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const long long idx = (long long)blockIdx.x * 8 + threadIdx.y;
+    if (idx >= (long long)pk.npairs * nel) return;
+    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
+    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
     if (r / T < q / T) { const int t = r; r = q; q = t; }
     const int tile = tmap[(r / T) * nblk + (q / T)];
-    const double v = S[(size_t)blockIdx.z * sstrideP + (size_t)tile * (T * T) + (r % T) * T + (q % T)];
-    out[(size_t)blockIdx.z * ostride + pk.elem_off + (size_t)e * pk.npad + ip] = (double)pk.symf[ip] * v;
+    const double* src = S + (size_t)tile * (T * T) + (r % T) * T + (q % T);
+    double* dst = out + ((size_t)pk.elem_off + (size_t)idx) * pbp;
+    const double f = (double)pk.symf[ip];
+    for (int P = threadIdx.x; P < np; P += 32) dst[P] = f * src[(size_t)P * sstrideP];
 }
 
 // out[pos][0..ld) = in[order[pos]][0..cols) zero padded: C_occ in spatial row order with an even leading dimension
@@ -552,26 +568,28 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     const int nao = c->nao, naux = c->naux;
-    const int nbmax = std::min(nbatch, RIS_NB_MAX);
+    const int nbmax = next_nb(nbatch);
     const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
     const long long blk = (long long)RIS_GTILE2 * RIS_GTILE2;
-    // per aux function: HT [nao][noccp], S blocks [ntiles][64*64], packed tiles [nb][slab]
+    // per aux function: HT [nao][noccp], S blocks [ntiles][64*64], packed tiles [nb][elements]
     int pb = c->opt.p_batch;
     if (pb <= 0) {
         size_t fr = 0, tot = 0;
         CU(cudaMemGetInfo(&fr, &tot));
         fr += c->ws_bytes[WS_TILE] + c->ws_bytes[WS_H] + c->ws_bytes[WS_G];
-        const double per = 8.0 * ((double)noccp * nao + (double)c->ntiles * blk + (double)nbmax * c->nelem_slab);
+        const double per = 8.0 * ((double)noccp * nao + (double)c->ntiles * blk + (double)nbmax * c->nelem_real);
         const double budget = std::min(0.5 * (double)fr, 24.0e9);
         pb = (int)std::max(1.0, std::min((double)naux, budget / per));
+        if (pb < naux && pb > 32) pb &= ~31;              // whole chunks of 32 aux lanes
     }
     pb = std::min(pb, naux);
     c->last_pbatch = pb;
+    const int pbp = (pb + 3) & ~3;                        // P-minor tile rows start on 32-byte sectors
     double *tile, *HT, *S, *Cop;
     int rc;
     unsigned long long* det;
     if ((rc = det_begin(c, nbatch, &det))) return rc;
-    if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pb * c->nelem_slab, (void**)&tile))) return rc;
+    if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pbp * c->nelem_real, (void**)&tile))) return rc;
     if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)nao * pb * noccp, (void**)&HT))) return rc;
     if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * c->ntiles * blk, (void**)&S))) return rc;
     if ((rc = ws_get(c, WS_COCC, sizeof(double) * (size_t)nao * noccp, (void**)&Cop))) return rc;
@@ -580,8 +598,8 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
         const long long n = (long long)nao * noccp;
         ris_k_pad_rows<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(nao, nocc, noccp, c->d_ao_order, C_occ, Cop);
     }
-    for (int s0 = 0; s0 < nbatch; s0 += RIS_NB_MAX) {
-        const int nb = std::min(RIS_NB_MAX, nbatch - s0);
+    for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
+        nb = next_nb(nbatch - s0);
         for (int p0 = 0; p0 < naux; p0 += pb) {
             const int np = std::min(pb, naux - p0);
             const long long ldh = (long long)pb * noccp;
@@ -597,7 +615,7 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                                  8.0 * ((double)np * nocc * nvir + (double)nao * nvir + (double)np * nocc * nao));
                     CU(ris_gemm_dense(c->stream, g, 1));
                 }
-                {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 128x128 blocks
+                {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 64x64 blocks
                     RisGemmParams g{};
                     g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, ldh, noccp, nocc};
                     g.seg[1] = RisGemmSeg{HT, ldh, noccp, Cop, noccp, 0, nocc};
@@ -608,18 +626,18 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                                  8.0 * np * ((double)noccp * nao + (double)c->ntiles * blk) + 8.0 * nao * noccp);
                     CU(ris_gemm_blocks(c->stream, g, np, c->ntiles));
                 }
-                double* out = tile + (size_t)s * pb * c->nelem_slab;
+                double* out = tile + (size_t)s * pbp * c->nelem_real;
                 for (int k = 0; k < RIS_NCLASS; ++k) {
                     const RisClassPack& pk = c->cls[k];
                     if (pk.npairs == 0) continue;
-                    const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs * np;
-                    ProfScope ps(c, "ris_k_pack_sym", nel, 16.0 * nel);
-                    dim3 grid((pk.npairs + 127) / 128, ris_ncart(pk.la) * ris_ncart(pk.lb), np);
-                    ris_k_pack_sym<<<grid, 128, 0, c->stream>>>(pk, S, (long long)c->ntiles * blk, c->d_ao_pos, c->d_tmap, c->nblk, out, c->nelem_slab);
+                    const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+                    ProfScope ps(c, "ris_k_pack_sym", (double)nelc * np, 16.0 * nelc * np);
+                    ris_k_pack_sym<<<(unsigned)((nelc + 7) / 8), dim3(32, 8), 0, c->stream>>>(
+                        pk, np, pbp, S, (long long)c->ntiles * blk, c->d_ao_pos, c->d_tmap, c->nblk, out);
                 }
                 CU(cudaGetLastError());
             }
-            if ((rc = launch_classes(c, tile, (long long)pb * c->nelem_slab, c->nelem_slab, nullptr, nb, p0, p0 + np,
+            if ((rc = launch_classes(c, tile, (long long)pbp * c->nelem_real, pbp, 1, nullptr, nb, p0, p0 + np,
                                      grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
                 return rc;
         }

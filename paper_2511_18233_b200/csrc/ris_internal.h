@@ -5,28 +5,41 @@
 
 constexpr int RIS_LMAX = 3;
 constexpr int RIS_NCLASS = 10;          // (la,lb), la >= lb, la <= 3
-constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a, 2b, coef   (Z = host centre)
-constexpr int RIS_PAIR_PAD = 128;       // pairs per class padded to a multiple of this
-constexpr int RIS_GRAD_THREADS = 128;
+constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a, 2b, coef   (Z = host centre); one 64-byte record
+constexpr int RIS_GRAD_WARPS = 4;       // warps per class-kernel block
+constexpr int RIS_GRAD_THREADS = 32 * RIS_GRAD_WARPS;
+constexpr int RIS_TASK_PRIMS = 64;      // a warp task = the shell pairs whose first primitive pair falls in one window of
+                                        // this many packed primitive pairs (so a task holds < RIS_TASK_PRIMS + kmax of them)
+constexpr int RIS_NB_MAX = 4;           // states per class-kernel launch (per-state gradients live in registers)
 
 __host__ __device__ inline int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
 __host__ __device__ inline int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
 
-// Packed shell pairs of one class (device pointers, SoA over the padded pair index).
+// One packed shell pair (64 bytes, read by a whole warp as a broadcast).
+struct __align__(16) RisPairRec {
+    double Ax, Ay, Az;       // centre of mu
+    double ABx, ABy, ABz;    // A - B
+    int atA, atB;            // atom of mu, atom of nu
+    int nkA, nkB;            // surviving primitive pairs hosted on A (a >= b; stored first) / on B (b > a)
+};
+static_assert(sizeof(RisPairRec) == 64, "pair record layout");
+
+// Packed shell pairs of one class (device pointers).  The pairs are sorted by (atom of mu, atom of nu), so that the
+// class kernel keeps the pair-side gradient of an atom pair in registers across its shell pairs.
 struct RisClassPack {
     int la, lb;
     int npairs;            // surviving shell pairs
-    int npad;              // padded count (multiple of RIS_PAIR_PAD); SoA stride
     int kmax;              // max surviving primitive pairs per shell pair
     long long nprim;       // surviving primitive pairs in the class
-    double* geom;          // [6][npad]  Ax,Ay,Az, ABx,ABy,ABz  (AB = A - B)
-    int* atoms;            // [2][npad]  atom of mu, atom of nu
-    int* ao;               // [2][npad]  first AO of mu, first AO of nu
-    int* nkA;              // [npad]     surviving primitive pairs hosted on A (a >= b); stored first
-    int* nkB;              // [npad]     surviving primitive pairs hosted on B (b > a)
-    float* symf;           // [npad]     1 (mu != nu shell) or 0.5 (same shell): folds D + D^T onto unique pairs
-    double* prim;          // [kmax][8][npad]
-    long long elem_off;    // offset of this class inside a packed tile slab
+    int ntasks;            // warp tasks (windows of RIS_TASK_PRIMS primitive pairs)
+    RisPairRec* pairs;     // [npairs]
+    int* ao;               // [2][npairs]  first AO of mu, first AO of nu
+    float* symf;           // [npairs]     1 (mu != nu shell) or 0.5 (same shell): folds D + D^T onto unique pairs
+    long long* prim_off;   // [npairs + 1] first primitive-pair record of the pair (exclusive scan)
+    double* prim;          // [nprim][8]
+    int* task_begin;       // [ntasks + 1] first pair of the task
+    long long elem_off;    // first packed Cartesian pair element of the class; pair ip holds elements
+                           // elem_off + ip * nca * ncb + (ca * ncb + cb)
 };
 
 // Launch description of one class kernel (by value to the kernel).
@@ -35,12 +48,14 @@ struct RisGradParams {
     int naux, natoms;
     const double* aux;       // [naux][5] Cx,Cy,Cz,alpha,auxfac
     const double* boys;      // table for M = E of this class
-    const double* tile;      // packed tiles: + s*sstride + (P-p0)*pstride + elem_off + e*npad + ip
-    long long sstride, pstride;
+    // packed tiles: element el of state s for aux P sits at tile[s*sstride + el*estride + (P - p0)*lstride]
+    //   J: estride 1, lstride 0 (D tile, the same for every P);  K: estride = padded P-batch, lstride 1 (Gamma^P)
+    const double* tile;
+    long long sstride, estride;
+    int lstride;
     const double* cscale;    // J: c_aux[nb][naux]; K: nullptr
     int nb;
-    int p0, p1;              // aux range of this launch
-    int pchunk;              // aux functions per blockIdx.y
+    int p0, p1;              // aux range of this launch; blockIdx.y selects 32 of them, one per lane
     double* grad;            // [nb][natoms][3], accumulated with atomics
     unsigned long long* det; // deterministic mode: [nb][natoms][3][2] fixed-point accumulators (hi, lo), else nullptr
     int* det_flag;           // set to 1 when a contribution leaves the fixed-point range
@@ -49,7 +64,7 @@ struct RisGradParams {
 // Deterministic reduction (ris_options.deterministic): a contribution x is added as the integer pair
 //   hi = floor(x 2^28),  lo = floor((x 2^28 - hi) 2^32)        value = hi 2^-28 + lo 2^-60
 // with two 64-bit INTEGER atomics; integer addition is associative, so the result does not depend on the order in
-// which blocks arrive (resolution 2^-60 ~ 8.7e-19 per contribution, range |x| < 2^34, |sum| < 2^35).
+// which warps arrive (resolution 2^-60 ~ 8.7e-19 per contribution, range |x| < 2^34, |sum| < 2^35).
 __device__ __forceinline__ void ris_grad_add(const RisGradParams& prm, size_t idx, double x)
 {
     if (prm.det == nullptr) { atomicAdd(prm.grad + idx, x); return; }
@@ -62,4 +77,12 @@ __device__ __forceinline__ void ris_grad_add(const RisGradParams& prm, size_t id
 }
 
 typedef void (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
-extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];
+extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS][RIS_NB_MAX];
+
+// dynamic shared memory of a class-kernel block (host + device agree through this)
+__host__ __device__ inline size_t ris_grad_warp_smem(int kmax, int nb)
+{
+    return (size_t)64 * (RIS_TASK_PRIMS + kmax)      // primitive-pair records of the task
+         + (size_t)64 * RIS_TASK_PRIMS               // pair records of the task
+         + (size_t)8 * 6 * nb * 33;                  // flush scratch [6 nb][33]
+}

@@ -39,13 +39,14 @@ __device__ __forceinline__ bool ris_prim_survives(const RisMolDev& m, double a, 
     return bound >= m.tol;
 }
 
-// Survey: packed[t] = cls | nkA << 8 | nkB << 16 with cls = 15 for a dropped pair; nkA / nkB = surviving
+// Survey: packed[t] = cls | nkA << 8 | nkB << 20 with cls = 15 for a dropped pair; nkA / nkB = surviving
 // primitive pairs hosted on A (a >= b) / on B (b > a).  Per-class max / total of surviving primitive pairs.
 constexpr int RIS_NBIN = 16;
 constexpr int RIS_DROPPED = 15;
 
-__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m, long long ntot, unsigned* packed, int* kmax,
-                                                                    unsigned long long* nprim)
+// key[t] = cls << 40 | atom(mu) << 20 | atom(nu): the sort key (class, atom pair).
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m, long long ntot, unsigned* packed,
+                                                                    unsigned long long* key, int* kmax, unsigned long long* nprim)
 {
     const long long t = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
     if (t >= ntot) return;
@@ -69,28 +70,23 @@ __global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m,
         atomicMax(&kmax[k], nA + nB);
         atomicAdd(&nprim[k], (unsigned long long)(nA + nB));
     }
-    packed[t] = k | ((unsigned)min(nA, 255) << 8) | ((unsigned)min(nB, 255) << 16);
+    packed[t] = k | ((unsigned)min(nA, 4095) << 8) | ((unsigned)min(nB, 4095) << 20);
+    key[t] = ((unsigned long long)k << 40) | ((unsigned long long)m.shell_atom[mu] << 20) | (unsigned long long)m.shell_atom[nu];
 }
 
-// Stable LSD radix sort of the pair list in three 16-bin passes: nkB, nkA (both DEscending), class.  After it, the
-// pairs of a class are contiguous and ordered by (nkA, nkB), so the lanes of a warp run equally long primitive
-// loops in both host phases, and the blocks with the longest loops start first.  (Measured on config 4: ordering
-// by the TOTAL number of primitive pairs instead costs 10 % of the class-kernel time in either direction.)
-__device__ __forceinline__ int ris_digit(unsigned packed, int pass)
-{
-    if (pass == 0) return 15 - min((int)((packed >> 16) & 255u), 15);
-    if (pass == 1) return 15 - min((int)((packed >> 8) & 255u), 15);
-    return (int)(packed & 255u);
-}
+// Stable LSD radix sort of the pair list on 4-bit digits of the key (atom of nu, atom of mu, class; `shift` selects
+// the digit).  After it the pairs of a class are contiguous and ordered by atom pair: the class kernel walks the shell
+// pairs of one atom pair back to back and keeps their pair-side gradient in registers.
+__device__ __forceinline__ int ris_digit(unsigned long long key, int shift) { return (int)((key >> shift) & 15ull); }
 
-__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_hist(long long n, const long long* list_in, const unsigned* packed,
-                                                                   int pass, int* hist)
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_hist(long long n, const long long* list_in, const unsigned long long* key,
+                                                                   int shift, int* hist)
 {
     __shared__ int sh[RIS_NBIN];
     if (threadIdx.x < RIS_NBIN) sh[threadIdx.x] = 0;
     __syncthreads();
     const long long i = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
-    if (i < n) atomicAdd(&sh[ris_digit(packed[list_in ? list_in[i] : i], pass)], 1);
+    if (i < n) atomicAdd(&sh[ris_digit(key[list_in ? list_in[i] : i], shift)], 1);
     __syncthreads();
     if (threadIdx.x < RIS_NBIN) hist[blockIdx.x * RIS_NBIN + threadIdx.x] = sh[threadIdx.x];
 }
@@ -112,13 +108,13 @@ __global__ void ris_k_radix_scan(int nblk, const int* hist, int* base, int* tota
 }
 
 // Stable scatter: list_out[start[d] + base[blk][d] + rank-in-block] = element.
-__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_scatter(long long n, const long long* list_in, const unsigned* packed,
-                                                                      int pass, const int* base, const int* start, long long* list_out)
+__global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_scatter(long long n, const long long* list_in, const unsigned long long* key,
+                                                                      int shift, const int* base, const int* start, long long* list_out)
 {
     __shared__ int wtot[RIS_SCAN_BLOCK / 32];
     const long long i = (long long)blockIdx.x * RIS_SCAN_BLOCK + threadIdx.x;
     const long long el = (i < n) ? (list_in ? list_in[i] : i) : -1;
-    const int k = (i < n) ? ris_digit(packed[el], pass) : -1;
+    const int k = (i < n) ? ris_digit(key[el], shift) : -1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (int c = 0; c < RIS_NBIN; ++c) {
         const unsigned bal = __ballot_sync(0xffffffffu, k == c);
@@ -133,8 +129,46 @@ __global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_scatter(long long 
     }
 }
 
-// Pack one class: geometry, atoms, AO offsets, symmetry factor, surviving primitive pairs -- those hosted on
-// A (a >= b) first, then those hosted on B.
+// prim_off[0 .. n] = exclusive scan of the surviving primitive-pair counts of the class's sorted pairs (one block).
+__global__ void __launch_bounds__(1024) ris_k_scan_nk(int n, const long long* list, const unsigned* packed, long long* prim_off)
+{
+    __shared__ long long part[1024];
+    const int t = threadIdx.x, per = (n + 1023) / 1024;
+    const int i0 = min(t * per, n), i1 = min(i0 + per, n);
+    long long sum = 0;
+    for (int i = i0; i < i1; ++i) { const unsigned pk = packed[list[i]]; sum += ((pk >> 8) & 4095u) + ((pk >> 20) & 4095u); }
+    part[t] = sum;
+    __syncthreads();
+    if (t == 0) {
+        long long run = 0;
+        for (int k = 0; k < 1024; ++k) { const long long v = part[k]; part[k] = run; run += v; }
+        prim_off[n] = run;
+    }
+    __syncthreads();
+    long long run = part[t];
+    for (int i = i0; i < i1; ++i) {
+        prim_off[i] = run;
+        const unsigned pk = packed[list[i]];
+        run += ((pk >> 8) & 4095u) + ((pk >> 20) & 4095u);
+    }
+}
+
+// task_begin[t] = first pair whose first primitive-pair record is >= t * RIS_TASK_PRIMS  (t = 0 .. ntasks)
+__global__ void ris_k_task_bounds(int npairs, int ntasks, const long long* prim_off, int* task_begin)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > ntasks) return;
+    const long long target = (long long)t * RIS_TASK_PRIMS;
+    int lo = 0, hi = npairs;             // first ip in [0, npairs] with prim_off[ip] >= target
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (prim_off[mid] >= target) hi = mid; else lo = mid + 1;
+    }
+    task_begin[t] = (t == ntasks) ? npairs : lo;
+}
+
+// Pack one class: pair records, AO offsets, symmetry factor, surviving primitive pairs -- those hosted on
+// A (a >= b) first, then those hosted on B -- as 64-byte records at prim_off[ip].
 __global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* list)
 {
     const int ip = blockIdx.x * blockDim.x + threadIdx.x;
@@ -147,13 +181,15 @@ __global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* l
     const double* B = m.coords + 3 * atB;
     const double dx = A[0] - B[0], dy = A[1] - B[1], dz = A[2] - B[2];
     const double AB2 = dx * dx + dy * dy + dz * dz;
-    const size_t n = (size_t)pk.npad;
-    pk.geom[0 * n + ip] = A[0]; pk.geom[1 * n + ip] = A[1]; pk.geom[2 * n + ip] = A[2];
-    pk.geom[3 * n + ip] = dx;   pk.geom[4 * n + ip] = dy;   pk.geom[5 * n + ip] = dz;
-    pk.atoms[ip] = atA; pk.atoms[n + ip] = atB;
+    const size_t n = (size_t)pk.npairs;
+    RisPairRec rec;
+    rec.Ax = A[0]; rec.Ay = A[1]; rec.Az = A[2];
+    rec.ABx = dx; rec.ABy = dy; rec.ABz = dz;
+    rec.atA = atA; rec.atB = atB;
     pk.ao[ip] = m.shell_ao[mu]; pk.ao[n + ip] = m.shell_ao[nu];
     pk.symf[ip] = (mu == nu) ? 0.5f : 1.0f;
-    int k = 0;
+    double* q = pk.prim + (size_t)pk.prim_off[ip] * RIS_PRIM_FIELDS;
+    int k = 0, kA = 0;
     for (int host = 0; host < 2; ++host) {
         for (int ka = 0; ka < m.shell_nprim[mu]; ++ka)
             for (int kb = 0; kb < m.shell_nprim[nu]; ++kb) {
@@ -162,21 +198,22 @@ __global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* l
                 const double da = m.pcoef[m.shell_poff[mu] + ka], db = m.pcoef[m.shell_poff[nu] + kb];
                 if (!ris_prim_survives(m, a, b, da, db, AB2)) continue;
                 const double p = a + b, ip_ = 1.0 / p;
-                double* q = pk.prim + (size_t)k * RIS_PRIM_FIELDS * n + ip;
-                q[0 * n] = p;
+                q[0] = p;
                 // P - Z (Z = host centre) from the centre difference: host A: -(b/p)(A-B); host B: (a/p)(A-B)
                 const double fz = (host == 0) ? -b * ip_ : a * ip_;
-                q[1 * n] = fz * dx;
-                q[2 * n] = fz * dy;
-                q[3 * n] = fz * dz;
-                q[4 * n] = 0.5 * ip_;
-                q[5 * n] = 2.0 * a;
-                q[6 * n] = 2.0 * b;
+                q[1] = fz * dx;
+                q[2] = fz * dy;
+                q[3] = fz * dz;
+                q[4] = 0.5 * ip_;
+                q[5] = 2.0 * a;
+                q[6] = 2.0 * b;
                 // d_a d_b K_ab 2 pi^{5/2} / p
-                q[7 * n] = da * db * exp(-a * b * ip_ * AB2) * (2.0 * 17.493418327624862846) * ip_;
+                q[7] = da * db * exp(-a * b * ip_ * AB2) * (2.0 * 17.493418327624862846) * ip_;
+                q += RIS_PRIM_FIELDS;
                 ++k;
             }
-        if (host == 0) pk.nkA[ip] = k;
+        if (host == 0) kA = k;
     }
-    pk.nkB[ip] = k - pk.nkA[ip];
+    rec.nkA = kA; rec.nkB = k - kA;
+    pk.pairs[ip] = rec;
 }

@@ -55,12 +55,16 @@ static void phase_t(int nk, const double* prim, bool hostA, const double* Z, con
                                  Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac, tab(K::E), acc);
     }
     if (!used) return;
-    ris_hrrc<LH, LO, TR>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)(K::NCA * K::NCB), nb,
-                         [&](int s, double h0, double h1, double h2, double o0, double o1, double o2) {
-                             double* o = out + 6 * s + (hostA ? 0 : 3);
-                             double* oo = out + 6 * s + (hostA ? 3 : 0);
-                             o[0] += h0; o[1] += h1; o[2] += h2; oo[0] += o0; oo[1] += o1; oo[2] += o2;
-                         });
+    // the kernels instantiate NB = 1..4 states per launch; the harness contracts one state at a time
+    for (int s = 0; s < nb; ++s) {
+        const double sc[1] = {1.0};
+        double gh[1][3] = {{0.0, 0.0, 0.0}}, go[1][3] = {{0.0, 0.0, 0.0}};
+        ris_hrrc<LH, LO, TR, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile + (size_t)s * (K::NCA * K::NCB), (size_t)1,
+                                (size_t)(K::NCA * K::NCB), sc, gh, go);
+        double* o = out + 6 * s + (hostA ? 0 : 3);
+        double* oo = out + 6 * s + (hostA ? 3 : 0);
+        for (int x = 0; x < 3; ++x) { o[x] += gh[0][x]; oo[x] += go[0][x]; }
+    }
 }
 
 template <int LA, int LB>
