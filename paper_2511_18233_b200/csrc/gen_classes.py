@@ -18,8 +18,8 @@ Emits `generated/ris_classes.cuh`: for every class (la >= lb, la <= 3) straight-
                       on the contracted targets, then
                         d/dA_i (ab|P) = (a+1_i,b|_{2a} - a_i (a-1_i,b|_1
                         d/dB_i (ab|P) = (a,b+1_i|_{2b} - b_i (a,b-1_i|_1
-                      contracted on the fly with the D / Gamma^P tile of each of the NB states
-                      (compile-time NB: the per-state gradients stay in registers).
+                      contracted on the fly with the D / Gamma^P tile of each state and added to the
+                      caller's per-lane accumulator slots (shared memory in the class kernel).
 
 What is computed is Eq. 27 terms 1-2 of the paper for the integrals of Eq. 21
 (PAPER.md:119); the evaluation scheme is ours (the paper is silent).  The aux-centre
@@ -208,13 +208,14 @@ def gen_hrrc(pl: ClassPlan) -> str:
     la, lb = pl.la, pl.lb
     out = []
     w = out.append
-    w(f"// contracted triplet of class ({la},{lb}): HRR, derivative assembly, contraction with the tile of each of the")
-    w("// NB states: gh[s] += sc[s] d/d(host centre), go[s] += sc[s] d/d(other centre).")
-    w("// tile element (c_host,c_other) of state s sits at tile[s*sstride + el*estride], el by TR (see gen_classes.py).")
-    w("template <bool TR, int NB>")
+    w(f"// contracted triplet of class ({la},{lb}): HRR, derivative assembly, contraction with the tile of each state,")
+    w("// accumulated into the caller's per-lane slots: slot[(s*6 + c)*SL] += sc[s*SC] * g, c = 0..2 centre A, 3..5 centre B")
+    w("// (the host centre is B in the TR instantiations).  tile element (c_host,c_other) of state s sits at")
+    w("// tile[s*sstride + el*estride], el by TR (see gen_classes.py).")
+    w("template <bool TR, int SL, int SC>")
     w(f"RIS_DEV void ris_hrrc_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
-    w("    const double* __restrict__ tile, size_t estride, size_t sstride, const double (&sc)[NB],")
-    w("    double (&gh)[NB][3], double (&go)[NB][3])")
+    w("    const double* __restrict__ tile, size_t estride, size_t sstride, int nb, const double* __restrict__ sc,")
+    w("    double* __restrict__ slot)")
     w("{")
     done = set()
     X2a = gen_hrr_chain(w, pl, "2a", la + 1, lb, "xa", done)
@@ -222,8 +223,8 @@ def gen_hrrc(pl: ClassPlan) -> str:
     X1m = gen_hrr_chain(w, pl, "1", la - 1, lb, "xm", done) if la >= 1 else None
     Y1m = gen_hrr_chain(w, pl, "1", la, lb - 1, "xm", done) if lb >= 1 else None
     nca, ncb = nc(la), nc(lb)
-    w("#pragma unroll")
-    w("    for (int s = 0; s < NB; ++s) {")
+    w("    constexpr int OH = TR ? 3 : 0, OO = TR ? 0 : 3;")
+    w("    for (int s = 0; s < nb; ++s) {")
     w("        const double* __restrict__ t = tile + (size_t)s * sstride;")
     w("        double ga0 = 0.0, ga1 = 0.0, ga2 = 0.0, gb0 = 0.0, gb1 = 0.0, gb2 = 0.0;")
     for ia, a in enumerate(comps(la)):
@@ -237,8 +238,12 @@ def gen_hrrc(pl: ClassPlan) -> str:
                 if b[i] >= 1:
                     w(f"          gb{i} = fma(-{float(b[i])} * w, {Y1m(a, lower(b, i))}, gb{i});")
             w("        }")
-    w("        gh[s][0] = fma(sc[s], ga0, gh[s][0]); gh[s][1] = fma(sc[s], ga1, gh[s][1]); gh[s][2] = fma(sc[s], ga2, gh[s][2]);")
-    w("        go[s][0] = fma(sc[s], gb0, go[s][0]); go[s][1] = fma(sc[s], gb1, go[s][1]); go[s][2] = fma(sc[s], gb2, go[s][2]);")
+    w("        const double c = sc[s * SC];")
+    w("        double* __restrict__ o = slot + s * 6 * SL;")
+    for i in range(3):
+        w(f"        o[(OH + {i}) * SL] = fma(c, ga{i}, o[(OH + {i}) * SL]);")
+    for i in range(3):
+        w(f"        o[(OO + {i}) * SL] = fma(c, gb{i}, o[(OO + {i}) * SL]);")
     w("    }")
     w("}")
     return "\n".join(out)
@@ -265,9 +270,9 @@ def generate() -> str:
     for la, lb in classes:
         parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_vrr_{la}{lb}(static_cast<A&&>(a)...);")
     parts.append("}")
-    parts.append("template <int LA, int LB, bool TR, int NB, class... A> RIS_DEV void ris_hrrc(A&&... a) {")
+    parts.append("template <int LA, int LB, bool TR, int SL, int SC, class... A> RIS_DEV void ris_hrrc(A&&... a) {")
     for la, lb in classes:
-        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrrc_{la}{lb}<TR, NB>(static_cast<A&&>(a)...);")
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrrc_{la}{lb}<TR, SL, SC>(static_cast<A&&>(a)...);")
     parts.append("}")
     return "\n".join(parts) + "\n"
 

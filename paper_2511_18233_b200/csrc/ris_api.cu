@@ -149,14 +149,12 @@ extern "C" int ris_profile_get_work(ris_ctx* c, int i, double* flops, double* by
 }
 
 // --------------------------------------------------------------------------------------- class launchers
-#define DECL(la, lb) void ris_launch_grad_##la##lb##_1(const RisGradParams&, cudaStream_t); void ris_launch_grad_##la##lb##_2(const RisGradParams&, cudaStream_t); \
-    void ris_launch_grad_##la##lb##_3(const RisGradParams&, cudaStream_t); void ris_launch_grad_##la##lb##_4(const RisGradParams&, cudaStream_t);
+#define DECL(la, lb) void ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
 #undef DECL
-#define ROW(la, lb) {ris_launch_grad_##la##lb##_1, ris_launch_grad_##la##lb##_2, ris_launch_grad_##la##lb##_3, ris_launch_grad_##la##lb##_4}
-ris_grad_launcher ris_grad_launchers[RIS_NCLASS][RIS_NB_MAX] = {
-    ROW(0, 0), ROW(1, 0), ROW(1, 1), ROW(2, 0), ROW(2, 1), ROW(2, 2), ROW(3, 0), ROW(3, 1), ROW(3, 2), ROW(3, 3)};
-#undef ROW
+ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
+    ris_launch_grad_00, ris_launch_grad_10, ris_launch_grad_11, ris_launch_grad_20, ris_launch_grad_21,
+    ris_launch_grad_22, ris_launch_grad_30, ris_launch_grad_31, ris_launch_grad_32, ris_launch_grad_33};
 static const char* const kGradNames[RIS_NCLASS] = {
     "ris_grad_kernel<0,0>", "ris_grad_kernel<1,0>", "ris_grad_kernel<1,1>", "ris_grad_kernel<2,0>", "ris_grad_kernel<2,1>",
     "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
@@ -459,7 +457,7 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
         ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
                      8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-        ris_grad_launchers[k][nb - 1](p, c->stream);
+        ris_grad_launchers[k](p, c->stream);
     }
     CU(cudaGetLastError());
     return RIS_OK;
@@ -548,7 +546,14 @@ __global__ void __launch_bounds__(256) ris_k_pack_sym(RisClassPack pk, int np, i
     const double* src = S + (size_t)tile * (T * T) + (r % T) * T + (q % T);
     double* dst = out + ((size_t)pk.elem_off + (size_t)idx) * pbp;
     const double f = (double)pk.symf[ip];
-    for (int P = threadIdx.x; P < np; P += 32) dst[P] = f * src[(size_t)P * sstrideP];
+    // four strided gathers in flight per thread (the reads are 8 bytes out of a 32-byte sector each)
+    for (int P = threadIdx.x; P < np; P += 128) {
+        double v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = (P + 32 * u < np) ? __ldg(src + (size_t)(P + 32 * u) * sstrideP) : 0.0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) if (P + 32 * u < np) dst[P + 32 * u] = f * v[u];
+    }
 }
 
 // out[pos][0..ld) = in[order[pos]][0..cols) zero padded: C_occ in spatial row order with an even leading dimension

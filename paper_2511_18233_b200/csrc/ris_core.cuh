@@ -99,20 +99,39 @@ RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 
 // Accuracy: the packed record carries PZ = P - Z = -(o/p)(Z - O) computed from the centre difference, never
 // as a difference of absolute coordinates: for a tight pair on one atom the whole derivative is the small
 // WP term, and a rounding residue of size eps*|coords| in P - Z would swamp it.  P - C = (Z - C) + PZ.
+// Split in two so the class kernel can software-pipeline the primitive loop: ris_prim_head (prefactor + Boys: one
+// long dependent chain through rsqrt, the table gather and two Horner schemes) of primitive k+1 is issued next to
+// the wide, independent recurrence of primitive k.
+template <int E>
+struct RisPrimHead {
+    double F[E + 1];          // kappa F_m(T)
+    double W0, W1, W2;        // W - P = -(rho/p)(P - C)
+    double q;                 // rho/p
+};
+
+template <int E>
+RIS_DEV void ris_prim_head(double p, double PZx, double PZy, double PZz, double coef, double ZCx, double ZCy, double ZCz,
+                           double alpha, double auxfac, const double* __restrict__ boys_tab, RisPrimHead<E>& h)
+{
+    const double s = ris_rsqrt(p + alpha);
+    const double q = alpha * s * s;          // rho/p
+    const double X0 = ZCx + PZx, X1 = ZCy + PZy, X2 = ZCz + PZz;
+    const double T = (p * q) * fma(X0, X0, fma(X1, X1, X2 * X2));
+    ris_boys<E>(T, boys_tab, h.F);
+    const double kappa = coef * auxfac * s;
+#pragma unroll
+    for (int m = 0; m <= E; ++m) h.F[m] *= kappa;
+    h.W0 = -q * X0; h.W1 = -q * X1; h.W2 = -q * X2;
+    h.q = q;
+}
+
 template <int LH, int LO>
 RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, double oo2p, double h2, double o2,
                               double coef, double ZCx, double ZCy, double ZCz, double alpha, double auxfac,
                               const double* __restrict__ boys_tab, double (&acc)[RisClass<LH, LO>::NACC])
 {
     constexpr int E = RisClass<LH, LO>::E;
-    const double s = ris_rsqrt(p + alpha);
-    const double q = alpha * s * s;          // rho/p
-    const double X0 = ZCx + PZx, X1 = ZCy + PZy, X2 = ZCz + PZz;
-    const double T = (p * q) * fma(X0, X0, fma(X1, X1, X2 * X2));
-    double F[E + 1];
-    ris_boys<E>(T, boys_tab, F);
-    const double kappa = coef * auxfac * s;
-#pragma unroll
-    for (int m = 0; m <= E; ++m) F[m] *= kappa;
-    ris_vrr<LH, LO>(F, PZx, PZy, PZz, -q * X0, -q * X1, -q * X2, oo2p, q, h2, o2, acc);
+    RisPrimHead<E> h;
+    ris_prim_head<E>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
+    ris_vrr<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc);
 }

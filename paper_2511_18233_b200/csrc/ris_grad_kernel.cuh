@@ -1,6 +1,6 @@
 // ris_grad_kernel.cuh -- the fused class kernel: S1 Boys + S2 derivative-integral recurrence +
 // S3 contraction with the D / Gamma^P tile + S4 reduction, one instantiation per
-// (l_mu,l_nu) class and number of states NB.  Eq. 27 terms 1-2 for the integrals of Eq. 21
+// (l_mu,l_nu) class.  Eq. 27 terms 1-2 for the integrals of Eq. 21
 // (PAPER.md:119).
 //
 // Mapping ("aux lanes"): the 32 lanes of a warp hold 32 different auxiliary functions P (blockIdx.y selects the
@@ -10,12 +10,14 @@
 // warp's shared memory with coalesced 16-byte copies and read back as broadcasts, there is no divergence except the
 // Boys-function branch, and what varies per lane (aux centre / exponent, W - P, Boys values, the Gamma^P tile of the
 // K term, stored P-minor so a warp reads 256 contiguous bytes) is exactly the per-lane arithmetic.
-//   aux side   g[A_P] = -(dA + dB) summed over the pairs (translational invariance): the lane owns P, so this is a
-//              register accumulator over ALL tasks of the warp; the four warps of a block (same P chunk) are summed
-//              in shared memory in fixed order, one atomic per (block, P, state, x).
-//   pair side  g[A_mu], g[A_nu]: registers across the consecutive shell pairs of one atom pair (the pairs of a class
-//              are sorted by atom pair), then a fixed-order sum over the lanes through shared memory and one atomic
-//              per (atom pair, state, centre, x).
+// The per-state gradient accumulators are per-lane shared-memory slots (conflict-free: lane-contiguous), which keeps the
+// register file for the recurrence and lets the light classes run 16 warps per SM:
+//   aux side   g[A_P] = -(dA + dB) summed over the pairs (translational invariance): the lane owns P, so this is one
+//              slot per (state, x) over ALL tasks of the warp; the four warps of a block (same P chunk) are summed
+//              in fixed order at the end, one atomic per (block, P, state, x).
+//   pair side  g[A_mu], g[A_nu]: slots across the consecutive shell pairs of one atom pair (the pairs of a class
+//              are sorted by atom pair), then a fixed-order sum over the lanes and one atomic per (atom pair, state,
+//              centre, x).
 // Every in-block sum has a fixed order; the global atomics are FP64 adds, or -- deterministic mode -- 64-bit integer
 // adds of a fixed-point split (ris_grad_add), which makes the result bitwise reproducible.
 #pragma once
@@ -23,12 +25,12 @@
 #include "ris_internal.h"
 
 // One host-centre phase of a contracted triplet: the primitive pairs q[0 .. nk) hosted on centre Z (host l = LH,
-// other l = LO), then HRR / derivative / tile contraction into gh (host centre) and go (other centre).
-template <int LH, int LO, bool TR, int NB>
+// other l = LO), then HRR / derivative / tile contraction into the lane's accumulator slots.
+template <int LH, int LO, bool TR>
 RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
                        double ZOz, double alpha, double auxfac, const double* __restrict__ boys,
-                       const double* __restrict__ tile, size_t estride, size_t sstride, const double (&sc)[NB],
-                       double (&gh)[NB][3], double (&go)[NB][3])
+                       const double* __restrict__ tile, size_t estride, size_t sstride, int nb, const double* __restrict__ sc,
+                       double* __restrict__ slot)
 {
     using K = RisClass<LH, LO>;
     double acc[K::NACC];
@@ -42,20 +44,28 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
         ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
                                  alpha, auxfac, boys, acc);
     }
-    ris_hrrc<LH, LO, TR, NB>(acc, ZOx, ZOy, ZOz, tile, estride, sstride, sc, gh, go);
+    ris_hrrc<LH, LO, TR, 33, 32>(acc, ZOx, ZOy, ZOz, tile, estride, sstride, nb, sc, slot);
 }
 
-template <int LA, int LB, int NB>
-__global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGradParams prm)
+// resident blocks per SM the register allocation aims at (light classes: latency-bound prefactor / Boys chains
+// want warps; heavy classes: the contracted targets want registers)
+template <int LA, int LB> struct RisGradTune { static constexpr int MINB = (LA + LB <= 1) ? 4 : (LA + LB == 2 ? 3 : 2); };
+
+template <int LA, int LB>
+__global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
 {
     constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
     extern __shared__ __align__(16) unsigned char sm_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const RisClassPack& pk = prm.pk;
-    const size_t wbytes = ris_grad_warp_smem(pk.kmax, NB);
+    const int nb = prm.nb;
+    const size_t wbytes = ris_grad_warp_smem(pk.kmax, nb);
     double* s_prim = reinterpret_cast<double*>(sm_raw + (size_t)warp * wbytes);
     RisPairRec* s_pair = reinterpret_cast<RisPairRec*>(s_prim + (size_t)RIS_PRIM_FIELDS * (RIS_TASK_PRIMS + pk.kmax));
-    double* s_red = reinterpret_cast<double*>(s_pair + RIS_TASK_PRIMS);      // [6 NB][33]
+    double* s_red = reinterpret_cast<double*>(s_pair + RIS_TASK_PRIMS);      // [6 nb][33]  pair side: A x,y,z, B x,y,z per state
+    double* s_gaux = s_red + 6 * nb * 33;                                    // [3 nb][32]  aux side
+    double* s_sc = s_gaux + 3 * nb * 32;                                     // [nb][32]    J: c_aux[s][P]; K: 1
+    const size_t gaux_off = (size_t)(reinterpret_cast<unsigned char*>(s_gaux) - (sm_raw + (size_t)warp * wbytes));
 
     // this lane's auxiliary function
     const int P = prm.p0 + blockIdx.y * 32 + lane;
@@ -64,33 +74,23 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
     const double* ax = prm.aux + 5 * (size_t)Pe;
     const double Cx = ax[0], Cy = ax[1], Cz = ax[2], alpha = ax[3];
     const double auxfac = live ? ax[4] : 0.0;          // a dead lane computes exact zeros
-    double sc[NB];
-#pragma unroll
-    for (int s = 0; s < NB; ++s) sc[s] = prm.cscale ? prm.cscale[(size_t)s * prm.naux + Pe] : 1.0;
+    for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale ? prm.cscale[(size_t)s * prm.naux + Pe] : 1.0;
+    for (int i = 0; i < 6 * nb; ++i) s_red[i * 33 + lane] = 0.0;
+    for (int i = 0; i < 3 * nb; ++i) s_gaux[i * 32 + lane] = 0.0;
     const double* __restrict__ tile_lane = prm.tile + (size_t)(Pe - prm.p0) * prm.lstride;
     const size_t estride = (size_t)prm.estride, sstride = (size_t)prm.sstride;
-
-    double gaux[NB][3], gA[NB][3], gB[NB][3];
-#pragma unroll
-    for (int s = 0; s < NB; ++s)
-#pragma unroll
-        for (int x = 0; x < 3; ++x) gaux[s][x] = gA[s][x] = gB[s][x] = 0.0;
     int curA = -1, curB = -1;
+    __syncwarp();
 
     // pair side: fixed-order sum over the lanes, one atomic per (state, centre, x); aux side keeps -(gA + gB)
     auto flush = [&]() {
         if (curA < 0) return;
+        for (int s = 0; s < nb; ++s)
 #pragma unroll
-        for (int s = 0; s < NB; ++s)
-#pragma unroll
-            for (int x = 0; x < 3; ++x) {
-                s_red[(s * 6 + x) * 33 + lane] = gA[s][x];
-                s_red[(s * 6 + 3 + x) * 33 + lane] = gB[s][x];
-                gaux[s][x] -= gA[s][x] + gB[s][x];
-                gA[s][x] = 0.0; gB[s][x] = 0.0;
-            }
+            for (int x = 0; x < 3; ++x)
+                s_gaux[(s * 3 + x) * 32 + lane] -= s_red[(s * 6 + x) * 33 + lane] + s_red[(s * 6 + 3 + x) * 33 + lane];
         __syncwarp();
-        if (lane < 6 * NB) {
+        if (lane < 6 * nb) {
             const double* r = s_red + lane * 33;
             double v = 0.0;
 #pragma unroll 8
@@ -99,6 +99,8 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
             const int at = c < 3 ? curA : curB;
             ris_grad_add(prm, ((size_t)s * prm.natoms + at) * 3 + (c < 3 ? c : c - 3), v);
         }
+        __syncwarp();
+        for (int i = 0; i < 6 * nb; ++i) s_red[i * 33 + lane] = 0.0;
         __syncwarp();
     };
 
@@ -125,12 +127,12 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
             const double* __restrict__ tile = tile_lane + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * estride;
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
             if (pr.nkA > 0)
-                ris_phase<LA, LB, false, NB>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
-                                             estride, sstride, sc, gA, gB);
+                ris_phase<LA, LB, false>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
+                                         estride, sstride, nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
             if (pr.nkB > 0)
-                ris_phase<LB, LA, true, NB>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz, alpha,
-                                            auxfac, prm.boys, tile, estride, sstride, sc, gB, gA);
+                ris_phase<LB, LA, true>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz, alpha,
+                                        auxfac, prm.boys, tile, estride, sstride, nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
     }
@@ -138,39 +140,32 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS) ris_grad_kernel(const RisGra
 
     // aux side: the four warps of the block hold the same 32 aux functions
     __syncthreads();
-    double* s_g = reinterpret_cast<double*>(sm_raw);          // [warps][3 NB][32]
-#pragma unroll
-    for (int s = 0; s < NB; ++s)
-#pragma unroll
-        for (int x = 0; x < 3; ++x) s_g[((size_t)warp * 3 * NB + s * 3 + x) * 32 + lane] = gaux[s][x];
-    __syncthreads();
     if (warp == 0 && live) {
+        for (int i = 0; i < 3 * nb; ++i) {
+            double v = 0.0;
 #pragma unroll
-        for (int s = 0; s < NB; ++s)
-#pragma unroll
-            for (int x = 0; x < 3; ++x) {
-                double v = 0.0;
-#pragma unroll
-                for (int w = 0; w < RIS_GRAD_WARPS; ++w) v += s_g[((size_t)w * 3 * NB + s * 3 + x) * 32 + lane];
-                ris_grad_add(prm, ((size_t)s * prm.natoms + P) * 3 + x, v);
-            }
+            for (int w = 0; w < RIS_GRAD_WARPS; ++w)
+                v += reinterpret_cast<const double*>(sm_raw + (size_t)w * wbytes + gaux_off)[i * 32 + lane];
+            const int s = i / 3, x = i - 3 * s;
+            ris_grad_add(prm, ((size_t)s * prm.natoms + P) * 3 + x, v);
+        }
     }
 }
 
-template <int LA, int LB, int NB>
+template <int LA, int LB>
 void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
 {
     if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
-    const size_t smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.kmax, NB);
+    const size_t smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.kmax, p.nb);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(ris_grad_kernel<LA, LB, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(ris_grad_kernel<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    // blockIdx.y: chunks of 32 aux functions; blockIdx.x: enough blocks for ~4 waves of 3 blocks per SM, each warp
+    // blockIdx.y: chunks of 32 aux functions; blockIdx.x: enough blocks for ~4 waves of the resident blocks, each warp
     // striding over the tasks (fewer, longer-lived warps = fewer aux-side atomics)
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
-    const int nx = std::max(1, std::min(nbt, (148 * 3 * 4 + ny - 1) / ny));
-    ris_grad_kernel<LA, LB, NB><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    const int nx = std::max(1, std::min(nbt, (148 * RisGradTune<LA, LB>::MINB * 4 + ny - 1) / ny));
+    ris_grad_kernel<LA, LB><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
 }

@@ -8,9 +8,9 @@ constexpr int RIS_NCLASS = 10;          // (la,lb), la >= lb, la <= 3
 constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a, 2b, coef   (Z = host centre); one 64-byte record
 constexpr int RIS_GRAD_WARPS = 4;       // warps per class-kernel block
 constexpr int RIS_GRAD_THREADS = 32 * RIS_GRAD_WARPS;
-constexpr int RIS_TASK_PRIMS = 64;      // a warp task = the shell pairs whose first primitive pair falls in one window of
+constexpr int RIS_TASK_PRIMS = 32;      // a warp task = the shell pairs whose first primitive pair falls in one window of
                                         // this many packed primitive pairs (so a task holds < RIS_TASK_PRIMS + kmax of them)
-constexpr int RIS_NB_MAX = 4;           // states per class-kernel launch (per-state gradients live in registers)
+constexpr int RIS_NB_MAX = 5;           // states per class-kernel launch (per-state gradient slots in shared memory)
 
 __host__ __device__ inline int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
 __host__ __device__ inline int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
@@ -77,12 +77,12 @@ __device__ __forceinline__ void ris_grad_add(const RisGradParams& prm, size_t id
 }
 
 typedef void (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
-extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS][RIS_NB_MAX];
+extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];
 
 // dynamic shared memory of a class-kernel block (host + device agree through this)
 __host__ __device__ inline size_t ris_grad_warp_smem(int kmax, int nb)
 {
     return (size_t)64 * (RIS_TASK_PRIMS + kmax)      // primitive-pair records of the task
          + (size_t)64 * RIS_TASK_PRIMS               // pair records of the task
-         + (size_t)8 * 6 * nb * 33;                  // flush scratch [6 nb][33]
+         + (size_t)8 * (6 * nb * 33 + 3 * nb * 32 + nb * 32);   // pair-side slots [6 nb][33], aux-side slots, scales
 }

@@ -6,6 +6,7 @@
 #include "ris_boys_table.h"
 #include <cstring>
 #include <map>
+#include <vector>
 
 static std::map<int, std::vector<double>> g_tabs;
 static const double* tab(int M)
@@ -55,16 +56,10 @@ static void phase_t(int nk, const double* prim, bool hostA, const double* Z, con
                                  Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac, tab(K::E), acc);
     }
     if (!used) return;
-    // the kernels instantiate NB = 1..4 states per launch; the harness contracts one state at a time
-    for (int s = 0; s < nb; ++s) {
-        const double sc[1] = {1.0};
-        double gh[1][3] = {{0.0, 0.0, 0.0}}, go[1][3] = {{0.0, 0.0, 0.0}};
-        ris_hrrc<LH, LO, TR, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile + (size_t)s * (K::NCA * K::NCB), (size_t)1,
-                                (size_t)(K::NCA * K::NCB), sc, gh, go);
-        double* o = out + 6 * s + (hostA ? 0 : 3);
-        double* oo = out + 6 * s + (hostA ? 3 : 0);
-        for (int x = 0; x < 3; ++x) { o[x] += gh[0][x]; oo[x] += go[0][x]; }
-    }
+    // slots as in the class kernel: slot[(s*6 + c)*SL], c = 0..2 centre A, 3..5 centre B (stride SL = 1 here), unit scales
+    std::vector<double> sc((size_t)nb, 1.0);
+    ris_hrrc<LH, LO, TR, 1, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)(K::NCA * K::NCB), nb,
+                               sc.data(), out);
 }
 
 template <int LA, int LB>
