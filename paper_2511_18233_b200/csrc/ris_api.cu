@@ -72,7 +72,7 @@ struct ris_ctx {
     std::vector<cudaEvent_t> ev_pool;
 };
 
-enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_N = 10 };
+enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9, WS_N = 10 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -317,7 +317,8 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             pk.npairs = meta[k];
             pk.kmax = meta[2 * RIS_NBIN + k];
             pk.nprim = (long long)nprim_c[k];
-            pk.ntasks = (int)((pk.nprim + RIS_TASK_PRIMS - 1) / RIS_TASK_PRIMS);
+            pk.task_prims = ris_task_prims(la, lb);
+            pk.ntasks = (int)((pk.nprim + pk.task_prims - 1) / pk.task_prims);
             pk.elem_off = off;
             off += (long long)ris_ncart(la) * ris_ncart(lb) * pk.npairs;
             c->nprim_surv += pk.nprim;
@@ -331,7 +332,7 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             if ((rc = dev_alloc(c, &pk.task_begin, (size_t)pk.ntasks + 1, false))) return rc;
             ProfScope ps(c, "ris_k_pair_pack");
             ris_k_scan_nk<<<1, 1024, 0, c->stream>>>(pk.npairs, d_sorted + meta[RIS_NBIN + k], d_packed, pk.prim_off);
-            ris_k_task_bounds<<<(pk.ntasks + 1 + 127) / 128, 128, 0, c->stream>>>(pk.npairs, pk.ntasks, pk.prim_off, pk.task_begin);
+            ris_k_task_bounds<<<(pk.ntasks + 1 + 127) / 128, 128, 0, c->stream>>>(pk.npairs, pk.ntasks, pk.task_prims, pk.prim_off, pk.task_begin);
             ris_k_pair_pack<<<(pk.npairs + 127) / 128, 128, 0, c->stream>>>(m, pk, d_sorted + meta[RIS_NBIN + k]);
         }
     c->nelem_real = off;
@@ -445,11 +446,16 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
 static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long estride, int lstride,
                           const double* cscale, int nb, int p0, int p1, double* grad, unsigned long long* det)
 {
+    const int ny = (p1 - p0 + 31) / 32;
+    int* ctr;
+    { int rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)RIS_NCLASS * ny, (void**)&ctr); if (rc) return rc; }
+    CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)RIS_NCLASS * ny, c->stream));
     for (int oi = 0; oi < RIS_NCLASS; ++oi) {
         const int k = kClassOrder[oi];
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
         RisGradParams p{};
+        p.task_ctr = ctr + (size_t)k * ny;
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
         p.tile = tile; p.sstride = sstride; p.estride = estride; p.lstride = lstride; p.cscale = cscale; p.nb = nb;
         p.p0 = p0; p.p1 = p1;

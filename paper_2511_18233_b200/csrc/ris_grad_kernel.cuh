@@ -47,9 +47,26 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
     ris_hrrc<LH, LO, TR, 33, 32>(acc, ZOx, ZOy, ZOz, tile, estride, sstride, nb, sc, slot);
 }
 
+template <int NEL>
+RIS_DEV void ris_prefetch_tile(const double* t, size_t estride, size_t sstride, int nb, int lstride)
+{
+    const int rows = lstride ? NEL : (NEL + 15) / 16;
+    const size_t step = lstride ? estride : 16;
+    for (int s = 0; s < nb; ++s)
+        for (int e = 0; e < rows; ++e) asm volatile("prefetch.global.L1 [%0];" ::"l"(t + (size_t)s * sstride + (size_t)e * step));
+}
+
 // resident blocks per SM the register allocation aims at (light classes: latency-bound prefactor / Boys chains
 // want warps; heavy classes: the contracted targets want registers)
-template <int LA, int LB> struct RisGradTune { static constexpr int MINB = (LA + LB <= 1) ? 4 : (LA + LB == 2 ? 3 : 2); };
+#ifndef RIS_MB1
+#define RIS_MB1 4
+#define RIS_MB2 3
+#define RIS_MB3 2
+#define RIS_MB4 2
+#endif
+template <int LA, int LB> struct RisGradTune {
+    static constexpr int MINB = (LA + LB <= 1) ? RIS_MB1 : (LA + LB == 2 ? RIS_MB2 : (LA + LB == 3 ? RIS_MB3 : RIS_MB4));
+};
 
 template <int LA, int LB>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
@@ -104,9 +121,16 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
         __syncwarp();
     };
 
-    for (int task = blockIdx.x * RIS_GRAD_WARPS + warp; task < pk.ntasks; task += gridDim.x * RIS_GRAD_WARPS) {
+    // Tasks are handed out by an atomic ticket counter per aux chunk; the ticket for the NEXT task is drawn before the
+    // current one starts, so its latency is hidden.  Every warp ends within one task of the others, and a block that
+    // becomes resident late finds the counter exhausted and leaves.
+    int task = 0;
+    if (lane == 0) task = atomicAdd(prm.task_ctr + blockIdx.y, 1);
+    task = __shfl_sync(0xffffffffu, task, 0);
+    while (task < pk.ntasks) {
+        int next = 0;
+        if (lane == 0) next = atomicAdd(prm.task_ctr + blockIdx.y, 1);
         const int ip0 = pk.task_begin[task], ip1 = pk.task_begin[task + 1];
-        if (ip1 <= ip0) continue;
         const long long q0 = pk.prim_off[ip0], q1 = pk.prim_off[ip1];
         __syncwarp();
         {   // stage the task: 16-byte copies, 4 per record
@@ -126,6 +150,11 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
             if (pr.atA != curA || pr.atB != curB) { flush(); curA = pr.atA; curB = pr.atB; }
             const double* __restrict__ tile = tile_lane + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * estride;
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
+#ifdef RIS_PREFETCH_TILE   // measured on config 4: no gain (7.6 -> 7.9 ms/step), kept for experiments
+            // the NEXT pair's tile rows start their way from HBM / L2 to L1 while this pair's primitives run
+            // (K: one 256-byte row per element and state across the warp; J: the pair's few contiguous lines)
+            if (ip0 + j + 1 < pk.npairs) ris_prefetch_tile<NEL>(tile + (size_t)NEL * estride, estride, sstride, nb, prm.lstride);
+#endif
             if (pr.nkA > 0)
                 ris_phase<LA, LB, false>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
                                          estride, sstride, nb, s_sc + lane, s_red + lane);
@@ -135,6 +164,18 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
                                         auxfac, prm.boys, tile, estride, sstride, nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
+        if (prm.det != nullptr) {
+            // deterministic mode: which warp runs which task varies from run to run, so every task hands over its own
+            // sums (integer atomics: exact, order-independent) instead of carrying FP64 partial sums into the next task
+            flush();
+            curA = curB = -1;
+            if (live)
+                for (int i = 0; i < 3 * nb; ++i) {
+                    ris_grad_add(prm, ((size_t)(i / 3) * prm.natoms + P) * 3 + (i % 3), s_gaux[i * 32 + lane]);
+                    s_gaux[i * 32 + lane] = 0.0;
+                }
+        }
+        task = __shfl_sync(0xffffffffu, next, 0);
     }
     flush();
 
@@ -162,10 +203,12 @@ void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
         cudaFuncSetAttribute(ris_grad_kernel<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
-    // blockIdx.y: chunks of 32 aux functions; blockIdx.x: enough blocks for ~4 waves of the resident blocks, each warp
-    // striding over the tasks (fewer, longer-lived warps = fewer aux-side atomics)
+    // blockIdx.y: chunks of 32 aux functions; blockIdx.x: the blocks of a chunk, together one resident wave of
+    // long-lived warps drawing tasks (few aux-side atomics, no wave quantisation)
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
-    const int nx = std::max(1, std::min(nbt, (148 * RisGradTune<LA, LB>::MINB * 4 + ny - 1) / ny));
+    static int nsm = 0;
+    if (nsm == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
+    const int nx = std::max(1, std::min(nbt, (nsm * RisGradTune<LA, LB>::MINB + ny - 1) / ny));
     ris_grad_kernel<LA, LB><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
 }

@@ -9,11 +9,14 @@ constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a
 constexpr int RIS_GRAD_WARPS = 4;       // warps per class-kernel block
 constexpr int RIS_GRAD_THREADS = 32 * RIS_GRAD_WARPS;
 constexpr int RIS_TASK_PRIMS = 32;      // a warp task = the shell pairs whose first primitive pair falls in one window of
-                                        // this many packed primitive pairs (so a task holds < RIS_TASK_PRIMS + kmax of them)
+                                        // ris_task_prims(class) <= RIS_TASK_PRIMS packed primitive pairs (so a task holds
+                                        // fewer than window + kmax of them)
 constexpr int RIS_NB_MAX = 5;           // states per class-kernel launch (per-state gradient slots in shared memory)
 
 __host__ __device__ inline int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
 __host__ __device__ inline int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
+// task window by class weight: a (d,d) primitive triplet costs ~10x an (s,s) one, and a task should stay ~10-20 us
+__host__ __device__ inline int ris_task_prims(int la, int lb) { return la + lb <= 2 ? 32 : (la + lb <= 3 ? 16 : 8); }
 
 // One packed shell pair (64 bytes, read by a whole warp as a broadcast).
 struct __align__(16) RisPairRec {
@@ -31,7 +34,8 @@ struct RisClassPack {
     int npairs;            // surviving shell pairs
     int kmax;              // max surviving primitive pairs per shell pair
     long long nprim;       // surviving primitive pairs in the class
-    int ntasks;            // warp tasks (windows of RIS_TASK_PRIMS primitive pairs)
+    int ntasks;            // warp tasks (windows of task_prims primitive pairs)
+    int task_prims;
     RisPairRec* pairs;     // [npairs]
     int* ao;               // [2][npairs]  first AO of mu, first AO of nu
     float* symf;           // [npairs]     1 (mu != nu shell) or 0.5 (same shell): folds D + D^T onto unique pairs
@@ -56,6 +60,7 @@ struct RisGradParams {
     const double* cscale;    // J: c_aux[nb][naux]; K: nullptr
     int nb;
     int p0, p1;              // aux range of this launch; blockIdx.y selects 32 of them, one per lane
+    int* task_ctr;           // [chunks of 32 aux] zeroed ticket counters of this launch (dynamic task hand-out)
     double* grad;            // [nb][natoms][3], accumulated with atomics
     unsigned long long* det; // deterministic mode: [nb][natoms][3][2] fixed-point accumulators (hi, lo), else nullptr
     int* det_flag;           // set to 1 when a contribution leaves the fixed-point range

@@ -153,12 +153,12 @@ __global__ void __launch_bounds__(1024) ris_k_scan_nk(int n, const long long* li
     }
 }
 
-// task_begin[t] = first pair whose first primitive-pair record is >= t * RIS_TASK_PRIMS  (t = 0 .. ntasks)
-__global__ void ris_k_task_bounds(int npairs, int ntasks, const long long* prim_off, int* task_begin)
+// task_begin[t] = first pair whose first primitive-pair record is >= t * task_prims  (t = 0 .. ntasks)
+__global__ void ris_k_task_bounds(int npairs, int ntasks, int task_prims, const long long* prim_off, int* task_begin)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t > ntasks) return;
-    const long long target = (long long)t * RIS_TASK_PRIMS;
+    const long long target = (long long)t * task_prims;
     int lo = 0, hi = npairs;             // first ip in [0, npairs] with prim_off[ip] >= target
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
