@@ -64,6 +64,12 @@ struct ris_ctx {
     int nblk = 0, ntiles = 0;
     int2* d_tiles = nullptr;           // [ntiles] (I, J)
     int* d_tmap = nullptr;             // [nblk][nblk] tile index of (I >= J), -1 if absent
+    // inverse map for the P-minor tile transpose: S position -> packed element
+    int* d_smap = nullptr;             // [ntiles][64][64]  (packed element << 1 | same-shell pair), -1 if no surviving element
+    int* d_srows = nullptr;            // [nsrows] rows (tile * 64 + r) of the block buffer that hold a surviving element
+    int nsrows = 0;
+    int* d_ovf = nullptr;              // [novf][2] (element code, S position) of the elements that share an S position
+    int novf = 0;
     // grow-only scratch
     void* ws[10] = {nullptr};
     size_t ws_bytes[10] = {0};
@@ -174,6 +180,40 @@ __global__ void ris_k_mark_blocks(RisClassPack pk, const int* __restrict__ ao_po
     const int r1 = r0 + ris_ncart(pk.la) - 1, q1 = q0 + ris_ncart(pk.lb) - 1;
     for (int I = r0 / RIS_GTILE2; I <= r1 / RIS_GTILE2; ++I)
         for (int J = q0 / RIS_GTILE2; J <= q1 / RIS_GTILE2; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
+}
+
+// Inverse map of the packed pair elements into the GEMM-2 block buffer: element (ip, ca, cb) of a class reads
+// S^P[pos(mu0+ca)][pos(nu0+cb)] (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
+__global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos, const int* __restrict__ tmap, int nblk,
+                                 int* __restrict__ smap, int* __restrict__ rowflag, int* __restrict__ ovf, int* __restrict__ novf)
+{
+    constexpr int T = RIS_GTILE2;
+    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)pk.npairs * nel) return;
+    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
+    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
+    if (r / T < q / T) { const int t = r; r = q; q = t; }
+    const int tile = tmap[(r / T) * nblk + (q / T)];
+    const int code = (int)(((pk.elem_off + idx) << 1) | (pk.symf[ip] < 0.75f ? 1 : 0));
+    const size_t pos = (size_t)tile * (T * T) + (r % T) * T + (q % T);
+    // elements (ca,cb) and (cb,ca) of a same-shell pair that straddles a block edge fold onto ONE position of the
+    // symmetric S: the second one goes to a short overflow list served by a gather
+    if (atomicCAS(&smap[pos], -1, code) != -1) {
+        const int k = atomicAdd(novf, 1);
+        ovf[2 * k] = code; ovf[2 * k + 1] = (int)pos;
+        return;
+    }
+    rowflag[tile * T + (r % T)] = 1;
+}
+
+// overflow elements of ris_k_build_smap: out[el * pbp + P] = symf * S^P[pos]
+__global__ void ris_k_pack_sym_ovf(int novf, const int* __restrict__ ovf, int np, int pbp, const double* __restrict__ S,
+                                   long long sstrideP, double* __restrict__ out)
+{
+    const int k = blockIdx.x, code = ovf[2 * k], pos = ovf[2 * k + 1];
+    for (int P = threadIdx.x; P < np; P += blockDim.x)
+        out[(size_t)(code >> 1) * pbp + P] = ((code & 1) ? 0.5 : 1.0) * S[(size_t)P * sstrideP + pos];
 }
 
 // Morton (Z-order) code of a point on a 3-bohr grid: the spatial AO order that keeps the surviving pairs of an
@@ -375,6 +415,27 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         c->ntiles = (int)tiles.size();
         if ((rc = dev_upload(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
         if ((rc = dev_upload(c, &c->d_tmap, mark.data(), mark.size()))) return rc;
+        // inverse element map + active-row list of the block buffer (for the P-minor transpose of the K tiles)
+        int *d_rowflag, *d_novf;
+        if ((rc = dev_alloc(c, &c->d_ovf, (size_t)2 * std::max<long long>(c->nelem_real, 1), false))) return rc;
+        if ((rc = dev_alloc(c, &d_novf, 1, true))) return rc;
+        if ((rc = dev_alloc(c, &c->d_smap, (size_t)std::max(c->ntiles, 1) * RIS_GTILE2 * RIS_GTILE2, false))) return rc;
+        if ((rc = dev_alloc(c, &d_rowflag, (size_t)std::max(c->ntiles, 1) * RIS_GTILE2, true))) return rc;
+        CU(cudaMemsetAsync(c->d_smap, 0xff, sizeof(int) * (size_t)std::max(c->ntiles, 1) * RIS_GTILE2 * RIS_GTILE2, c->stream));
+        for (int k = 0; k < RIS_NCLASS; ++k) {
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+            ris_k_build_smap<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, c->d_tmap, c->nblk, c->d_smap, d_rowflag, c->d_ovf, d_novf);
+        }
+        CU(cudaGetLastError());
+        std::vector<int> rowflag((size_t)c->ntiles * RIS_GTILE2), srows;
+        CU(cudaMemcpyAsync(rowflag.data(), d_rowflag, rowflag.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(&c->novf, d_novf, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        for (size_t i = 0; i < rowflag.size(); ++i) if (rowflag[i]) srows.push_back((int)i);
+        c->nsrows = (int)srows.size();
+        if ((rc = dev_upload(c, &c->d_srows, srows.data(), srows.size()))) return rc;
         CU(cudaStreamSynchronize(c->stream));      // host vectors go out of scope
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -534,31 +595,25 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
 }
 
 // --------------------------------------------------------------------------------------- K
-// K tiles, P-minor: out[(elem_off + ip*nel + e) * pbp + P] = symf[ip] * S^P[pos(mu0+ca)][pos(nu0+cb)] read from the block
-// buffer of GEMM-2 (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).  threadIdx.x runs over P (the
-// contiguous output index: a warp writes 256 bytes), threadIdx.y over 8 consecutive elements (neighbours in S).
-__global__ void __launch_bounds__(256) ris_k_pack_sym(RisClassPack pk, int np, int pbp, const double* __restrict__ S, long long sstrideP,
-                                                      const int* __restrict__ ao_pos, const int* __restrict__ tmap, int nblk,
+// K tiles, P-minor: out[el * pbp + P] = symf * S^P[position of el], a transpose through shared memory: one block takes
+// one row (64 doubles) of one S block for 32 aux functions -- 32 coalesced 512-byte reads -- and writes, for every
+// surviving element of the row, its 32 consecutive P values (256 bytes).
+__global__ void __launch_bounds__(256) ris_k_pack_sym(int np, int pbp, const double* __restrict__ S, long long sstrideP,
+                                                      const int* __restrict__ srows, const int* __restrict__ smap,
                                                       double* __restrict__ out)
 {
     constexpr int T = RIS_GTILE2;
-    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
-    const long long idx = (long long)blockIdx.x * 8 + threadIdx.y;
-    if (idx >= (long long)pk.npairs * nel) return;
-    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
-    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
-    if (r / T < q / T) { const int t = r; r = q; q = t; }
-    const int tile = tmap[(r / T) * nblk + (q / T)];
-    const double* src = S + (size_t)tile * (T * T) + (r % T) * T + (q % T);
-    double* dst = out + ((size_t)pk.elem_off + (size_t)idx) * pbp;
-    const double f = (double)pk.symf[ip];
-    // four strided gathers in flight per thread (the reads are 8 bytes out of a 32-byte sector each)
-    for (int P = threadIdx.x; P < np; P += 128) {
-        double v[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) v[u] = (P + 32 * u < np) ? __ldg(src + (size_t)(P + 32 * u) * sstrideP) : 0.0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) if (P + 32 * u < np) dst[P + 32 * u] = f * v[u];
+    __shared__ double sm[32][T + 1];
+    const int row = srows[blockIdx.x], P0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & (T - 1), ty = threadIdx.x / T;              // 64 x 4
+    const double* src = S + (size_t)row * T + tx;
+    for (int pl = ty; pl < 32; pl += 4) sm[pl][tx] = (P0 + pl < np) ? src[(size_t)(P0 + pl) * sstrideP] : 0.0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (P0 + lane >= np) return;
+    for (int q = w; q < T; q += 8) {
+        const int m = smap[(size_t)row * T + q];
+        if (m >= 0) out[(size_t)(m >> 1) * pbp + P0 + lane] = ((m & 1) ? 0.5 : 1.0) * sm[lane][q];
     }
 }
 
@@ -638,13 +693,12 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                     CU(ris_gemm_blocks(c->stream, g, np, c->ntiles));
                 }
                 double* out = tile + (size_t)s * pbp * c->nelem_real;
-                for (int k = 0; k < RIS_NCLASS; ++k) {
-                    const RisClassPack& pk = c->cls[k];
-                    if (pk.npairs == 0) continue;
-                    const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
-                    ProfScope ps(c, "ris_k_pack_sym", (double)nelc * np, 16.0 * nelc * np);
-                    ris_k_pack_sym<<<(unsigned)((nelc + 7) / 8), dim3(32, 8), 0, c->stream>>>(
-                        pk, np, pbp, S, (long long)c->ntiles * blk, c->d_ao_pos, c->d_tmap, c->nblk, out);
+                {
+                    ProfScope ps(c, "ris_k_pack_sym", (double)c->nelem_real * np, 8.0 * np * ((double)c->nsrows * RIS_GTILE2 + (double)c->nelem_real));
+                    ris_k_pack_sym<<<dim3(c->nsrows, (np + 31) / 32), 256, 0, c->stream>>>(np, pbp, S, (long long)c->ntiles * blk,
+                                                                                        c->d_srows, c->d_smap, out);
+                    if (c->novf > 0)
+                        ris_k_pack_sym_ovf<<<c->novf, 64, 0, c->stream>>>(c->novf, c->d_ovf, np, pbp, S, (long long)c->ntiles * blk, out);
                 }
                 CU(cudaGetLastError());
             }
