@@ -30,6 +30,10 @@ if ROOT not in sys.path:
 
 METRIC = "TDDFT-ris gradient ms/state"
 UNIT = "ms/state"
+# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/r01_v5_ncu.md);
+# None where no capture of that (config, kernel) is committed.
+NCU_TRAFFIC = {(4, "ris_gemm_dmma(HT=Cvir*B^T)"): 1.434842e9 + 3.779255e9}
+
 ORACLE_CUTOFF = {4: 1e-22}      # the oracle's documented primitive cutoff on config 4
 
 
@@ -206,8 +210,10 @@ def run_ours(args):
     achieved = dom["flops"] / (dom["ms"] * 1e-3) * 1e-12 if dom["ms"] > 0 else 0.0
     roofline = {"kernel": dom_name, "bound": "tensor" if is_gemm else "alu", "achieved": round(achieved, 3),
                 "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4) if peak else None,
-                "traffic": None, "launches": dom["launches"], "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
+                "traffic": NCU_TRAFFIC.get((args.config, dom_name)), "launches": dom["launches"], "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
                 "share_of_kernel_time": round(dom["ms"] / ksum, 4),
+                "traffic_unit": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum (profiles/r01_v5_ncu.md)",
+                "algorithmic_bytes_per_launch": round(dom["bytes"] / dom["launches"]),
                 "peak_source": ("measured in this run by ris_probe_fp64_mma_peak (mma.sync f64 chains)" if is_gemm else
                                 "measured in this run by ris_probe_fp64_peak (independent DFMA chains)")
                                + "; MEASURED_PEAKS.json carries no FP64 figure"}
