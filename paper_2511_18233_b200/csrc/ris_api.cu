@@ -509,14 +509,15 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
 {
     const int ny = (p1 - p0 + 31) / 32;
     int* ctr;
-    { int rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)RIS_NCLASS * ny, (void**)&ctr); if (rc) return rc; }
-    CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)RIS_NCLASS * ny, c->stream));
+    // two ticket arrays per class: the heavy classes run their host-centre phases as two launches
+    { int rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr); if (rc) return rc; }
+    CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
     for (int oi = 0; oi < RIS_NCLASS; ++oi) {
         const int k = kClassOrder[oi];
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
         RisGradParams p{};
-        p.task_ctr = ctr + (size_t)k * ny;
+        p.task_ctr = ctr + (size_t)2 * k * ny;
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
         p.tile = tile; p.sstride = sstride; p.estride = estride; p.lstride = lstride; p.cscale = cscale; p.nb = nb;
         p.p0 = p0; p.p1 = p1;

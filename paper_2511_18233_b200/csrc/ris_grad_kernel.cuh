@@ -64,11 +64,18 @@ RIS_DEV void ris_prefetch_tile(const double* t, size_t estride, size_t sstride, 
 #define RIS_MB3 2
 #define RIS_MB4 2
 #endif
+// SPLIT: the heavy classes (l_mu + l_nu >= 4) run their two host-centre phases as two launches (PH = 1: primitive pairs
+// hosted on A, PH = 2: hosted on B; PH = 0: both in one kernel).  With both phases inlined the (2,2) kernel is 94 KB of
+// SASS and stalls on instruction fetch (profiles/r01_v5_ncu.md: no_instruction 7.1 cycles per issue); one phase is 47 KB.
+#ifndef RIS_SPLIT_L
+#define RIS_SPLIT_L 4
+#endif
 template <int LA, int LB> struct RisGradTune {
     static constexpr int MINB = (LA + LB <= 1) ? RIS_MB1 : (LA + LB == 2 ? RIS_MB2 : (LA + LB == 3 ? RIS_MB3 : RIS_MB4));
+    static constexpr bool SPLIT = (LA + LB >= RIS_SPLIT_L);
 };
 
-template <int LA, int LB>
+template <int LA, int LB, int PH>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
 {
     constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
@@ -155,11 +162,11 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
             // (K: one 256-byte row per element and state across the warp; J: the pair's few contiguous lines)
             if (ip0 + j + 1 < pk.npairs) ris_prefetch_tile<NEL>(tile + (size_t)NEL * estride, estride, sstride, nb, prm.lstride);
 #endif
-            if (pr.nkA > 0)
+            if (PH != 2 && pr.nkA > 0)
                 ris_phase<LA, LB, false>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
                                          estride, sstride, nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
-            if (pr.nkB > 0)
+            if (PH != 1 && pr.nkB > 0)
                 ris_phase<LB, LA, true>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz, alpha,
                                         auxfac, prm.boys, tile, estride, sstride, nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
@@ -193,14 +200,13 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
     }
 }
 
-template <int LA, int LB>
-void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
+template <int LA, int LB, int PH>
+void ris_launch_grad_phase(const RisGradParams& p, cudaStream_t st)
 {
-    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
     const size_t smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.kmax, p.nb);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(ris_grad_kernel<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(ris_grad_kernel<LA, LB, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
     // blockIdx.y: chunks of 32 aux functions; blockIdx.x: the blocks of a chunk, together one resident wave of
@@ -210,5 +216,20 @@ void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
     static int nsm = 0;
     if (nsm == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
     const int nx = std::max(1, std::min(nbt, (nsm * RisGradTune<LA, LB>::MINB + ny - 1) / ny));
-    ris_grad_kernel<LA, LB><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    ris_grad_kernel<LA, LB, PH><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+}
+
+// p.task_ctr holds two zeroed ticket arrays of ny counters each (one per phase launch)
+template <int LA, int LB>
+void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
+{
+    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
+    if constexpr (RisGradTune<LA, LB>::SPLIT) {
+        RisGradParams q = p;
+        ris_launch_grad_phase<LA, LB, 1>(q, st);
+        q.task_ctr = p.task_ctr + (p.p1 - p.p0 + 31) / 32;
+        ris_launch_grad_phase<LA, LB, 2>(q, st);
+    } else {
+        ris_launch_grad_phase<LA, LB, 0>(p, st);
+    }
 }
