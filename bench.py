@@ -261,7 +261,7 @@ def run_ours(args):
         e2e = {"value": round(t_e2e / (world * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
                "how": "ris_grad_{J,K,PQ}_host on pinned host buffers; host wall clock around the calls (they return "
-                      "after the D2H copy of the gradient)"}
+                      "after the D2H copy of the gradient); B goes up in P chunks on a copy stream, GEMM-1 follows chunk by chunk"}
 
     line = {
         "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -102,7 +102,9 @@ int ris_grad_K(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ
 int ris_grad_PQ(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
 
 /* The same three calls on HOST buffers: host->device copies, the kernels, and the device->host copy of
- * the gradient all happen inside the call, which returns when grad (host) is complete. */
+ * the gradient all happen inside the call, which returns when grad (host) is complete.  Pinned (page-locked) host
+ * buffers let ris_grad_K_host stream B up in ranges of P on a second stream while the Gamma^P GEMMs of the
+ * ranges already resident run; pageable buffers are accepted and simply copy synchronously. */
 int ris_grad_J_host(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, double* grad);
 int ris_grad_K_host(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                     const double* B, double* grad);

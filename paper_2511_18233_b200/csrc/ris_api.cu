@@ -71,6 +71,9 @@ struct ris_ctx {
     int* d_ovf = nullptr;              // [novf][2] (element code, S position) of the elements that share an S position
     int novf = 0;
     // grow-only scratch
+    cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
+    std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
+    cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
     void* ws[10] = {nullptr};
     size_t ws_bytes[10] = {0};
     int last_pbatch = 0;
@@ -450,6 +453,9 @@ extern "C" int ris_destroy(ris_ctx* c)
     cudaStreamSynchronize(c->stream);
     for (void* p : c->owned) cudaFree(p);
     for (int i = 0; i < WS_N; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
+    for (cudaEvent_t e : c->copy_ev) cudaEventDestroy(e);
+    if (c->copy_gate) cudaEventDestroy(c->copy_gate);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     ris_profile_reset(c);
     delete c;
     return RIS_OK;
@@ -628,8 +634,12 @@ __global__ void ris_k_pad_rows(int rows, int cols, int ld, const int* __restrict
     out[i] = cidx < cols ? in[(size_t)order[r] * cols + cidx] : 0.0;
 }
 
-extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
-                          const double* B, double* grad)
+// b_ready (nullable): b_ready[s * RIS_COPY_CHUNKS + ch] is recorded (on another stream) once chunk ch (a range of P) of
+// B of state s is resident; the compute stream waits for it right before that chunk's GEMM-1, so the H2D copy runs
+// ahead of the GEMMs instead of in front of them.
+constexpr int RIS_COPY_CHUNKS = 4;     // *_host: B of a state goes up in this many P ranges, GEMM-1 follows chunk by chunk
+static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                       const double* B, double* grad, const cudaEvent_t* b_ready)
 {
     if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
@@ -672,14 +682,23 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
             const long long ldh = (long long)pb * noccp;
             for (int s = 0; s < nb; ++s) {
                 const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
-                {   // GEMM-1: HT[nu][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]
+                // GEMM-1: HT[nu][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]; with b_ready, in RIS_COPY_CHUNKS column chunks
+                // (ranges of P), each waiting only for its own slice of B
+                const int nch = (b_ready && p0 == 0 && np == naux) ? RIS_COPY_CHUNKS : 1;
+                for (int ch = 0; ch < nch; ++ch) {
+                    const int q0 = (int)((long long)np * ch / nch), q1 = (int)((long long)np * (ch + 1) / nch);
+                    if (q1 <= q0) continue;
+                    if (b_ready) {
+                        if (nch > 1) CU(cudaStreamWaitEvent(c->stream, b_ready[(s0 + s) * RIS_COPY_CHUNKS + ch], 0));
+                        else if (p0 == 0) CU(cudaStreamWaitEvent(c->stream, b_ready[(s0 + s) * RIS_COPY_CHUNKS + RIS_COPY_CHUNKS - 1], 0));
+                    }
                     RisGemmParams g{};
-                    g.seg[0] = RisGemmSeg{C_vir, nvir, 0, Bs, nvir, 0, nvir};
-                    g.nseg = 1; g.M = nao; g.N = np * nocc; g.C = HT; g.ldc = ldh; g.bsC = 0;
+                    g.seg[0] = RisGemmSeg{C_vir, nvir, 0, Bs + (size_t)q0 * nocc * nvir, nvir, 0, nvir};
+                    g.nseg = 1; g.M = nao; g.N = (q1 - q0) * nocc; g.C = HT + (size_t)q0 * noccp; g.ldc = ldh; g.bsC = 0;
                     g.rowsA = c->d_ao_order;                  // HT rows in spatial order
                     g.cdiv = (noccp != nocc) ? nocc : 0; g.cpad = noccp;
-                    ProfScope ps(c, "ris_gemm_dmma(HT=Cvir*B^T)", 2.0 * np * nocc * (double)nao * nvir,
-                                 8.0 * ((double)np * nocc * nvir + (double)nao * nvir + (double)np * nocc * nao));
+                    ProfScope ps(c, "ris_gemm_dmma(HT=Cvir*B^T)", 2.0 * (q1 - q0) * nocc * (double)nao * nvir,
+                                 8.0 * ((double)(q1 - q0) * nocc * nvir + (double)nao * nvir + (double)(q1 - q0) * nocc * nao));
                     CU(ris_gemm_dense(c->stream, g, 1));
                 }
                 {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 64x64 blocks
@@ -709,6 +728,12 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
         }
     }
     return det_end(c, nbatch, det, grad);
+}
+
+extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                          const double* B, double* grad)
+{
+    return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B, grad, nullptr);
 }
 
 // --------------------------------------------------------------------------------------- PQ (S5)
@@ -795,11 +820,35 @@ extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const
     double *dCo, *dCv, *dB, *dg;
     int rc;
     const size_t ng = (size_t)nbatch * c->natoms * 3;
-    if ((rc = h2d(c, WS_IN0, B, (size_t)nbatch * c->naux * nocc * nvir, &dB))) return rc;
+    // B (the bulk of the input: naux*nocc*nvir doubles per state) goes up state by state on a second stream, each
+    // state's GEMMs waiting only for their own slice: the PCIe transfer of state s+1 hides behind the GEMMs of state s.
+    // The small operands go first: the H2D copy engine serves transfers in issue order across streams.
     if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
     if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    const size_t nB = (size_t)c->naux * nocc * nvir;
+    if ((rc = ws_get(c, WS_IN0, nbatch * nB * sizeof(double), (void**)&dB))) return rc;
+    if (!c->copy_stream) CU(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    if (!c->copy_gate) CU(cudaEventCreateWithFlags(&c->copy_gate, cudaEventDisableTiming));
+    while ((int)c->copy_ev.size() < nbatch * RIS_COPY_CHUNKS) {
+        cudaEvent_t e;
+        CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        c->copy_ev.push_back(e);
+    }
+    CU(cudaEventRecord(c->copy_gate, c->stream));                 // earlier readers of the staging buffer are done
+    CU(cudaStreamWaitEvent(c->copy_stream, c->copy_gate, 0));
+    for (int s = 0; s < nbatch; ++s)
+        for (int ch = 0; ch < RIS_COPY_CHUNKS; ++ch) {
+            const size_t q0 = (size_t)((long long)c->naux * ch / RIS_COPY_CHUNKS) * nocc * nvir;
+            const size_t q1 = (size_t)((long long)c->naux * (ch + 1) / RIS_COPY_CHUNKS) * nocc * nvir;
+            if (q1 > q0)
+                CU(cudaMemcpyAsync(dB + s * nB + q0, B + s * nB + q0, (q1 - q0) * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream));
+            CU(cudaEventRecord(c->copy_ev[s * RIS_COPY_CHUNKS + ch], c->copy_stream));
+        }
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
-    if ((rc = ris_grad_K(c, nbatch, nocc, nvir, dCo, dCv, dB, dg))) return rc;
+    if ((rc = grad_K_impl(c, nbatch, nocc, nvir, dCo, dCv, dB, dg, c->copy_ev.data()))) {
+        cudaStreamSynchronize(c->copy_stream);
+        return rc;
+    }
     return d2h_grad(c, dg, grad, ng);
 }
 
