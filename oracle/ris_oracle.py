@@ -197,3 +197,57 @@ def grad_PQ(mol, c_aux, d_aux):
     e = np.zeros(nb, dtype=np.longdouble)
     lib().ris_oracle_grad_PQ(C.byref(h.c), nb, c_aux.ctypes.data, d_aux.ctypes.data, g.ctypes.data, e.ctypes.data)
     return g.astype(np.float64), e.astype(np.float64)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1: the J-type fitting step either side of the derivative path, Eqs. 21-22
+# with the Coulomb pairing of Eq. 21's first term:
+#   v_P   = sum_{mu nu} D_{mu nu} (mu nu|P)                        (undifferentiated three-centre contraction)
+#   M_PQ  = (P|Q)  with N_P N_Q                                    (Eq. 22)
+#   c     = M^-1 v                                                 (numpy.linalg.solve: a library step)
+#   E_RIJ = 1/2 v^T M^-1 v = 1/2 sum_{pq,sr} D_pq (pq|A) M^-1_AB (B|sr) D_sr
+# and, for fixed symmetric-or-not D, Eq. 27 gives
+#   dE_RIJ/dxi = sum_P c_P v_P^xi - 1/2 c^T M^xi c = G_J(D, c) - 1/2 G_PQ(c, c).
+def vec_J(mol, D, *, prim_cutoff=0.0):
+    """v[s][P] = sum_{mu nu} D^s_{mu nu} (mu nu|P) over all ordered (mu, nu)."""
+    h = _Held(mol)
+    D = _f64(D).reshape(-1, h.nao, h.nao)
+    nb = D.shape[0]
+    one = np.ones(nb)
+    v = np.zeros((nb, h.natoms))
+    for P in range(h.natoms):
+        g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
+        e = np.zeros(nb, dtype=np.longdouble)
+        rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, one.ctypes.data, None, prim_cutoff,
+                                         g.ctypes.data, e.ctypes.data)
+        assert rc == 0
+        v[:, P] = e.astype(np.float64)
+    return v
+
+
+def metric(mol):
+    """M[P][Q] = N_P N_Q (P|Q), Eq. 22."""
+    al = _f64(mol.aux_exponents)
+    R = _f64(mol.coords)
+    n = al.shape[0]
+    N = (2.0 * al / np.pi) ** 0.75
+    M = np.zeros((n, n))
+    for P in range(n):
+        for Q in range(n):
+            M[P, Q] = N[P] * N[Q] * prim2c(al[P], al[Q], R[P], R[Q])[0]
+    return M
+
+
+def fit_J(mol, D, *, prim_cutoff=0.0):
+    """(v, c, E_RIJ): c = M^-1 v, E_RIJ[s] = 1/2 v[s].c[s]."""
+    v = vec_J(mol, D, prim_cutoff=prim_cutoff)
+    c = np.linalg.solve(metric(mol), v.T).T
+    return v, c, 0.5 * np.einsum("sp,sp->s", v, c)
+
+
+def grad_RIJ(mol, D, *, prim_cutoff=0.0):
+    """dE_RIJ/dR at fixed D: G_J(D, c) - 1/2 G_PQ(c, c) with the fitted c (Eq. 27)."""
+    _, c, _ = fit_J(mol, D, prim_cutoff=prim_cutoff)
+    gJ, _ = grad_J(mol, D, c, prim_cutoff=prim_cutoff)
+    gQ, _ = grad_PQ(mol, c, c)
+    return gJ - 0.5 * gQ
