@@ -263,6 +263,18 @@ def run_ours(args):
                "how": "ris_grad_{J,K,PQ}_host on pinned host buffers; host wall clock around the calls (they return "
                       "after the D2H copy of the gradient); B goes up in P chunks on a copy stream, GEMM-1 follows chunk by chunk"}
 
+    # ---- NEXT-1 (reported beside the metric, outside the timed step): the J-type fitting step on the same workload
+    ctx.fit_J(d["D"])                                       # builds the metric's Cholesky factor (one-off per geometry)
+    torch.cuda.synchronize()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(3):
+        ctx.fit_J(d["D"])
+    f1.record()
+    torch.cuda.synchronize()
+    fit = {"ris_fit_J_ms_per_state": round(f0.elapsed_time(f1) / 3 / nbJ, 4), "nbatch": nbJ,
+           "what": "v_P = sum D (mu nu|P) on the undifferentiated class kernels + Cholesky solve c = M^-1 v"}
+
     line = {
         "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
@@ -277,7 +289,7 @@ def run_ours(args):
         "gamma_gemm": {"ms_per_step": round(gemm_ms / args.steps, 4),
                        "tflops": round(gemm_fl / (gemm_ms * 1e-3) * 1e-12, 3) if gemm_ms else None,
                        "fp64_mma_peak_tflops": round(mma_peak, 2)},
-        "kernels": kernels, "clocks": clocks,
+        "kernels": kernels, "fit_step": fit, "clocks": clocks,
     }
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:

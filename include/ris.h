@@ -101,6 +101,17 @@ int ris_grad_K(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ
 /* Two-centre term.  c_aux, d_aux device [nbatch][naux], grad device [nbatch][natoms][3]. */
 int ris_grad_PQ(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
 
+/* ---- Fitting step, J type (Eqs. 21-22) --------------------------------
+ * ris_fit_J:   v[s][P] = sum_{mu nu} D^s_{mu nu} (mu nu|P)   (undifferentiated three-centre contraction, all ordered mu nu)
+ *              c[s]    = M^-1 v[s],  M[P][Q] = N_P N_Q (P|Q)  (Cholesky factor built on the device by the first call,
+ *                                                              kept in ctx)
+ *   D device [nbatch][nao][nao] (any symmetry), v_out device [nbatch][naux] or NULL, c_out device [nbatch][naux].
+ *   With these c, for fixed D:  d/dxi (1/2 v^T M^-1 v) = ris_grad_J(D, c) - 1/2 ris_grad_PQ(c, c)   (Eq. 27).
+ *   RIS_EINVAL when the metric is not positive definite (coincident aux centres) or naux > 6144.
+ * ris_metric:  M_out device [naux][naux], row-major, full (symmetric) matrix. */
+int ris_fit_J(ris_ctx* ctx, int nbatch, const double* D, double* v_out, double* c_out);
+int ris_metric(ris_ctx* ctx, double* M_out);
+
 /* The same three calls on HOST buffers: host->device copies, the kernels, and the device->host copy of
  * the gradient all happen inside the call, which returns when grad (host) is complete.  Pinned (page-locked) host
  * buffers let ris_grad_K_host stream B up in ranges of P on a second stream while the Gamma^P GEMMs of the

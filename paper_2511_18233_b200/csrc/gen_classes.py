@@ -91,6 +91,29 @@ class ClassPlan:
                 self.off[(tag, e)] = n
                 n += nc(e)
         self.nacc = n
+        self.fams = [("2a", self.r2a, "a2"), ("2b", self.r2b, "b2"), ("1", self.r1, None)]
+        self.vrr_name = f"ris_vrr_{la}{lb}"
+
+    def acc(self, tag, e, c):
+        return f"acc[{self.off[(tag, e)] + cidx(c)}]"
+
+
+class ClassPlan0:
+    """Undifferentiated integrals (mu nu|P) of one class (the fitting step): the VRR stops at
+    e = la + lb and the contracted targets are the unscaled [e0|s], e = la .. la+lb."""
+
+    def __init__(self, la, lb):
+        self.la, self.lb = la, lb
+        self.E = la + lb
+        self.r0 = list(range(la, self.E + 1))
+        self.off = {}
+        n = 0
+        for e in self.r0:
+            self.off[("0", e)] = n
+            n += nc(e)
+        self.nacc = n
+        self.fams = [("0", self.r0, None)]
+        self.vrr_name = f"ris_vrr0_{la}{lb}"
 
     def acc(self, tag, e, c):
         return f"acc[{self.off[(tag, e)] + cidx(c)}]"
@@ -103,13 +126,13 @@ def gen_vrr(pl: ClassPlan) -> str:
     out = []
     w = out.append
     w(f"// class ({la},{lb}): E={E}, {pl.nacc} contracted targets")
-    w(f"RIS_DEV void ris_vrr_{la}{lb}(const double (&F)[{E + 1}], double PA0, double PA1, double PA2,")
+    w(f"RIS_DEV void {pl.vrr_name}(const double (&F)[{E + 1}], double PA0, double PA1, double PA2,")
     w("    double WP0, double WP1, double WP2, double oo2p, double q, double a2, double b2,")
     w(f"    double (&acc)[{pl.nacc}])")
     w("{")
     PA = ["PA0", "PA1", "PA2"]
     WP = ["WP0", "WP1", "WP2"]
-    emin_target = min([pl.r2b[0]] + (pl.r1[:1] if pl.r1 else []))
+    emin_target = min(rng[0] for _, rng, _ in pl.fams if rng)
     # needed set by backward closure
     need = set()
 
@@ -166,12 +189,13 @@ def gen_vrr(pl: ClassPlan) -> str:
     for e in range(0, E + 1):
         for c in comps(e):
             val = v(e, c, 0)
-            if e in pl.r2a:
-                w(f"    {pl.acc('2a', e, c)} = fma(a2, {val}, {pl.acc('2a', e, c)});")
-            if e in pl.r2b:
-                w(f"    {pl.acc('2b', e, c)} = fma(b2, {val}, {pl.acc('2b', e, c)});")
-            if e in pl.r1:
-                w(f"    {pl.acc('1', e, c)} += {val};")
+            for tag, rng, scale in pl.fams:
+                if e not in rng:
+                    continue
+                if scale:
+                    w(f"    {pl.acc(tag, e, c)} = fma({scale}, {val}, {pl.acc(tag, e, c)});")
+                else:
+                    w(f"    {pl.acc(tag, e, c)} += {val};")
     w("}")
     return "\n".join(out)
 
@@ -249,6 +273,31 @@ def gen_hrrc(pl: ClassPlan) -> str:
     return "\n".join(out)
 
 
+def gen_hrr0c(pl: ClassPlan0) -> str:
+    la, lb = pl.la, pl.lb
+    out = []
+    w = out.append
+    w(f"// contracted undifferentiated triplet of class ({la},{lb}): HRR to (a b|P), dot with the tile of each state:")
+    w("// slot[s*SL] += sum_{ab} tile_s[el] (ab|P).  Tile element order as in ris_hrrc (TR).")
+    w("template <bool TR, int SL>")
+    w(f"RIS_DEV void ris_hrr0c_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
+    w("    const double* __restrict__ tile, size_t estride, size_t sstride, int nb, double* __restrict__ slot)")
+    w("{")
+    done = set()
+    X = gen_hrr_chain(w, pl, "0", la, lb, "x", done)
+    nca, ncb = nc(la), nc(lb)
+    w("    for (int s = 0; s < nb; ++s) {")
+    w("        const double* __restrict__ t = tile + (size_t)s * sstride;")
+    w("        double v = 0.0;")
+    for ia, a in enumerate(comps(la)):
+        for ib, b in enumerate(comps(lb)):
+            w(f"        v = fma(t[(TR ? {ib * nca + ia} : {ia * ncb + ib}) * estride], {X(a, b)}, v);")
+    w("        slot[s * SL] += v;")
+    w("    }")
+    w("}")
+    return "\n".join(out)
+
+
 def generate() -> str:
     parts = ["// GENERATED by gen_classes.py -- do not edit.  See that file for the recurrences.",
              "#pragma once", ""]
@@ -258,6 +307,9 @@ def generate() -> str:
         parts.append(f"template <> struct RisClass<{la},{lb}> {{ static constexpr int E = {pl.E}; "
                      f"static constexpr int NACC = {pl.nacc}; static constexpr int NCA = {nc(la)}; "
                      f"static constexpr int NCB = {nc(lb)}; }};")
+        p0 = ClassPlan0(la, lb)
+        parts.append(f"template <> struct RisClass0<{la},{lb}> {{ static constexpr int E = {p0.E}; "
+                     f"static constexpr int NACC = {p0.nacc}; }};")
     parts.append("")
     for la, lb in classes:
         pl = ClassPlan(la, lb)
@@ -265,10 +317,23 @@ def generate() -> str:
         parts.append("")
         parts.append(gen_hrrc(pl))
         parts.append("")
+        p0 = ClassPlan0(la, lb)
+        parts.append(gen_vrr(p0))
+        parts.append("")
+        parts.append(gen_hrr0c(p0))
+        parts.append("")
     # dispatch helpers
     parts.append("template <int LA, int LB, class... A> RIS_DEV void ris_vrr(A&&... a) {")
     for la, lb in classes:
         parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_vrr_{la}{lb}(static_cast<A&&>(a)...);")
+    parts.append("}")
+    parts.append("template <int LA, int LB, class... A> RIS_DEV void ris_vrr0(A&&... a) {")
+    for la, lb in classes:
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_vrr0_{la}{lb}(static_cast<A&&>(a)...);")
+    parts.append("}")
+    parts.append("template <int LA, int LB, bool TR, int SL, class... A> RIS_DEV void ris_hrr0c(A&&... a) {")
+    for la, lb in classes:
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrr0c_{la}{lb}<TR, SL>(static_cast<A&&>(a)...);")
     parts.append("}")
     parts.append("template <int LA, int LB, bool TR, int SL, int SC, class... A> RIS_DEV void ris_hrrc(A&&... a) {")
     for la, lb in classes:

@@ -57,6 +57,7 @@ struct ris_ctx {
     std::vector<void*> owned;          // every device allocation of the packed data
     long long nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[8] = {nullptr};
+    double* d_chol = nullptr;          // [naux][naux] lower Cholesky factor of the aux metric (built by the first ris_fit_J)
     // Gamma^P GEMM-2 block list: RIS_GTILE2^2 blocks (I >= J) of the spatially (Morton) ordered AO index that
     // contain a surviving shell pair
     int* d_ao_pos = nullptr;           // [nao] spatial position of AO
@@ -164,12 +165,21 @@ DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DEC
 ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
     ris_launch_grad_00, ris_launch_grad_10, ris_launch_grad_11, ris_launch_grad_20, ris_launch_grad_21,
     ris_launch_grad_22, ris_launch_grad_30, ris_launch_grad_31, ris_launch_grad_32, ris_launch_grad_33};
+#define DECL(la, lb) void ris_launch_int_##la##lb(const RisGradParams&, cudaStream_t);
+DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
+#undef DECL
+static const ris_grad_launcher ris_int_launchers[RIS_NCLASS] = {
+    ris_launch_int_00, ris_launch_int_10, ris_launch_int_11, ris_launch_int_20, ris_launch_int_21,
+    ris_launch_int_22, ris_launch_int_30, ris_launch_int_31, ris_launch_int_32, ris_launch_int_33};
+static const char* const kIntNames[RIS_NCLASS] = {
+    "ris_int_kernel<0,0>", "ris_int_kernel<1,0>", "ris_int_kernel<1,1>", "ris_int_kernel<2,0>", "ris_int_kernel<2,1>",
+    "ris_int_kernel<2,2>", "ris_int_kernel<3,0>", "ris_int_kernel<3,1>", "ris_int_kernel<3,2>", "ris_int_kernel<3,3>"};
 static const char* const kGradNames[RIS_NCLASS] = {
     "ris_grad_kernel<0,0>", "ris_grad_kernel<1,0>", "ris_grad_kernel<1,1>", "ris_grad_kernel<2,0>", "ris_grad_kernel<2,1>",
     "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
 // Algorithmic FP64 flops per primitive triplet by E = la + lb + 1 (SURVEY.md 8(d) model: setup ~45, Boys ~30 + 4E,
 // 7 flops per OS-VRR intermediate, scaled accumulation), plus 12 nca ncb flops per contracted triplet and state.
-static const double kModelFlopsByE[8] = {0.0, 140.0, 250.0, 450.0, 750.0, 1250.0, 2000.0, 3100.0};
+static const double kModelFlopsByE[8] = {90.0, 140.0, 250.0, 450.0, 750.0, 1250.0, 2000.0, 3100.0};
 // heaviest class first (flops per primitive triplet), so the tail is made of light kernels
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
@@ -291,8 +301,8 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     }
     if ((rc = dev_upload(c, &c->d_aux, aux.data(), aux.size()))) return rc;
 
-    // Boys tables, one per top order M = 1..7
-    for (int M = 1; M <= 7; ++M) {
+    // Boys tables, one per top order M = 0..7 (M = 0: the undifferentiated (ss|P) of the fitting step)
+    for (int M = 0; M <= 7; ++M) {
         std::vector<double> t;
         ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, t);
         if ((rc = dev_upload(c, &c->d_boys[M], t.data(), t.size()))) return rc;
@@ -599,6 +609,152 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
             return rc;
     }
     return det_end(c, nbatch, det, grad);
+}
+
+// --------------------------------------------------------------------------------------- fitting step, J type (NEXT-1)
+// M[P][Q] = N_P N_Q (P|Q) = fP fQ 2 pi^{5/2} / sqrt(alpha+beta) F_0(rho R^2), fP = N_P / alpha   (Eq. 22)
+__global__ void ris_k_metric(int n, const double* __restrict__ aux, const double* __restrict__ boys0, double* __restrict__ M)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n * n) return;
+    const int P = (int)(t / n), Q = (int)(t - (long long)P * n);
+    const double X0 = aux[5 * P] - aux[5 * Q], X1 = aux[5 * P + 1] - aux[5 * Q + 1], X2 = aux[5 * P + 2] - aux[5 * Q + 2];
+    const double al = aux[5 * P + 3], be = aux[5 * Q + 3];
+    const double sI = ris_rsqrt(al + be);
+    double F[1];
+    ris_boys<0>(al * be * sI * sI * (X0 * X0 + X1 * X1 + X2 * X2), boys0, F);
+    M[t] = aux[5 * P + 4] * aux[5 * Q + 4] * (2.0 * 17.493418327624862846) * sI * F[0];
+}
+
+// In-place Cholesky factor M = L L^T (lower triangle) by ONE block, right-looking, column by column: naux = natoms is a
+// few hundred to a few thousand, the factorisation runs once per geometry.  flag = 1 when a pivot is not positive.
+__global__ void __launch_bounds__(1024) ris_k_cholesky(int n, double* __restrict__ M, int* flag)
+{
+    __shared__ double piv;
+    for (int j = 0; j < n; ++j) {
+        if (threadIdx.x == 0) {
+            const double d = M[(size_t)j * n + j];
+            if (!(d > 0.0)) *flag = 1;
+            piv = sqrt(d);
+            M[(size_t)j * n + j] = piv;
+        }
+        __syncthreads();
+        const double inv = 1.0 / piv;
+        for (int i = j + 1 + threadIdx.x; i < n; i += blockDim.x) M[(size_t)i * n + j] *= inv;
+        __syncthreads();
+        // trailing update of the lower triangle: M[i][k] -= L[i][j] L[k][j], j < k <= i; thread -> row i, k runs along the row
+        const int m = n - j - 1;
+        for (long long t = threadIdx.x; t < (long long)m * m; t += blockDim.x) {
+            const int i = j + 1 + (int)(t / m), k = j + 1 + (int)(t % m);
+            if (k <= i) M[(size_t)i * n + k] = fma(-M[(size_t)i * n + j], M[(size_t)k * n + j], M[(size_t)i * n + k]);
+        }
+        __syncthreads();
+    }
+}
+
+// c[s] = (L L^T)^-1 v[s]: one block per state, column-oriented forward and backward substitution in shared memory.
+__global__ void __launch_bounds__(256) ris_k_chol_solve(int n, const double* __restrict__ L, const double* __restrict__ v,
+                                                        double* __restrict__ cout)
+{
+    extern __shared__ double y[];
+    const int s = blockIdx.x;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) y[i] = v[(size_t)s * n + i];
+    __syncthreads();
+    for (int j = 0; j < n; ++j) {
+        if (threadIdx.x == 0) y[j] /= L[(size_t)j * n + j];
+        __syncthreads();
+        const double yj = y[j];
+        for (int i = j + 1 + threadIdx.x; i < n; i += blockDim.x) y[i] = fma(-L[(size_t)i * n + j], yj, y[i]);
+        __syncthreads();
+    }
+    for (int j = n - 1; j >= 0; --j) {
+        if (threadIdx.x == 0) y[j] /= L[(size_t)j * n + j];
+        __syncthreads();
+        const double yj = y[j];
+        for (int i = threadIdx.x; i < j; i += blockDim.x) y[i] = fma(-L[(size_t)j * n + i], yj, y[i]);
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) cout[(size_t)s * n + i] = y[i];
+}
+
+static int metric_factor(ris_ctx* c)
+{
+    if (c->d_chol) return RIS_OK;
+    const int n = c->naux;
+    int rc;
+    double* L;
+    int* flag;
+    if ((rc = dev_alloc(c, &L, (size_t)n * n, false))) return rc;
+    if ((rc = dev_alloc(c, &flag, 1, true))) return rc;
+    {
+        ProfScope ps(c, "ris_k_metric", 40.0 * n * (double)n, 8.0 * n * (double)n);
+        ris_k_metric<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_aux, c->d_boys[0], L);
+    }
+    {
+        ProfScope ps(c, "ris_k_cholesky", (double)n * n * n / 3.0, 8.0 * n * (double)n);
+        ris_k_cholesky<<<1, 1024, 0, c->stream>>>(n, L, flag);
+    }
+    int hflag = 0;
+    CU(cudaMemcpyAsync(&hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (hflag) return RIS_EINVAL;          // metric not positive definite (coincident aux centres)
+    c->d_chol = L;
+    return RIS_OK;
+}
+
+extern "C" int ris_metric(ris_ctx* c, double* M)
+{
+    if (!c || !M) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    const int n = c->naux;
+    ris_k_metric<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_aux, c->d_boys[0], M);
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out, double* c_out)
+{
+    if (!c || nbatch < 1 || !D || !c_out) return RIS_EINVAL;
+    if ((size_t)c->naux * sizeof(double) > 48 * 1024) return RIS_EINVAL;     // substitution vector in static-size shared memory
+    CU(cudaSetDevice(c->device));
+    int rc;
+    if ((rc = metric_factor(c))) return rc;
+    const long long nao2 = (long long)c->nao * c->nao;
+    const int naux = c->naux;
+    double* v = v_out;
+    if (!v && (rc = ws_get(c, WS_OUT, sizeof(double) * (size_t)nbatch * naux, (void**)&v))) return rc;
+    CU(cudaMemsetAsync(v, 0, sizeof(double) * (size_t)nbatch * naux, c->stream));
+    const int ny = (naux + 31) / 32;
+    for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
+        nb = next_nb(nbatch - s0);
+        double* tile;
+        if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile))) return rc;
+        if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
+        int* ctr;
+        if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr))) return rc;
+        CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
+        for (int oi = 0; oi < RIS_NCLASS; ++oi) {
+            const int k = kClassOrder[oi];
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            RisGradParams p{};
+            p.task_ctr = ctr + (size_t)2 * k * ny;
+            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
+            p.tile = tile; p.sstride = c->nelem_real; p.estride = 1; p.lstride = 0; p.nb = nb;
+            p.p0 = 0; p.p1 = naux; p.grad = v + (size_t)s0 * naux;
+            const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
+            ProfScope ps(c, kIntNames[k], (double)naux * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb] + 2.0 * nel * pk.npairs * nb),
+                         8.0 * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
+            ris_int_launchers[k](p, c->stream);
+        }
+        CU(cudaGetLastError());
+    }
+    {
+        ProfScope ps(c, "ris_k_chol_solve", 2.0 * naux * (double)naux * nbatch, 8.0 * naux * (double)naux * nbatch);
+        ris_k_chol_solve<<<nbatch, 256, sizeof(double) * naux, c->stream>>>(naux, c->d_chol, v, c_out);
+    }
+    CU(cudaGetLastError());
+    return RIS_OK;
 }
 
 // --------------------------------------------------------------------------------------- K

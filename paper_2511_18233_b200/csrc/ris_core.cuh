@@ -12,6 +12,7 @@
 #endif
 
 template <int LA, int LB> struct RisClass;
+template <int LA, int LB> struct RisClass0;     // undifferentiated integrals (fitting step)
 #include "generated/ris_classes.cuh"
 
 // ---------------------------------------------------------------------------------------------
@@ -134,4 +135,17 @@ RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, doub
     RisPrimHead<E> h;
     ris_prim_head<E>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
     ris_vrr<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc);
+}
+
+// Undifferentiated primitive triplet (v_P = sum D_{mu nu} (mu nu|P), Eq. 21):
+// the same head, the VRR up to e = lh + lo, unscaled accumulation of [e0|s].
+template <int LH, int LO>
+RIS_DEV void ris_prim_triplet0(double p, double PZx, double PZy, double PZz, double oo2p, double coef, double ZCx,
+                               double ZCy, double ZCz, double alpha, double auxfac, const double* __restrict__ boys_tab,
+                               double (&acc)[RisClass0<LH, LO>::NACC])
+{
+    constexpr int E = RisClass0<LH, LO>::E;
+    RisPrimHead<E> h;
+    ris_prim_head<E>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
+    ris_vrr0<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, 0.0, 0.0, acc);
 }

@@ -17,6 +17,7 @@ _lib = None
 
 EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host",
+    "ris_fit_J", "ris_metric",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
     "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work", "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak",
@@ -45,6 +46,8 @@ def load_library():
     lib.ris_grad_J.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_grad_K.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_fit_J.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_metric.argtypes = [vp, vp]
     lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_grad_K_host.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ_host.argtypes = [vp, ci, vp, vp, vp]
@@ -182,6 +185,21 @@ class RisContext:
         _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux)), self._dev(d_aux, (nb, self.naux)),
                                      self._dev(out, (nb, self.natoms, 3))))
         return out
+
+    # ---- fitting step, J type (argument marshalling only)
+    def fit_J(self, D):
+        """(v, c): v[s][P] = sum D^s_{mu nu} (mu nu|P), c = M^-1 v; both [nbatch][naux] on the device."""
+        nb = D.shape[0]
+        v = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
+        c = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux)),
+                                   self._dev(c, (nb, self.naux))))
+        return v, c
+
+    def metric(self):
+        M = self._torch.empty((self.naux, self.naux), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_metric(self._h, self._dev(M, (self.naux, self.naux))))
+        return M
 
     # ---- host-buffer calls (numpy arrays or pinned CPU tensors; copies happen inside the C call)
     @staticmethod

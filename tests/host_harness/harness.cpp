@@ -30,6 +30,7 @@ template <int M> static void boys_t(double T, double* F)
 extern "C" int harness_boys(int M, double T, double* F)
 {
     switch (M) {
+    case 0: boys_t<0>(T, F); break;
     case 1: boys_t<1>(T, F); break; case 2: boys_t<2>(T, F); break; case 3: boys_t<3>(T, F); break;
     case 4: boys_t<4>(T, F); break; case 5: boys_t<5>(T, F); break; case 6: boys_t<6>(T, F); break;
     case 7: boys_t<7>(T, F); break; default: return -1;
@@ -76,6 +77,46 @@ extern "C" int harness_triplet(int la, int lb, int nk, const double* prim, const
                                const double* C, double alpha, double auxfac, const double* tile, int nb, double* out)
 {
 #define CASE(a, b) if (la == a && lb == b) { triplet_t<a, b>(nk, prim, A, AB, C, alpha, auxfac, tile, nb, out); return 0; }
+    CASE(0, 0) CASE(1, 0) CASE(1, 1) CASE(2, 0) CASE(2, 1) CASE(2, 2) CASE(3, 0) CASE(3, 1) CASE(3, 2) CASE(3, 3)
+#undef CASE
+    return -1;
+}
+
+// The undifferentiated contracted triplet (fitting step): out[nb] = sum_{ab} tile[s][a][b] (ab|P), phases as above.
+template <int LH, int LO, bool TR>
+static void phase0_t(int nk, const double* prim, bool hostA, const double* Z, const double* ZO, const double* C,
+                     double alpha, double auxfac, const double* tile, int nb, int nel, double* out)
+{
+    using K = RisClass0<LH, LO>;
+    double acc[K::NACC];
+    for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
+    int used = 0;
+    for (int k = 0; k < nk; ++k) {
+        const double* q = prim + 8 * k;
+        if ((q[5] >= q[6]) != hostA) continue;
+        ++used;
+        ris_prim_triplet0<LH, LO>(q[0], q[1], q[2], q[3], q[4], q[7], Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac,
+                                  tab(K::E), acc);
+    }
+    if (!used) return;
+    ris_hrr0c<LH, LO, TR, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)nel, nb, out);
+}
+
+template <int LA, int LB>
+static void triplet0_t(int nk, const double* prim, const double* A, const double* AB, const double* C, double alpha,
+                       double auxfac, const double* tile, int nb, double* out)
+{
+    const double B[3] = {A[0] - AB[0], A[1] - AB[1], A[2] - AB[2]};
+    constexpr int nel = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
+    for (int i = 0; i < nb; ++i) out[i] = 0.0;
+    phase0_t<LA, LB, false>(nk, prim, true, A, B, C, alpha, auxfac, tile, nb, nel, out);
+    phase0_t<LB, LA, true>(nk, prim, false, B, A, C, alpha, auxfac, tile, nb, nel, out);
+}
+
+extern "C" int harness_triplet0(int la, int lb, int nk, const double* prim, const double* A, const double* AB,
+                                const double* C, double alpha, double auxfac, const double* tile, int nb, double* out)
+{
+#define CASE(a, b) if (la == a && lb == b) { triplet0_t<a, b>(nk, prim, A, AB, C, alpha, auxfac, tile, nb, out); return 0; }
     CASE(0, 0) CASE(1, 0) CASE(1, 1) CASE(2, 0) CASE(2, 1) CASE(2, 2) CASE(3, 0) CASE(3, 1) CASE(3, 2) CASE(3, 3)
 #undef CASE
     return -1;

@@ -1,0 +1,99 @@
+"""Parity of the CUDA fitting step (ris_fit_J, ris_metric) with the oracle
+(oracle.ris_oracle.vec_J / metric / fit_J / grad_RIJ), through the C ABI.
+
+Tolerances.  v_P is a plain contraction: the gradient tolerance of test_gpu_parity.py (1e-10 relative + 1e-12 of the
+scale, and < 5e-14 of the scale).  M: closed form, 1e-13 relative.  c = M^-1 v is the solution of a linear system whose
+condition number is 1e2 .. 1e7 on the configs (diffuse s functions on neighbouring atoms overlap strongly): two
+backward-stable solvers (device Cholesky, numpy LU) may differ by ~ cond(M) eps |c|, so c -- and everything composed
+from it -- is compared at  64 cond(M) eps  of its scale; the residual M c = v is checked at 1e-12 of |v| on top."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import ris_oracle as orc
+from paper_2511_18233_b200 import ris_setup, synth
+
+from test_gpu_parity import assert_parity, dev
+
+pytestmark = pytest.mark.gpu
+EPS = 2.220446049250313e-16
+
+
+def _check_fit(mol, D, what):
+    ctx = ris_setup(mol)
+    v, c = ctx.fit_J(dev(D))
+    M = ctx.metric().cpu().numpy()
+    v, c = v.cpu().numpy(), c.cpu().numpy()
+    v_ref, c_ref, e_ref = orc.fit_J(mol, D)
+    M_ref = orc.metric(mol)
+    assert_parity(v, v_ref, what + " v")
+    np.testing.assert_allclose(M, M_ref, rtol=1e-13, atol=0)
+    cond = np.linalg.cond(M_ref)
+    ctol = 64.0 * cond * EPS
+    assert np.abs(c - c_ref).max() <= ctol * np.abs(c_ref).max(), (what, np.abs(c - c_ref).max(), ctol, cond)
+    res = c @ M_ref - v_ref                                  # M symmetric
+    assert np.abs(res).max() <= 1e-12 * np.abs(v_ref).max() * max(1.0, np.abs(M_ref).max()), (what, np.abs(res).max())
+    # composed RI-J gradient with the DEVICE c: G_J(D, c) - 1/2 G_PQ(c, c)  (Eq. 27)
+    cd = dev(c)
+    g = (ctx.grad_J(dev(D), cd) - 0.5 * ctx.grad_PQ(cd, cd)).cpu().numpy()
+    g_ref = orc.grad_RIJ(mol, D)
+    assert np.abs(g - g_ref).max() <= max(ctol, 5e-14) * max(1.0, np.abs(orc.grad_J(mol, D, c_ref)[0]).max()), what
+    # fitted energy 1/2 v.c
+    e = 0.5 * np.einsum("sp,sp->s", v, c)
+    assert np.all(np.abs(e - e_ref) <= max(ctol, 1e-13) * np.abs(e_ref).max())
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_fit_J_small_configs(cfg):
+    wl = synth.make_workload(cfg)
+    _check_fit(wl.mol, wl.D, f"config {cfg}")
+
+
+def test_fit_J_all_classes_up_to_f_and_many_states():
+    mol = synth.tiny_molecule(21, [[0, 1, 2, 3], [3, 2, 0], [1, 3], [0]],
+                              [[0, 0, 0], [1.9, 0.4, -0.3], [-0.8, 1.7, 1.0], [0.5, -2.2, 1.4]], nprim=2)
+    rng = np.random.default_rng(9)
+    _check_fit(mol, rng.standard_normal((7, mol.nao, mol.nao)), "all classes")
+
+
+def test_fit_J_single_atom_and_repeat_calls():
+    """One atom: M is 1x1, c = v / M; a second call on the same ctx reuses the Cholesky factor."""
+    mol = synth.tiny_molecule(4, [[0, 1, 2]], [[0.3, -0.1, 0.2]])
+    rng = np.random.default_rng(1)
+    D = rng.standard_normal((2, mol.nao, mol.nao))
+    ctx = ris_setup(mol)
+    v1, c1 = ctx.fit_J(dev(D))
+    v2, c2 = ctx.fit_J(dev(D[:1]))
+    v_ref, c_ref, _ = orc.fit_J(mol, D)
+    assert_parity(v1.cpu().numpy(), v_ref, "single atom v")
+    np.testing.assert_allclose(c1.cpu().numpy(), c_ref, rtol=1e-13)
+    np.testing.assert_allclose(v2.cpu().numpy(), v1.cpu().numpy()[:1], rtol=1e-13, atol=1e-13 * np.abs(v_ref).max())
+    ctx.close()
+
+
+def test_fit_J_full_size_config3():
+    """Config 3 (100 atoms, 1100 AO, 5 states) at full size: v against the oracle on sampled aux functions (each v_P is
+    an independent output the oracle computes on its own), the solve through its residual."""
+    wl = synth.make_workload(3)
+    ctx = ris_setup(wl.mol, schwarz_tol=wl.schwarz_tol)
+    v, c = ctx.fit_J(dev(wl.D))
+    v, c = v.cpu().numpy(), c.cpu().numpy()
+    import ctypes as C
+    h = orc._Held(wl.mol)
+    D = np.ascontiguousarray(wl.D, dtype=np.float64)
+    nb = D.shape[0]
+    one = np.ones(nb)
+    scale = np.abs(v).max()
+    for P in (0, 57, 99):
+        g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
+        e = np.zeros(nb, dtype=np.longdouble)
+        assert orc.lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, one.ctypes.data, None, 0.0,
+                                               g.ctypes.data, e.ctypes.data) == 0
+        ref = e.astype(np.float64)
+        assert np.all(np.abs(v[:, P] - ref) <= 1e-10 * np.abs(ref) + 1e-12 * scale), (P, v[:, P], ref)
+    M_ref = orc.metric(wl.mol)
+    res = c @ M_ref - v
+    assert np.abs(res).max() <= 1e-11 * np.abs(v).max() * max(1.0, np.abs(M_ref).max())
+    ctx.close()

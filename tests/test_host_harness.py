@@ -33,10 +33,11 @@ def harness():
     lib.harness_boys.argtypes = [C.c_int, C.c_double, C.c_void_p]
     lib.harness_triplet.argtypes = [C.c_int, C.c_int, C.c_int] + [C.c_void_p] * 4 + [C.c_double, C.c_double,
                                                                                     C.c_void_p, C.c_int, C.c_void_p]
+    lib.harness_triplet0.argtypes = lib.harness_triplet.argtypes
     return lib
 
 
-@pytest.mark.parametrize("M", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("M", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_device_boys_interpolation_vs_mpmath(harness, M):
     mpmath.mp.dps = 40
     rng = np.random.default_rng(M)
@@ -97,3 +98,41 @@ def test_class_recurrence_vs_oracle(harness, la, lb):
         np.testing.assert_allclose(out, ref, rtol=0, atol=2e-13 * scale)
         # translational invariance closes the aux centre
         np.testing.assert_allclose(-(out[:, :3] + out[:, 3:]), g[:, 2, :], rtol=0, atol=2e-13 * scale)
+
+
+@pytest.mark.parametrize("la,lb", CLASSES)
+def test_undifferentiated_class_recurrence_vs_oracle(harness, la, lb):
+    """Fitting step (NEXT-1): one contracted triplet per class, sum_ab tile_ab (ab|P), against the oracle's v_P."""
+    rng = np.random.default_rng(50 + 10 * la + lb)
+    for trial, dist in enumerate([1.5, 6.0, 40.0]):
+        coords = np.array([[0.1, -0.2, 0.3], [1.1, 0.7, -0.6], [0, 0, 0]], dtype=float)
+        v = rng.normal(size=3)
+        coords[2] = coords[0] + dist * v / np.linalg.norm(v)
+        mol = synth.tiny_molecule(200 + trial, [[la], [lb], []], coords, lo=0.15, hi=4.0, nprim=3)
+        nca, ncb = synth.ncart(la), synth.ncart(lb)
+        nb = 2
+        tile = rng.standard_normal((nb, nca, ncb))
+        G = np.zeros((nb, mol.nao, mol.nao))
+        G[:, :nca, nca:] = tile
+        P = 2
+        ref = orc.vec_J(mol, G)[:, P]
+        A, B = coords[0], coords[1]
+        prim = []
+        for ka in range(3):
+            for kb in range(3):
+                a, b = mol.prim_exp[ka], mol.prim_exp[3 + kb]
+                p = a + b
+                PZ = -(b / p) * (A - B) if a >= b else (a / p) * (A - B)
+                Kab = math.exp(-a * b / p * np.dot(A - B, A - B))
+                coef = mol.prim_coef[ka] * mol.prim_coef[3 + kb] * Kab * 2 * math.pi ** 2.5 / p
+                prim.append([p, PZ[0], PZ[1], PZ[2], 0.5 / p, 2 * a, 2 * b, coef])
+        prim = np.ascontiguousarray(prim)
+        alpha = mol.aux_exponents[P]
+        auxfac = (2 * alpha / math.pi) ** 0.75 / alpha
+        out = np.zeros(nb)
+        AB = A - B
+        Cc = np.ascontiguousarray(coords[P])
+        rc = harness.harness_triplet0(la, lb, 9, prim.ctypes.data, A.ctypes.data, AB.ctypes.data, Cc.ctypes.data,
+                                      alpha, auxfac, np.ascontiguousarray(tile).ctypes.data, nb, out.ctypes.data)
+        assert rc == 0
+        np.testing.assert_allclose(out, ref, rtol=0, atol=2e-13 * max(np.abs(ref).max(), 1e-3))
