@@ -393,6 +393,74 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
     return 0;
 }
 
+/* ---------------------------------------------------------------- undifferentiated integral matrix
+ * out[mu][nu] = (mu nu|P) for aux P, all ordered (mu, nu)  (first factor of Eq. 21; O2-O4 with
+ * N_P and the contraction coefficients).  Used by the fitting step (NEXT-1): T^P = C_occ^T (mu nu|P) C_vir.
+ */
+int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, double *out)
+{
+    int nsh = mol->nshells;
+    int *ao_off = malloc(sizeof(int) * (size_t)(nsh + 1));
+    ao_off[0] = 0;
+    for (int s = 0; s < nsh; ++s) {
+        if (mol->shell_l[s] < 0 || mol->shell_l[s] > LMAX) { free(ao_off); return -1; }
+        ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
+    }
+    int nao = ao_off[nsh];
+    double alpha = mol->aux_exponents[P];
+    double NP = aux_norm(alpha);
+    const double *C = mol->coords + 3 * P;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int sa = 0; sa < nsh; ++sa) {
+        int la = mol->shell_l[sa], na = ncart(la);
+        int compa[10][3];
+        cart_components(la, compa);
+        const double *A = mol->coords + 3 * mol->shell_atom[sa];
+        for (int sb = 0; sb < nsh; ++sb) {
+            int lb = mol->shell_l[sb], nb = ncart(lb);
+            int compb[10][3];
+            cart_components(lb, compb);
+            const double *Bc = mol->coords + 3 * mol->shell_atom[sb];
+            double buf[100];
+            memset(buf, 0, sizeof buf);
+            double AB2 = 0.0;
+            for (int d = 0; d < 3; ++d) AB2 += (A[d] - Bc[d]) * (A[d] - Bc[d]);
+            for (int ka = 0; ka < mol->shell_nprim[sa]; ++ka) {
+                double a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
+                double da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
+                for (int kb = 0; kb < mol->shell_nprim[sb]; ++kb) {
+                    double b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
+                    double db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
+                    double p = a + b;
+                    if (prim_cutoff > 0.0 && fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, 1.5) < prim_cutoff)
+                        continue;
+                    double rho = p * alpha / (p + alpha);
+                    double X[3];
+                    Etab E[3];
+                    for (int d = 0; d < 3; ++d) {
+                        X[d] = (a * A[d] + b * Bc[d]) / p - C[d];
+                        hermite_E(la, lb, a, b, A[d] - Bc[d], E[d]);
+                    }
+                    Rtab R;
+                    hermite_R(la + lb, rho, X, R);
+                    double pref = NP * da * db * 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+                    for (int ca = 0; ca < na; ++ca)
+                        for (int cb = 0; cb < nb; ++cb) {
+                            const int *ia = compa[ca], *ib = compb[cb];
+                            buf[ca * 10 + cb] += pref * hsum(E[0][ia[0]][ib[0]], ia[0] + ib[0], E[1][ia[1]][ib[1]], ia[1] + ib[1],
+                                                             E[2][ia[2]][ib[2]], ia[2] + ib[2], R, 0, 0, 0);
+                        }
+                }
+            }
+            for (int ca = 0; ca < na; ++ca)
+                for (int cb = 0; cb < nb; ++cb)
+                    out[(size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb] = buf[ca * 10 + cb];
+        }
+    }
+    free(ao_off);
+    return 0;
+}
+
 /* ---------------------------------------------------------------- O7: G_PQ and E_PQ
  * gacc[s][A][x] += sum_{PQ} c^s_P d^s_Q d(P|Q)/dR_{A,x};  eacc[s] += sum_{PQ} c_P d_Q (P|Q),
  * with N_P N_Q included.  P and Q run over all ordered pairs; P = Q contributes no gradient.

@@ -62,6 +62,8 @@ def lib():
         _lib.ris_oracle_contract_P.restype = C.c_int
         _lib.ris_oracle_grad_PQ.argtypes = [C.POINTER(_Mol), C.c_int, C.c_void_p, C.c_void_p,
                                             C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_int3c_P.argtypes = [C.POINTER(_Mol), C.c_int, C.c_double, C.c_void_p]
+        _lib.ris_oracle_int3c_P.restype = C.c_int
         _lib.ris_oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -251,3 +253,63 @@ def grad_RIJ(mol, D, *, prim_cutoff=0.0):
     gJ, _ = grad_J(mol, D, c, prim_cutoff=prim_cutoff)
     gQ, _ = grad_PQ(mol, c, c)
     return gJ - 0.5 * gQ
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1, K-type fitting step: the MO-transformed three-index tensor and its fit (Eqs. 21-22, PAPER.md:119-121;
+# "transformed from the AO to the MO basis and stored in the reduced-size MO basis"):
+#   T^P_ia = sum_{mu nu} C_occ[mu,i] (mu nu|P) C_vir[nu,a]
+#   B      = M^-1 T                                    (per (i,a) column; numpy.linalg.solve)
+#   E_RIK  = 1/2 sum_{PQ} sum_ia T^P_ia M^-1_PQ T^Q_ia = 1/2 sum_P sum_ia T^P_ia B^P_ia
+# and for fixed C_occ, C_vir (Eq. 27; A9: the metric term carries the FULL matrix G, not a rank-1 one)
+#   dE_RIK/dxi = G_K(C_occ, C_vir, B) - 1/2 sum_{PQ} G_PQ M^xi_PQ,   G_PQ = sum_ia B^P_ia B^Q_ia.
+def int3c(mol, P, *, prim_cutoff=0.0):
+    """(mu nu|P) as a dense [nao][nao] matrix."""
+    h = _Held(mol)
+    out = np.zeros((h.nao, h.nao))
+    rc = lib().ris_oracle_int3c_P(C.byref(h.c), int(P), prim_cutoff, out.ctypes.data)
+    assert rc == 0
+    return out
+
+
+def tensor_K(mol, C_occ, C_vir, *, prim_cutoff=0.0):
+    """T[P][i][a] = sum C_occ[mu,i] (mu nu|P) C_vir[nu,a]."""
+    C_occ, C_vir = _f64(C_occ), _f64(C_vir)
+    n = np.asarray(mol.coords).shape[0]
+    return np.stack([C_occ.T @ int3c(mol, P, prim_cutoff=prim_cutoff) @ C_vir for P in range(n)])
+
+
+def fit_K(mol, C_occ, C_vir, *, prim_cutoff=0.0):
+    """(T, B, E_RIK): B = M^-1 T, E_RIK = 1/2 sum T.B."""
+    T = tensor_K(mol, C_occ, C_vir, prim_cutoff=prim_cutoff)
+    n = T.shape[0]
+    B = np.linalg.solve(metric(mol), T.reshape(n, -1)).reshape(T.shape)
+    return T, B, 0.5 * float(np.sum(T * B))
+
+
+def grad_PQ_full(mol, G):
+    """sum_{PQ} G[s][P][Q] d(P|Q)/dR with N_P N_Q (the metric term of Eq. 27 for a full matrix G; positive sign)."""
+    al = _f64(mol.aux_exponents)
+    R = _f64(mol.coords)
+    n = al.shape[0]
+    G = _f64(G).reshape(-1, n, n)
+    N = (2.0 * al / np.pi) ** 0.75
+    g = np.zeros((G.shape[0], n, 3), dtype=np.longdouble)
+    for P in range(n):
+        for Q in range(n):
+            if P == Q:
+                continue
+            d = N[P] * N[Q] * prim2c(al[P], al[Q], R[P], R[Q])[1:]
+            for s in range(G.shape[0]):
+                g[s, P] += G[s, P, Q] * d
+                g[s, Q] -= G[s, P, Q] * d
+    return g.astype(np.float64)
+
+
+def grad_RIK(mol, C_occ, C_vir, *, prim_cutoff=0.0):
+    """dE_RIK/dR at fixed C_occ, C_vir: G_K(C_occ, C_vir, B) - 1/2 G_PQ_full(B B^T) with the fitted B."""
+    _, B, _ = fit_K(mol, C_occ, C_vir, prim_cutoff=prim_cutoff)
+    n = B.shape[0]
+    gK, _ = grad_K(mol, C_occ, C_vir, B[None], prim_cutoff=prim_cutoff)
+    Bf = B.reshape(n, -1)
+    return gK[0] - 0.5 * grad_PQ_full(mol, (Bf @ Bf.T)[None])[0]

@@ -122,3 +122,62 @@ def test_vec_J_far_field_limit():
     ref = S * (2 * al / math.pi) ** 0.75 * (math.pi / al) ** 1.5 / 200.0
     got = orc.vec_J(mol, np.ones((1, 1, 1)))[0, 1]
     assert abs(got - ref) < 1e-8 * ref
+
+
+# ------------------------------------------------------------------ K-type fitting step
+
+def test_int3c_consistent_with_pinned_contraction_and_symmetric():
+    """(mu nu|P) as a matrix against the pinned contraction: sum D.I^P = v_P; symmetric in mu nu."""
+    mol, D = _tiny()
+    v = orc.vec_J(mol, D)
+    for P in range(3):
+        I = orc.int3c(mol, P)
+        np.testing.assert_allclose(I, I.T, rtol=0, atol=1e-14 * np.abs(I).max())
+        np.testing.assert_allclose(np.einsum("smn,mn->s", D, I), v[:, P], rtol=0, atol=1e-12 * np.abs(v).max())
+
+
+def test_int3c_single_element_by_quadrature():
+    coords = np.array([[0.2, -0.1, 0.3], [1.1, 0.6, -0.4]])
+    mol = synth.tiny_molecule(7, [[0], [0]], coords, nprim=1)
+    a, b = mol.prim_exp
+    da, db = mol.prim_coef
+    A, B = coords
+    p = a + b
+    Pc = (a * A + b * B) / p
+    x, w = np.polynomial.hermite.hermgauss(48)
+    g = [Pc[d] + x / math.sqrt(p) for d in range(3)]
+    X, Y, Z = np.meshgrid(*g, indexing="ij")
+    W = w[:, None, None] * w[None, :, None] * w[None, None, :] / p ** 1.5
+    al = mol.aux_exponents[0]
+    r = np.sqrt((X - A[0]) ** 2 + (Y - A[1]) ** 2 + (Z - A[2]) ** 2)
+    V = (2 * al / math.pi) ** 0.75 * (math.pi / al) ** 1.5 * erf(math.sqrt(al) * r) / r
+    ref = da * db * math.exp(-a * b / p * np.sum((A - B) ** 2)) * np.sum(W * V)
+    assert abs(orc.int3c(mol, 0)[0, 1] - ref) < 1e-11 * abs(ref)
+
+
+def test_grad_PQ_full_reduces_to_rank_one():
+    mol, _ = _tiny()
+    rng = np.random.default_rng(2)
+    c, d = rng.standard_normal((2, 3)), rng.standard_normal((2, 3))
+    ref, _ = orc.grad_PQ(mol, c, d)
+    got = orc.grad_PQ_full(mol, np.einsum("sp,sq->spq", c, d))
+    np.testing.assert_allclose(got, ref, rtol=0, atol=1e-13 * np.abs(ref).max())
+
+
+def test_fitted_K_energy_finite_difference():
+    """d/dR [1/2 sum T M^-1 T] with the fit re-solved at every displaced geometry
+    = G_K(C_occ, C_vir, B) - 1/2 sum_PQ (B B^T)_PQ M^xi_PQ   (Eq. 27 with a full-matrix metric term)."""
+    mol, _ = _tiny()
+    rng = np.random.default_rng(8)
+    nao = sum(synth.ncart(int(l)) for l in mol.shell_l)
+    Co, Cv = rng.standard_normal((nao, 3)), rng.standard_normal((nao, 4))
+    g = orc.grad_RIK(mol, Co, Cv)
+    h = 5e-6
+    scale = np.abs(g).max()
+    for atom, d in itertools.product(range(3), range(3)):
+        mp_, mm_ = copy.copy(mol), copy.copy(mol)
+        mp_.coords = mol.coords.copy(); mp_.coords[atom, d] += h
+        mm_.coords = mol.coords.copy(); mm_.coords[atom, d] -= h
+        fd = (orc.fit_K(mp_, Co, Cv)[2] - orc.fit_K(mm_, Co, Cv)[2]) / (2 * h)
+        assert abs(g[atom, d] - fd) < 5e-7 * scale, (atom, d, g[atom, d], fd)
+    assert np.all(np.abs(g.sum(axis=0)) < 1e-10 * np.abs(g).sum())
