@@ -112,6 +112,19 @@ int ris_grad_PQ(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_a
 int ris_fit_J(ris_ctx* ctx, int nbatch, const double* D, double* v_out, double* c_out);
 int ris_metric(ris_ctx* ctx, double* M_out);
 
+/* ---- Fitting step, K type (NEXT-1; Eqs. 21-22; MO-basis three-index tensor) ---------
+ * ris_fit_K:  T[P][i][a] = sum_{mu nu} C_occ[mu,i] (mu nu|P) C_vir[nu,a]      (surviving shell pairs only)
+ *             B[P][i][a] = sum_Q M^-1[P][Q] T[Q][i][a]                        -> the B that ris_grad_K takes (nbatch 1)
+ *   C_occ device [nao][nocc], C_vir device [nao][nvir] (any two matrices with nao rows), T_out device
+ *   [naux][nocc][nvir] or NULL, B_out device [naux][nocc][nvir].  Scratch (integral buffer, band slabs, half-transformed
+ *   tensor: about 8 (naux nvir nao + naux * band) bytes) is ctx-owned.  For fixed C_occ, C_vir:
+ *     d/dxi (1/2 sum_{PQ,ia} T^P_ia M^-1_PQ T^Q_ia) = ris_grad_K(C_occ, C_vir, B) - 1/2 ris_grad_PQ_full(G),
+ *     G[P][Q] = sum_ia B[P][i][a] B[Q][i][a]                                  (Eq. 27).
+ * ris_grad_PQ_full:  grad[s][A][x] = sum_{PQ} G[s][P][Q] d(P|Q)/dR_{A,x}  -- the metric term for a full matrix
+ *   (SURVEY.md 8(c) A9); G device [nbatch][naux][naux] (any symmetry), grad device [nbatch][natoms][3], overwritten. */
+int ris_fit_K(ris_ctx* ctx, int nocc, int nvir, const double* C_occ, const double* C_vir, double* T_out, double* B_out);
+int ris_grad_PQ_full(ris_ctx* ctx, int nbatch, const double* G, double* grad);
+
 /* The same three calls on HOST buffers: host->device copies, the kernels, and the device->host copy of
  * the gradient all happen inside the call, which returns when grad (host) is complete.  Pinned (page-locked) host
  * buffers let ris_grad_K_host stream B up in ranges of P on a second stream while the Gamma^P GEMMs of the

@@ -298,6 +298,26 @@ def gen_hrr0c(pl: ClassPlan0) -> str:
     return "\n".join(out)
 
 
+def gen_hrr0w(pl: ClassPlan0) -> str:
+    la, lb = pl.la, pl.lb
+    out = []
+    w = out.append
+    w(f"// contracted undifferentiated triplet of class ({la},{lb}): HRR to (a b|P), ADDED to out[el * estride] (the two")
+    w("// host-centre phases of a pair add into the same, pre-zeroed elements).  Element order by TR as in ris_hrrc.")
+    w("template <bool TR>")
+    w(f"RIS_DEV void ris_hrr0w_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
+    w("    double* __restrict__ out, size_t estride)")
+    w("{")
+    done = set()
+    X = gen_hrr_chain(w, pl, "0", la, lb, "x", done)
+    nca, ncb = nc(la), nc(lb)
+    for ia, a in enumerate(comps(la)):
+        for ib, b in enumerate(comps(lb)):
+            w(f"    out[(TR ? {ib * nca + ia} : {ia * ncb + ib}) * estride] += {X(a, b)};")
+    w("}")
+    return "\n".join(out)
+
+
 def generate() -> str:
     parts = ["// GENERATED by gen_classes.py -- do not edit.  See that file for the recurrences.",
              "#pragma once", ""]
@@ -322,6 +342,8 @@ def generate() -> str:
         parts.append("")
         parts.append(gen_hrr0c(p0))
         parts.append("")
+        parts.append(gen_hrr0w(p0))
+        parts.append("")
     # dispatch helpers
     parts.append("template <int LA, int LB, class... A> RIS_DEV void ris_vrr(A&&... a) {")
     for la, lb in classes:
@@ -334,6 +356,10 @@ def generate() -> str:
     parts.append("template <int LA, int LB, bool TR, int SL, class... A> RIS_DEV void ris_hrr0c(A&&... a) {")
     for la, lb in classes:
         parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrr0c_{la}{lb}<TR, SL>(static_cast<A&&>(a)...);")
+    parts.append("}")
+    parts.append("template <int LA, int LB, bool TR, class... A> RIS_DEV void ris_hrr0w(A&&... a) {")
+    for la, lb in classes:
+        parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrr0w_{la}{lb}<TR>(static_cast<A&&>(a)...);")
     parts.append("}")
     parts.append("template <int LA, int LB, bool TR, int SL, int SC, class... A> RIS_DEV void ris_hrrc(A&&... a) {")
     for la, lb in classes:

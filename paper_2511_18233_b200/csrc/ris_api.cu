@@ -57,6 +57,14 @@ struct ris_ctx {
     std::vector<void*> owned;          // every device allocation of the packed data
     long long nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[8] = {nullptr};
+    double* d_minv = nullptr;          // [naux][nauxp] inverse metric (built by the first ris_fit_K)
+    // band of the spatially ordered AO index per 64-row block (from the GEMM-2 block list): columns
+    // [rb_jlo*64, (rb_jlo*64 + rb_kw)) hold every surviving partner of the block's rows
+    std::vector<int> rb_jlo, rb_kw;
+    std::vector<long long> rb_off;     // offset (doubles) of the block's [64][rb_kw] slab within one P
+    long long slab_stride = 0;
+    int *d_rb_jlo = nullptr, *d_rb_kw = nullptr;
+    long long* d_rb_off = nullptr;
     double* d_chol = nullptr;          // [naux][naux] lower Cholesky factor of the aux metric (built by the first ris_fit_J)
     // Gamma^P GEMM-2 block list: RIS_GTILE2^2 blocks (I >= J) of the spatially (Morton) ordered AO index that
     // contain a surviving shell pair
@@ -75,14 +83,15 @@ struct ris_ctx {
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
-    void* ws[10] = {nullptr};
-    size_t ws_bytes[10] = {0};
+    void* ws[20] = {nullptr};
+    size_t ws_bytes[20] = {0};
     int last_pbatch = 0;
     std::vector<ProfRec> prof;
     std::vector<cudaEvent_t> ev_pool;
 };
 
-enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9, WS_N = 10 };
+enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
+       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_N = 17 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -171,6 +180,12 @@ DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DEC
 static const ris_grad_launcher ris_int_launchers[RIS_NCLASS] = {
     ris_launch_int_00, ris_launch_int_10, ris_launch_int_11, ris_launch_int_20, ris_launch_int_21,
     ris_launch_int_22, ris_launch_int_30, ris_launch_int_31, ris_launch_int_32, ris_launch_int_33};
+#define DECL(la, lb) void ris_launch_ints_##la##lb(const RisGradParams&, cudaStream_t);
+DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
+#undef DECL
+static const ris_grad_launcher ris_ints_launchers[RIS_NCLASS] = {
+    ris_launch_ints_00, ris_launch_ints_10, ris_launch_ints_11, ris_launch_ints_20, ris_launch_ints_21,
+    ris_launch_ints_22, ris_launch_ints_30, ris_launch_ints_31, ris_launch_ints_32, ris_launch_ints_33};
 static const char* const kIntNames[RIS_NCLASS] = {
     "ris_int_kernel<0,0>", "ris_int_kernel<1,0>", "ris_int_kernel<1,1>", "ris_int_kernel<2,0>", "ris_int_kernel<2,1>",
     "ris_int_kernel<2,2>", "ris_int_kernel<3,0>", "ris_int_kernel<3,1>", "ris_int_kernel<3,2>", "ris_int_kernel<3,3>"};
@@ -426,6 +441,24 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
                 if (m_) { m_ = (int)tiles.size(); tiles.push_back(make_int2(I, J)); } else m_ = -1;
             }
         c->ntiles = (int)tiles.size();
+        {   // row-block bands for the fitting step's sparse transform (ris_fit_K)
+            std::vector<int> jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
+            for (const int2& t : tiles) {
+                jlo[t.x] = std::min(jlo[t.x], t.y); jhi[t.x] = std::max(jhi[t.x], t.y);
+                jlo[t.y] = std::min(jlo[t.y], t.x); jhi[t.y] = std::max(jhi[t.y], t.x);
+            }
+            c->rb_jlo.resize(c->nblk); c->rb_kw.resize(c->nblk); c->rb_off.resize(c->nblk);
+            long long off2 = 0;
+            for (int I = 0; I < c->nblk; ++I) {
+                if (jhi[I] < 0) jlo[I] = jhi[I] = I;
+                c->rb_jlo[I] = jlo[I]; c->rb_kw[I] = (jhi[I] - jlo[I] + 1) * RIS_GTILE2; c->rb_off[I] = off2;
+                off2 += (long long)RIS_GTILE2 * c->rb_kw[I];
+            }
+            c->slab_stride = off2;
+            if ((rc = dev_upload(c, &c->d_rb_jlo, c->rb_jlo.data(), c->rb_jlo.size()))) return rc;
+            if ((rc = dev_upload(c, &c->d_rb_kw, c->rb_kw.data(), c->rb_kw.size()))) return rc;
+            if ((rc = dev_upload(c, &c->d_rb_off, c->rb_off.data(), c->rb_off.size()))) return rc;
+        }
         if ((rc = dev_upload(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
         if ((rc = dev_upload(c, &c->d_tmap, mark.data(), mark.size()))) return rc;
         // inverse element map + active-row list of the block buffer (for the P-minor transpose of the K tiles)
@@ -753,6 +786,238 @@ extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out,
         ProfScope ps(c, "ris_k_chol_solve", 2.0 * naux * (double)naux * nbatch, 8.0 * naux * (double)naux * nbatch);
         ris_k_chol_solve<<<nbatch, 256, sizeof(double) * naux, c->stream>>>(naux, c->d_chol, v, c_out);
     }
+    CU(cudaGetLastError());
+    return RIS_OK;
+}
+
+// --------------------------------------------------------------------------------------- fitting step, K type (NEXT-1)
+//   T^P_ia = sum_{mu nu} C_occ[mu,i] (mu nu|P) C_vir[nu,a],   B = M^-1 T        (Eqs. 21-22)
+// 1. ris_int_kernel<.., STORE>: the surviving (mu nu|P) into the P-minor integral buffer I[element][P]
+// 2. ris_k_unpack_band: I -> per-P band slabs of the spatially ordered AO index: slab[P][row block][64][kw] (both
+//    triangles; the band [jlo*64, jlo*64 + kw) of a row block covers every surviving partner of its rows)
+// 3. GEMM-A (per row block, batched over P):  Ut[P][a][mu'] = sum_{nu' in band} C_vir^T[a][nu'] slab[P][mu'][nu']
+// 4. GEMM-B (batched over P):                  T[P][i][a]   = sum_{mu'} C_occ^T[i][mu'] Ut[P][a][mu']
+// 5. transpose T -> Tt[(i,a)][Q];  GEMM-C:     B[P][(i,a)]  = sum_Q Minv[P][Q] Tt[(i,a)][Q]
+// all three GEMMs on the DMMA kernel of ris_gemm.cuh (K-contiguous "NT" operands).
+__global__ void ris_k_unpack_band(RisClassPack pk, const int* __restrict__ ao_pos, int np, int pbp,
+                                  const double* __restrict__ I, const int* __restrict__ rb_jlo, const int* __restrict__ rb_kw,
+                                  const long long* __restrict__ rb_off, long long slab_stride, double* __restrict__ slab)
+{
+    const int nca = ris_ncart(pk.la), ncb = ris_ncart(pk.lb), nel = nca * ncb;
+    const long long el = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (el >= (long long)nel * pk.npairs) return;
+    const int P = blockIdx.y * 32 + (threadIdx.x & 31);
+    if (P >= np) return;
+    const int ip = (int)(el / nel), e = (int)(el - (long long)ip * nel);
+    const int a0 = pk.ao[ip], b0 = pk.ao[(size_t)pk.npairs + ip];
+    const int r = ao_pos[a0] + e / ncb, q = ao_pos[b0] + e % ncb;
+    const double v = I[((size_t)pk.elem_off + (size_t)el) * pbp + P];
+    double* s = slab + (size_t)P * slab_stride;
+    {
+        const int Ib = r / RIS_GTILE2;
+        s[rb_off[Ib] + (long long)(r - Ib * RIS_GTILE2) * rb_kw[Ib] + (q - rb_jlo[Ib] * RIS_GTILE2)] = v;
+    }
+    if (a0 != b0) {          // a same-shell pair holds both (ca,cb) and (cb,ca) as elements of its own
+        const int Ib = q / RIS_GTILE2;
+        s[rb_off[Ib] + (long long)(q - Ib * RIS_GTILE2) * rb_kw[Ib] + (r - rb_jlo[Ib] * RIS_GTILE2)] = v;
+    }
+}
+
+// out[col][pos] = in[order[pos]][col], pos < rows; zero for rows <= pos < ld   (C^T in spatial AO order, K-contiguous)
+__global__ void ris_k_transpose_rows(int rows, int cols, int ld, const int* __restrict__ order, const double* __restrict__ in,
+                                     double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)cols * ld) return;
+    const int col = (int)(i / ld), pos = (int)(i - (long long)col * ld);
+    out[i] = pos < rows ? in[(size_t)order[pos] * cols + col] : 0.0;
+}
+
+// out[c][r] (ld ldo, zero padded) = in[r][c]: 32x32 tiles through shared memory
+__global__ void ris_k_transpose(int rows, long long cols, int ldo, const double* __restrict__ in, double* __restrict__ out)
+{
+    __shared__ double t[32][33];
+    const long long c0 = (long long)blockIdx.x * 32;
+    const int r0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+        const int r = r0 + j;
+        const long long cc = c0 + threadIdx.x;
+        t[j][threadIdx.x] = (r < rows && cc < cols) ? in[(size_t)r * cols + cc] : 0.0;
+    }
+    __syncthreads();
+    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+        const long long cc = c0 + j;
+        const int r = r0 + threadIdx.x;
+        if (cc < cols && r < ldo) out[(size_t)cc * ldo + r] = t[threadIdx.x][j];
+    }
+}
+
+__global__ void ris_k_eye(int n, double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < (long long)n * n) out[i] = (i / n == i % n) ? 1.0 : 0.0;
+}
+
+__global__ void ris_k_pad2d(int rows, int cols, int ld, const double* __restrict__ in, double* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)rows * ld) return;
+    const int r = (int)(i / ld), cidx = (int)(i - (long long)r * ld);
+    out[i] = cidx < cols ? in[(size_t)r * cols + cidx] : 0.0;
+}
+
+static int metric_inverse(ris_ctx* c)
+{
+    if (c->d_minv) return RIS_OK;
+    int rc;
+    if ((rc = metric_factor(c))) return rc;
+    const int n = c->naux, np_ = (n + 1) & ~1;
+    double *eye, *inv, *minv;
+    if ((rc = dev_alloc(c, &eye, (size_t)n * n, false))) return rc;
+    if ((rc = dev_alloc(c, &inv, (size_t)n * n, false))) return rc;
+    if ((rc = dev_alloc(c, &minv, (size_t)n * np_, false))) return rc;
+    const unsigned nb1 = (unsigned)(((long long)n * n + 255) / 256), nb2 = (unsigned)(((long long)n * np_ + 255) / 256);
+    ris_k_eye<<<nb1, 256, 0, c->stream>>>(n, eye);
+    ris_k_chol_solve<<<n, 256, sizeof(double) * n, c->stream>>>(n, c->d_chol, eye, inv);
+    ris_k_pad2d<<<nb2, 256, 0, c->stream>>>(n, n, np_, inv, minv);
+    CU(cudaGetLastError());
+    c->d_minv = minv;
+    return RIS_OK;
+}
+
+extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir, double* T_out, double* B_out)
+{
+    if (!c || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B_out) return RIS_EINVAL;
+    if ((size_t)c->naux * sizeof(double) > 48 * 1024) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    int rc;
+    if ((rc = metric_inverse(c))) return rc;
+    const int nao = c->nao, naux = c->naux;
+    const int naop = (nao + 1) & ~1, nauxp = (naux + 1) & ~1, pbp = (naux + 3) & ~3;
+    const long long nia = (long long)nocc * nvir;
+    double *I, *slab, *Ut, *T, *Tt, *CvT, *CoT;
+    if ((rc = ws_get(c, WS_FIT_I, sizeof(double) * (size_t)std::max<long long>(c->nelem_real, 1) * pbp, (void**)&I))) return rc;
+    if ((rc = ws_get(c, WS_FIT_SLAB, sizeof(double) * (size_t)naux * c->slab_stride, (void**)&slab))) return rc;
+    if ((rc = ws_get(c, WS_FIT_UT, sizeof(double) * (size_t)naux * nvir * naop, (void**)&Ut))) return rc;
+    if ((rc = ws_get(c, WS_FIT_TT, sizeof(double) * (size_t)nia * nauxp, (void**)&Tt))) return rc;
+    if ((rc = ws_get(c, WS_FIT_CV, sizeof(double) * (size_t)nvir * naop, (void**)&CvT))) return rc;
+    if ((rc = ws_get(c, WS_FIT_CO, sizeof(double) * (size_t)nocc * naop, (void**)&CoT))) return rc;
+    T = T_out;
+    if (!T && (rc = ws_get(c, WS_FIT_T, sizeof(double) * (size_t)naux * nia, (void**)&T))) return rc;
+    CU(cudaMemsetAsync(I, 0, sizeof(double) * (size_t)std::max<long long>(c->nelem_real, 1) * pbp, c->stream));
+    CU(cudaMemsetAsync(slab, 0, sizeof(double) * (size_t)naux * c->slab_stride, c->stream));
+    const int ny = (naux + 31) / 32;
+    {   // 1. integrals
+        int* ctr;
+        if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr))) return rc;
+        CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
+        for (int oi = 0; oi < RIS_NCLASS; ++oi) {
+            const int k = kClassOrder[oi];
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            RisGradParams p{};
+            p.task_ctr = ctr + (size_t)2 * k * ny;
+            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
+            p.estride = pbp; p.nb = 0; p.p0 = 0; p.p1 = naux; p.grad = I;
+            const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
+            ProfScope ps(c, kIntNames[k], (double)naux * (double)pk.nprim * kModelFlopsByE[pk.la + pk.lb],
+                         8.0 * nel * pk.npairs * naux + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
+            ris_ints_launchers[k](p, c->stream);
+        }
+        CU(cudaGetLastError());
+    }
+    {   // 2. band slabs
+        ProfScope ps(c, "ris_k_unpack_band", 0.0, 24.0 * (double)c->nelem_real * naux);
+        for (int k = 0; k < RIS_NCLASS; ++k) {
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+            ris_k_unpack_band<<<dim3((unsigned)((nelc + 7) / 8), ny), 256, 0, c->stream>>>(pk, c->d_ao_pos, naux, pbp, I, c->d_rb_jlo,
+                                                                                         c->d_rb_kw, c->d_rb_off, c->slab_stride, slab);
+        }
+        CU(cudaGetLastError());
+    }
+    {
+        const long long n1 = (long long)nvir * naop, n2 = (long long)nocc * naop;
+        ris_k_transpose_rows<<<(unsigned)((n1 + 255) / 256), 256, 0, c->stream>>>(nao, nvir, naop, c->d_ao_order, C_vir, CvT);
+        ris_k_transpose_rows<<<(unsigned)((n2 + 255) / 256), 256, 0, c->stream>>>(nao, nocc, naop, c->d_ao_order, C_occ, CoT);
+        CU(cudaGetLastError());
+    }
+    double flopsA = 0.0;
+    for (int Ib = 0; Ib < c->nblk; ++Ib) flopsA += 2.0 * naux * (double)nvir * std::min(RIS_GTILE2, nao - Ib * RIS_GTILE2) * c->rb_kw[Ib];
+    {   // 3. GEMM-A, one launch per row block, batched over P
+        ProfScope ps(c, "ris_gemm_dmma(Ut=CvirT*slab^T,band)", flopsA, 8.0 * ((double)naux * c->slab_stride + (double)naux * nvir * nao));
+        for (int Ib = 0; Ib < c->nblk; ++Ib) {
+            const int col0 = c->rb_jlo[Ib] * RIS_GTILE2;
+            RisGemmParams g{};
+            g.seg[0] = RisGemmSeg{CvT + col0, naop, 0, slab + c->rb_off[Ib], c->rb_kw[Ib], c->slab_stride,
+                                  std::min(c->rb_kw[Ib], naop - col0)};
+            g.nseg = 1; g.M = nvir; g.N = std::min(RIS_GTILE2, nao - Ib * RIS_GTILE2);
+            g.C = Ut + (size_t)Ib * RIS_GTILE2; g.ldc = naop; g.bsC = (long long)nvir * naop;
+            CU((ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3, 3>(c->stream, g, naux, 0)));
+        }
+    }
+    {   // 4. GEMM-B: T[P][i][a]
+        RisGemmParams g{};
+        g.seg[0] = RisGemmSeg{CoT, naop, 0, Ut, naop, (long long)nvir * naop, nao};
+        g.nseg = 1; g.M = nocc; g.N = nvir; g.C = T; g.ldc = nvir; g.bsC = nia;
+        ProfScope ps(c, "ris_gemm_dmma(T=CoccT*Ut^T)", 2.0 * naux * (double)nocc * nvir * nao,
+                     8.0 * ((double)naux * nvir * nao + (double)naux * nia));
+        CU(ris_gemm_dense(c->stream, g, naux));
+    }
+    {   // 5. Tt[(i,a)][Q], then B[P][(i,a)] = sum_Q Minv[P][Q] Tt[(i,a)][Q]
+        ProfScope ps(c, "ris_k_transpose", 0.0, 16.0 * naux * (double)nia);
+        ris_k_transpose<<<dim3((unsigned)((nia + 31) / 32), (nauxp + 31) / 32), dim3(32, 8), 0, c->stream>>>(naux, nia, nauxp, T, Tt);
+        CU(cudaGetLastError());
+    }
+    {
+        RisGemmParams g{};
+        g.seg[0] = RisGemmSeg{Tt, nauxp, 0, c->d_minv, nauxp, 0, naux};
+        g.nseg = 1; g.M = (int)nia; g.N = naux; g.C = B_out; g.ldc = 1; g.bsC = 0;
+        g.cdiv = 1; g.cpad = (int)nia;
+        ProfScope ps(c, "ris_gemm_dmma(B=Minv*T)", 2.0 * naux * (double)naux * nia, 16.0 * naux * (double)nia);
+        CU(ris_gemm_dense(c->stream, g, 1));
+    }
+    return RIS_OK;
+}
+
+// Metric term of Eq. 27 with a FULL matrix: g[s][A] = sum_{PQ} G[s][P][Q] d(P|Q)/dR_A, positive sign.
+__global__ void __launch_bounds__(128) ris_k_grad_pq_full(int naux, const double* __restrict__ aux, const double* __restrict__ boys1,
+                                                          const double* __restrict__ G, double* __restrict__ grad)
+{
+    const int P = blockIdx.x, s = blockIdx.y;
+    const double* Gs = G + (size_t)s * naux * naux;
+    const double Px = aux[5 * P], Py = aux[5 * P + 1], Pz = aux[5 * P + 2], al = aux[5 * P + 3], fP = aux[5 * P + 4];
+    double g0 = 0.0, g1 = 0.0, g2 = 0.0;
+    for (int Q = threadIdx.x; Q < naux; Q += blockDim.x) {
+        if (Q == P) continue;
+        const double X0 = Px - aux[5 * Q], X1 = Py - aux[5 * Q + 1], X2 = Pz - aux[5 * Q + 2];
+        const double be = aux[5 * Q + 3], fQ = aux[5 * Q + 4];
+        const double sI = ris_rsqrt(al + be);
+        const double rho = al * be * sI * sI;
+        double F[2];
+        ris_boys<1>(rho * (X0 * X0 + X1 * X1 + X2 * X2), boys1, F);
+        const double w = (Gs[(size_t)P * naux + Q] + Gs[(size_t)Q * naux + P]) * fP * fQ * (2.0 * 17.493418327624862846) * sI *
+                         (-2.0 * rho) * F[1];
+        g0 = fma(w, X0, g0); g1 = fma(w, X1, g1); g2 = fma(w, X2, g2);
+    }
+    __shared__ double red[3][128];
+    red[0][threadIdx.x] = g0; red[1][threadIdx.x] = g1; red[2][threadIdx.x] = g2;
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if (threadIdx.x < o)
+            for (int x = 0; x < 3; ++x) red[x][threadIdx.x] += red[x][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) grad[((size_t)s * naux + P) * 3 + threadIdx.x] = red[threadIdx.x][0];
+}
+
+extern "C" int ris_grad_PQ_full(ris_ctx* c, int nbatch, const double* G, double* grad)
+{
+    if (!c || nbatch < 1 || !G || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    ProfScope ps(c, "ris_k_grad_pq_full", 60.0 * c->naux * (double)c->naux * nbatch, 8.0 * c->naux * (double)c->naux * nbatch);
+    ris_k_grad_pq_full<<<dim3(c->naux, nbatch), 128, 0, c->stream>>>(c->naux, c->d_aux, c->d_boys[1], G, grad);
     CU(cudaGetLastError());
     return RIS_OK;
 }

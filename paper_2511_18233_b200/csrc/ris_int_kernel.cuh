@@ -10,10 +10,13 @@
 #include "ris_core.cuh"
 #include "ris_internal.h"
 
-template <int LH, int LO, bool TR>
+// STORE: instead of the dot with a tile, the contracted integrals themselves are added to out[el * ostride] (the
+// P-minor integral buffer of ris_fit_K); tile / slot are unused then.
+template <int LH, int LO, bool TR, bool STORE>
 RIS_DEV void ris_phase0(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
                         double ZOz, double alpha, double auxfac, const double* __restrict__ boys,
-                        const double* __restrict__ tile, size_t sstride, int nb, double* __restrict__ slot)
+                        const double* __restrict__ tile, size_t sstride, int nb, double* __restrict__ slot,
+                        double* __restrict__ out, size_t ostride)
 {
     using K = RisClass0<LH, LO>;
     double acc[K::NACC];
@@ -26,7 +29,8 @@ RIS_DEV void ris_phase0(int nk, const double* __restrict__ q, double ZCx, double
         const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
         ris_prim_triplet0<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, r3.y, ZCx, ZCy, ZCz, alpha, auxfac, boys, acc);
     }
-    ris_hrr0c<LH, LO, TR, 32>(acc, ZOx, ZOy, ZOz, tile, (size_t)1, sstride, nb, slot);
+    if constexpr (STORE) ris_hrr0w<LH, LO, TR>(acc, ZOx, ZOy, ZOz, out, ostride);
+    else ris_hrr0c<LH, LO, TR, 32>(acc, ZOx, ZOy, ZOz, tile, (size_t)1, sstride, nb, slot);
 }
 
 // dynamic shared memory per warp: the task's primitive-pair and pair records + [nb][32] sums
@@ -35,8 +39,10 @@ __host__ __device__ inline size_t ris_int_warp_smem(int kmax, int nb)
     return (size_t)64 * (RIS_TASK_PRIMS + kmax) + (size_t)64 * RIS_TASK_PRIMS + (size_t)8 * nb * 32;
 }
 
-// prm.tile: J tile [nb][packed elements] (estride 1); prm.grad: v [nb][naux] (zeroed by the caller)
-template <int LA, int LB>
+// prm.tile: J tile [nb][packed elements] (estride 1); prm.grad: v [nb][naux] (zeroed by the caller).
+// STORE: prm.grad is the integral buffer [packed elements][estride] (P-minor, zeroed by the caller), element el of aux P
+// at grad[el * estride + (P - p0)]; nb is 0.
+template <int LA, int LB, bool STORE>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisGradParams prm)
 {
     constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
@@ -83,21 +89,24 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
         const double* __restrict__ q = s_prim;
         for (int j = 0; j < ip1 - ip0; ++j) {
             const RisPairRec pr = s_pair[j];
-            const double* __restrict__ tile = prm.tile + (size_t)pk.elem_off + (size_t)(ip0 + j) * NEL;
+            const double* __restrict__ tile = STORE ? nullptr : prm.tile + (size_t)pk.elem_off + (size_t)(ip0 + j) * NEL;
+            // a dead lane (P beyond the range) must not write: the phases below are skipped for it
+            double* __restrict__ out = STORE ? prm.grad + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * (size_t)prm.estride + (Pe - prm.p0)
+                                            : nullptr;
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
-            if (pr.nkA > 0)
-                ris_phase0<LA, LB, false>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
-                                          sstride, nb, s_v + lane);
+            if (pr.nkA > 0 && (!STORE || live))
+                ris_phase0<LA, LB, false, STORE>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
+                                                 sstride, nb, s_v + lane, out, (size_t)prm.estride);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
-            if (pr.nkB > 0)
-                ris_phase0<LB, LA, true>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
-                                         alpha, auxfac, prm.boys, tile, sstride, nb, s_v + lane);
+            if (pr.nkB > 0 && (!STORE || live))
+                ris_phase0<LB, LA, true, STORE>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
+                                                alpha, auxfac, prm.boys, tile, sstride, nb, s_v + lane, out, (size_t)prm.estride);
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
         task = __shfl_sync(0xffffffffu, next, 0);
     }
     __syncthreads();
-    if (warp == 0 && live) {
+    if (!STORE && warp == 0 && live) {
         for (int s = 0; s < nb; ++s) {
             double v = 0.0;
 #pragma unroll
@@ -108,14 +117,14 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
     }
 }
 
-template <int LA, int LB>
+template <int LA, int LB, bool STORE>
 void ris_launch_int(const RisGradParams& p, cudaStream_t st)
 {
     if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
     const size_t smem = RIS_GRAD_WARPS * ris_int_warp_smem(p.pk.kmax, p.nb);
     static size_t configured = 0;
     if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(ris_int_kernel<LA, LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(ris_int_kernel<LA, LB, STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = smem;
     }
     const int ny = (p.p1 - p.p0 + 31) / 32;
@@ -123,5 +132,5 @@ void ris_launch_int(const RisGradParams& p, cudaStream_t st)
     static int nsm = 0;
     if (nsm == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
     const int nx = std::max(1, std::min(nbt, (nsm * 3 + ny - 1) / ny));
-    ris_int_kernel<LA, LB><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    ris_int_kernel<LA, LB, STORE><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
 }

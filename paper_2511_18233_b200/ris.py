@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host",
-    "ris_fit_J", "ris_metric",
+    "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
     "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work", "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak",
@@ -48,6 +48,8 @@ def load_library():
     lib.ris_grad_PQ.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_fit_J.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_metric.argtypes = [vp, vp]
+    lib.ris_fit_K.argtypes = [vp, ci, ci, vp, vp, vp, vp]
+    lib.ris_grad_PQ_full.argtypes = [vp, ci, vp, vp]
     lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_grad_K_host.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ_host.argtypes = [vp, ci, vp, vp, vp]
@@ -195,6 +197,23 @@ class RisContext:
         _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux)),
                                    self._dev(c, (nb, self.naux))))
         return v, c
+
+    def fit_K(self, C_occ, C_vir):
+        """(T, B): T[P][i][a] = sum C_occ[mu,i] (mu nu|P) C_vir[nu,a], B = M^-1 T; both on the device."""
+        nocc, nvir = C_occ.shape[1], C_vir.shape[1]
+        T = self._torch.empty((self.naux, nocc, nvir), dtype=self._torch.float64, device=self.device)
+        B = self._torch.empty((self.naux, nocc, nvir), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_fit_K(self._h, nocc, nvir, self._dev(C_occ, (self.nao, nocc)), self._dev(C_vir, (self.nao, nvir)),
+                                   self._dev(T, (self.naux, nocc, nvir)), self._dev(B, (self.naux, nocc, nvir))))
+        return T, B
+
+    def grad_PQ_full(self, G, out=None):
+        nb = G.shape[0]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        _check(self._lib.ris_grad_PQ_full(self._h, nb, self._dev(G, (nb, self.naux, self.naux)),
+                                          self._dev(out, (nb, self.natoms, 3))))
+        return out
 
     def metric(self):
         M = self._torch.empty((self.naux, self.naux), dtype=self._torch.float64, device=self.device)

@@ -97,3 +97,57 @@ def test_fit_J_full_size_config3():
     res = c @ M_ref - v
     assert np.abs(res).max() <= 1e-11 * np.abs(v).max() * max(1.0, np.abs(M_ref).max())
     ctx.close()
+
+
+# ------------------------------------------------------------------ K-type fitting step
+
+def _check_fit_K(mol, C_occ, C_vir, what):
+    ctx = ris_setup(mol)
+    T, B = ctx.fit_K(dev(C_occ), dev(C_vir))
+    T_ref, B_ref, e_ref = orc.fit_K(mol, C_occ, C_vir)
+    assert_parity(T.cpu().numpy(), T_ref, what + " T")
+    M_ref = orc.metric(mol)
+    cond = np.linalg.cond(M_ref)
+    ctol = 64.0 * cond * EPS
+    Bh = B.cpu().numpy()
+    assert np.abs(Bh - B_ref).max() <= ctol * np.abs(B_ref).max(), (what, np.abs(Bh - B_ref).max(), ctol)
+    n = M_ref.shape[0]
+    res = M_ref @ Bh.reshape(n, -1) - T_ref.reshape(n, -1)
+    assert np.abs(res).max() <= 1e-12 * np.abs(T_ref).max() * max(1.0, np.abs(M_ref).max()), (what, np.abs(res).max())
+    # composed RI-K gradient with the DEVICE B: G_K(C_occ, C_vir, B) - 1/2 G_PQ_full(B B^T)   (Eq. 27)
+    Bf = B.reshape(n, -1)
+    G = (Bf @ Bf.T)[None].contiguous()
+    g = (ctx.grad_K(dev(C_occ), dev(C_vir), B[None].contiguous()) - 0.5 * ctx.grad_PQ_full(G)).cpu().numpy()[0]
+    g_ref = orc.grad_RIK(mol, C_occ, C_vir)
+    gscale = max(1.0, np.abs(orc.grad_K(mol, C_occ, C_vir, B_ref[None])[0]).max())
+    assert np.abs(g - g_ref).max() <= max(ctol, 5e-14) * gscale, (what, np.abs(g - g_ref).max(), ctol * gscale)
+    e = 0.5 * float((T * B).sum())
+    assert abs(e - e_ref) <= max(ctol, 1e-13) * abs(e_ref)
+    ctx.close()
+
+
+def test_grad_PQ_full_parity_and_rank_one():
+    wl = synth.make_workload(2)
+    ctx = ris_setup(wl.mol)
+    rng = np.random.default_rng(3)
+    n = wl.mol.natoms
+    G = rng.standard_normal((2, n, n))
+    assert_parity(ctx.grad_PQ_full(dev(G)).cpu().numpy(), orc.grad_PQ_full(wl.mol, G), "PQ full")
+    c, d = rng.standard_normal((2, n)), rng.standard_normal((2, n))
+    r1 = ctx.grad_PQ_full(dev(np.einsum("sp,sq->spq", c, d))).cpu().numpy()
+    assert_parity(r1, ctx.grad_PQ(dev(c), dev(d)).cpu().numpy(), "PQ full rank one")
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_fit_K_small_configs(cfg):
+    wl = synth.make_workload(cfg)
+    _check_fit_K(wl.mol, wl.C_occ, wl.C_vir, f"config {cfg}")
+
+
+def test_fit_K_all_classes_up_to_f_ragged_sizes():
+    """Every class incl. f shells; odd nao / nocc / nvir / naux exercise the padded leading dimensions."""
+    mol = synth.tiny_molecule(22, [[0, 1, 2, 3], [3, 2, 0], [1, 3]],
+                              [[0, 0, 0], [1.9, 0.4, -0.3], [-0.8, 1.7, 1.0]], nprim=2)
+    rng = np.random.default_rng(4)
+    _check_fit_K(mol, rng.standard_normal((mol.nao, 3)), rng.standard_normal((mol.nao, 5)), "all classes")
