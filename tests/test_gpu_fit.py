@@ -151,3 +151,23 @@ def test_fit_K_all_classes_up_to_f_ragged_sizes():
                               [[0, 0, 0], [1.9, 0.4, -0.3], [-0.8, 1.7, 1.0]], nprim=2)
     rng = np.random.default_rng(4)
     _check_fit_K(mol, rng.standard_normal((mol.nao, 3)), rng.standard_normal((mol.nao, 5)), "all classes")
+
+
+def test_fit_K_full_size_config4_sampled_aux():
+    """Config 4 (300 atoms, 3000 AO, nocc 525, nvir 1050) at full size, in the launch configuration bench.py times:
+    T[P] against the oracle for sampled aux P (each T[P] = C_occ^T (mu nu|P) C_vir is an output the oracle computes on
+    its own; oracle primitive cutoff 1e-22, DESIGN.md R-screen), B through the residual M B = T."""
+    wl = synth.make_workload(4)
+    ctx = ris_setup(wl.mol, schwarz_tol=wl.schwarz_tol)
+    T, B = ctx.fit_K(dev(wl.C_occ), dev(wl.C_vir))
+    scale = float(T.abs().max())
+    for P in (0, 149, 299):
+        ref = wl.C_occ.T @ orc.int3c(wl.mol, P, prim_cutoff=1e-22) @ wl.C_vir
+        err = np.abs(T[P].cpu().numpy() - ref)
+        assert np.all(err <= 1e-10 * np.abs(ref) + 1e-12 * scale), (P, err.max(), scale)
+        assert err.max() <= 5e-14 * scale
+    M = torch.as_tensor(orc.metric(wl.mol), device="cuda")
+    n = M.shape[0]
+    res = (M @ B.reshape(n, -1) - T.reshape(n, -1)).abs().max().item()
+    assert res <= 1e-11 * scale * max(1.0, float(M.abs().max())), res
+    ctx.close()
