@@ -313,3 +313,57 @@ def grad_RIK(mol, C_occ, C_vir, *, prim_cutoff=0.0):
     gK, _ = grad_K(mol, C_occ, C_vir, B[None], prim_cutoff=prim_cutoff)
     Bf = B.reshape(n, -1)
     return gK[0] - 0.5 * grad_PQ_full(mol, (Bf @ Bf.T)[None])[0]
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1, the composed term <g^ris,(xi); {D1, D2}> of Eqs. 25-27 for two AO matrices D1, D2
+# (Eq. 38-39: <g; {D1, D2}> = sum_{pqrs} g_{pq,rs} [D1]_pq [D2]_rs), with Eq. 5 / 21 read in the
+# index order of Eq. 39, g_{pq,rs} = (pq|rs) - c_x (ps|rq):
+#   S(R) = sum_AB M^-1_AB ( Tr[I^A D1] Tr[I^B D2] - c_x sum_{pqrs} I^A_ps I^B_rq D1_pq D2_rs ),   I^A_pq = (pq|A)
+# written out in the AO basis with dense matrices (tiny molecules only).  Its derivative at FIXED D1, D2 by Eq. 27:
+#   J part:  G_J(D1, c2) + G_J(D2, c1) - G_PQ(c1, c2),                c_i = M^-1 Tr[I D_i]
+#   K part:  sum_A <I^A,xi; G1^A + G2^A> - sum_CD N_CD M^xi_CD,
+#            G1^A = sum_B M^-1_AB D1 I^B D2,  G2^A = sum_B M^-1_AB D1^T I^B D2^T,  N = M^-1 K M^-1,
+#            K_AB = sum_ps I^A_ps (D1 I^B D2)_ps.
+def ris_pair_scalar(mol, D1, D2, c_x):
+    n = np.asarray(mol.coords).shape[0]
+    I = [int3c(mol, P) for P in range(n)]
+    Minv = np.linalg.inv(metric(mol))
+    v1 = np.array([np.sum(I[A] * D1) for A in range(n)])
+    v2 = np.array([np.sum(I[A] * D2) for A in range(n)])
+    K = np.array([[np.sum(I[A] * (D1 @ I[B] @ D2)) for B in range(n)] for A in range(n)])
+    return float(v1 @ Minv @ v2 - c_x * np.sum(Minv * K))
+
+
+def grad_dense_K(mol, G):
+    """sum_P sum_{mu nu} G[P][mu][nu] d(mu nu|P)/dR for dense AO matrices G[P] (the K-type contraction of
+    ris_oracle_contract_P with the matrices given directly)."""
+    h = _Held(mol)
+    G = _f64(G).reshape(h.natoms, h.nao, h.nao)
+    g = np.zeros((1, h.natoms, 3), dtype=np.longdouble)
+    e = np.zeros(1, dtype=np.longdouble)
+    one = np.ones(1)
+    for P in range(h.natoms):
+        GP = _f64(G[P])
+        rc = lib().ris_oracle_contract_P(C.byref(h.c), P, 1, GP.ctypes.data, one.ctypes.data, None, 0.0,
+                                         g.ctypes.data, e.ctypes.data)
+        assert rc == 0
+    return g.astype(np.float64)[0]
+
+
+def ris_pair_gradient(mol, D1, D2, c_x):
+    n = np.asarray(mol.coords).shape[0]
+    I = [int3c(mol, P) for P in range(n)]
+    Minv = np.linalg.inv(metric(mol))
+    v1 = np.array([np.sum(I[A] * D1) for A in range(n)])
+    v2 = np.array([np.sum(I[A] * D2) for A in range(n)])
+    c1, c2 = Minv @ v1, Minv @ v2
+    gJ = grad_J(mol, D1[None], c2[None])[0][0] + grad_J(mol, D2[None], c1[None])[0][0] \
+        - grad_PQ(mol, c1[None], c2[None])[0][0]
+    K = np.array([[np.sum(I[A] * (D1 @ I[B] @ D2)) for B in range(n)] for A in range(n)])
+    N = Minv @ K @ Minv
+    X1 = [D1 @ I[B] @ D2 for B in range(n)]
+    X2 = [D1.T @ I[B] @ D2.T for B in range(n)]
+    G = np.stack([sum(Minv[A, B] * (X1[B] + X2[B]) for B in range(n)) for A in range(n)])
+    gK = grad_dense_K(mol, G) - grad_PQ_full(mol, N[None])[0]
+    return gJ - c_x * gK

@@ -181,3 +181,40 @@ def test_fitted_K_energy_finite_difference():
         fd = (orc.fit_K(mp_, Co, Cv)[2] - orc.fit_K(mm_, Co, Cv)[2]) / (2 * h)
         assert abs(g[atom, d] - fd) < 5e-7 * scale, (atom, d, g[atom, d], fd)
     assert np.all(np.abs(g.sum(axis=0)) < 1e-10 * np.abs(g).sum())
+
+
+# ------------------------------------------------------------------ composed <g^ris,(xi); {D1, D2}>
+
+def test_ris_pair_gradient_finite_difference():
+    """Eq. 27 for the full ris kernel of Eq. 21 (Coulomb and exchange pairing, c_x = 0.25), D1 != D2, neither
+    symmetric: central differences of S(R) = <g^ris(R); {D1, D2}> at fixed AO matrices."""
+    mol, D = _tiny()
+    D1, D2 = D[0] + 0.3 * D[1], D[1]
+    cx = 0.25
+    g = orc.ris_pair_gradient(mol, D1, D2, cx)
+    h = 5e-6
+    scale = np.abs(g).max()
+    for atom, d in itertools.product(range(3), range(3)):
+        mp_, mm_ = copy.copy(mol), copy.copy(mol)
+        mp_.coords = mol.coords.copy(); mp_.coords[atom, d] += h
+        mm_.coords = mol.coords.copy(); mm_.coords[atom, d] -= h
+        fd = (orc.ris_pair_scalar(mp_, D1, D2, cx) - orc.ris_pair_scalar(mm_, D1, D2, cx)) / (2 * h)
+        assert abs(g[atom, d] - fd) < 5e-7 * scale, (atom, d, g[atom, d], fd)
+    assert np.all(np.abs(g.sum(axis=0)) < 1e-10 * np.abs(g).sum())
+
+
+def test_ris_pair_scalar_exchange_index_pairing():
+    """The exchange term pairs (ps|A)(B|rq): for rank-one D1 = x y^T, D2 = z w^T it factorises into
+    sum_AB M^-1_AB (x^T I^A w)(z^T I^B y); the Coulomb term into (x^T I^A y)(z^T I^B w)."""
+    mol, _ = _tiny()
+    rng = np.random.default_rng(11)
+    nao = sum(synth.ncart(int(l)) for l in mol.shell_l)
+    x, y, z, w = rng.standard_normal((4, nao))
+    I = [orc.int3c(mol, P) for P in range(3)]
+    Minv = np.linalg.inv(orc.metric(mol))
+    coul = sum(Minv[A, B] * (x @ I[A] @ y) * (z @ I[B] @ w) for A in range(3) for B in range(3))
+    exch = sum(Minv[A, B] * (x @ I[A] @ w) * (z @ I[B] @ y) for A in range(3) for B in range(3))
+    D1, D2 = np.outer(x, y), np.outer(z, w)
+    assert abs(orc.ris_pair_scalar(mol, D1, D2, 0.0) - coul) < 1e-12 * abs(coul)
+    s = orc.ris_pair_scalar(mol, D1, D2, 1.0)
+    assert abs((coul - s) - exch) < 1e-11 * max(abs(exch), abs(coul))
