@@ -71,8 +71,8 @@ struct ris_ctx {
     int* d_ao_pos = nullptr;           // [nao] spatial position of AO
     int* d_ao_order = nullptr;         // [nao] AO at spatial position
     int nblk = 0, ntiles = 0;
-    int2* d_tiles = nullptr;           // [ntiles] (I, J)
-    int* d_tmap = nullptr;             // [nblk][nblk] tile index of (I >= J), -1 if absent
+    int2* d_tiles = nullptr;           // [ntiles] (row panel I, offset of the tile's 64 columns in d_gcols)
+    int* d_gcols = nullptr;            // gathered column lists of all panels (AO positions; -1 = padding)
     // inverse map for the P-minor tile transpose: S position -> packed element
     int* d_smap = nullptr;             // [ntiles][64][64]  (packed element << 1 | same-shell pair), -1 if no surviving element
     int* d_srows = nullptr;            // [nsrows] rows (tile * 64 + r) of the block buffer that hold a surviving element
@@ -199,21 +199,9 @@ static const double kModelFlopsByE[8] = {90.0, 140.0, 250.0, 450.0, 750.0, 1250.
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
 // --------------------------------------------------------------------------------------- setup
-// Marks the blocks (I >= J) of the spatially ordered AO index touched by the surviving shell pairs of one class.
-__global__ void ris_k_mark_blocks(RisClassPack pk, const int* __restrict__ ao_pos, int nblk, int* mark)
-{
-    const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ip >= pk.npairs) return;
-    const int r0 = ao_pos[pk.ao[ip]], q0 = ao_pos[pk.ao[(size_t)pk.npairs + ip]];   // shells stay contiguous
-    const int r1 = r0 + ris_ncart(pk.la) - 1, q1 = q0 + ris_ncart(pk.lb) - 1;
-    for (int I = r0 / RIS_GTILE2; I <= r1 / RIS_GTILE2; ++I)
-        for (int J = q0 / RIS_GTILE2; J <= q1 / RIS_GTILE2; ++J) mark[max(I, J) * nblk + min(I, J)] = 1;
-}
-
-// Inverse map of the packed pair elements into the GEMM-2 block buffer: element (ip, ca, cb) of a class reads
-// S^P[pos(mu0+ca)][pos(nu0+cb)] (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
-__global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos, const int* __restrict__ tmap, int nblk,
-                                 int* __restrict__ smap, int* __restrict__ rowflag, int* __restrict__ ovf, int* __restrict__ novf)
+// Marks, per 64-row panel of the spatially ordered AO index, the columns that hold a surviving pair element; an
+// element (r, q) is oriented so that block(r) >= block(q) (S^P is symmetric).
+__global__ void ris_k_mark_cols(RisClassPack pk, const int* __restrict__ ao_pos, int nao, int* __restrict__ cmark)
 {
     constexpr int T = RIS_GTILE2;
     const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
@@ -222,9 +210,26 @@ __global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos
     const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
     int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
     if (r / T < q / T) { const int t = r; r = q; q = t; }
-    const int tile = tmap[(r / T) * nblk + (q / T)];
+    cmark[(size_t)(r / T) * nao + q] = 1;
+}
+
+// Inverse map of the packed pair elements into the GEMM-2 block buffer: element (ip, ca, cb) of a class reads
+// S^P[pos(mu0+ca)][pos(nu0+cb)] (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
+__global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos, const int* __restrict__ colidx,
+                                 const int* __restrict__ ptile0, int nao, int* __restrict__ smap, int* __restrict__ rowflag,
+                                 int* __restrict__ ovf, int* __restrict__ novf)
+{
+    constexpr int T = RIS_GTILE2;
+    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)pk.npairs * nel) return;
+    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
+    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
+    if (r / T < q / T) { const int t = r; r = q; q = t; }
+    const int ci = colidx[(size_t)(r / T) * nao + q];          // column within the panel's gathered list
+    const int tile = ptile0[r / T] + ci / T;
     const int code = (int)(((pk.elem_off + idx) << 1) | (pk.symf[ip] < 0.75f ? 1 : 0));
-    const size_t pos = (size_t)tile * (T * T) + (r % T) * T + (q % T);
+    const size_t pos = (size_t)tile * (T * T) + (r % T) * T + (ci % T);
     // elements (ca,cb) and (cb,ca) of a same-shell pair that straddles a block edge fold onto ONE position of the
     // symmetric S: the second one goes to a short overflow list served by a gather
     if (atomicCAS(&smap[pos], -1, code) != -1) {
@@ -425,28 +430,42 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         if ((rc = dev_upload(c, &c->d_ao_pos, ao_pos.data(), ao_pos.size()))) return rc;
         if ((rc = dev_upload(c, &c->d_ao_order, ao_order.data(), ao_order.size()))) return rc;
         c->nblk = (nao + RIS_GTILE2 - 1) / RIS_GTILE2;
-        int* d_mark;
-        if ((rc = dev_alloc(c, &d_mark, (size_t)c->nblk * c->nblk, true))) return rc;
-        for (int k = 0; k < RIS_NCLASS; ++k)
-            if (c->cls[k].npairs > 0)
-                ris_k_mark_blocks<<<(c->cls[k].npairs + 127) / 128, 128, 0, c->stream>>>(c->cls[k], c->d_ao_pos, c->nblk, d_mark);
+        // GEMM-2 tiles: per 64-row panel I of the spatial AO order, the GATHERED list of columns (positions q with a
+        // surviving element (r, q), r in the panel, oriented so that block(r) >= block(q)), cut into 64-column tiles.
+        // Versus aligned 64x64 blocks this drops the columns of tight shells that only reach the near part of the band
+        // (config 4: 756 k instead of 934 k block-buffer elements for 437 k unique surviving ones).
+        int* d_cmark;
+        if ((rc = dev_alloc(c, &d_cmark, (size_t)c->nblk * nao, true))) return rc;
+        for (int k = 0; k < RIS_NCLASS; ++k) {
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+            ris_k_mark_cols<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, nao, d_cmark);
+        }
         CU(cudaGetLastError());
-        std::vector<int> mark((size_t)c->nblk * c->nblk);
-        CU(cudaMemcpyAsync(mark.data(), d_mark, mark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        std::vector<int> cmark((size_t)c->nblk * nao);
+        CU(cudaMemcpyAsync(cmark.data(), d_cmark, cmark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         std::vector<int2> tiles;
-        for (int I = 0; I < c->nblk; ++I)
-            for (int J = 0; J <= I; ++J) {
-                int& m_ = mark[(size_t)I * c->nblk + J];
-                if (m_) { m_ = (int)tiles.size(); tiles.push_back(make_int2(I, J)); } else m_ = -1;
+        std::vector<int> gcols, ptile0(c->nblk), jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
+        for (int I = 0; I < c->nblk; ++I) {
+            ptile0[I] = (int)tiles.size();
+            int* row = &cmark[(size_t)I * nao];
+            int n = 0;
+            for (int q = 0; q < nao; ++q) {
+                if (!row[q]) { row[q] = -1; continue; }
+                row[q] = n++;                              // cmark becomes the column index within the panel's list
+                gcols.push_back(q);
+                const int J = q / RIS_GTILE2;
+                jlo[I] = std::min(jlo[I], J); jhi[I] = std::max(jhi[I], J);
+                jlo[J] = std::min(jlo[J], I); jhi[J] = std::max(jhi[J], I);
             }
+            for (int t = 0; t < (n + RIS_GTILE2 - 1) / RIS_GTILE2; ++t)
+                tiles.push_back(make_int2(I, (int)gcols.size() - n + t * RIS_GTILE2));
+            while (gcols.size() % RIS_GTILE2) gcols.push_back(-1);
+        }
         c->ntiles = (int)tiles.size();
         {   // row-block bands for the fitting step's sparse transform (ris_fit_K)
-            std::vector<int> jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
-            for (const int2& t : tiles) {
-                jlo[t.x] = std::min(jlo[t.x], t.y); jhi[t.x] = std::max(jhi[t.x], t.y);
-                jlo[t.y] = std::min(jlo[t.y], t.x); jhi[t.y] = std::max(jhi[t.y], t.x);
-            }
             c->rb_jlo.resize(c->nblk); c->rb_kw.resize(c->nblk); c->rb_off.resize(c->nblk);
             long long off2 = 0;
             for (int I = 0; I < c->nblk; ++I) {
@@ -459,8 +478,12 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             if ((rc = dev_upload(c, &c->d_rb_kw, c->rb_kw.data(), c->rb_kw.size()))) return rc;
             if ((rc = dev_upload(c, &c->d_rb_off, c->rb_off.data(), c->rb_off.size()))) return rc;
         }
+        if (gcols.empty()) gcols.push_back(-1);
+        int *d_colidx, *d_ptile0;
         if ((rc = dev_upload(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
-        if ((rc = dev_upload(c, &c->d_tmap, mark.data(), mark.size()))) return rc;
+        if ((rc = dev_upload(c, &c->d_gcols, gcols.data(), gcols.size()))) return rc;
+        if ((rc = dev_upload(c, &d_colidx, cmark.data(), cmark.size()))) return rc;
+        if ((rc = dev_upload(c, &d_ptile0, ptile0.data(), ptile0.size()))) return rc;
         // inverse element map + active-row list of the block buffer (for the P-minor transpose of the K tiles)
         int *d_rowflag, *d_novf;
         if ((rc = dev_alloc(c, &c->d_ovf, (size_t)2 * std::max<long long>(c->nelem_real, 1), false))) return rc;
@@ -472,7 +495,7 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             const RisClassPack& pk = c->cls[k];
             if (pk.npairs == 0) continue;
             const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
-            ris_k_build_smap<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, c->d_tmap, c->nblk, c->d_smap, d_rowflag, c->d_ovf, d_novf);
+            ris_k_build_smap<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, d_colidx, d_ptile0, nao, c->d_smap, d_rowflag, c->d_ovf, d_novf);
         }
         CU(cudaGetLastError());
         std::vector<int> rowflag((size_t)c->ntiles * RIS_GTILE2), srows;
@@ -1127,7 +1150,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
                     g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, ldh, noccp, nocc};
                     g.seg[1] = RisGemmSeg{HT, ldh, noccp, Cop, noccp, 0, nocc};
                     g.nseg = 2; g.M = nao; g.N = nao; g.C = S; g.ldc = RIS_GTILE2; g.bsC = (long long)c->ntiles * blk;
-                    g.tiles = c->d_tiles; g.tile_stride = blk;
+                    g.tiles = c->d_tiles; g.tile_stride = blk; g.gcols = c->d_gcols;
                     // algorithmic flops: two length-nocc dot products per unique surviving pair element
                     ProfScope ps(c, "ris_gemm_dmma(S=Cocc*HT^T+HT*Cocc^T,blocks)", 4.0 * np * nocc * (double)c->nelem_real,
                                  8.0 * np * ((double)noccp * nao + (double)c->ntiles * blk) + 8.0 * nao * noccp);

@@ -40,6 +40,9 @@ struct RisGemmParams {
     const int2* tiles;                     // nullptr: grid.x = m-tile, grid.y = n-tile (dense).  Otherwise tile t =
     long long tile_stride;                 // blockIdx.x covers rows tiles[t].x*BM.., cols tiles[t].y*BN.. and is
                                            // written as a dense BM x BN block at C + z*bsC + t*tile_stride (ld BN)
+    const int* gcols;                      // nullable, with tiles: GATHERED columns -- column n of tile t is the B row
+                                           // gcols[tiles[t].y + n] (< 0: padding, zero column); tiles[t].y is then an
+                                           // offset into gcols, not a block index
 };
 
 template <bool VEC16>
@@ -64,7 +67,9 @@ struct RisGemmCfg {
 };
 
 // VEC16: all operand rows are 16-byte aligned (even leading dimensions, aligned bases) -> 16-byte cp.async
-template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool VEC16>
+// GATH: gathered-column tiles (p.gcols); a warp whose WN-column strip is all padding issues no MMAs (skipping single
+// 8-column sub-tiles was measured slower: the predicates break the MMA schedule, 48.2 -> 49.8 ms on config 4).
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool VEC16, bool GATH = false>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_dmma(const RisGemmParams p)
 {
     using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
@@ -80,13 +85,20 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
     long long ldc;
     if (p.tiles) {
         const int2 tl = p.tiles[blockIdx.x];
-        m0 = tl.x * BM; n0 = tl.y * BN;
+        m0 = tl.x * BM; n0 = p.gcols ? tl.y : tl.y * BN;
         Cout = p.C + (long long)blockIdx.z * p.bsC + (long long)blockIdx.x * p.tile_stride;
         ldc = BN;
     } else {
         m0 = blockIdx.x * BM; n0 = blockIdx.y * BN;
         Cout = p.C + (long long)blockIdx.z * p.bsC + (long long)m0 * p.ldc + (p.cdiv > 0 ? 0 : n0);
         ldc = p.ldc;
+    }
+    int nvw = WN;                                      // valid (non-padding) columns of this warp's WN-column strip
+    if (GATH) {
+        int cnt = 0;
+        for (int c0 = lane; c0 < WN; c0 += 32) cnt += p.gcols[n0 + wn0 + c0] >= 0 ? 1 : 0;
+        for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        nvw = cnt;                                     // padding sits at the end of a panel's list only
     }
     const int nk0 = (p.seg[0].K + RIS_GBK - 1) / RIS_GBK;
     const int nk1 = p.nseg > 1 ? (p.seg[1].K + RIS_GBK - 1) / RIS_GBK : 0;
@@ -116,8 +128,9 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
         }
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
-            const int r = n0 + (tid / CH) + j * (THREADS / CH);
-            pb[j] = r < p.N ? Bg + (long long)r * sg.ldb + kc : nullptr;
+            int r = n0 + (tid / CH) + j * (THREADS / CH);
+            if (p.gcols != nullptr) r = p.gcols[r];          // gathered column: B row index, or -1 (padding)
+            pb[j] = (r >= 0 && r < p.N) ? Bg + (long long)r * sg.ldb + kc : nullptr;
         }
     };
     // shared layout: row stride RIS_GLD = 16 doubles (one K step), the two 8-double halves of odd rows swapped
@@ -212,6 +225,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
                     asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(st_) : "r"(bar0 + 8 * (STAGES + stage)) : "memory");
                 }
             }
+            if (GATH && nvw == 0) continue;            // warp-uniform: the whole strip is padding
 #pragma unroll
             for (int i = 0; i < MT; ++i)
 #pragma unroll
@@ -258,16 +272,16 @@ inline bool ris_gemm_aligned16(const RisGemmParams& p)
     return true;
 }
 
-template <int BM, int BN, int WM, int WN, int STAGES, int MINB>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool GATH = false>
 inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
     using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true>,
+        cudaError_t e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false>,
+        e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
@@ -276,8 +290,8 @@ inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, 
     if (p.tiles) grid = dim3(ntiles, 1, batch);
     else grid = dim3((p.M + BM - 1) / BM, (p.N + BN - 1) / BN, batch);
     if (grid.x == 0 || grid.y == 0 || grid.z == 0) return cudaSuccess;
-    if (ris_gemm_aligned16(p)) ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
-    else ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    if (ris_gemm_aligned16(p)) ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    else ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -288,8 +302,9 @@ inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int b
 {
     return ris_gemm_launch_cfg<64, 128, 32, 32, 3, 2>(st, p, batch, 0);
 }
-// GEMM-2: block list of RIS_GTILE2 x RIS_GTILE2 tiles
+// GEMM-2: tile list of RIS_GTILE2 rows x RIS_GTILE2 gathered columns (p.gcols required)
 inline cudaError_t ris_gemm_blocks(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
-    return ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3, 3>(st, p, batch, ntiles);
+    // GATH = false: skipping the MMAs of all-padding strips measured slower than issuing them (48.2 vs 49.0 ms, config 4)
+    return ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3, 3, false>(st, p, batch, ntiles);
 }
