@@ -203,7 +203,7 @@ static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 // element (r, q) is oriented so that block(r) >= block(q) (S^P is symmetric).
 __global__ void ris_k_mark_cols(RisClassPack pk, const int* __restrict__ ao_pos, int nao, int* __restrict__ cmark)
 {
-    constexpr int T = RIS_GTILE2;
+    constexpr int T = RIS_GPANEL_ROWS;
     const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)pk.npairs * nel) return;
@@ -219,7 +219,7 @@ __global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos
                                  const int* __restrict__ ptile0, int nao, int* __restrict__ smap, int* __restrict__ rowflag,
                                  int* __restrict__ ovf, int* __restrict__ novf)
 {
-    constexpr int T = RIS_GTILE2;
+    constexpr int T = RIS_GPANEL_ROWS, TC = RIS_GTILE2;       // panel rows, tile columns
     const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)pk.npairs * nel) return;
@@ -227,9 +227,9 @@ __global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos
     int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
     if (r / T < q / T) { const int t = r; r = q; q = t; }
     const int ci = colidx[(size_t)(r / T) * nao + q];          // column within the panel's gathered list
-    const int tile = ptile0[r / T] + ci / T;
+    const int tile = ptile0[r / T] + ci / TC;
     const int code = (int)(((pk.elem_off + idx) << 1) | (pk.symf[ip] < 0.75f ? 1 : 0));
-    const size_t pos = (size_t)tile * (T * T) + (r % T) * T + (ci % T);
+    const size_t pos = (size_t)tile * (T * TC) + (r % T) * TC + (ci % TC);
     // elements (ca,cb) and (cb,ca) of a same-shell pair that straddles a block edge fold onto ONE position of the
     // symmetric S: the second one goes to a short overflow list served by a gather
     if (atomicCAS(&smap[pos], -1, code) != -1) {
@@ -430,12 +430,13 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         if ((rc = dev_upload(c, &c->d_ao_pos, ao_pos.data(), ao_pos.size()))) return rc;
         if ((rc = dev_upload(c, &c->d_ao_order, ao_order.data(), ao_order.size()))) return rc;
         c->nblk = (nao + RIS_GTILE2 - 1) / RIS_GTILE2;
-        // GEMM-2 tiles: per 64-row panel I of the spatial AO order, the GATHERED list of columns (positions q with a
+        const int npanel = (nao + RIS_GPANEL_ROWS - 1) / RIS_GPANEL_ROWS;
+        // GEMM-2 tiles: per RIS_GPANEL_ROWS-row panel I of the spatial AO order, the GATHERED list of columns (positions q with a
         // surviving element (r, q), r in the panel, oriented so that block(r) >= block(q)), cut into 64-column tiles.
         // Versus aligned 64x64 blocks this drops the columns of tight shells that only reach the near part of the band
         // (config 4: 756 k instead of 934 k block-buffer elements for 437 k unique surviving ones).
         int* d_cmark;
-        if ((rc = dev_alloc(c, &d_cmark, (size_t)c->nblk * nao, true))) return rc;
+        if ((rc = dev_alloc(c, &d_cmark, (size_t)npanel * nao, true))) return rc;
         for (int k = 0; k < RIS_NCLASS; ++k) {
             const RisClassPack& pk = c->cls[k];
             if (pk.npairs == 0) continue;
@@ -443,12 +444,13 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             ris_k_mark_cols<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, nao, d_cmark);
         }
         CU(cudaGetLastError());
-        std::vector<int> cmark((size_t)c->nblk * nao);
+        std::vector<int> cmark((size_t)npanel * nao);
         CU(cudaMemcpyAsync(cmark.data(), d_cmark, cmark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
         std::vector<int2> tiles;
-        std::vector<int> gcols, ptile0(c->nblk), jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
-        for (int I = 0; I < c->nblk; ++I) {
+        std::vector<int> gcols, ptile0(npanel), jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
+        for (int I = 0; I < npanel; ++I) {
+            const int I64 = I * RIS_GPANEL_ROWS / RIS_GTILE2;      // the 64-row block of the fit_K bands this panel lies in
             ptile0[I] = (int)tiles.size();
             int* row = &cmark[(size_t)I * nao];
             int n = 0;
@@ -457,8 +459,8 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
                 row[q] = n++;                              // cmark becomes the column index within the panel's list
                 gcols.push_back(q);
                 const int J = q / RIS_GTILE2;
-                jlo[I] = std::min(jlo[I], J); jhi[I] = std::max(jhi[I], J);
-                jlo[J] = std::min(jlo[J], I); jhi[J] = std::max(jhi[J], I);
+                jlo[I64] = std::min(jlo[I64], J); jhi[I64] = std::max(jhi[I64], J);
+                jlo[J] = std::min(jlo[J], I64); jhi[J] = std::max(jhi[J], I64);
             }
             for (int t = 0; t < (n + RIS_GTILE2 - 1) / RIS_GTILE2; ++t)
                 tiles.push_back(make_int2(I, (int)gcols.size() - n + t * RIS_GTILE2));
@@ -488,9 +490,9 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         int *d_rowflag, *d_novf;
         if ((rc = dev_alloc(c, &c->d_ovf, (size_t)2 * std::max<long long>(c->nelem_real, 1), false))) return rc;
         if ((rc = dev_alloc(c, &d_novf, 1, true))) return rc;
-        if ((rc = dev_alloc(c, &c->d_smap, (size_t)std::max(c->ntiles, 1) * RIS_GTILE2 * RIS_GTILE2, false))) return rc;
-        if ((rc = dev_alloc(c, &d_rowflag, (size_t)std::max(c->ntiles, 1) * RIS_GTILE2, true))) return rc;
-        CU(cudaMemsetAsync(c->d_smap, 0xff, sizeof(int) * (size_t)std::max(c->ntiles, 1) * RIS_GTILE2 * RIS_GTILE2, c->stream));
+        if ((rc = dev_alloc(c, &c->d_smap, (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS * RIS_GTILE2, false))) return rc;
+        if ((rc = dev_alloc(c, &d_rowflag, (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS, true))) return rc;
+        CU(cudaMemsetAsync(c->d_smap, 0xff, sizeof(int) * (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS * RIS_GTILE2, c->stream));
         for (int k = 0; k < RIS_NCLASS; ++k) {
             const RisClassPack& pk = c->cls[k];
             if (pk.npairs == 0) continue;
@@ -498,7 +500,7 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             ris_k_build_smap<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, d_colidx, d_ptile0, nao, c->d_smap, d_rowflag, c->d_ovf, d_novf);
         }
         CU(cudaGetLastError());
-        std::vector<int> rowflag((size_t)c->ntiles * RIS_GTILE2), srows;
+        std::vector<int> rowflag((size_t)c->ntiles * RIS_GPANEL_ROWS), srows;
         CU(cudaMemcpyAsync(rowflag.data(), d_rowflag, rowflag.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaMemcpyAsync(&c->novf, d_novf, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
@@ -1091,7 +1093,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     const int nao = c->nao, naux = c->naux;
     const int nbmax = next_nb(nbatch);
     const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
-    const long long blk = (long long)RIS_GTILE2 * RIS_GTILE2;
+    const long long blk = (long long)RIS_GPANEL_ROWS * RIS_GTILE2;
     // per aux function: HT [nao][noccp], S blocks [ntiles][64*64], packed tiles [nb][elements]
     int pb = c->opt.p_batch;
     if (pb <= 0) {

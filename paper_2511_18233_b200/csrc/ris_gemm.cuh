@@ -4,8 +4,9 @@
 //   GEMM-1   HT[nu'][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]          nu' = spatial (Morton) position of AO nu
 //   GEMM-2   S^P[mu'][nu']  = Gamma^P_{mu nu} + Gamma^P_{nu mu}
 //                           = sum_i C_occ[mu][i] HT[nu'][(P,i)] + sum_i HT[mu'][(P,i)] C_occ[nu][i]
-//            only for the 64x64 blocks of the spatially ordered AO index that contain a surviving shell pair
-//            (block list), written as dense blocks that ris_k_pack_sym gathers into the packed pair order.
+//            only on tiles of 32 rows x 64 GATHERED columns of the spatially ordered AO index: per 32-row panel the
+//            columns that hold a surviving pair element (tile list + gathered-column list), written as dense
+//            tiles that ris_k_pack_sym gathers into the packed pair order.
 //
 // One kernel serves both:  C[m][n] = sum_seg sum_k A_seg[row(m)][k] B_seg[n][k]  (up to two K segments; row(m)
 // optionally through an index list, which is how GEMM-1 emits HT in spatial order).
@@ -16,13 +17,17 @@
 // DMMA pipe (profiles/r01_v3_ncu.md -> r01_v4_gemm.md).  Fragments are read with 128-bit shared loads from a
 // 16-double row whose halves are swapped on odd rows (bank-conflict free, no padding).
 //   GEMM-1: CTA tile 64x128, K step 16, 8 warps as 2 x 4, warp tile 32x32, 3 stages, 2 CTAs/SM
-//   GEMM-2: CTA tile 64x64,  K step 16, 4 warps as 2 x 2, warp tile 32x32, 3 stages, 3 CTAs/SM
+//   GEMM-2: CTA tile 32x64,  K step 16, 2 warps as 1 x 2, warp tile 32x32, 3 stages, 5 CTAs/SM
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 constexpr int RIS_GBK = 16, RIS_GLD = 16;   // K step; shared row stride in doubles (swizzled, see the kernel)
-constexpr int RIS_GTILE2 = 64;           // AO block edge of the GEMM-2 block list
+constexpr int RIS_GTILE2 = 64;           // GEMM-2 tile width (gathered columns); also the AO block edge of the fit_K bands
+#ifndef RIS_GPANEL
+#define RIS_GPANEL 32
+#endif
+constexpr int RIS_GPANEL_ROWS = RIS_GPANEL;   // GEMM-2 row-panel height (rows of the spatial AO order per tile)
 
 struct RisGemmSeg {
     const double* A; long long lda, bsA;   // A operand rows m, K contiguous; bsA = batch (blockIdx.z) stride in doubles
@@ -306,5 +311,9 @@ inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int b
 inline cudaError_t ris_gemm_blocks(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
     // GATH = false: skipping the MMAs of all-padding strips measured slower than issuing them (48.2 vs 49.0 ms, config 4)
-    return ris_gemm_launch_cfg<RIS_GTILE2, RIS_GTILE2, 32, 32, 3, 3, false>(st, p, batch, ntiles);
+#ifndef RIS_G2_STAGES
+#define RIS_G2_STAGES 3
+#define RIS_G2_MINB (RIS_GPANEL_ROWS == 32 ? 5 : 3)   // measured on config 4: 5 -> 44.3 ms, 6 -> 45.4, 3 or 4 -> 47.1
+#endif
+    return ris_gemm_launch_cfg<RIS_GPANEL_ROWS, RIS_GTILE2, 32, 32, RIS_G2_STAGES, RIS_G2_MINB, false>(st, p, batch, ntiles);
 }
