@@ -30,9 +30,9 @@ if ROOT not in sys.path:
 
 METRIC = "TDDFT-ris gradient ms/state"
 UNIT = "ms/state"
-# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/r01_v5_ncu.md);
+# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/r01_v9_ncu.md);
 # None where no capture of that (config, kernel) is committed.
-NCU_TRAFFIC = {(4, "ris_gemm_dmma(HT=Cvir*B^T)"): 1.434842e9 + 3.779255e9}
+NCU_TRAFFIC = {(4, "ris_gemm_dmma(HT=Cvir*B^T)"): 1.399466e9 + 3.755925e9}
 
 ORACLE_CUTOFF = {4: 1e-22}      # the oracle's documented primitive cutoff on config 4
 
@@ -212,7 +212,7 @@ def run_ours(args):
                 "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4) if peak else None,
                 "traffic": NCU_TRAFFIC.get((args.config, dom_name)), "launches": dom["launches"], "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
                 "share_of_kernel_time": round(dom["ms"] / ksum, 4),
-                "traffic_unit": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum (profiles/r01_v5_ncu.md)",
+                "traffic_unit": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum (profiles/r01_v9_ncu.md)",
                 "algorithmic_bytes_per_launch": round(dom["bytes"] / dom["launches"]),
                 "peak_source": ("measured in this run by ris_probe_fp64_mma_peak (mma.sync f64 chains)" if is_gemm else
                                 "measured in this run by ris_probe_fp64_peak (independent DFMA chains)")
