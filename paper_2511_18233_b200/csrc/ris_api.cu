@@ -15,6 +15,7 @@ constexpr int RIS_NPRIM_MAX = 24;        // primitives per shell (kmax <= 576: t
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -322,11 +323,16 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     if ((rc = dev_upload(c, &c->d_aux, aux.data(), aux.size()))) return rc;
 
     // Boys tables, one per top order M = 0..7 (M = 0: the undifferentiated (ss|P) of the fitting step)
-    for (int M = 0; M <= 7; ++M) {
-        std::vector<double> t;
-        ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, t);
-        if ((rc = dev_upload(c, &c->d_boys[M], t.data(), t.size()))) return rc;
-        CU(cudaStreamSynchronize(c->stream));      // t goes out of scope
+    // (geometry-independent: the host tables are built once per process, in long double, and kept)
+    {
+        static std::vector<double> tabs[8];
+        static std::mutex tabs_mu;
+        std::lock_guard<std::mutex> lk(tabs_mu);
+        for (int M = 0; M <= 7; ++M) {
+            if (tabs[M].empty()) ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, tabs[M]);
+            if ((rc = dev_upload(c, &c->d_boys[M], tabs[M].data(), tabs[M].size()))) return rc;
+        }
+        CU(cudaStreamSynchronize(c->stream));
     }
 
     // ---- S0 on device: survey -> scan -> scatter -> pack
