@@ -305,7 +305,10 @@ inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, 
 // CTA/SM reach 31.3-31.6, 128x64 x 2 CTAs 31.9, the same tile with 4 stages 32.4.
 inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int batch)
 {
-    return ris_gemm_launch_cfg<64, 128, 32, 32, 3, 2>(st, p, batch, 0);
+#ifndef RIS_G1_STAGES
+#define RIS_G1_STAGES 3
+#endif
+    return ris_gemm_launch_cfg<64, 128, 32, 32, RIS_G1_STAGES, 2>(st, p, batch, 0);
 }
 // GEMM-2: tile list of RIS_GTILE2 rows x RIS_GTILE2 gathered columns (p.gcols required)
 inline cudaError_t ris_gemm_blocks(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
