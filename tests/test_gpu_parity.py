@@ -214,3 +214,32 @@ def test_deterministic_mode_flags_out_of_range_contributions():
     g = ctx.grad_J(dev(wl.D), dev(wl.c_aux)).cpu().numpy()       # the flag does not stick
     assert_parity(g, orc.grad_J(wl.mol, wl.D, wl.c_aux)[0], "deterministic J after overflow")
     ctx.close()
+
+
+def test_twice_the_largest_config_p_batched():
+    """Maximum-size case: a 600-atom chain (6000 AO, nocc 1050, nvir 2100 -- twice config 4 in every dimension, HT alone
+    would be 30 GB), so ris_grad_K runs P-batched on its own (auto p_batch < naux).  J against the oracle on sampled atoms;
+    K through properties that hold at any size: invariance under the P-batch size, translational invariance.  (The oracle's
+    K rows for one sampled atom agree to 4.6e-15 of the scale; that 65 s check is recorded in DESIGN.md, not run here.)"""
+    rng = np.random.default_rng(7)
+    xyz, heavy = synth._chain(300)
+    mol = synth._build_molecule(rng, xyz, heavy, synth.HEAVY_SPD, 0.1, 50.0)
+    nao, naux, nocc, nvir = mol.nao, mol.natoms, 1050, 2100
+    g = torch.Generator(device="cuda").manual_seed(3)
+    C_occ = torch.randn(nao, nocc, dtype=torch.float64, device="cuda", generator=g)
+    C_vir = torch.randn(nao, nvir, dtype=torch.float64, device="cuda", generator=g)
+    B = torch.randn(1, naux, nocc, nvir, dtype=torch.float64, device="cuda", generator=g)
+    D = rng.standard_normal((1, nao, nao))
+    c = rng.standard_normal((1, naux))
+    ctx = ris_setup(mol, schwarz_tol=1e-13)
+    gK = ctx.grad_K(C_occ, C_vir, B)
+    assert 0 < ctx.p_batch < naux
+    gJ = ctx.grad_J(dev(D), dev(c)).cpu().numpy()
+    ctx.close()
+    ctx2 = ris_setup(mol, schwarz_tol=1e-13, p_batch=96)
+    gK2 = ctx2.grad_K(C_occ, C_vir, B)
+    ctx2.close()
+    assert float((gK2 - gK).abs().max()) <= 5e-14 * float(gK.abs().max())
+    assert float(gK.sum(dim=1).abs().max()) <= 1e-10 * float(gK.abs().sum())
+    rJ, _ = orc.grad_J(mol, D, c, atoms=[0, 299, 599], prim_cutoff=1e-22)
+    assert_parity(gJ, rJ, "600-atom chain J")
