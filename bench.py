@@ -244,9 +244,7 @@ def run_ours(args):
         hJ = np.empty((nbJ, mol.natoms, 3)); hK = np.empty((nbK, mol.natoms, 3)); hQ = np.empty((nbJ, mol.natoms, 3))
 
         def step_host():
-            ctx.grad_J_host(host["D"], host["c_aux"], out=hJ)
-            ctx.grad_K_host(host["C_occ"], host["C_vir"], host["B"], out=hK)
-            ctx.grad_PQ_host(host["c_aux"], host["d_aux"], out=hQ)
+            ctx.grad_host(host["D"], host["c_aux"], host["d_aux"], host["C_occ"], host["C_vir"], host["B"], out=(hJ, hK, hQ))
 
         step_host()
         barrier()
@@ -262,13 +260,14 @@ def run_ours(args):
             t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             t_e2e = float(t.item())
-        h2d = 8 * (host["D"].numel() + 2 * host["c_aux"].numel() + host["C_occ"].numel() + host["C_vir"].numel()
-                   + host["B"].numel() + host["c_aux"].numel() + host["d_aux"].numel())
+        h2d = 8 * (host["D"].numel() + host["c_aux"].numel() + host["d_aux"].numel() + host["C_occ"].numel()
+                   + host["C_vir"].numel() + host["B"].numel())
         d2h = 8 * (hJ.size + hK.size + hQ.size)
         e2e = {"value": round(t_e2e / (world * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "ms_per_step_each": [round(r, 2) for r in reps],
-               "how": "ris_grad_{J,K,PQ}_host on pinned host buffers; host wall clock around the calls (they return "
-                      "after the D2H copy of the gradient); B goes up in P chunks on a copy stream, GEMM-1 follows chunk by chunk"}
+               "median_ms_per_state": round(sorted(reps)[len(reps) // 2] / (world * nstates), 4),
+               "how": "ris_grad_host (J + K + PQ in one call) on pinned host buffers; host wall clock around the call, which returns "
+                      "after the D2H copy of the gradients; B goes up in P chunks on a copy stream under the J kernels and the GEMMs"}
 
     # ---- NEXT-1 (reported beside the metric, outside the timed step): the J-type fitting step on the same workload
     ctx.fit_J(d["D"])                                       # builds the metric's Cholesky factor (one-off per geometry)

@@ -133,6 +133,12 @@ int ris_grad_J_host(ris_ctx* ctx, int nbatch, const double* D, const double* c_a
 int ris_grad_K_host(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                     const double* B, double* grad);
 int ris_grad_PQ_host(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
+/* All three terms in one call on host buffers (same argument meaning as above; nbatch_J states for D / c_aux / d_aux and
+ * the J and PQ outputs, nbatch_K states for B and the K output).  The upload of B runs behind the J class kernels and the
+ * GEMMs of the parts of B already resident; one synchronisation at the end. */
+int ris_grad_host(ris_ctx* ctx, int nbatch_J, const double* D, const double* c_aux, const double* d_aux, int nbatch_K,
+                  int nocc, int nvir, const double* C_occ, const double* C_vir, const double* B, double* grad_J,
+                  double* grad_K, double* grad_PQ);
 
 int ris_destroy(ris_ctx* ctx);
 const char* ris_strerror(int status);

@@ -83,6 +83,7 @@ struct ris_ctx {
     // grow-only scratch
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
+    cudaEvent_t copy_extra = nullptr;             // the extra payload of upload_B_chunked has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
     void* ws[20] = {nullptr};
     size_t ws_bytes[20] = {0};
@@ -92,7 +93,7 @@ struct ris_ctx {
 };
 
 enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
-       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_N = 17 };
+       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_N = 20 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -529,6 +530,7 @@ extern "C" int ris_destroy(ris_ctx* c)
     for (int i = 0; i < WS_N; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
     for (cudaEvent_t e : c->copy_ev) cudaEventDestroy(e);
     if (c->copy_gate) cudaEventDestroy(c->copy_gate);
+    if (c->copy_extra) cudaEventDestroy(c->copy_extra);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     ris_profile_reset(c);
     delete c;
@@ -1089,7 +1091,7 @@ __global__ void ris_k_pad_rows(int rows, int cols, int ld, const int* __restrict
 // b_ready (nullable): b_ready[s * RIS_COPY_CHUNKS + ch] is recorded (on another stream) once chunk ch (a range of P) of
 // B of state s is resident; the compute stream waits for it right before that chunk's GEMM-1, so the H2D copy runs
 // ahead of the GEMMs instead of in front of them.
-constexpr int RIS_COPY_CHUNKS = 4;     // *_host: B of a state goes up in this many P ranges, GEMM-1 follows chunk by chunk
+constexpr int RIS_COPY_CHUNKS = 8;     // *_host: B of a state goes up in this many P ranges, GEMM-1 follows chunk by chunk
 static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                        const double* B, double* grad, const cudaEvent_t* b_ready)
 {
@@ -1264,19 +1266,14 @@ extern "C" int ris_grad_J_host(ris_ctx* c, int nbatch, const double* D, const do
     return d2h_grad(c, dg, grad, ng);
 }
 
-extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
-                               const double* B, double* grad)
+// B [nbatch][naux][nocc][nvir] host -> device staging (WS_IN0) on the copy stream, in RIS_COPY_CHUNKS ranges of P per state,
+// one event per chunk (c->copy_ev[s * RIS_COPY_CHUNKS + ch]).  The caller has already enqueued the small operands: the
+// H2D copy engine serves transfers in issue order across streams.
+static int upload_B_chunked(ris_ctx* c, int nbatch, int nocc, int nvir, const double* B, double** dB_out,
+                            const double* extra_h = nullptr, double* extra_d = nullptr, size_t extra_n = 0)
 {
-    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
-    CU(cudaSetDevice(c->device));
-    double *dCo, *dCv, *dB, *dg;
     int rc;
-    const size_t ng = (size_t)nbatch * c->natoms * 3;
-    // B (the bulk of the input: naux*nocc*nvir doubles per state) goes up state by state on a second stream, each
-    // state's GEMMs waiting only for their own slice: the PCIe transfer of state s+1 hides behind the GEMMs of state s.
-    // The small operands go first: the H2D copy engine serves transfers in issue order across streams.
-    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
-    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    double* dB;
     const size_t nB = (size_t)c->naux * nocc * nvir;
     if ((rc = ws_get(c, WS_IN0, nbatch * nB * sizeof(double), (void**)&dB))) return rc;
     if (!c->copy_stream) CU(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
@@ -1295,7 +1292,31 @@ extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const
             if (q1 > q0)
                 CU(cudaMemcpyAsync(dB + s * nB + q0, B + s * nB + q0, (q1 - q0) * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream));
             CU(cudaEventRecord(c->copy_ev[s * RIS_COPY_CHUNKS + ch], c->copy_stream));
+            if (s == 0 && ch == RIS_COPY_CHUNKS - 1 && extra_n > 0) {
+                // a second payload (D of the combined call) rides behind the first state's B: its consumer runs last
+                if (!c->copy_extra) CU(cudaEventCreateWithFlags(&c->copy_extra, cudaEventDisableTiming));
+                CU(cudaMemcpyAsync(extra_d, extra_h, extra_n * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream));
+                CU(cudaEventRecord(c->copy_extra, c->copy_stream));
+            }
         }
+    *dB_out = dB;
+    return RIS_OK;
+}
+
+extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                               const double* B, double* grad)
+{
+    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    double *dCo, *dCv, *dB, *dg;
+    int rc;
+    const size_t ng = (size_t)nbatch * c->natoms * 3;
+    // B (the bulk of the input: naux*nocc*nvir doubles per state) goes up state by state on a second stream, each
+    // state's GEMMs waiting only for their own slice: the PCIe transfer of state s+1 hides behind the GEMMs of state s.
+    // The small operands go first: the H2D copy engine serves transfers in issue order across streams.
+    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
+    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    if ((rc = upload_B_chunked(c, nbatch, nocc, nvir, B, &dB))) return rc;
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = grad_K_impl(c, nbatch, nocc, nvir, dCo, dCv, dB, dg, c->copy_ev.data()))) {
         cudaStreamSynchronize(c->copy_stream);
@@ -1316,6 +1337,42 @@ extern "C" int ris_grad_PQ_host(ris_ctx* c, int nbatch, const double* c_aux, con
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = ris_grad_PQ(c, nbatch, dc, dd, dg))) return rc;
     return d2h_grad(c, dg, grad, ng);
+}
+
+// All three terms on host buffers in ONE call: the chunked upload of B starts right behind the small operands and D,
+// so it runs under the J class kernels and the GEMMs of the chunks already resident; one synchronisation at the end.
+extern "C" int ris_grad_host(ris_ctx* c, int nbJ, const double* D, const double* c_aux, const double* d_aux, int nbK, int nocc,
+                             int nvir, const double* C_occ, const double* C_vir, const double* B, double* grad_J, double* grad_K,
+                             double* grad_PQ)
+{
+    if (!c || nbJ < 1 || nbK < 1 || nocc < 1 || nvir < 1 || !D || !c_aux || !d_aux || !C_occ || !C_vir || !B || !grad_J || !grad_K ||
+        !grad_PQ)
+        return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    int rc;
+    double *dc, *dd, *dCo, *dCv, *dD, *dB, *dg;
+    const size_t nJ = (size_t)nbJ * c->natoms * 3, nK = (size_t)nbK * c->natoms * 3;
+    if ((rc = h2d(c, WS_HC, c_aux, (size_t)nbJ * c->naux, &dc))) return rc;
+    if ((rc = h2d(c, WS_HDQ, d_aux, (size_t)nbJ * c->naux, &dd))) return rc;
+    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
+    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    const size_t nD = (size_t)nbJ * c->nao * c->nao;
+    if ((rc = ws_get(c, WS_HD, nD * sizeof(double), (void**)&dD))) return rc;
+    if ((rc = upload_B_chunked(c, nbK, nocc, nvir, B, &dB, D, dD, nD))) return rc;
+    if ((rc = ws_get(c, WS_OUT, (2 * nJ + nK) * sizeof(double), (void**)&dg))) return rc;
+    // compute order: PQ (needs only c, d), K (follows the chunks of B), J last (D rode up behind the first state's B)
+    if ((rc = ris_grad_PQ(c, nbJ, dc, dd, dg + nJ)) ||
+        (rc = grad_K_impl(c, nbK, nocc, nvir, dCo, dCv, dB, dg + 2 * nJ, c->copy_ev.data()))) {
+        cudaStreamSynchronize(c->copy_stream);
+        return rc;
+    }
+    CU(cudaStreamWaitEvent(c->stream, c->copy_extra, 0));
+    if ((rc = ris_grad_J(c, nbJ, dD, dc, dg))) { cudaStreamSynchronize(c->copy_stream); return rc; }
+    CU(cudaMemcpyAsync(grad_J, dg, nJ * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(grad_PQ, dg + nJ, nJ * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(grad_K, dg + 2 * nJ, nK * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return RIS_OK;
 }
 
 // --------------------------------------------------------------------------------------- FP64 probe

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libris_b200.so")
 _lib = None
 
 EXPORTS = [
-    "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host",
+    "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host", "ris_grad_host",
     "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
@@ -53,6 +53,7 @@ def load_library():
     lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_grad_K_host.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ_host.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_grad_host.argtypes = [vp, ci, vp, vp, vp, ci, ci, ci, vp, vp, vp, vp, vp, vp]
     lib.ris_destroy.argtypes = [vp]
     lib.ris_strerror.argtypes = [ci]
     lib.ris_strerror.restype = C.c_char_p
@@ -252,6 +253,17 @@ class RisContext:
         if out is None:
             out = np.empty((nb, self.natoms, 3))
         _check(self._lib.ris_grad_PQ_host(self._h, nb, pc[0], pd[0], self._host(out)[0]))
+        return out
+
+    def grad_host(self, D, c_aux, d_aux, C_occ, C_vir, B, out=None):
+        """(gJ, gK, gPQ) from host buffers in one call (H2D of B overlapped with the kernels)."""
+        pD, pc, pd = self._host(D), self._host(c_aux), self._host(d_aux)
+        po, pv, pB = self._host(C_occ), self._host(C_vir), self._host(B)
+        nbJ, nbK, nocc, nvir = pD[1][0], pB[1][0], po[1][1], pv[1][1]
+        if out is None:
+            out = (np.empty((nbJ, self.natoms, 3)), np.empty((nbK, self.natoms, 3)), np.empty((nbJ, self.natoms, 3)))
+        _check(self._lib.ris_grad_host(self._h, nbJ, pD[0], pc[0], pd[0], nbK, nocc, nvir, po[0], pv[0], pB[0],
+                                       self._host(out[0])[0], self._host(out[1])[0], self._host(out[2])[0]))
         return out
 
     # ---- profiling

@@ -124,6 +124,10 @@ def test_host_buffer_entry_points_match_device():
     hK = ctx.grad_K_host(pin(wl.C_occ), pin(wl.C_vir), pin(wl.B))
     hQ = ctx.grad_PQ_host(wl.c_aux, wl.d_aux)
     assert_parity(hJ, gJ, "host J"); assert_parity(hK, gK, "host K"); assert np.array_equal(hQ, gQ)
+    # all three terms in one call (pinned and pageable buffers mixed; config 2 has nbatch_J = 2, nbatch_K = 1)
+    for rep in range(2):            # the second call reuses the staging buffers and the copy stream
+        aJ, aK, aQ = ctx.grad_host(pin(wl.D), wl.c_aux, wl.d_aux, pin(wl.C_occ), wl.C_vir, pin(wl.B))
+        assert_parity(aJ, gJ, "host all J"); assert_parity(aK, gK, "host all K"); assert np.array_equal(aQ, gQ)
 
 
 def test_properties_symmetry_linearity_K_reduces_to_J():
