@@ -1098,6 +1098,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
+    if (c->nelem_real == 0) return RIS_OK;                // every shell pair screened out: the gradient is exactly zero
     const int nao = c->nao, naux = c->naux;
     const int nbmax = next_nb(nbatch);
     const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
@@ -1169,8 +1170,9 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
                 double* out = tile + (size_t)s * pbp * c->nelem_real;
                 {
                     ProfScope ps(c, "ris_k_pack_sym", (double)c->nelem_real * np, 8.0 * np * ((double)c->nsrows * RIS_GTILE2 + (double)c->nelem_real));
-                    ris_k_pack_sym<<<dim3(c->nsrows, (np + 31) / 32), 256, 0, c->stream>>>(np, pbp, S, (long long)c->ntiles * blk,
-                                                                                        c->d_srows, c->d_smap, out);
+                    if (c->nsrows > 0)
+                        ris_k_pack_sym<<<dim3(c->nsrows, (np + 31) / 32), 256, 0, c->stream>>>(np, pbp, S, (long long)c->ntiles * blk,
+                                                                                            c->d_srows, c->d_smap, out);
                     if (c->novf > 0)
                         ris_k_pack_sym_ovf<<<c->novf, 64, 0, c->stream>>>(c->novf, c->d_ovf, np, pbp, S, (long long)c->ntiles * blk, out);
                 }

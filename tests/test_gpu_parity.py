@@ -247,3 +247,21 @@ def test_twice_the_largest_config_p_batched():
     assert float(gK.sum(dim=1).abs().max()) <= 1e-10 * float(gK.abs().sum())
     rJ, _ = orc.grad_J(mol, D, c, atoms=[0, 299, 599], prim_cutoff=1e-22)
     assert_parity(gJ, rJ, "600-atom chain J")
+
+
+def test_everything_screened_out_is_an_empty_problem():
+    """Degenerate case: a screening tolerance that drops every primitive pair leaves no shell pair in any class -- the
+    calls must run on the empty lists and return exact zeros for J and K (PQ has no screening)."""
+    wl = synth.make_workload(1)
+    ctx = ris_setup(wl.mol, schwarz_tol=1e30)
+    assert ctx.ntriplets == 0
+    gJ = ctx.grad_J(dev(wl.D), dev(wl.c_aux)).cpu().numpy()
+    gK = ctx.grad_K(dev(wl.C_occ), dev(wl.C_vir), dev(wl.B)).cpu().numpy()
+    gQ = ctx.grad_PQ(dev(wl.c_aux), dev(wl.d_aux)).cpu().numpy()
+    assert not gJ.any() and not gK.any()
+    assert_parity(gQ, orc.grad_PQ(wl.mol, wl.c_aux, wl.d_aux)[0], "PQ")
+    v, c = ctx.fit_J(dev(wl.D))
+    assert not v.cpu().numpy().any() and not c.cpu().numpy().any()
+    T, B = ctx.fit_K(dev(wl.C_occ), dev(wl.C_vir))
+    assert not T.cpu().numpy().any() and not B.cpu().numpy().any()
+    ctx.close()
