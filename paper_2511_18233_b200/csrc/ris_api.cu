@@ -696,11 +696,17 @@ __global__ void ris_k_metric(int n, const double* __restrict__ aux, const double
 // few hundred to a few thousand, the factorisation runs once per geometry.  flag = 1 when a pivot is not positive.
 __global__ void __launch_bounds__(1024) ris_k_cholesky(int n, double* __restrict__ M, int* flag)
 {
-    __shared__ double piv;
+    __shared__ double piv, dmax;
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int j = 0; j < n; ++j) m = fmax(m, M[(size_t)j * n + j]);
+        dmax = m;
+    }
+    __syncthreads();
     for (int j = 0; j < n; ++j) {
         if (threadIdx.x == 0) {
             const double d = M[(size_t)j * n + j];
-            if (!(d > 0.0)) *flag = 1;
+            if (!(d > 1e-12 * dmax)) *flag = 1;        // numerically singular: (nearly) coincident aux functions
             piv = sqrt(d);
             M[(size_t)j * n + j] = piv;
         }

@@ -171,3 +171,21 @@ def test_fit_K_full_size_config4_sampled_aux():
     res = (M @ B.reshape(n, -1) - T.reshape(n, -1)).abs().max().item()
     assert res <= 1e-11 * scale * max(1.0, float(M.abs().max())), res
     ctx.close()
+
+
+def test_singular_metric_is_reported_not_crashed():
+    """Two atoms on one point: identical aux functions (same exponent) make M singular -- ris_fit_J / ris_fit_K return
+    RIS_EINVAL (raised as RisError); the derivative calls still work on that geometry (T = 0 paths)."""
+    from paper_2511_18233_b200 import RisError
+    mol = synth.tiny_molecule(5, [[0, 1], [0, 1]], [[0.1, 0.2, 0.3], [0.1, 0.2, 0.3]])
+    mol.aux_exponents[1] = mol.aux_exponents[0]
+    rng = np.random.default_rng(0)
+    D = rng.standard_normal((1, mol.nao, mol.nao))
+    ctx = ris_setup(mol)
+    with pytest.raises(RisError):
+        ctx.fit_J(dev(D))
+    with pytest.raises(RisError):
+        ctx.fit_K(dev(rng.standard_normal((mol.nao, 2))), dev(rng.standard_normal((mol.nao, 3))))
+    g = ctx.grad_J(dev(D), dev(rng.standard_normal((1, 2)))).cpu().numpy()
+    assert np.all(np.isfinite(g)) and np.all(np.abs(g.sum(axis=1)) < 1e-10 * max(np.abs(g).sum(), 1e-300))
+    ctx.close()
