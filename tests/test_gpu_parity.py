@@ -265,3 +265,33 @@ def test_everything_screened_out_is_an_empty_problem():
     T, B = ctx.fit_K(dev(wl.C_occ), dev(wl.C_vir))
     assert not T.cpu().numpy().any() and not B.cpu().numpy().any()
     ctx.close()
+
+
+def test_maximum_contraction_length():
+    """24 primitives per shell (RIS_NPRIM_MAX: up to 576 primitive pairs per shell pair, the largest warp task that has
+    to fit in shared memory) with 5 states per launch; 25 primitives are refused."""
+    coords = [[0, 0, 0], [1.7, 0.5, -0.3]]
+    mol = synth.tiny_molecule(12, [[0, 2], [1, 0]], coords, lo=0.05, hi=300.0, nprim=24)
+    wl = _workload_for(mol, 2, 5)
+    ctx, gJ, gK, gQ = run_all(wl, schwarz_tol=0.0)
+    assert_parity(gJ, orc.grad_J(mol, wl.D, wl.c_aux)[0], "J")
+    assert_parity(gK, orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B)[0], "K")
+    v, _ = ctx.fit_J(dev(wl.D))
+    assert_parity(v.cpu().numpy(), orc.vec_J(mol, wl.D), "v")
+    ctx.close()
+    big = synth.tiny_molecule(12, [[0], [0]], coords, nprim=25)
+    with pytest.raises(RisError):
+        ris_setup(big)
+
+
+@pytest.mark.parametrize("nocc,nvir", [(1, 1), (2, 17), (16, 1)])
+def test_smallest_and_odd_mo_dimensions(nocc, nvir):
+    """K term with one-column coefficient matrices and K dimensions far below one MMA step (16)."""
+    wl0 = synth.make_workload(1)
+    wl = _workload_for(wl0.mol, 10 + nocc + nvir, 2, nocc=nocc, nvir=nvir)
+    ctx = ris_setup(wl.mol)
+    gK = ctx.grad_K(dev(wl.C_occ), dev(wl.C_vir), dev(wl.B)).cpu().numpy()
+    assert_parity(gK, orc.grad_K(wl.mol, wl.C_occ, wl.C_vir, wl.B)[0], "K")
+    T, B = ctx.fit_K(dev(wl.C_occ), dev(wl.C_vir))
+    assert_parity(T.cpu().numpy(), orc.tensor_K(wl.mol, wl.C_occ, wl.C_vir), "T")
+    ctx.close()
