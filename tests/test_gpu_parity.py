@@ -295,3 +295,26 @@ def test_smallest_and_odd_mo_dimensions(nocc, nvir):
     T, B = ctx.fit_K(dev(wl.C_occ), dev(wl.C_vir))
     assert_parity(T.cpu().numpy(), orc.tensor_K(wl.mol, wl.C_occ, wl.C_vir), "T")
     ctx.close()
+
+
+def test_runs_on_a_caller_stream():
+    """The library enqueues everything on the stream given at setup (here a non-default torch stream): results match the
+    default-stream run, and nothing was left on the legacy stream (the outputs are complete after synchronising ONLY the
+    caller's stream)."""
+    wl = synth.make_workload(2)
+    _, gJ, gK, gQ = run_all(wl)
+    st = torch.cuda.Stream()
+    D, c, d = dev(wl.D), dev(wl.c_aux), dev(wl.d_aux)
+    Co, Cv, B = dev(wl.C_occ), dev(wl.C_vir), dev(wl.B)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        ctx = ris_setup(wl.mol)
+        a = ctx.grad_J(D, c); b = ctx.grad_K(Co, Cv, B); q = ctx.grad_PQ(c, d)
+        v, cf = ctx.fit_J(D)
+        T, Bf = ctx.fit_K(Co, Cv)
+    st.synchronize()
+    assert_parity(a.cpu().numpy(), gJ, "J on stream"); assert_parity(b.cpu().numpy(), gK, "K on stream")
+    assert np.array_equal(q.cpu().numpy(), gQ)
+    assert_parity(v.cpu().numpy(), orc.vec_J(wl.mol, wl.D), "v on stream")
+    assert_parity(T.cpu().numpy(), orc.tensor_K(wl.mol, wl.C_occ, wl.C_vir), "T on stream")
+    ctx.close()
