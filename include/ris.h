@@ -81,7 +81,7 @@ typedef struct ris_options {
 /* Build the context: copies the molecule to the device and runs shell-pair screening, sorting by
  * (l_mu,l_nu) class and SoA packing ON THE DEVICE (north_star; the paper is silent).
  *   coords[natoms][3] bohr; shell s sits on atom shell_atom[s], has angular momentum shell_l[s] in 0..3 and
- *   shell_nprim[s] >= 1 primitives at prim_exp/prim_coef[shell_prim_off[s] ...]; aux P sits on atom P with
+ *   1 <= shell_nprim[s] <= 24 primitives at prim_exp/prim_coef[shell_prim_off[s] ...] (RIS_EINVAL beyond); aux P sits on atom P with
  *   exponent aux_exponents[P] (bohr^-2).  opt may be NULL (defaults).  cuda_stream is a cudaStream_t
  *   (NULL = default stream) on which every later call of this context is enqueued. */
 int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
