@@ -151,11 +151,13 @@ def run_ours(args):
     ctx = ris_setup(mol, schwarz_tol=wl.schwarz_tol, profile=True)
     torch.cuda.synchronize()
     setup_first_ms = (time.perf_counter() - t0) * 1e3      # includes CUDA context creation and module load
-    ctx.close()
-    t0 = time.perf_counter()
-    ctx = ris_setup(mol, schwarz_tol=wl.schwarz_tol, profile=True)
-    torch.cuda.synchronize()
-    setup_ms = (time.perf_counter() - t0) * 1e3            # what a new geometry costs in a running process
+    setup_ms = float("inf")                                # what a new geometry costs in a running process (best of 3)
+    for _ in range(3):
+        ctx.close()
+        t0 = time.perf_counter()
+        ctx = ris_setup(mol, schwarz_tol=wl.schwarz_tol, profile=True)
+        torch.cuda.synchronize()
+        setup_ms = min(setup_ms, (time.perf_counter() - t0) * 1e3)
 
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k))).pin_memory()
             for k in ("D", "c_aux", "d_aux", "C_occ", "C_vir", "B")}
