@@ -83,6 +83,8 @@ struct ris_ctx {
     // grow-only scratch
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
+    cudaStream_t side[RIS_NCLASS] = {nullptr};    // class kernels of small molecules run concurrently on these
+    cudaEvent_t join_ev[RIS_NCLASS] = {nullptr}, fork_ev = nullptr;
     cudaEvent_t copy_extra = nullptr;             // the extra payload of upload_B_chunked has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
     void* ws[20] = {nullptr};
@@ -130,18 +132,20 @@ template <class T> static int dev_upload(ris_ctx* c, T** p, const T* h, size_t n
 
 // profiling: events around a launch when opt.profile is set
 struct ProfScope {
-    ris_ctx* c; int idx = -1;
-    // flops / bytes: ALGORITHMIC work of the launch
-    ProfScope(ris_ctx* c_, const char* name, double flops = 0.0, double bytes = 0.0) : c(c_)
+    ris_ctx* c; int idx = -1; cudaStream_t st;
+    // flops / bytes: ALGORITHMIC work of the launch; st: the stream the launch
+    // goes to when it is not the context's own (concurrent class kernels of small molecules)
+    ProfScope(ris_ctx* c_, const char* name, double flops = 0.0, double bytes = 0.0, cudaStream_t st_ = nullptr, bool own = true)
+        : c(c_), st(own ? c_->stream : st_)
     {
         if (!c->opt.profile) return;
         ProfRec r; r.name = name; r.flops = flops; r.bytes = bytes;
         if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) return;
-        cudaEventRecord(r.e0, c->stream);
+        cudaEventRecord(r.e0, st);
         c->prof.push_back(r);
         idx = (int)c->prof.size() - 1;
     }
-    ~ProfScope() { if (idx >= 0) cudaEventRecord(c->prof[idx].e1, c->stream); }
+    ~ProfScope() { if (idx >= 0) cudaEventRecord(c->prof[idx].e1, st); }
 };
 
 extern "C" int ris_profile_reset(ris_ctx* c)
@@ -531,6 +535,11 @@ extern "C" int ris_destroy(ris_ctx* c)
     for (cudaEvent_t e : c->copy_ev) cudaEventDestroy(e);
     if (c->copy_gate) cudaEventDestroy(c->copy_gate);
     if (c->copy_extra) cudaEventDestroy(c->copy_extra);
+    if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+    for (int k = 0; k < RIS_NCLASS; ++k) {
+        if (c->join_ev[k]) cudaEventDestroy(c->join_ev[k]);
+        if (c->side[k]) cudaStreamDestroy(c->side[k]);
+    }
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     ris_profile_reset(c);
     delete c;
@@ -594,10 +603,30 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
     // two ticket arrays per class: the heavy classes run their host-centre phases as two launches
     { int rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr); if (rc) return rc; }
     CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
+    // Small molecules: no class has enough warp tasks to fill the GPU with its one resident wave, so the class kernels
+    // run side by side on their own streams (fork from / join into the context's stream); large ones run back to back.
+    int nsm = 0;
+    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
+    long long most = 0;
+    int nclass = 0;
+    for (int k = 0; k < RIS_NCLASS; ++k)
+        if (c->cls[k].npairs > 0) { most = std::max(most, (long long)((c->cls[k].ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS) * ny); ++nclass; }
+    const bool side = nclass > 1 && most <= (long long)2 * nsm;
+    if (side) {
+        if (!c->fork_ev) CU(cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
+        for (int k = 0; k < RIS_NCLASS; ++k)
+            if (!c->side[k]) {
+                CU(cudaStreamCreateWithFlags(&c->side[k], cudaStreamNonBlocking));
+                CU(cudaEventCreateWithFlags(&c->join_ev[k], cudaEventDisableTiming));
+            }
+        CU(cudaEventRecord(c->fork_ev, c->stream));
+    }
     for (int oi = 0; oi < RIS_NCLASS; ++oi) {
         const int k = kClassOrder[oi];
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
+        const cudaStream_t st = side ? c->side[k] : c->stream;
+        if (side) CU(cudaStreamWaitEvent(st, c->fork_ev, 0));
         RisGradParams p{};
         p.task_ctr = ctr + (size_t)2 * k * ny;
         p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
@@ -605,9 +634,15 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         p.p0 = p0; p.p1 = p1;
         p.grad = grad; p.det = det; p.det_flag = det ? (int*)c->ws[WS_DET] : nullptr;
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
-        ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
-                     8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-        ris_grad_launchers[k](p, c->stream);
+        {
+            ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
+                         8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS, st, false);
+            ris_grad_launchers[k](p, st);
+        }
+        if (side) {
+            CU(cudaEventRecord(c->join_ev[k], st));
+            CU(cudaStreamWaitEvent(c->stream, c->join_ev[k], 0));
+        }
     }
     CU(cudaGetLastError());
     return RIS_OK;
