@@ -32,6 +32,7 @@
  * as-is to UNnormalised primitives; the aux function carries N_P = (2 alpha/pi)^(3/4).
  */
 #include <math.h>
+#include <tgmath.h>            /* exp / sqrt / pow / fabs pick the precision of their argument */
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -44,7 +45,16 @@
 #define TMAX (2 * EMAX + 2)    /* Hermite order bound (+1 for the aux derivative) */
 #define MMAX (TMAX + 1)
 
-static const double PI = 3.14159265358979323846264338327950288;
+/* Working precision of every intermediate (E, R, Boys values, prefactors, per-pair buffers).  The oracle IS the
+ * default build (double: "FP64 unless the paper fixes the precision"); `-DORACLE_REAL="long double"` builds the same
+ * source with x87 extended intermediates, used only by tests/test_oracle_pins.py to measure the oracle's own FP64
+ * rounding error (the evidence behind the parity tolerance, reading R-tol).  Inputs / outputs stay double. */
+#ifndef ORACLE_REAL
+#define ORACLE_REAL double
+#endif
+typedef ORACLE_REAL real;
+
+static const real PI = (real)3.14159265358979323846264338327950288L;
 
 /* ---------------------------------------------------------------- O1: Boys function
  * F_m(T) = int_0^1 t^(2m) exp(-T t^2) dt.
@@ -52,7 +62,7 @@ static const double PI = 3.14159265358979323846264338327950288;
  *         F_m = (2T F_{m+1} + e^-T)/(2m+1).
  * T >= 35: F_0 = 1/2 sqrt(pi/T) erf(sqrt T), upward F_{m+1} = ((2m+1)F_m - e^-T)/(2T).
  */
-void ris_oracle_boys(int mmax, double T, double *F)
+static void boys_real(int mmax, real T, real *F)
 {
     if (T < 35.0) {
         long double t = (long double)T;
@@ -65,21 +75,28 @@ void ris_oracle_boys(int mmax, double T, double *F)
             if (term < 1e-22L * sum) break;
         }
         long double f = et * sum;
-        F[mmax] = (double)f;
+        F[mmax] = (real)f;
         for (int m = mmax - 1; m >= 0; --m) {
             f = (2.0L * t * f + et) / (2 * m + 1);
-            F[m] = (double)f;
+            F[m] = (real)f;
         }
     } else {
         long double t = (long double)T;
         long double et = expl(-t);
-        long double f = 0.5L * sqrtl((long double)PI / t) * erfl(sqrtl(t));
-        F[0] = (double)f;
+        long double f = 0.5L * sqrtl(3.14159265358979323846264338327950288L / t) * erfl(sqrtl(t));
+        F[0] = (real)f;
         for (int m = 0; m < mmax; ++m) {
             f = ((2 * m + 1) * f - et) / (2.0L * t);
-            F[m + 1] = (double)f;
+            F[m + 1] = (real)f;
         }
     }
+}
+
+void ris_oracle_boys(int mmax, double T, double *F)
+{
+    real Fr[64];
+    boys_real(mmax, (real)T, Fr);
+    for (int m = 0; m <= mmax; ++m) F[m] = (double)Fr[m];
 }
 
 /* ---------------------------------------------------------------- O2: Hermite expansion
@@ -88,18 +105,18 @@ void ris_oracle_boys(int mmax, double T, double *F)
  *   E^{i+1,j}_t = E^{ij}_{t-1}/(2p) - (q Q/a) E^{ij}_t + (t+1) E^{ij}_{t+1}
  *   E^{i,j+1}_t = E^{ij}_{t-1}/(2p) + (q Q/b) E^{ij}_t + (t+1) E^{ij}_{t+1}
  */
-typedef double Etab[EMAX + 1][EMAX + 1][2 * EMAX + 2];
+typedef real Etab[EMAX + 1][EMAX + 1][2 * EMAX + 2];
 
-static void hermite_E(int imax, int jmax, double a, double b, double Q, Etab E)
+static void hermite_E(int imax, int jmax, real a, real b, real Q, Etab E)
 {
-    double p = a + b, q = a * b / p;
+    real p = a + b, q = a * b / p;
     memset(E, 0, sizeof(Etab));
     E[0][0][0] = exp(-q * Q * Q);
     for (int i = 0; i <= imax; ++i) {
         for (int j = 0; j <= jmax; ++j) {
             if (i == 0 && j == 0) continue;
             for (int t = 0; t <= i + j; ++t) {
-                double lo, mid, hi;
+                real lo, mid, hi;
                 if (j == 0) {           /* raise i from (i-1, 0) */
                     lo = (t > 0) ? E[i - 1][j][t - 1] : 0.0;
                     mid = E[i - 1][j][t];
@@ -120,24 +137,24 @@ static void hermite_E(int imax, int jmax, double a, double b, double Q, Etab E)
  * R^n_{000} = (-2 rho)^n F_n(T);  R^n_{t+1,u,v} = t R^{n+1}_{t-1,u,v} + X_x R^{n+1}_{t,u,v}
  * (same in y and z).  Output R[t][u][v] = R^0_{tuv} for t+u+v <= nmax.
  */
-typedef double Rtab[TMAX + 1][TMAX + 1][TMAX + 1];
+typedef real Rtab[TMAX + 1][TMAX + 1][TMAX + 1];
 
-static void hermite_R(int nmax, double rho, const double X[3], Rtab R0)
+static void hermite_R(int nmax, real rho, const real X[3], Rtab R0)
 {
-    double F[MMAX + 1];
-    double T = rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
-    ris_oracle_boys(nmax, T, F);
+    real F[MMAX + 1];
+    real T = rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
+    boys_real(nmax, T, F);
     /* Rn[n][t][u][v]; every entry read below has been written before it is read */
     int N = nmax + 1;
-    double Rn[N][N][N][N];
-    double pw = 1.0;
+    real Rn[N][N][N][N];
+    real pw = 1.0;
     for (int n = 0; n <= nmax; ++n) { Rn[n][0][0][0] = pw * F[n]; pw *= -2.0 * rho; }
     for (int tot = 1; tot <= nmax; ++tot)
         for (int t = 0; t <= tot; ++t)
             for (int u = 0; u <= tot - t; ++u) {
                 int v = tot - t - u;
                 for (int n = 0; n <= nmax - tot; ++n) {
-                    double val;
+                    real val;
                     if (t > 0)
                         val = ((t > 1) ? (t - 1) * Rn[n + 1][t - 2][u][v] : 0.0) + X[0] * Rn[n + 1][t - 1][u][v];
                     else if (u > 0)
@@ -153,14 +170,14 @@ static void hermite_R(int nmax, double rho, const double X[3], Rtab R0)
 }
 
 /* sum_{tuv} Ex[t] Ey[u] Ez[v] R[t+dt][u+du][v+dv] */
-static double hsum(const double *Ex, int nx, const double *Ey, int ny, const double *Ez, int nz,
-                   Rtab R, int dt, int du, int dv)
+static real hsum(const real *Ex, int nx, const real *Ey, int ny, const real *Ez, int nz,
+                 Rtab R, int dt, int du, int dv)
 {
     long double s = 0.0L;
     for (int t = 0; t <= nx; ++t)
         for (int u = 0; u <= ny; ++u)
             for (int v = 0; v <= nz; ++v) s += (long double)(Ex[t] * Ey[u] * Ez[v]) * R[t + dt][u + du][v + dv];
-    return (double)s;
+    return (real)s;
 }
 
 /* ---------------------------------------------------------------- O4/O5: one primitive integral
@@ -171,26 +188,27 @@ static double hsum(const double *Ex, int nx, const double *Ey, int ny, const dou
  *   d/dC_x[ab|P] = -pref sum E_tuv R^0_{t+1,u,v}              (explicit aux derivative)
  * out[0] = value, out[1..3] = d/dA, out[4..6] = d/dB, out[7..9] = d/dC.
  */
-void ris_oracle_prim3c(const int la[3], const int lb[3], double a, double b, double alpha,
+void ris_oracle_prim3c(const int la[3], const int lb[3], double a_, double b_, double alpha_,
                        const double A[3], const double B[3], const double C[3], double out[10])
 {
-    double p = a + b, rho = p * alpha / (p + alpha);
-    double P[3], X[3];
+    real a = a_, b = b_, alpha = alpha_;
+    real p = a + b, rho = p * alpha / (p + alpha);
+    real P[3], X[3];
     Etab E[3];
     for (int d = 0; d < 3; ++d) {
         P[d] = (a * A[d] + b * B[d]) / p;
         X[d] = P[d] - C[d];
-        hermite_E(la[d] + 1, lb[d] + 1, a, b, A[d] - B[d], E[d]);
+        hermite_E(la[d] + 1, lb[d] + 1, a, b, (real)A[d] - B[d], E[d]);
     }
     int L = la[0] + la[1] + la[2] + lb[0] + lb[1] + lb[2];
     Rtab *R = malloc(sizeof(Rtab));
     hermite_R(L + 2, rho, X, *R);
-    double pref = 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+    real pref = 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
 #define EE(d, i, j) E[d][i][j], (i) + (j)
     out[0] = pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R, 0, 0, 0);
     for (int d = 0; d < 3; ++d) {
         int ia[3] = {la[0], la[1], la[2]}, ib[3] = {lb[0], lb[1], lb[2]};
-        double up, dn;
+        real up, dn;
         /* bra centre A */
         ia[d] = la[d] + 1;
         up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
@@ -224,13 +242,14 @@ void ris_oracle_prim3c(const int la[3], const int lb[3], double a, double b, dou
  * d/dR_P = -2 rho (R_P-R_Q) * 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)) * F_1(rho R^2) = -d/dR_Q.
  * WITHOUT N_P N_Q.  out[0]=value, out[1..3] = d/dR_P.
  */
-void ris_oracle_prim2c(double alpha, double beta, const double RP[3], const double RQ[3], double out[4])
+void ris_oracle_prim2c(double alpha_, double beta_, const double RP[3], const double RQ[3], double out[4])
 {
-    double rho = alpha * beta / (alpha + beta);
-    double X[3] = {RP[0] - RQ[0], RP[1] - RQ[1], RP[2] - RQ[2]};
-    double F[2];
-    ris_oracle_boys(1, rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]), F);
-    double pref = 2.0 * pow(PI, 2.5) / (alpha * beta * sqrt(alpha + beta));
+    real alpha = alpha_, beta = beta_;
+    real rho = alpha * beta / (alpha + beta);
+    real X[3] = {(real)RP[0] - RQ[0], (real)RP[1] - RQ[1], (real)RP[2] - RQ[2]};
+    real F[2];
+    boys_real(1, rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]), F);
+    real pref = 2.0 * pow(PI, (real)2.5) / (alpha * beta * sqrt(alpha + beta));
     out[0] = pref * F[0];
     for (int d = 0; d < 3; ++d) out[1 + d] = -2.0 * rho * X[d] * pref * F[1];
 }
@@ -256,7 +275,7 @@ static void cart_components(int l, int comp[][3])
         }
 }
 
-static double aux_norm(double alpha) { return pow(2.0 * alpha / PI, 0.75); }
+static real aux_norm(real alpha) { return pow(2.0 * alpha / PI, (real)0.75); }
 
 /* ---------------------------------------------------------------- O6: contraction for one aux P
  * For aux function P (on atom P) and nmat dense matrices G_s[nao][nao] with scale factors
@@ -282,8 +301,8 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
         ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
     }
     int nao = ao_off[nsh];
-    double alpha = mol->aux_exponents[P];
-    double NP = aux_norm(alpha);
+    real alpha = mol->aux_exponents[P];
+    real NP = aux_norm(alpha);
     const double *C = mol->coords + 3 * P;
     int Pmasked = atom_mask ? atom_mask[P] : 1;
     size_t ng = (size_t)nmat * natoms * 3;
@@ -292,7 +311,7 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
     {
         long double *gl = calloc(ng, sizeof(long double));
         long double *el = calloc((size_t)nmat, sizeof(long double));
-        double *buf = malloc(sizeof(double) * 10 * 10 * 10);   /* [ca][cb][10] */
+        real *buf = malloc(sizeof(real) * 10 * 10 * 10);   /* [ca][cb][10] */
 #pragma omp for schedule(dynamic, 1)
         for (int sa = 0; sa < nsh; ++sa) {
             int la = mol->shell_l[sa], at_a = mol->shell_atom[sa];
@@ -307,40 +326,40 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
                 int compb[10][3];
                 cart_components(lb, compb);
                 const double *Bc = mol->coords + 3 * at_b;
-                memset(buf, 0, sizeof(double) * 1000);
-                double AB2 = 0.0;
-                for (int d = 0; d < 3; ++d) AB2 += (A[d] - Bc[d]) * (A[d] - Bc[d]);
+                memset(buf, 0, sizeof(real) * 1000);
+                real AB2 = 0.0;
+                for (int d = 0; d < 3; ++d) AB2 += ((real)A[d] - Bc[d]) * ((real)A[d] - Bc[d]);
                 for (int ka = 0; ka < mol->shell_nprim[sa]; ++ka) {
-                    double a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
-                    double da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
+                    real a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
+                    real da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
                     for (int kb = 0; kb < mol->shell_nprim[sb]; ++kb) {
-                        double b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
-                        double db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
-                        double p = a + b;
+                        real b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
+                        real db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
+                        real p = a + b;
                         if (prim_cutoff > 0.0 &&
-                            fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, 1.5) < prim_cutoff)
+                            fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, (real)1.5) < prim_cutoff)
                             continue;
                         /* O2-O5 for every Cartesian component pair of this primitive pair */
-                        double rho = p * alpha / (p + alpha);
-                        double Pc[3], X[3];
+                        real rho = p * alpha / (p + alpha);
+                        real Pc[3], X[3];
                         Etab E[3];
                         for (int d = 0; d < 3; ++d) {
                             Pc[d] = (a * A[d] + b * Bc[d]) / p;
                             X[d] = Pc[d] - C[d];
-                            hermite_E(la + 1, lb + 1, a, b, A[d] - Bc[d], E[d]);
+                            hermite_E(la + 1, lb + 1, a, b, (real)A[d] - Bc[d], E[d]);
                         }
                         Rtab R;
                         hermite_R(la + lb + 2, rho, X, R);
-                        double pref = NP * da * db * 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+                        real pref = NP * da * db * 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
                         for (int ca = 0; ca < na; ++ca)
                             for (int cb = 0; cb < nb; ++cb) {
                                 const int *ia = compa[ca], *ib = compb[cb];
-                                double *o = buf + (ca * 10 + cb) * 10;
+                                real *o = buf + (ca * 10 + cb) * 10;
 #define EE(d, i, j) E[d][i][j], (i) + (j)
                                 o[0] += pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R, 0, 0, 0);
                                 for (int d = 0; d < 3; ++d) {
                                     int ja[3] = {ia[0], ia[1], ia[2]}, jb[3] = {ib[0], ib[1], ib[2]};
-                                    double up, dn = 0.0;
+                                    real up, dn = 0.0;
                                     ja[d] = ia[d] + 1;
                                     up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
                                     if (ia[d] > 0) {
@@ -371,7 +390,7 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
                     for (int ca = 0; ca < na; ++ca)
                         for (int cb = 0; cb < nb; ++cb) {
                             long double w = (long double)scale[s] * Gs[(size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb];
-                            const double *o = buf + (ca * 10 + cb) * 10;
+                            const real *o = buf + (ca * 10 + cb) * 10;
                             el[s] += w * o[0];
                             for (int d = 0; d < 3; ++d) {
                                 g[at_a * 3 + d] += w * o[1 + d];
@@ -407,8 +426,8 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
         ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
     }
     int nao = ao_off[nsh];
-    double alpha = mol->aux_exponents[P];
-    double NP = aux_norm(alpha);
+    real alpha = mol->aux_exponents[P];
+    real NP = aux_norm(alpha);
     const double *C = mol->coords + 3 * P;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int sa = 0; sa < nsh; ++sa) {
@@ -421,29 +440,29 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
             int compb[10][3];
             cart_components(lb, compb);
             const double *Bc = mol->coords + 3 * mol->shell_atom[sb];
-            double buf[100];
+            real buf[100];
             memset(buf, 0, sizeof buf);
-            double AB2 = 0.0;
-            for (int d = 0; d < 3; ++d) AB2 += (A[d] - Bc[d]) * (A[d] - Bc[d]);
+            real AB2 = 0.0;
+            for (int d = 0; d < 3; ++d) AB2 += ((real)A[d] - Bc[d]) * ((real)A[d] - Bc[d]);
             for (int ka = 0; ka < mol->shell_nprim[sa]; ++ka) {
-                double a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
-                double da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
+                real a = mol->prim_exp[mol->shell_prim_off[sa] + ka];
+                real da = mol->prim_coef[mol->shell_prim_off[sa] + ka];
                 for (int kb = 0; kb < mol->shell_nprim[sb]; ++kb) {
-                    double b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
-                    double db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
-                    double p = a + b;
-                    if (prim_cutoff > 0.0 && fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, 1.5) < prim_cutoff)
+                    real b = mol->prim_exp[mol->shell_prim_off[sb] + kb];
+                    real db = mol->prim_coef[mol->shell_prim_off[sb] + kb];
+                    real p = a + b;
+                    if (prim_cutoff > 0.0 && fabs(da * db) * exp(-a * b / p * AB2) * pow(PI / p, (real)1.5) < prim_cutoff)
                         continue;
-                    double rho = p * alpha / (p + alpha);
-                    double X[3];
+                    real rho = p * alpha / (p + alpha);
+                    real X[3];
                     Etab E[3];
                     for (int d = 0; d < 3; ++d) {
                         X[d] = (a * A[d] + b * Bc[d]) / p - C[d];
-                        hermite_E(la, lb, a, b, A[d] - Bc[d], E[d]);
+                        hermite_E(la, lb, a, b, (real)A[d] - Bc[d], E[d]);
                     }
                     Rtab R;
                     hermite_R(la + lb, rho, X, R);
-                    double pref = NP * da * db * 2.0 * pow(PI, 2.5) / (p * alpha * sqrt(p + alpha));
+                    real pref = NP * da * db * 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
                     for (int ca = 0; ca < na; ++ca)
                         for (int cb = 0; cb < nb; ++cb) {
                             const int *ia = compa[ca], *ib = compb[cb];
@@ -454,7 +473,7 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
             }
             for (int ca = 0; ca < na; ++ca)
                 for (int cb = 0; cb < nb; ++cb)
-                    out[(size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb] = buf[ca * 10 + cb];
+                    out[(size_t)(ao_off[sa] + ca) * nao + ao_off[sb] + cb] = (double)buf[ca * 10 + cb];
         }
     }
     free(ao_off);
@@ -475,7 +494,7 @@ int ris_oracle_grad_PQ(const ris_oracle_mol *mol, int nbatch, const double *c, c
                 double o[4];
                 double aP = mol->aux_exponents[P], aQ = mol->aux_exponents[Q];
                 ris_oracle_prim2c(aP, aQ, mol->coords + 3 * P, mol->coords + 3 * Q, o);
-                long double w = (long double)c[s * n + P] * dq[s * n + Q] * aux_norm(aP) * aux_norm(aQ);
+                long double w = (long double)c[s * n + P] * dq[s * n + Q] * (double)aux_norm(aP) * (double)aux_norm(aQ);
                 eacc[s] += w * o[0];
                 if (P == Q) continue;
                 for (int d = 0; d < 3; ++d) {

@@ -33,12 +33,18 @@ _SRC = os.path.join(_HERE, "ris_oracle.c")
 _lib = None
 
 
-def build(force: bool = False) -> str:
-    """gcc -O2 -fopenmp -shared.  No -ffast-math: IEEE semantics, long double accumulators."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-fopenmp", "-fPIC", "-shared",
-                               "-o", _SO, _SRC, "-lm"])
-    return _SO
+_SO_EXT = os.path.join(_HERE, "libris_oracle_ext.so")
+
+
+def build(force: bool = False, extended: bool = False) -> str:
+    """gcc -O2 -fopenmp -shared.  No -ffast-math: IEEE semantics, long double accumulators.
+    extended=True builds the SAME source with every intermediate in `long double` (-DORACLE_REAL): not the oracle,
+    but the yardstick tests/test_oracle_pins.py measures the oracle's own FP64 rounding error with."""
+    so = _SO_EXT if extended else _SO
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-fopenmp", "-fPIC", "-shared"]
+                              + (['-DORACLE_REAL=long double'] if extended else []) + ["-o", so, _SRC, "-lm"])
+    return so
 
 
 class _Mol(C.Structure):
@@ -48,11 +54,30 @@ class _Mol(C.Structure):
                 ("aux_exponents", C.c_void_p)]
 
 
+class extended_precision:
+    """`with extended_precision(): ...` routes every call of this module to the long-double-intermediate build."""
+
+    def __enter__(self):
+        global _lib
+        self._saved = _lib
+        _lib = None
+        _load(build(extended=True))
+
+    def __exit__(self, *exc):
+        global _lib
+        _lib = self._saved
+
+
 def lib():
-    global _lib
     if _lib is None:
-        build()
-        _lib = C.CDLL(_SO)
+        _load(build())
+    return _lib
+
+
+def _load(so):
+    global _lib
+    if True:
+        _lib = C.CDLL(so)
         _lib.ris_oracle_boys.argtypes = [C.c_int, C.c_double, C.c_void_p]
         _lib.ris_oracle_prim3c.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double,
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -65,7 +90,6 @@ def lib():
         _lib.ris_oracle_int3c_P.argtypes = [C.POINTER(_Mol), C.c_int, C.c_double, C.c_void_p]
         _lib.ris_oracle_int3c_P.restype = C.c_int
         _lib.ris_oracle_num_threads.restype = C.c_int
-    return _lib
 
 
 def num_threads() -> int:

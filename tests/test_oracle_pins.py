@@ -205,6 +205,25 @@ def test_quadrature_finite_difference_of_derivatives():
             assert abs(got[1 + 3 * which + d] - fd) < 1e-6, (which, d)
 
 
+def test_quadrature_finite_difference_of_f_shell_derivatives():
+    """l = 3 in the differentiated function: all nine derivative numbers of an f-d primitive pair (the `2a[a+1|`
+    branch with l_a + 1 = 4: E table index 4, Hermite R order 8; Eq. 27 terms 1-2) vs central
+    differences of the brute-force quadrature.  Two component pairs so that every Cartesian direction is raised to 4."""
+    a, b, alpha = 0.9, 0.6, 0.35
+    A, B, Cc = np.array([0.2, -0.1, 0.3]), np.array([-0.4, 0.5, 0.1]), np.array([1.9, -1.4, 1.1])
+    h = 1e-4
+    for xa, xb in (((3, 0, 0), (0, 1, 1)), ((0, 2, 1), (1, 0, 1)), ((0, 0, 3), (0, 2, 0))):
+        got = orc.prim3c(xa, xb, a, b, alpha, A, B, Cc)
+        scale = max(1.0, np.abs(got[1:]).max())
+        for which in range(3):
+            for d in range(3):
+                args_p, args_m = [A.copy(), B.copy(), Cc.copy()], [A.copy(), B.copy(), Cc.copy()]
+                args_p[which][d] += h
+                args_m[which][d] -= h
+                fd = (_quad3c(xa, xb, a, b, alpha, *args_p, n=44) - _quad3c(xa, xb, a, b, alpha, *args_m, n=44)) / (2 * h)
+                assert abs(got[1 + 3 * which + d] - fd) < 2e-6 * scale, (xa, xb, which, d, got[1 + 3 * which + d], fd)
+
+
 # ------------------------------------------------------------------ P12: far-aux limit
 
 def test_far_aux_limit():
@@ -265,6 +284,29 @@ def test_finite_difference_config1_all_atoms():
             fd = (f(mp_)[0] - f(mm_)[0]) / (2 * h)
             scale = np.abs(g[0]).max()
             assert abs(g[0, atom, d] - fd) < 2e-7 * scale, (name, atom, d, g[0, atom, d], fd)
+
+
+def test_finite_difference_f_shells_all_atoms():
+    """P6 at l = 3: central differences (5e-6 bohr) of E_J and E_K for every atom and direction of a
+    3-atom molecule with shells [[f, s], [f, d], [p]] -- classes (3,3), (3,2), (3,1), (3,0) differentiate an f shell, i.e.
+    the oracle's table bounds EMAX = 4 / Hermite order 8 are exercised without the CUDA path vouching for them."""
+    mol = synth.tiny_molecule(31, [[3, 0], [3, 2], [1]], [[0.0, 0.0, 0.0], [1.7, 0.4, -0.3], [-0.6, 1.6, 0.8]])
+    rng = np.random.default_rng(32)
+    nao, nocc, nvir = mol.nao, 3, 4
+    D = rng.standard_normal((1, nao, nao))
+    c = rng.standard_normal((1, 3))
+    Co, Cv = rng.standard_normal((nao, nocc)), rng.standard_normal((nao, nvir))
+    B = rng.standard_normal((1, 3, nocc, nvir))
+    gJ, _ = orc.grad_J(mol, D, c)
+    gK, _ = orc.grad_K(mol, Co, Cv, B)
+    assert np.all(np.abs(gJ.sum(axis=1)) < 1e-12 * np.abs(gJ).sum())
+    assert np.all(np.abs(gK.sum(axis=1)) < 1e-12 * np.abs(gK).sum())
+    h = 5e-6
+    for atom, d in itertools.product(range(3), range(3)):
+        mp_, mm_ = _displaced(mol, atom, d, h), _displaced(mol, atom, d, -h)
+        for name, g, f in (("J", gJ, lambda m: orc.grad_J(m, D, c)[1]), ("K", gK, lambda m: orc.grad_K(m, Co, Cv, B)[1])):
+            fd = (f(mp_)[0] - f(mm_)[0]) / (2 * h)
+            assert abs(g[0, atom, d] - fd) < 2e-7 * np.abs(g[0]).max(), (name, atom, d, g[0, atom, d], fd)
 
 
 def test_finite_difference_directional_all_classes():
@@ -369,3 +411,32 @@ def test_sampled_atoms_and_cutoff_equal_full():
         assert np.all(np.isnan(sJ[:, others]))
     cJ, _ = orc.grad_J(wl.mol, wl.D, wl.c_aux, prim_cutoff=1e-22)
     np.testing.assert_allclose(cJ, gJ, rtol=0, atol=1e-14 * np.abs(gJ).max())
+
+
+# ------------------------------------------------------------------ the oracle's own FP64 rounding error (R-tol evidence)
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_fp64_oracle_against_its_extended_precision_build(cfg):
+    """DESIGN.md reading R-tol rests on this measurement: the oracle (FP64 intermediates) against the SAME source built
+    with every intermediate in `long double` (-DORACLE_REAL, 64-bit mantissa) differs by a few 1e-15 of the gradient's
+    largest component -- so `5e-14 * max|ref|` (tests/test_gpu_parity.py) is ~30x the oracle's own rounding noise, and an
+    absolute floor has to be expressed in units of the gradient.  Also: against the extended build the FP64 oracle passes
+    north_star's LITERAL tolerance 1e-12 + 1e-10 |ref| on every component."""
+    wl = synth.make_workload(cfg)
+    mol = wl.mol
+    ref64 = (orc.grad_J(mol, wl.D, wl.c_aux)[0], orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B)[0],
+             orc.grad_PQ(mol, wl.c_aux, wl.d_aux)[0])
+    with orc.extended_precision():
+        ext = (orc.grad_J(mol, wl.D, wl.c_aux)[0], orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B)[0],
+               orc.grad_PQ(mol, wl.c_aux, wl.d_aux)[0])
+    again = orc.grad_J(mol, wl.D, wl.c_aux)[0]
+    # the context manager restored the FP64 build (OpenMP merges the threads' long double partial sums in arrival
+    # order, so two runs agree to the last bit or so, not necessarily bitwise)
+    assert np.abs(again - ref64[0]).max() <= 3e-16 * np.abs(again).max()
+    # measured: config 1  J 1.4e-14 (tight same-atom pairs, exponent ratio up to 500), K 2.4e-15, PQ 1.9e-16;
+    #           config 2  J 1.7e-15, K 1.6e-15, PQ 2.0e-16
+    bound = {1: 3e-14, 2: 5e-15}[cfg]
+    for name, a, b in zip("J K PQ".split(), ref64, ext):
+        err = np.abs(a - b)
+        assert err.max() <= bound * np.abs(b).max(), (name, err.max() / np.abs(b).max())
+        assert np.all(err <= 1e-12 + 1e-10 * np.abs(b)), (name, (err / (1e-12 + 1e-10 * np.abs(b))).max())
