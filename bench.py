@@ -30,9 +30,15 @@ if ROOT not in sys.path:
 
 METRIC = "TDDFT-ris gradient ms/state"
 UNIT = "ms/state"
-# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/r01_v9_ncu.md);
-# None where no capture of that (config, kernel) is committed.
-NCU_TRAFFIC = {(4, "ris_gemm_dmma(HT=Cvir*B^T)"): 1.399466e9 + 3.755925e9}
+# ncu counters of the committed `ncu --set full` captures, keyed by config and kernel (profiles/ncu_counters.json, written
+# by hand from the profile summaries it names); a (config, kernel) without a committed capture reports null.
+def ncu_counters(config: int) -> dict:
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_counters.json")) as f:
+            return json.load(f).get(f"config{config}", {})
+    except (OSError, ValueError):
+        return {}
+
 
 ORACLE_CUTOFF = {4: 1e-22}      # the oracle's documented primitive cutoff on config 4
 
@@ -46,6 +52,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-baseline-full", action="store_true",
+                    help="time the oracle over the WHOLE workload (minutes on config 3; not for config 4) and single-threaded")
     ap.add_argument("--oracle-aux", type=int, default=0, help="aux functions in the oracle's timed sample (0 = auto)")
     return ap.parse_args()
 
@@ -96,33 +104,85 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle leg
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def set_oracle_threads(n: int):
+    """The oracle's OpenMP team size (it is loaded already: set through the OpenMP runtime it linked)."""
+    import ctypes
+    ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+
+
 def oracle_sample_time(wl, cfg: int, n_aux: int, nstate: int = 1):
     """Time the oracle AS IT STANDS on a bounded sample of the workload: aux functions P in [0, n_aux) (of naux),
-    `nstate` state(s): J + K (incl. its Gamma^P assembly, numpy matmul) for the sample, PQ in full.  Returns
-    (seconds for the sample, extrapolated ms/state for the whole workload, threads, description)."""
+    `nstate` state(s): J, K (its Gamma^P assembly -- numpy matmul -- and its integral contraction timed separately) for
+    the sample, PQ in full.  n_aux >= naux and nstate = all states: the whole workload, nothing extrapolated.
+    Returns a dict: seconds of the sample, ms/state for the whole workload (extrapolated linearly in naux when the sample
+    is a part), threads, parts, description."""
     from oracle import ris_oracle as orc
     mol = wl.mol
     cut = ORACLE_CUTOFF.get(cfg, 0.0)
     aux = list(range(min(n_aux, mol.natoms)))
+    nsJ, nsK = min(nstate, wl.D.shape[0]), min(nstate, wl.B.shape[0])
     t0 = time.perf_counter()
-    orc.grad_J(mol, wl.D[:nstate], wl.c_aux[:nstate], prim_cutoff=cut, aux=aux)
+    orc.grad_J(mol, wl.D[:nsJ], wl.c_aux[:nsJ], prim_cutoff=cut, aux=aux)
     tJ = time.perf_counter()
-    orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B[:nstate], prim_cutoff=cut, aux=aux)
+    orc.grad_K(mol, wl.C_occ, wl.C_vir, wl.B[:nsK], prim_cutoff=cut, aux=aux)
     tK = time.perf_counter()
-    orc.grad_PQ(mol, wl.c_aux[:nstate], wl.d_aux[:nstate])
+    for P in aux:                       # the Gamma^P assembly step of grad_K once more, by itself
+        for st in range(nsK):
+            orc.gamma_P(wl.C_occ, wl.C_vir, wl.B[st, P])
+    tG = time.perf_counter()
+    orc.grad_PQ(mol, wl.c_aux[:nsJ], wl.d_aux[:nsJ])
     tQ = time.perf_counter()
     frac = len(aux) / mol.natoms
-    ms_state = ((tK - t0) / frac + (tQ - tK)) / nstate * 1e3
-    desc = (f"aux P in [0,{len(aux)}) of {mol.natoms}, {nstate} state of the batch: oracle grad_J {tJ - t0:.2f}s + grad_K "
-            f"(numpy Gamma^P + integrals) {tK - tJ:.2f}s, PQ in full {tQ - tK:.3f}s; ms/state extrapolated x{1 / frac:.1f}"
+    sJ, sK, sG, sQ = tJ - t0, tK - tJ, tG - tK, tQ - tG
+    ms_state = (sJ / nsJ / frac + sK / nsK / frac + sQ / nsJ) * 1e3
+    full = frac >= 1.0 and nsJ == wl.D.shape[0] and nsK == wl.B.shape[0]
+    desc = (("the whole workload, all aux functions and states" if full else
+             f"aux P in [0,{len(aux)}) of {mol.natoms}, {nsJ} J / {nsK} K state(s) of the batch") +
+            f": oracle grad_J {sJ:.2f}s + grad_K {sK:.2f}s (of which numpy Gamma^P assembly {sG:.2f}s, integral "
+            f"contraction {max(sK - sG, 0.0):.2f}s), PQ in full {sQ:.3f}s"
+            + ("" if full else f"; ms/state extrapolated x{1 / frac:.1f} in naux")
             + (f"; oracle primitive cutoff {cut:g}" if cut else ""))
-    return tQ - t0, ms_state, orc.num_threads(), desc
+    return {"seconds": sJ + sK + sQ, "ms_state": ms_state, "threads": orc.num_threads(), "desc": desc,
+            "extrapolated": not full, "factor": round(1.0 / frac, 2),
+            "parts_s": {"J": round(sJ, 3), "K_total": round(sK, 3), "K_gamma_assembly": round(sG, 3),
+                        "K_integrals": round(max(sK - sG, 0.0), 3), "PQ": round(sQ, 4)}}
 
 
 def auto_oracle_aux(wl) -> int:
-    # about 10-30 s of CPU work: cost per aux ~ ordered primitive pairs + Gamma^P matmul
-    est = {1: 3, 2: 30, 3: 12, 4: 6, 5: 4}
+    # about 10-30 s of CPU work on 16 threads: cost per aux ~ ordered primitive pairs + Gamma^P matmul
+    est = {1: 3, 2: 30, 3: 12, 4: 40, 5: 6}
     return est.get(wl.meta.get("config", 0), 4)
+
+
+def cpu_baseline_block(wl, cfg: int, n_aux: int, full: bool):
+    """The `cpu_baseline` object of the JSON line.  full: the oracle over the whole workload (configs 1-3, 5: nothing
+    extrapolated; `--cpu-baseline-full`), plus its single-thread time on configs 1-2 (whole) / 3 (a sample)."""
+    nst = max(wl.D.shape[0], wl.B.shape[0]) if full else 1
+    r = oracle_sample_time(wl, cfg, wl.mol.natoms if full else n_aux, nst)
+    blk = {"value": round(r["ms_state"], 2), "unit": UNIT, "cores": r["threads"], "cpu_model": cpu_model(), "kind": "oracle",
+           "sample": r["desc"], "sample_seconds": round(r["seconds"], 2), "extrapolated": r["extrapolated"],
+           "extrapolation_factor": r["factor"] if r["extrapolated"] else 1.0, "parts_s": r["parts_s"]}
+    if full and cfg in (1, 2, 3):
+        nthr = r["threads"]
+        set_oracle_threads(1)
+        try:
+            r1 = oracle_sample_time(wl, cfg, wl.mol.natoms if cfg < 3 else 2, nst if cfg < 3 else 1)
+        finally:
+            set_oracle_threads(nthr)
+        blk["single_thread"] = {"value": round(r1["ms_state"], 2), "unit": UNIT, "sample": r1["desc"],
+                                "extrapolated": r1["extrapolated"], "parts_s": r1["parts_s"]}
+    return blk
 
 
 # ------------------------------------------------------------------------------------------ our arm
@@ -131,6 +191,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2511_18233_b200 import probe_fp64_peak, ris_setup, synth
     from paper_2511_18233_b200.ris import probe_fp64_mma_peak
+    counters = ncu_counters(args.config)
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -167,10 +228,22 @@ def run_ours(args):
     gQ = torch.empty((nbJ, mol.natoms, 3), dtype=torch.float64, device=dev)
     torch.cuda.synchronize()
 
-    def step():
+    marks = []                              # per step: events before J, after J, after K, after PQ (same stream)
+
+    def step(timed=False):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if timed else None
+        if timed:
+            ev[0].record()
         ctx.grad_J(d["D"], d["c_aux"], out=gJ)
+        if timed:
+            ev[1].record()
         ctx.grad_K(d["C_occ"], d["C_vir"], d["B"], out=gK)
+        if timed:
+            ev[2].record()
         ctx.grad_PQ(d["c_aux"], d["d_aux"], out=gQ)
+        if timed:
+            ev[3].record()
+            marks.append(ev)
 
     def barrier():
         torch.cuda.synchronize()
@@ -191,18 +264,26 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        step()
+        step(timed=True)
     e1.record()
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
     prof = ctx.profile()
+    ms_J = sum(ev[0].elapsed_time(ev[1]) for ev in marks)
+    ms_K = sum(ev[1].elapsed_time(ev[2]) for ev in marks)
+    ms_Q = sum(ev[2].elapsed_time(ev[3]) for ev in marks)
     if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        t = torch.tensor([ms_total, ms_J, ms_K, ms_Q], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+        ms_total, ms_J, ms_K, ms_Q = (float(x) for x in t.tolist())
     ms_step = ms_total / args.steps
-    value = ms_step / (world * nstates)
+    # ms per state: every term divided by ITS OWN number of states (config 2 runs 2 J/PQ states and 1 K state); the
+    # remainder of the step (launch gaps between the calls) is charged to the larger batch.  Equal batches: ms_step/nbatch.
+    gap = max(ms_total - (ms_J + ms_K + ms_Q), 0.0)
+    value = (ms_J / nbJ + ms_K / nbK + ms_Q / nbJ + gap / nstates) / args.steps / world
+    per_term = {"J_ms_per_state": round(ms_J / nbJ / args.steps, 4), "K_ms_per_state": round(ms_K / nbK / args.steps, 4),
+                "PQ_ms_per_state": round(ms_Q / nbJ / args.steps, 4), "nbatch_J": nbJ, "nbatch_K": nbK}
 
     # ---- per-kernel accounting from the CUDA events the library records around every launch (same stream)
     groups = {}
@@ -217,9 +298,12 @@ def run_ours(args):
     achieved = dom["flops"] / (dom["ms"] * 1e-3) * 1e-12 if dom["ms"] > 0 else 0.0
     roofline = {"kernel": dom_name, "bound": "tensor" if is_gemm else "alu", "achieved": round(achieved, 3),
                 "peak": round(peak, 3), "unit": "TFLOP/s", "frac": round(achieved / peak, 4) if peak else None,
-                "traffic": NCU_TRAFFIC.get((args.config, dom_name)), "launches": dom["launches"], "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
+                "traffic": counters.get(dom_name, {}).get("dram_bytes_per_launch"), "launches": dom["launches"],
+                "avg_launch_ms": round(dom["ms"] / dom["launches"], 4),
                 "share_of_kernel_time": round(dom["ms"] / ksum, 4),
-                "traffic_unit": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum (profiles/r01_v9_ncu.md)",
+                "kernel_times_overlap": bool(ctx.p_batch >= 0 and mol.natoms <= 64),   # small molecules: class kernels run side by side
+                "traffic_unit": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum; source: "
+                                + str(counters.get(dom_name, {}).get("source", "no committed ncu capture of this (config, kernel)")),
                 "algorithmic_bytes_per_launch": round(dom["bytes"] / dom["launches"]),
                 "peak_source": ("measured in this run by ris_probe_fp64_mma_peak (mma.sync f64 chains)" if is_gemm else
                                 "measured in this run by ris_probe_fp64_peak (independent DFMA chains)")
@@ -229,7 +313,9 @@ def run_ours(args):
     cls_fl = sum(g["flops"] for g in cls)
     ncalls = 2 * args.steps                      # J and K each run the class kernels over all triplets
     integrals = {"tflops_model": round(cls_fl / (cls_ms * 1e-3) * 1e-12, 3) if cls_ms else None,
-                 "frac_of_fp64_peak": round(cls_fl / (cls_ms * 1e-3) * 1e-12 / fp64_peak, 4) if cls_ms else None,
+                 "frac_model": round(cls_fl / (cls_ms * 1e-3) * 1e-12 / fp64_peak, 4) if cls_ms else None,
+                 "frac_model_note": "textbook operation model of SURVEY.md 8(d) / live time; NOT the ncu instruction count",
+                 "frac_ncu": counters.get("integral_kernels"),
                  "fp64_peak_tflops": round(fp64_peak, 2), "ms_per_step": round(cls_ms / args.steps, 4),
                  "triplets_per_s": round(ctx.ntriplets * ncalls / (cls_ms * 1e-3), 1) if cls_ms else None,
                  "ntriplets": ctx.ntriplets, "ntriplets_unscreened": ctx.ntriplets_unscreened}
@@ -262,11 +348,16 @@ def run_ours(args):
             t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             t_e2e = float(t.item())
+        # the end-to-end result is the resident-input result (same kernels, other copy schedule)
+        e2e_err = max(float(np.abs(h - g.cpu().numpy()).max() / max(1e-300, float(g.abs().max())))
+                      for h, g in ((hJ, gJ), (hK, gK), (hQ, gQ)))
+        if not e2e_err <= 5e-14:
+            raise SystemExit(f"bench.py: ris_grad_host deviates from the resident-input path by {e2e_err:.3g} of the scale")
         h2d = 8 * (host["D"].numel() + host["c_aux"].numel() + host["d_aux"].numel() + host["C_occ"].numel()
                    + host["C_vir"].numel() + host["B"].numel())
         d2h = 8 * (hJ.size + hK.size + hQ.size)
         e2e = {"value": round(t_e2e / (world * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "ms_per_step_each": [round(r, 2) for r in reps],
+               "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "e2e_checked": True, "e2e_max_dev_of_scale": e2e_err, "ms_per_step_each": [round(r, 2) for r in reps],
                "median_ms_per_state": round(sorted(reps)[len(reps) // 2] / (world * nstates), 4),
                "how": "ris_grad_host (J + K + PQ in one call) on pinned host buffers; host wall clock around the call, which returns "
                       "after the D2H copy of the gradients; B goes up in P chunks on a copy stream under the J kernels and the GEMMs"}
@@ -306,6 +397,7 @@ def run_ours(args):
                    "p_batch": ctx.p_batch, "l2": "inputs larger than L2 (B alone is %.2f GB)" % (host["B"].numel() * 8e-9)
                    if host["B"].numel() * 8 > 200e6 else "inputs smaller than L2; no flush (latency-bound case)",
                    "step": "ris_grad_J + ris_grad_K + ris_grad_PQ, all states; ris_setup excluded (one-off per geometry)"},
+        "per_term": per_term,
         "setup_ms": round(setup_ms, 2), "setup_first_ms": round(setup_first_ms, 2), "e2e": e2e, "gpu_launches": len(prof),
         "roofline": roofline, "integral_kernels": integrals,
         "gamma_gemm": {"ms_per_step": round(gemm_ms / args.steps, 4),
@@ -316,9 +408,7 @@ def run_ours(args):
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             n_aux = args.oracle_aux or auto_oracle_aux(wl)
-            secs, ms_state, thr, desc = oracle_sample_time(wl, args.config, n_aux)
-            line["cpu_baseline"] = {"value": round(ms_state, 2), "unit": UNIT, "cores": thr, "kind": "oracle",
-                                    "sample": desc, "sample_seconds": round(secs, 2)}
+            line["cpu_baseline"] = cpu_baseline_block(wl, args.config, n_aux, args.cpu_baseline_full)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -326,28 +416,33 @@ def run_ours(args):
 
 # ------------------------------------------------------------------------------------------ reference arm
 def run_reference(args):
-    """The oracle, as it stands, on the host cores (rank 0 only); each step = the bounded sample."""
+    """The oracle, as it stands, on the host cores (rank 0 only).  Exactly `--warmup` untimed and `--steps` timed steps;
+    each step = one bounded sample of the workload (a few aux functions of one state; the whole workload on configs 1-2),
+    so that the run ends within minutes.  `ms_per_step` is the MEASURED time of one such step; `value` is ms/state of the
+    whole workload, extrapolated linearly in naux from the sample (`cpu_baseline.extrapolated`, `.extrapolation_factor`)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     from paper_2511_18233_b200 import synth        # input generator only (no arithmetic of the method)
     wl = synth.make_workload(args.config)
-    n_aux = args.oracle_aux or auto_oracle_aux(wl)
-    for _ in range(max(0, min(args.warmup, 1))):
-        oracle_sample_time(wl, args.config, 1)
-    vals, secs = [], 0.0
-    steps = max(1, min(args.steps, 3))
+    n_aux = args.oracle_aux or {1: 3, 2: 30, 3: 3, 4: 6, 5: 2}[args.config]
+    for _ in range(max(0, args.warmup)):
+        oracle_sample_time(wl, args.config, n_aux)
+    vals, secs, r = [], [], None
+    steps = max(1, args.steps)
     for _ in range(steps):
-        s, ms_state, thr, desc = oracle_sample_time(wl, args.config, n_aux)
-        vals.append(ms_state); secs += s
+        r = oracle_sample_time(wl, args.config, n_aux)
+        vals.append(r["ms_state"]); secs.append(r["seconds"])
     v = float(np.mean(vals))
-    nstates = max(wl.D.shape[0], wl.B.shape[0])
     line = {"impl": "reference", "metric": METRIC, "value": round(v, 2), "unit": UNIT,
-            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": steps, "warmup": min(args.warmup, 1),
-            "ms_per_step": round(v * nstates, 2), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": steps, "warmup": max(0, args.warmup),
+            "ms_per_step": round(float(np.mean(secs)) * 1e3, 2), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "natoms": wl.mol.natoms, "nao": wl.mol.nao, "nocc": wl.nocc, "nvir": wl.nvir},
-            "cpu_baseline": {"value": round(v, 2), "unit": UNIT, "cores": thr, "kind": "oracle", "sample": desc,
-                             "sample_seconds": round(secs / steps, 2)},
+            "config": {"workload": wl.name, "natoms": wl.mol.natoms, "nao": wl.mol.nao, "nocc": wl.nocc, "nvir": wl.nvir,
+                       "step": "one bounded sample of the workload (see cpu_baseline.sample); ms_per_step is its measured time"},
+            "cpu_baseline": {"value": round(v, 2), "unit": UNIT, "cores": r["threads"], "cpu_model": cpu_model(), "kind": "oracle",
+                             "sample": r["desc"], "sample_seconds": round(float(np.mean(secs)), 2),
+                             "extrapolated": r["extrapolated"], "extrapolation_factor": r["factor"] if r["extrapolated"] else 1.0,
+                             "parts_s": r["parts_s"]},
             "e2e": {"value": round(v, 2), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 

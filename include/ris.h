@@ -165,12 +165,6 @@ int ris_profile_get(ris_ctx* ctx, int i, const char** name, float* ms);
  * FP64 flops and HBM bytes, from the per-unit figures of DESIGN.md ("Algorithmic work per unit"). */
 int ris_profile_get_work(ris_ctx* ctx, int i, double* flops, double* bytes);
 
-/* Measurement helper: runs an independent-DFMA-chain kernel on every SM and returns the achieved
- * FP64 rate in TFLOP/s (the denominator of the "% FP64 peak" metric; MEASURED_PEAKS.json has none). */
-int ris_probe_fp64_peak(double* tflops, void* cuda_stream);
-/* Same for the FP64 tensor path: independent mma.sync.m8n8k4.f64 chains (the denominator for the Gamma^P GEMMs). */
-int ris_probe_fp64_mma_peak(double* tflops, void* cuda_stream);
-
 #ifdef __cplusplus
 }
 #endif

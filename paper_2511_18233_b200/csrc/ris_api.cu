@@ -2,6 +2,7 @@
 // tile packing, two-centre term (S5), FP64 probe.  The class kernels live in ris_grad_kernel.cuh
 // (one translation unit per class under generated/), the Gamma^P GEMMs in ris_gemm.cuh.
 #include "../../include/ris.h"
+#include "../../include/ris_bench.h"
 #include "ris_boys_table.h"
 #include "ris_core.cuh"
 #include "ris_gemm.cuh"
@@ -1476,6 +1477,21 @@ static int probe_fp64(int kind, double* tflops, void* cuda_stream)
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     *tflops = best;
+    return RIS_OK;
+}
+
+extern "C" int ris_diag_gemm2_layout(ris_ctx* c, int32_t* ao_pos_host, int* panel_rows, int* tile_cols, int* ntiles, int* novf)
+{
+    if (!c) return RIS_EINVAL;
+    CU(cudaSetDevice(c->device));
+    if (ao_pos_host) {
+        CU(cudaMemcpyAsync(ao_pos_host, c->d_ao_pos, sizeof(int) * (size_t)c->nao, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    if (panel_rows) *panel_rows = RIS_GPANEL_ROWS;
+    if (tile_cols) *tile_cols = RIS_GTILE2;
+    if (ntiles) *ntiles = c->ntiles;
+    if (novf) *novf = c->novf;
     return RIS_OK;
 }
 

@@ -20,7 +20,9 @@ EXPORTS = [
     "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
-    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work", "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak",
+    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
+    # include/ris_bench.h: measurement / diagnostics, not the product boundary
+    "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak", "ris_diag_gemm2_layout",
 ]
 
 
@@ -69,6 +71,7 @@ def load_library():
     lib.ris_profile_get_work.argtypes = [vp, ci, C.POINTER(cd), C.POINTER(cd)]
     lib.ris_probe_fp64_peak.argtypes = [C.POINTER(cd), vp]
     lib.ris_probe_fp64_mma_peak.argtypes = [C.POINTER(cd), vp]
+    lib.ris_diag_gemm2_layout.argtypes = [vp, vp, C.POINTER(ci), C.POINTER(ci), C.POINTER(ci), C.POINTER(ci)]
     _lib = lib
     return lib
 
@@ -128,6 +131,26 @@ class RisContext:
         self.naux = self._lib.ris_naux(h)
         self.natoms = self._lib.ris_natoms(h)
 
+    # ---- stream ordering: the library enqueues on the stream given at setup.  When the caller's CURRENT torch stream
+    # is a different one (where its inputs were produced and where it will read the outputs), the setup stream first
+    # waits for the current stream and the current stream afterwards waits for the setup stream.
+    class _Ordered:
+        def __init__(self, ctx):
+            self.ctx = ctx
+
+        def __enter__(self):
+            torch = self.ctx._torch
+            self.cur = torch.cuda.current_stream(self.ctx.device)
+            if self.cur != self.ctx.stream:
+                self.ctx.stream.wait_stream(self.cur)
+
+        def __exit__(self, *exc):
+            if self.cur != self.ctx.stream:
+                self.cur.wait_stream(self.ctx.stream)
+
+    def _ordered(self):
+        return RisContext._Ordered(self)
+
     # ---- queries
     def npairs(self, la, lb):
         return int(self._lib.ris_npairs(self._h, la, lb))
@@ -168,25 +191,28 @@ class RisContext:
         nb = D.shape[0]
         if out is None:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_grad_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)),
-                                    self._dev(c_aux, (nb, self.naux)), self._dev(out, (nb, self.natoms, 3))))
+        with self._ordered():
+            _check(self._lib.ris_grad_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)),
+                                        self._dev(c_aux, (nb, self.naux)), self._dev(out, (nb, self.natoms, 3))))
         return out
 
     def grad_K(self, C_occ, C_vir, B, out=None):
         nb, nocc, nvir = B.shape[0], C_occ.shape[1], C_vir.shape[1]
         if out is None:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_grad_K(self._h, nb, nocc, nvir, self._dev(C_occ, (self.nao, nocc)),
-                                    self._dev(C_vir, (self.nao, nvir)), self._dev(B, (nb, self.naux, nocc, nvir)),
-                                    self._dev(out, (nb, self.natoms, 3))))
+        with self._ordered():
+            _check(self._lib.ris_grad_K(self._h, nb, nocc, nvir, self._dev(C_occ, (self.nao, nocc)),
+                                        self._dev(C_vir, (self.nao, nvir)), self._dev(B, (nb, self.naux, nocc, nvir)),
+                                        self._dev(out, (nb, self.natoms, 3))))
         return out
 
     def grad_PQ(self, c_aux, d_aux, out=None):
         nb = c_aux.shape[0]
         if out is None:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux)), self._dev(d_aux, (nb, self.naux)),
-                                     self._dev(out, (nb, self.natoms, 3))))
+        with self._ordered():
+            _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux)), self._dev(d_aux, (nb, self.naux)),
+                                         self._dev(out, (nb, self.natoms, 3))))
         return out
 
     # ---- fitting step, J type (argument marshalling only)
@@ -195,8 +221,9 @@ class RisContext:
         nb = D.shape[0]
         v = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
         c = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux)),
-                                   self._dev(c, (nb, self.naux))))
+        with self._ordered():
+            _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux)),
+                                       self._dev(c, (nb, self.naux))))
         return v, c
 
     def fit_K(self, C_occ, C_vir):
@@ -204,67 +231,96 @@ class RisContext:
         nocc, nvir = C_occ.shape[1], C_vir.shape[1]
         T = self._torch.empty((self.naux, nocc, nvir), dtype=self._torch.float64, device=self.device)
         B = self._torch.empty((self.naux, nocc, nvir), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_fit_K(self._h, nocc, nvir, self._dev(C_occ, (self.nao, nocc)), self._dev(C_vir, (self.nao, nvir)),
-                                   self._dev(T, (self.naux, nocc, nvir)), self._dev(B, (self.naux, nocc, nvir))))
+        with self._ordered():
+            _check(self._lib.ris_fit_K(self._h, nocc, nvir, self._dev(C_occ, (self.nao, nocc)), self._dev(C_vir, (self.nao, nvir)),
+                                       self._dev(T, (self.naux, nocc, nvir)), self._dev(B, (self.naux, nocc, nvir))))
         return T, B
 
     def grad_PQ_full(self, G, out=None):
         nb = G.shape[0]
         if out is None:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_grad_PQ_full(self._h, nb, self._dev(G, (nb, self.naux, self.naux)),
-                                          self._dev(out, (nb, self.natoms, 3))))
+        with self._ordered():
+            _check(self._lib.ris_grad_PQ_full(self._h, nb, self._dev(G, (nb, self.naux, self.naux)),
+                                              self._dev(out, (nb, self.natoms, 3))))
         return out
 
     def metric(self):
         M = self._torch.empty((self.naux, self.naux), dtype=self._torch.float64, device=self.device)
-        _check(self._lib.ris_metric(self._h, self._dev(M, (self.naux, self.naux))))
+        with self._ordered():
+            _check(self._lib.ris_metric(self._h, self._dev(M, (self.naux, self.naux))))
         return M
 
-    # ---- host-buffer calls (numpy arrays or pinned CPU tensors; copies happen inside the C call)
+    # ---- host-buffer calls (numpy arrays or CPU tensors, float64, C-contiguous; copies happen inside the C call)
     @staticmethod
-    def _host(x):
+    def _host(x, what="input"):
+        """(pointer, shape, keep-alive).  float64 and C-contiguous are REQUIRED of tensors and of numpy arrays alike: a silent
+        conversion copy would make the C call read (or, for outputs, fill) a temporary."""
         if hasattr(x, "data_ptr"):
-            if x.is_cuda or not x.is_contiguous():
-                raise RisError("expected a contiguous CPU tensor")
-            return C.c_void_p(x.data_ptr()), tuple(x.shape)
-        a = _np(x, np.float64)
+            import torch
+            if x.is_cuda or not x.is_contiguous() or x.dtype != torch.float64:
+                raise RisError(f"{what}: expected a contiguous float64 CPU tensor, got {x.dtype} on {x.device}")
+            return C.c_void_p(x.data_ptr()), tuple(x.shape), x
+        a = np.asarray(x)
+        if a.dtype != np.float64 or not a.flags.c_contiguous:
+            raise RisError(f"{what}: expected a C-contiguous float64 array, got dtype {a.dtype}, "
+                           f"c_contiguous={a.flags.c_contiguous}")
         return C.c_void_p(a.ctypes.data), a.shape, a
 
-    def grad_J_host(self, D, c_aux, out=None):
-        pD, pc = self._host(D), self._host(c_aux)
-        nb = pD[1][0]
+    def _host_out(self, out, shape):
         if out is None:
-            out = np.empty((nb, self.natoms, 3))
-        _check(self._lib.ris_grad_J_host(self._h, nb, pD[0], pc[0], self._host(out)[0]))
+            out = np.empty(shape)
+        p = self._host(out, "out")
+        if tuple(p[1]) != tuple(shape):
+            raise RisError(f"out: shape {tuple(p[1])} != expected {tuple(shape)}")
+        return out, p
+
+    def grad_J_host(self, D, c_aux, out=None):
+        pD, pc = self._host(D, "D"), self._host(c_aux, "c_aux")
+        nb = pD[1][0]
+        out, po = self._host_out(out, (nb, self.natoms, 3))
+        with self._ordered():
+            _check(self._lib.ris_grad_J_host(self._h, nb, pD[0], pc[0], po[0]))
         return out
 
     def grad_K_host(self, C_occ, C_vir, B, out=None):
-        po, pv, pB = self._host(C_occ), self._host(C_vir), self._host(B)
+        po, pv, pB = self._host(C_occ, "C_occ"), self._host(C_vir, "C_vir"), self._host(B, "B")
         nb, nocc, nvir = pB[1][0], po[1][1], pv[1][1]
-        if out is None:
-            out = np.empty((nb, self.natoms, 3))
-        _check(self._lib.ris_grad_K_host(self._h, nb, nocc, nvir, po[0], pv[0], pB[0], self._host(out)[0]))
+        out, pg = self._host_out(out, (nb, self.natoms, 3))
+        with self._ordered():
+            _check(self._lib.ris_grad_K_host(self._h, nb, nocc, nvir, po[0], pv[0], pB[0], pg[0]))
         return out
 
     def grad_PQ_host(self, c_aux, d_aux, out=None):
-        pc, pd = self._host(c_aux), self._host(d_aux)
+        pc, pd = self._host(c_aux, "c_aux"), self._host(d_aux, "d_aux")
         nb = pc[1][0]
-        if out is None:
-            out = np.empty((nb, self.natoms, 3))
-        _check(self._lib.ris_grad_PQ_host(self._h, nb, pc[0], pd[0], self._host(out)[0]))
+        out, pg = self._host_out(out, (nb, self.natoms, 3))
+        with self._ordered():
+            _check(self._lib.ris_grad_PQ_host(self._h, nb, pc[0], pd[0], pg[0]))
         return out
 
     def grad_host(self, D, c_aux, d_aux, C_occ, C_vir, B, out=None):
         """(gJ, gK, gPQ) from host buffers in one call (H2D of B overlapped with the kernels)."""
-        pD, pc, pd = self._host(D), self._host(c_aux), self._host(d_aux)
-        po, pv, pB = self._host(C_occ), self._host(C_vir), self._host(B)
+        pD, pc, pd = self._host(D, "D"), self._host(c_aux, "c_aux"), self._host(d_aux, "d_aux")
+        po, pv, pB = self._host(C_occ, "C_occ"), self._host(C_vir, "C_vir"), self._host(B, "B")
         nbJ, nbK, nocc, nvir = pD[1][0], pB[1][0], po[1][1], pv[1][1]
         if out is None:
-            out = (np.empty((nbJ, self.natoms, 3)), np.empty((nbK, self.natoms, 3)), np.empty((nbJ, self.natoms, 3)))
-        _check(self._lib.ris_grad_host(self._h, nbJ, pD[0], pc[0], pd[0], nbK, nocc, nvir, po[0], pv[0], pB[0],
-                                       self._host(out[0])[0], self._host(out[1])[0], self._host(out[2])[0]))
-        return out
+            out = (None, None, None)
+        oJ, pJ = self._host_out(out[0], (nbJ, self.natoms, 3))
+        oK, pK = self._host_out(out[1], (nbK, self.natoms, 3))
+        oQ, pQ = self._host_out(out[2], (nbJ, self.natoms, 3))
+        with self._ordered():
+            _check(self._lib.ris_grad_host(self._h, nbJ, pD[0], pc[0], pd[0], nbK, nocc, nvir, po[0], pv[0], pB[0],
+                                           pJ[0], pK[0], pQ[0]))
+        return oJ, oK, oQ
+
+    # ---- measurement / diagnostics (include/ris_bench.h)
+    def gemm2_layout(self):
+        """(ao_pos[nao], panel_rows, tile_cols, ntiles, novf) of the pair-restricted Gamma^P GEMM-2."""
+        pos = np.empty(self.nao, dtype=np.int32)
+        r, c, nt, nv = C.c_int(), C.c_int(), C.c_int(), C.c_int()
+        _check(self._lib.ris_diag_gemm2_layout(self._h, pos.ctypes.data, C.byref(r), C.byref(c), C.byref(nt), C.byref(nv)))
+        return pos, r.value, c.value, nt.value, nv.value
 
     # ---- profiling
     def profile_reset(self):
