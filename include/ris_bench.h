@@ -21,10 +21,10 @@ int ris_probe_fp64_peak(double* tflops, void* cuda_stream);
 int ris_probe_fp64_mma_peak(double* tflops, void* cuda_stream);
 
 /* Layout of the pair-restricted Gamma^P GEMM-2: the spatial position of every AO
- * (ao_pos_host[nao], host pointer, filled by the call) and the tile geometry: rows of a row panel, gathered columns of
- * a tile, number of tiles, number of same-shell elements served by the overflow gather.  Any output pointer may be
- * NULL.  RIS_EINVAL on a null context. */
-int ris_diag_gemm2_layout(ris_ctx* ctx, int32_t* ao_pos_host, int* panel_rows, int* tile_cols, int* ntiles, int* novf);
+ * (ao_pos_host[nao], host pointer, filled by the call) and the tile geometry: gathered partner rows of a tile
+ * (panel_rows), aux functions of a tile (tile_cols), number of tiles, number of partner-list entries (two per packed
+ * pair element).  Any output pointer may be NULL.  RIS_EINVAL on a null context. */
+int ris_diag_gemm2_layout(ris_ctx* ctx, int32_t* ao_pos_host, int* panel_rows, int* tile_cols, int* ntiles, int* nentries);
 
 #ifdef __cplusplus
 }

@@ -234,12 +234,12 @@ def gen_hrrc(pl: ClassPlan) -> str:
     w = out.append
     w(f"// contracted triplet of class ({la},{lb}): HRR, derivative assembly, contraction with the tile of each state,")
     w("// accumulated into the caller's per-lane slots: slot[(s*6 + c)*SL] += sc[s*SC] * g, c = 0..2 centre A, 3..5 centre B")
-    w("// (the host centre is B in the TR instantiations).  tile element (c_host,c_other) of state s sits at")
-    w("// tile[s*sstride + el*estride], el by TR (see gen_classes.py).")
-    w("template <bool TR, int SL, int SC>")
+    w("// (the host centre is B in the TR instantiations).  The tile comes from a provider: ring.get(s) returns the tile of")
+    w("// state s (shared-memory ring of the class kernel, or plain memory), element (c_host,c_other) at t[el * ring.es()],")
+    w("// el by TR (see gen_classes.py).")
+    w("template <bool TR, int SL, int SC, class Ring>")
     w(f"RIS_DEV void ris_hrrc_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
-    w("    const double* __restrict__ tile, size_t estride, size_t sstride, int nb, const double* __restrict__ sc,")
-    w("    double* __restrict__ slot)")
+    w("    Ring& ring, int nb, const double* __restrict__ sc, double* __restrict__ slot)")
     w("{")
     done = set()
     X2a = gen_hrr_chain(w, pl, "2a", la + 1, lb, "xa", done)
@@ -248,8 +248,9 @@ def gen_hrrc(pl: ClassPlan) -> str:
     Y1m = gen_hrr_chain(w, pl, "1", la, lb - 1, "xm", done) if lb >= 1 else None
     nca, ncb = nc(la), nc(lb)
     w("    constexpr int OH = TR ? 3 : 0, OO = TR ? 0 : 3;")
+    w("    const size_t estride = ring.es();")
     w("    for (int s = 0; s < nb; ++s) {")
-    w("        const double* __restrict__ t = tile + (size_t)s * sstride;")
+    w("        const double* __restrict__ t = ring.get(s);")
     w("        double ga0 = 0.0, ga1 = 0.0, ga2 = 0.0, gb0 = 0.0, gb1 = 0.0, gb2 = 0.0;")
     for ia, a in enumerate(comps(la)):
         for ib, b in enumerate(comps(lb)):
@@ -262,7 +263,7 @@ def gen_hrrc(pl: ClassPlan) -> str:
                 if b[i] >= 1:
                     w(f"          gb{i} = fma(-{float(b[i])} * w, {Y1m(a, lower(b, i))}, gb{i});")
             w("        }")
-    w("        const double c = sc[s * SC];")
+    w("        const double c = SC ? sc[s * SC] : 1.0;       // SC = 0: no scale (K type)")
     w("        double* __restrict__ o = slot + s * 6 * SL;")
     for i in range(3):
         w(f"        o[(OH + {i}) * SL] = fma(c, ga{i}, o[(OH + {i}) * SL]);")

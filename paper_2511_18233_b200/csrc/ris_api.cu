@@ -48,6 +48,7 @@ struct ProfRec { const char* name; cudaEvent_t e0, e1; double flops, bytes; };
 
 struct ris_ctx {
     int device = 0;
+    int nsm = 0;                       // SMs of `device` (grid sizing of the class kernels)
     cudaStream_t stream = nullptr;
     ris_options opt{};
     int natoms = 0, nshells = 0, nao = 0, naux = 0;
@@ -68,19 +69,15 @@ struct ris_ctx {
     int *d_rb_jlo = nullptr, *d_rb_kw = nullptr;
     long long* d_rb_off = nullptr;
     double* d_chol = nullptr;          // [naux][naux] lower Cholesky factor of the aux metric (built by the first ris_fit_J)
-    // Gamma^P GEMM-2 block list: RIS_GTILE2^2 blocks (I >= J) of the spatially (Morton) ordered AO index that
-    // contain a surviving shell pair
+    // Gamma^P GEMM-2 (ris_gemm.cuh, scatter mode): per AO position nu' the gathered list of its surviving partners
     int* d_ao_pos = nullptr;           // [nao] spatial position of AO
     int* d_ao_order = nullptr;         // [nao] AO at spatial position
-    int nblk = 0, ntiles = 0;
-    int2* d_tiles = nullptr;           // [ntiles] (row panel I, offset of the tile's 64 columns in d_gcols)
-    int* d_gcols = nullptr;            // gathered column lists of all panels (AO positions; -1 = padding)
-    // inverse map for the P-minor tile transpose: S position -> packed element
-    int* d_smap = nullptr;             // [ntiles][64][64]  (packed element << 1 | same-shell pair), -1 if no surviving element
-    int* d_srows = nullptr;            // [nsrows] rows (tile * 64 + r) of the block buffer that hold a surviving element
-    int nsrows = 0;
-    int* d_ovf = nullptr;              // [novf][2] (element code, S position) of the elements that share an S position
-    int novf = 0;
+    int nblk = 0;                      // 64-row blocks of the spatial AO order (fit_K bands)
+    int ntiles = 0;                    // GEMM-2 tiles: RIS_G2_BM partner rows of one column problem each
+    long long g2_entries = 0;          // partner-list entries (2 per packed pair element)
+    int2* d_g2tiles = nullptr;         // [ntiles] (column problem nu', first entry of the tile in d_g2rows / d_g2code)
+    int* d_g2rows = nullptr;           // [ntiles * RIS_G2_BM] partner position mu' (A row), -1 = padding
+    int* d_g2code = nullptr;           // [ntiles * RIS_G2_BM] packed element << 1 | (symmetry factor 1/2), -1 = padding
     // grow-only scratch
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
@@ -95,7 +92,7 @@ struct ris_ctx {
     std::vector<cudaEvent_t> ev_pool;
 };
 
-enum { WS_TILE = 0, WS_H = 1, WS_G = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
+enum { WS_TILE = 0, WS_H = 1, WS_UNUSED2 = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
        WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_N = 20 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
@@ -175,19 +172,19 @@ extern "C" int ris_profile_get_work(ris_ctx* c, int i, double* flops, double* by
 }
 
 // --------------------------------------------------------------------------------------- class launchers
-#define DECL(la, lb) void ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
+#define DECL(la, lb) cudaError_t ris_launch_grad_##la##lb(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
 #undef DECL
 ris_grad_launcher ris_grad_launchers[RIS_NCLASS] = {
     ris_launch_grad_00, ris_launch_grad_10, ris_launch_grad_11, ris_launch_grad_20, ris_launch_grad_21,
     ris_launch_grad_22, ris_launch_grad_30, ris_launch_grad_31, ris_launch_grad_32, ris_launch_grad_33};
-#define DECL(la, lb) void ris_launch_int_##la##lb(const RisGradParams&, cudaStream_t);
+#define DECL(la, lb) cudaError_t ris_launch_int_##la##lb(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
 #undef DECL
 static const ris_grad_launcher ris_int_launchers[RIS_NCLASS] = {
     ris_launch_int_00, ris_launch_int_10, ris_launch_int_11, ris_launch_int_20, ris_launch_int_21,
     ris_launch_int_22, ris_launch_int_30, ris_launch_int_31, ris_launch_int_32, ris_launch_int_33};
-#define DECL(la, lb) void ris_launch_ints_##la##lb(const RisGradParams&, cudaStream_t);
+#define DECL(la, lb) cudaError_t ris_launch_ints_##la##lb(const RisGradParams&, cudaStream_t);
 DECL(0, 0) DECL(1, 0) DECL(1, 1) DECL(2, 0) DECL(2, 1) DECL(2, 2) DECL(3, 0) DECL(3, 1) DECL(3, 2) DECL(3, 3)
 #undef DECL
 static const ris_grad_launcher ris_ints_launchers[RIS_NCLASS] = {
@@ -206,54 +203,71 @@ static const double kModelFlopsByE[8] = {90.0, 140.0, 250.0, 450.0, 750.0, 1250.
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
 // --------------------------------------------------------------------------------------- setup
-// Marks, per 64-row panel of the spatially ordered AO index, the columns that hold a surviving pair element; an
-// element (r, q) is oriented so that block(r) >= block(q) (S^P is symmetric).
-__global__ void ris_k_mark_cols(RisClassPack pk, const int* __restrict__ ao_pos, int nao, int* __restrict__ cmark)
+// GEMM-2 partner lists.  Every packed pair element e = (mu, nu) with symmetry factor f emits two entries:
+//   into the list of column nu':  (row mu', e, f)   -- adds f Gamma^P_{mu nu} to tile[e][P]
+//   into the list of column mu':  (row nu', e, f)   -- adds f Gamma^P_{nu mu}
+// (a same-shell pair holds (ca,cb) and (cb,ca) as elements of their own, each with f = 1/2; its diagonal elements get
+// two entries of 1/2 Gamma_{mu mu}).  Pass 1 counts per column and records, per 64-row block of the spatial AO order,
+// the range of partner blocks (the bands of ris_fit_K).
+__global__ void ris_k_g2_count(RisClassPack pk, const int* __restrict__ ao_pos, int* __restrict__ cnt, volatile int* jlo,
+                               volatile int* jhi)
 {
-    constexpr int T = RIS_GPANEL_ROWS;
     const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)pk.npairs * nel) return;
     const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
-    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
-    if (r / T < q / T) { const int t = r; r = q; q = t; }
-    cmark[(size_t)(r / T) * nao + q] = 1;
+    const int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
+    atomicAdd(&cnt[q], 1);
+    atomicAdd(&cnt[r], 1);
+    const int I = r / RIS_GTILE2, J = q / RIS_GTILE2;
+    // (read first: after the first few elements of a block pair nothing changes any more, and ~50 addresses would
+    // otherwise serialise a million atomics)
+    if (J < jlo[I]) atomicMin((int*)&jlo[I], J);
+    if (J > jhi[I]) atomicMax((int*)&jhi[I], J);
+    if (I < jlo[J]) atomicMin((int*)&jlo[J], I);
+    if (I > jhi[J]) atomicMax((int*)&jhi[J], I);
 }
 
-// Inverse map of the packed pair elements into the GEMM-2 block buffer: element (ip, ca, cb) of a class reads
-// S^P[pos(mu0+ca)][pos(nu0+cb)] (S^P = Gamma^P + Gamma^P^T is symmetric; only blocks I >= J exist).
-__global__ void ris_k_build_smap(RisClassPack pk, const int* __restrict__ ao_pos, const int* __restrict__ colidx,
-                                 const int* __restrict__ ptile0, int nao, int* __restrict__ smap, int* __restrict__ rowflag,
-                                 int* __restrict__ ovf, int* __restrict__ novf)
+// One block: tiles per column = ceil(cnt / BM); tbase[nu] = exclusive scan; tbase[nao] = total.
+__global__ void __launch_bounds__(1024) ris_k_g2_scan(int nao, int bm, const int* __restrict__ cnt, int* __restrict__ tbase)
 {
-    constexpr int T = RIS_GPANEL_ROWS, TC = RIS_GTILE2;       // panel rows, tile columns
-    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (long long)pk.npairs * nel) return;
-    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
-    int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
-    if (r / T < q / T) { const int t = r; r = q; q = t; }
-    const int ci = colidx[(size_t)(r / T) * nao + q];          // column within the panel's gathered list
-    const int tile = ptile0[r / T] + ci / TC;
-    const int code = (int)(((pk.elem_off + idx) << 1) | (pk.symf[ip] < 0.75f ? 1 : 0));
-    const size_t pos = (size_t)tile * (T * TC) + (r % T) * TC + (ci % TC);
-    // elements (ca,cb) and (cb,ca) of a same-shell pair that straddles a block edge fold onto ONE position of the
-    // symmetric S: the second one goes to a short overflow list served by a gather
-    if (atomicCAS(&smap[pos], -1, code) != -1) {
-        const int k = atomicAdd(novf, 1);
-        ovf[2 * k] = code; ovf[2 * k + 1] = (int)pos;
-        return;
+    __shared__ int part[1024];
+    const int t = threadIdx.x, per = (nao + 1023) / 1024;
+    const int i0 = min(t * per, nao), i1 = min(i0 + per, nao);
+    int sum = 0;
+    for (int i = i0; i < i1; ++i) sum += (cnt[i] + bm - 1) / bm;
+    part[t] = sum;
+    __syncthreads();
+    if (t == 0) {
+        int run = 0;
+        for (int k = 0; k < 1024; ++k) { const int v = part[k]; part[k] = run; run += v; }
+        tbase[nao] = run;
     }
-    rowflag[tile * T + (r % T)] = 1;
+    __syncthreads();
+    int run = part[t];
+    for (int i = i0; i < i1; ++i) { tbase[i] = run; run += (cnt[i] + bm - 1) / bm; }
 }
 
-// overflow elements of ris_k_build_smap: out[el * pbp + P] = symf * S^P[pos]
-__global__ void ris_k_pack_sym_ovf(int novf, const int* __restrict__ ovf, int np, int pbp, const double* __restrict__ S,
-                                   long long sstrideP, double* __restrict__ out)
+__global__ void ris_k_g2_fill(RisClassPack pk, const int* __restrict__ ao_pos, int bm, const int* __restrict__ tbase,
+                              int* __restrict__ fillctr, int* __restrict__ rows, int* __restrict__ code)
 {
-    const int k = blockIdx.x, code = ovf[2 * k], pos = ovf[2 * k + 1];
-    for (int P = threadIdx.x; P < np; P += blockDim.x)
-        out[(size_t)(code >> 1) * pbp + P] = ((code & 1) ? 0.5 : 1.0) * S[(size_t)P * sstrideP + pos];
+    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)pk.npairs * nel) return;
+    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
+    const int r = ao_pos[pk.ao[ip]] + ca, q = ao_pos[pk.ao[(size_t)pk.npairs + ip]] + cb;
+    const int c = (int)(((pk.elem_off + idx) << 1) | (pk.symf[ip] < 0.75f ? 1 : 0));
+    int k = atomicAdd(&fillctr[q], 1);
+    rows[(size_t)tbase[q] * bm + k] = r; code[(size_t)tbase[q] * bm + k] = c;
+    k = atomicAdd(&fillctr[r], 1);
+    rows[(size_t)tbase[r] * bm + k] = q; code[(size_t)tbase[r] * bm + k] = c;
+}
+
+__global__ void ris_k_g2_tiles(int nao, int bm, const int* __restrict__ tbase, int2* __restrict__ tiles)
+{
+    const int nu = blockIdx.x * blockDim.x + threadIdx.x;
+    if (nu >= nao) return;
+    for (int t = tbase[nu]; t < tbase[nu + 1]; ++t) tiles[t] = make_int2(nu, t * bm);
 }
 
 // Morton (Z-order) code of a point on a 3-bohr grid: the spatial AO order that keeps the surviving pairs of an
@@ -302,6 +316,7 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     if (!c) return RIS_ENOMEM;
     struct Guard { ris_ctx* c; bool ok = false; ~Guard() { if (!ok) ris_destroy(c); } } guard{c};
     CU(cudaGetDevice(&c->device));
+    CU(cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device));
     c->stream = (cudaStream_t)cuda_stream;
     c->opt.schwarz_tol = 1e-13;
     if (opt) c->opt = *opt;
@@ -442,48 +457,49 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         if ((rc = dev_upload(c, &c->d_ao_pos, ao_pos.data(), ao_pos.size()))) return rc;
         if ((rc = dev_upload(c, &c->d_ao_order, ao_order.data(), ao_order.size()))) return rc;
         c->nblk = (nao + RIS_GTILE2 - 1) / RIS_GTILE2;
-        const int npanel = (nao + RIS_GPANEL_ROWS - 1) / RIS_GPANEL_ROWS;
-        // GEMM-2 tiles: per RIS_GPANEL_ROWS-row panel I of the spatial AO order, the GATHERED list of columns (positions q with a
-        // surviving element (r, q), r in the panel, oriented so that block(r) >= block(q)), cut into 64-column tiles.
-        // Versus aligned 64x64 blocks this drops the columns of tight shells that only reach the near part of the band
-        // (config 4: 756 k instead of 934 k block-buffer elements for 437 k unique surviving ones).
-        int* d_cmark;
-        if ((rc = dev_alloc(c, &d_cmark, (size_t)npanel * nao, true))) return rc;
+        // GEMM-2 partner lists and the fit_K bands, built on the device (two small D2H reads: tile count, band ranges)
+        constexpr int BM = RIS_G2_BM;
+        int *d_cnt, *d_tbase, *d_fill, *d_jlo, *d_jhi;
+        if ((rc = dev_alloc(c, &d_cnt, (size_t)nao, true))) return rc;
+        if ((rc = dev_alloc(c, &d_fill, (size_t)nao, true))) return rc;
+        if ((rc = dev_alloc(c, &d_tbase, (size_t)nao + 1, true))) return rc;
+        if ((rc = dev_alloc(c, &d_jlo, (size_t)c->nblk, false))) return rc;
+        if ((rc = dev_alloc(c, &d_jhi, (size_t)c->nblk, false))) return rc;
+        CU(cudaMemsetAsync(d_jlo, 0x7f, sizeof(int) * (size_t)c->nblk, c->stream));
+        CU(cudaMemsetAsync(d_jhi, 0xff, sizeof(int) * (size_t)c->nblk, c->stream));
         for (int k = 0; k < RIS_NCLASS; ++k) {
             const RisClassPack& pk = c->cls[k];
             if (pk.npairs == 0) continue;
             const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
-            ris_k_mark_cols<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, nao, d_cmark);
+            ris_k_g2_count<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, d_cnt, d_jlo, d_jhi);
         }
+        ris_k_g2_scan<<<1, 1024, 0, c->stream>>>(nao, BM, d_cnt, d_tbase);
         CU(cudaGetLastError());
-        std::vector<int> cmark((size_t)npanel * nao);
-        CU(cudaMemcpyAsync(cmark.data(), d_cmark, cmark.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        std::vector<int> jlo(c->nblk), jhi(c->nblk);
+        CU(cudaMemcpyAsync(&c->ntiles, d_tbase + nao, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(jlo.data(), d_jlo, sizeof(int) * (size_t)c->nblk, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaMemcpyAsync(jhi.data(), d_jhi, sizeof(int) * (size_t)c->nblk, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
-        std::vector<int2> tiles;
-        std::vector<int> gcols, ptile0(npanel), jlo(c->nblk, 1 << 30), jhi(c->nblk, -1);
-        for (int I = 0; I < npanel; ++I) {
-            const int I64 = I * RIS_GPANEL_ROWS / RIS_GTILE2;      // the 64-row block of the fit_K bands this panel lies in
-            ptile0[I] = (int)tiles.size();
-            int* row = &cmark[(size_t)I * nao];
-            int n = 0;
-            for (int q = 0; q < nao; ++q) {
-                if (!row[q]) { row[q] = -1; continue; }
-                row[q] = n++;                              // cmark becomes the column index within the panel's list
-                gcols.push_back(q);
-                const int J = q / RIS_GTILE2;
-                jlo[I64] = std::min(jlo[I64], J); jhi[I64] = std::max(jhi[I64], J);
-                jlo[J] = std::min(jlo[J], I64); jhi[J] = std::max(jhi[J], I64);
-            }
-            for (int t = 0; t < (n + RIS_GTILE2 - 1) / RIS_GTILE2; ++t)
-                tiles.push_back(make_int2(I, (int)gcols.size() - n + t * RIS_GTILE2));
-            while (gcols.size() % RIS_GTILE2) gcols.push_back(-1);
+        c->g2_entries = 2 * c->nelem_real;
+        const size_t nrow = (size_t)std::max(c->ntiles, 1) * BM;
+        if ((rc = dev_alloc(c, &c->d_g2tiles, (size_t)std::max(c->ntiles, 1), false))) return rc;
+        if ((rc = dev_alloc(c, &c->d_g2rows, nrow, false))) return rc;
+        if ((rc = dev_alloc(c, &c->d_g2code, nrow, false))) return rc;
+        CU(cudaMemsetAsync(c->d_g2rows, 0xff, sizeof(int) * nrow, c->stream));
+        CU(cudaMemsetAsync(c->d_g2code, 0xff, sizeof(int) * nrow, c->stream));
+        for (int k = 0; k < RIS_NCLASS; ++k) {
+            const RisClassPack& pk = c->cls[k];
+            if (pk.npairs == 0) continue;
+            const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+            ris_k_g2_fill<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, BM, d_tbase, d_fill, c->d_g2rows, c->d_g2code);
         }
-        c->ntiles = (int)tiles.size();
+        ris_k_g2_tiles<<<(nao + 127) / 128, 128, 0, c->stream>>>(nao, BM, d_tbase, c->d_g2tiles);
+        CU(cudaGetLastError());
         {   // row-block bands for the fitting step's sparse transform (ris_fit_K)
             c->rb_jlo.resize(c->nblk); c->rb_kw.resize(c->nblk); c->rb_off.resize(c->nblk);
             long long off2 = 0;
             for (int I = 0; I < c->nblk; ++I) {
-                if (jhi[I] < 0) jlo[I] = jhi[I] = I;
+                if (jhi[I] < 0 || jlo[I] > jhi[I]) jlo[I] = jhi[I] = I;
                 c->rb_jlo[I] = jlo[I]; c->rb_kw[I] = (jhi[I] - jlo[I] + 1) * RIS_GTILE2; c->rb_off[I] = off2;
                 off2 += (long long)RIS_GTILE2 * c->rb_kw[I];
             }
@@ -492,33 +508,6 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
             if ((rc = dev_upload(c, &c->d_rb_kw, c->rb_kw.data(), c->rb_kw.size()))) return rc;
             if ((rc = dev_upload(c, &c->d_rb_off, c->rb_off.data(), c->rb_off.size()))) return rc;
         }
-        if (gcols.empty()) gcols.push_back(-1);
-        int *d_colidx, *d_ptile0;
-        if ((rc = dev_upload(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
-        if ((rc = dev_upload(c, &c->d_gcols, gcols.data(), gcols.size()))) return rc;
-        if ((rc = dev_upload(c, &d_colidx, cmark.data(), cmark.size()))) return rc;
-        if ((rc = dev_upload(c, &d_ptile0, ptile0.data(), ptile0.size()))) return rc;
-        // inverse element map + active-row list of the block buffer (for the P-minor transpose of the K tiles)
-        int *d_rowflag, *d_novf;
-        if ((rc = dev_alloc(c, &c->d_ovf, (size_t)2 * std::max<long long>(c->nelem_real, 1), false))) return rc;
-        if ((rc = dev_alloc(c, &d_novf, 1, true))) return rc;
-        if ((rc = dev_alloc(c, &c->d_smap, (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS * RIS_GTILE2, false))) return rc;
-        if ((rc = dev_alloc(c, &d_rowflag, (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS, true))) return rc;
-        CU(cudaMemsetAsync(c->d_smap, 0xff, sizeof(int) * (size_t)std::max(c->ntiles, 1) * RIS_GPANEL_ROWS * RIS_GTILE2, c->stream));
-        for (int k = 0; k < RIS_NCLASS; ++k) {
-            const RisClassPack& pk = c->cls[k];
-            if (pk.npairs == 0) continue;
-            const long long nelc = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
-            ris_k_build_smap<<<(unsigned)((nelc + 255) / 256), 256, 0, c->stream>>>(pk, c->d_ao_pos, d_colidx, d_ptile0, nao, c->d_smap, d_rowflag, c->d_ovf, d_novf);
-        }
-        CU(cudaGetLastError());
-        std::vector<int> rowflag((size_t)c->ntiles * RIS_GPANEL_ROWS), srows;
-        CU(cudaMemcpyAsync(rowflag.data(), d_rowflag, rowflag.size() * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaMemcpyAsync(&c->novf, d_novf, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CU(cudaStreamSynchronize(c->stream));
-        for (size_t i = 0; i < rowflag.size(); ++i) if (rowflag[i]) srows.push_back((int)i);
-        c->nsrows = (int)srows.size();
-        if ((rc = dev_upload(c, &c->d_srows, srows.data(), srows.size()))) return rc;
         CU(cudaStreamSynchronize(c->stream));      // host vectors go out of scope
     }
     CU(cudaStreamSynchronize(c->stream));
@@ -606,8 +595,7 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
     CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
     // Small molecules: no class has enough warp tasks to fill the GPU with its one resident wave, so the class kernels
     // run side by side on their own streams (fork from / join into the context's stream); large ones run back to back.
-    int nsm = 0;
-    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
+    const int nsm = c->nsm;
     long long most = 0;
     int nclass = 0;
     for (int k = 0; k < RIS_NCLASS; ++k)
@@ -630,7 +618,7 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         if (side) CU(cudaStreamWaitEvent(st, c->fork_ev, 0));
         RisGradParams p{};
         p.task_ctr = ctr + (size_t)2 * k * ny;
-        p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
+        p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
         p.tile = tile; p.sstride = sstride; p.estride = estride; p.lstride = lstride; p.cscale = cscale; p.nb = nb;
         p.p0 = p0; p.p1 = p1;
         p.grad = grad; p.det = det; p.det_flag = det ? (int*)c->ws[WS_DET] : nullptr;
@@ -638,7 +626,7 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         {
             ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
                          8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS, st, false);
-            ris_grad_launchers[k](p, st);
+            CU(ris_grad_launchers[k](p, st));
         }
         if (side) {
             CU(cudaEventRecord(c->join_ev[k], st));
@@ -649,11 +637,19 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
     return RIS_OK;
 }
 
-// states per class-kernel launch: as even as possible, at most RIS_NB_MAX
-static int next_nb(int remaining)
+// states per class-kernel launch: as even as possible, at most `cap` (<= RIS_NB_MAX)
+static int next_nb(int remaining, int cap)
 {
-    const int launches = (remaining + RIS_NB_MAX - 1) / RIS_NB_MAX;
+    const int launches = (remaining + cap - 1) / cap;
     return (remaining + launches - 1) / launches;
+}
+// the cap: every class present must fit its block into shared memory (long contractions: kmax up to 576 records per task)
+static int nb_cap(const ris_ctx* c, bool ktype)
+{
+    int cap = RIS_NB_MAX;
+    for (int k = 0; k < RIS_NCLASS; ++k)
+        if (c->cls[k].npairs > 0) cap = std::min(cap, ris_grad_nb_cap(c->cls[k].la, c->cls[k].lb, c->cls[k].kmax, ktype));
+    return cap;
 }
 
 // --------------------------------------------------------------------------------------- deterministic reduction
@@ -700,8 +696,10 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
     const long long nao2 = (long long)c->nao * c->nao;
     unsigned long long* det;
     { int rc = det_begin(c, nbatch, &det); if (rc) return rc; }
+    const int cap = nb_cap(c, false);
+    if (cap < 1) return RIS_ENOMEM;
     for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
-        nb = next_nb(nbatch - s0);
+        nb = next_nb(nbatch - s0, cap);
         double* tile;
         int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile);
         if (rc) return rc;
@@ -834,7 +832,7 @@ extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out,
     CU(cudaMemsetAsync(v, 0, sizeof(double) * (size_t)nbatch * naux, c->stream));
     const int ny = (naux + 31) / 32;
     for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
-        nb = next_nb(nbatch - s0);
+        nb = next_nb(nbatch - s0, RIS_NB_MAX);
         double* tile;
         if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile))) return rc;
         if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
@@ -847,13 +845,13 @@ extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out,
             if (pk.npairs == 0) continue;
             RisGradParams p{};
             p.task_ctr = ctr + (size_t)2 * k * ny;
-            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
+            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
             p.tile = tile; p.sstride = c->nelem_real; p.estride = 1; p.lstride = 0; p.nb = nb;
             p.p0 = 0; p.p1 = naux; p.grad = v + (size_t)s0 * naux;
             const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
             ProfScope ps(c, kIntNames[k], (double)naux * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb] + 2.0 * nel * pk.npairs * nb),
                          8.0 * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-            ris_int_launchers[k](p, c->stream);
+            CU(ris_int_launchers[k](p, c->stream));
         }
         CU(cudaGetLastError());
     }
@@ -992,12 +990,12 @@ extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, co
             if (pk.npairs == 0) continue;
             RisGradParams p{};
             p.task_ctr = ctr + (size_t)2 * k * ny;
-            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
+            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
             p.estride = pbp; p.nb = 0; p.p0 = 0; p.p1 = naux; p.grad = I;
             const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
             ProfScope ps(c, kIntNames[k], (double)naux * (double)pk.nprim * kModelFlopsByE[pk.la + pk.lb],
                          8.0 * nel * pk.npairs * naux + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-            ris_ints_launchers[k](p, c->stream);
+            CU(ris_ints_launchers[k](p, c->stream));
         }
         CU(cudaGetLastError());
     }
@@ -1098,28 +1096,6 @@ extern "C" int ris_grad_PQ_full(ris_ctx* c, int nbatch, const double* G, double*
 }
 
 // --------------------------------------------------------------------------------------- K
-// K tiles, P-minor: out[el * pbp + P] = symf * S^P[position of el], a transpose through shared memory: one block takes
-// one row (64 doubles) of one S block for 32 aux functions -- 32 coalesced 512-byte reads -- and writes, for every
-// surviving element of the row, its 32 consecutive P values (256 bytes).
-__global__ void __launch_bounds__(256) ris_k_pack_sym(int np, int pbp, const double* __restrict__ S, long long sstrideP,
-                                                      const int* __restrict__ srows, const int* __restrict__ smap,
-                                                      double* __restrict__ out)
-{
-    constexpr int T = RIS_GTILE2;
-    __shared__ double sm[32][T + 1];
-    const int row = srows[blockIdx.x], P0 = blockIdx.y * 32;
-    const int tx = threadIdx.x & (T - 1), ty = threadIdx.x / T;              // 64 x 4
-    const double* src = S + (size_t)row * T + tx;
-    for (int pl = ty; pl < 32; pl += 4) sm[pl][tx] = (P0 + pl < np) ? src[(size_t)(P0 + pl) * sstrideP] : 0.0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (P0 + lane >= np) return;
-    for (int q = w; q < T; q += 8) {
-        const int m = smap[(size_t)row * T + q];
-        if (m >= 0) out[(size_t)(m >> 1) * pbp + P0 + lane] = ((m & 1) ? 0.5 : 1.0) * sm[lane][q];
-    }
-}
-
 // out[pos][0..ld) = in[order[pos]][0..cols) zero padded: C_occ in spatial row order with an even leading dimension
 __global__ void ris_k_pad_rows(int rows, int cols, int ld, const int* __restrict__ order, const double* __restrict__ in,
                                double* __restrict__ out)
@@ -1142,16 +1118,17 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     if (c->nelem_real == 0) return RIS_OK;                // every shell pair screened out: the gradient is exactly zero
     const int nao = c->nao, naux = c->naux;
-    const int nbmax = next_nb(nbatch);
+    const int cap = nb_cap(c, true);
+    if (cap < 1) return RIS_ENOMEM;
+    const int nbmax = next_nb(nbatch, cap);
     const int noccp = (nocc + 1) & ~1;                    // even: 16-byte aligned sub-blocks of HT
-    const long long blk = (long long)RIS_GPANEL_ROWS * RIS_GTILE2;
-    // per aux function: HT [nao][noccp], S blocks [ntiles][64*64], packed tiles [nb][elements]
+    // per aux function: HT [nao][noccp], packed tiles [nb][elements]
     int pb = c->opt.p_batch;
     if (pb <= 0) {
         size_t fr = 0, tot = 0;
         CU(cudaMemGetInfo(&fr, &tot));
-        fr += c->ws_bytes[WS_TILE] + c->ws_bytes[WS_H] + c->ws_bytes[WS_G];
-        const double per = 8.0 * ((double)noccp * nao + (double)c->ntiles * blk + (double)nbmax * c->nelem_real);
+        fr += c->ws_bytes[WS_TILE] + c->ws_bytes[WS_H];
+        const double per = 8.0 * ((double)noccp * nao + (double)nbmax * c->nelem_real);
         const double budget = std::min(0.5 * (double)fr, 24.0e9);
         pb = (int)std::max(1.0, std::min((double)naux, budget / per));
         if (pb < naux && pb > 32) pb &= ~31;              // whole chunks of 32 aux lanes
@@ -1159,13 +1136,12 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     pb = std::min(pb, naux);
     c->last_pbatch = pb;
     const int pbp = (pb + 3) & ~3;                        // P-minor tile rows start on 32-byte sectors
-    double *tile, *HT, *S, *Cop;
+    double *tile, *HT, *Cop;
     int rc;
     unsigned long long* det;
     if ((rc = det_begin(c, nbatch, &det))) return rc;
     if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nbmax * pbp * c->nelem_real, (void**)&tile))) return rc;
     if ((rc = ws_get(c, WS_H, sizeof(double) * (size_t)nao * pb * noccp, (void**)&HT))) return rc;
-    if ((rc = ws_get(c, WS_G, sizeof(double) * (size_t)pb * c->ntiles * blk, (void**)&S))) return rc;
     if ((rc = ws_get(c, WS_COCC, sizeof(double) * (size_t)nao * noccp, (void**)&Cop))) return rc;
     {
         ProfScope ps(c, "ris_k_pad_rows", 0.0, 16.0 * nao * (double)noccp);
@@ -1173,10 +1149,14 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
         ris_k_pad_rows<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(nao, nocc, noccp, c->d_ao_order, C_occ, Cop);
     }
     for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
-        nb = next_nb(nbatch - s0);
+        nb = next_nb(nbatch - s0, cap);
         for (int p0 = 0; p0 < naux; p0 += pb) {
             const int np = std::min(pb, naux - p0);
             const long long ldh = (long long)pb * noccp;
+            {   // the GEMM-2 epilogue ADDS the two halves of every element
+                ProfScope ps(c, "memset(K tiles)", 0.0, 8.0 * nb * (double)pbp * c->nelem_real);
+                CU(cudaMemsetAsync(tile, 0, sizeof(double) * (size_t)nb * pbp * c->nelem_real, c->stream));
+            }
             for (int s = 0; s < nb; ++s) {
                 const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
                 // GEMM-1: HT[nu][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]; with b_ready, in RIS_COPY_CHUNKS column chunks
@@ -1198,27 +1178,17 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
                                  8.0 * ((double)(q1 - q0) * nocc * nvir + (double)nao * nvir + (double)(q1 - q0) * nocc * nao));
                     CU(ris_gemm_dense(c->stream, g, 1));
                 }
-                {   // GEMM-2: S^P = C_occ HT_P^T + HT_P C_occ^T on the surviving 64x64 blocks
+                {   // GEMM-2: tile[e][P] += f Gamma^P_{mu nu}, one column problem per AO, P as the N dimension (scatter mode)
+                    double* out = tile + (size_t)s * pbp * c->nelem_real;
                     RisGemmParams g{};
-                    g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, ldh, noccp, nocc};
-                    g.seg[1] = RisGemmSeg{HT, ldh, noccp, Cop, noccp, 0, nocc};
-                    g.nseg = 2; g.M = nao; g.N = nao; g.C = S; g.ldc = RIS_GTILE2; g.bsC = (long long)c->ntiles * blk;
-                    g.tiles = c->d_tiles; g.tile_stride = blk; g.gcols = c->d_gcols;
+                    g.seg[0] = RisGemmSeg{Cop, noccp, 0, HT, noccp, ldh, nocc};
+                    g.nseg = 1; g.M = nao; g.N = np; g.C = out; g.ldc = pbp; g.bsC = 0;
+                    g.tiles = c->d_g2tiles; g.srows = c->d_g2rows; g.scode = c->d_g2code;
                     // algorithmic flops: two length-nocc dot products per unique surviving pair element
-                    ProfScope ps(c, "ris_gemm_dmma(S=Cocc*HT^T+HT*Cocc^T,blocks)", 4.0 * np * nocc * (double)c->nelem_real,
-                                 8.0 * np * ((double)noccp * nao + (double)c->ntiles * blk) + 8.0 * nao * noccp);
-                    CU(ris_gemm_blocks(c->stream, g, np, c->ntiles));
+                    ProfScope ps(c, "ris_gemm_dmma(tile+=Cocc*HT^T,scatter)", 4.0 * np * nocc * (double)c->nelem_real,
+                                 8.0 * np * ((double)noccp * nao + 3.0 * (double)c->nelem_real) + 8.0 * nao * noccp);
+                    CU(ris_gemm_scatter(c->stream, g, c->ntiles));
                 }
-                double* out = tile + (size_t)s * pbp * c->nelem_real;
-                {
-                    ProfScope ps(c, "ris_k_pack_sym", (double)c->nelem_real * np, 8.0 * np * ((double)c->nsrows * RIS_GTILE2 + (double)c->nelem_real));
-                    if (c->nsrows > 0)
-                        ris_k_pack_sym<<<dim3(c->nsrows, (np + 31) / 32), 256, 0, c->stream>>>(np, pbp, S, (long long)c->ntiles * blk,
-                                                                                            c->d_srows, c->d_smap, out);
-                    if (c->novf > 0)
-                        ris_k_pack_sym_ovf<<<c->novf, 64, 0, c->stream>>>(c->novf, c->d_ovf, np, pbp, S, (long long)c->ntiles * blk, out);
-                }
-                CU(cudaGetLastError());
             }
             if ((rc = launch_classes(c, tile, (long long)pbp * c->nelem_real, pbp, 1, nullptr, nb, p0, p0 + np,
                                      grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
@@ -1488,10 +1458,10 @@ extern "C" int ris_diag_gemm2_layout(ris_ctx* c, int32_t* ao_pos_host, int* pane
         CU(cudaMemcpyAsync(ao_pos_host, c->d_ao_pos, sizeof(int) * (size_t)c->nao, cudaMemcpyDeviceToHost, c->stream));
         CU(cudaStreamSynchronize(c->stream));
     }
-    if (panel_rows) *panel_rows = RIS_GPANEL_ROWS;
-    if (tile_cols) *tile_cols = RIS_GTILE2;
+    if (panel_rows) *panel_rows = RIS_G2_BM;
+    if (tile_cols) *tile_cols = RIS_G2_BN;
     if (ntiles) *ntiles = c->ntiles;
-    if (novf) *novf = c->novf;
+    if (novf) *novf = (int)std::min<long long>(c->g2_entries, 2147483647LL);
     return RIS_OK;
 }
 

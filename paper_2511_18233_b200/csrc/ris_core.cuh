@@ -31,17 +31,37 @@ constexpr int RIS_BOYS_PER_UNIT = 32;
 constexpr int RIS_BOYS_NGRID = 40 * 32 + 1;
 constexpr int RIS_BOYS_ROW = 8;
 
+// 1/sqrt(x) for positive, normal x (p + alpha, T >= 40), branch-free: the hardware seed (MUFU.RSQ64H, relative error
+// < 2^-22) and ONE third-order step  y (1 + e/2 + 3 e^2/8),  e = 1 - x y^2  (error ~ e^3 = 2^-66; the result is within an
+// ulp or two of the correctly rounded value).  CUDA's rsqrt() adds special-case branches this path never needs.
 RIS_DEV double ris_rsqrt(double x)
 {
 #ifdef __CUDA_ARCH__
-    return rsqrt(x);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
 #else
     return 1.0 / sqrt(x);
 #endif
 }
 
+// e^{-T} for T >= 40, single precision (see the error budget above): one FMUL + MUFU.EX2
+RIS_DEV double ris_exp_neg_f32(double T)
+{
+#ifdef __CUDA_ARCH__
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-1.44269504088896340736f * (float)T));
+    return (double)r;
+#else
+    return (double)expf(-(float)T);
+#endif
+}
+
+// F[m] = scale * F_m(T), m = 0..M.  The scale (kappa of the primitive triplet) rides along: the recursions are linear
+// in (F, e^{-T}), so two multiplications replace M + 1.
 template <int M>
-RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 1])
+RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 1], double scale = 1.0)
 {
     if (T < RIS_BOYS_TMAX) {
         const int i = (int)(T * RIS_BOYS_PER_UNIT + 0.5);
@@ -68,7 +88,8 @@ RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 
         ex = fma(ex, x, 0.5);
         ex = fma(ex, x, -1.0);
         ex = fma(ex, x, 1.0);
-        ex *= e0;
+        ex *= e0 * scale;
+        f *= scale;
         F[M] = f;
         const double t2 = T + T;
 #pragma unroll
@@ -79,8 +100,8 @@ RIS_DEV void ris_boys(double T, const double* __restrict__ tab, double (&F)[M + 
     } else {
         const double rt = ris_rsqrt(T);
         const double i2t = 0.5 * rt * rt;
-        const double ex = (double)expf(-(float)T);
-        double f = 0.88622692545275801365 * rt;     // sqrt(pi)/2 / sqrt(T)
+        const double ex = ris_exp_neg_f32(T) * scale;
+        double f = (0.88622692545275801365 * scale) * rt;     // sqrt(pi)/2 / sqrt(T)
         F[0] = f;
 #pragma unroll
         for (int m = 0; m < M; ++m) {
@@ -118,13 +139,33 @@ RIS_DEV void ris_prim_head(double p, double PZx, double PZy, double PZz, double 
     const double q = alpha * s * s;          // rho/p
     const double X0 = ZCx + PZx, X1 = ZCy + PZy, X2 = ZCz + PZz;
     const double T = (p * q) * fma(X0, X0, fma(X1, X1, X2 * X2));
-    ris_boys<E>(T, boys_tab, h.F);
-    const double kappa = coef * auxfac * s;
-#pragma unroll
-    for (int m = 0; m <= E; ++m) h.F[m] *= kappa;
+    ris_boys<E>(T, boys_tab, h.F, (coef * auxfac) * s);
     h.W0 = -q * X0; h.W1 = -q * X1; h.W2 = -q * X2;
     h.q = q;
 }
+
+// The branch-free front of the head (everything before the Boys function), used by the software-pipelined primitive
+// loop of the class kernel: it is issued for primitive k+1 next to the recurrence of primitive k.
+struct RisPrimFront {
+    double T, kappa, q, X0, X1, X2;       // rho |P-C|^2, coef auxfac / sqrt(p+alpha), rho/p, P - C
+};
+
+RIS_DEV void ris_prim_front(double p, double PZx, double PZy, double PZz, double coef, double ZCx, double ZCy, double ZCz,
+                            double alpha, double auxfac, RisPrimFront& f)
+{
+    const double s = ris_rsqrt(p + alpha);
+    f.q = alpha * s * s;
+    f.X0 = ZCx + PZx; f.X1 = ZCy + PZy; f.X2 = ZCz + PZz;
+    f.T = (p * f.q) * fma(f.X0, f.X0, fma(f.X1, f.X1, f.X2 * f.X2));
+    f.kappa = (coef * auxfac) * s;
+}
+
+// plain-memory tile provider of the generated contraction code (the class kernel passes its shared-memory ring instead)
+struct RisTilePlain {
+    const double* tile; size_t estride, sstride;
+    RIS_DEV size_t es() const { return estride; }
+    RIS_DEV const double* get(int s) const { return tile + (size_t)s * sstride; }
+};
 
 template <int LH, int LO>
 RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, double oo2p, double h2, double o2,

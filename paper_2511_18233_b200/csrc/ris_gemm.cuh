@@ -2,14 +2,19 @@
 //   Gamma^P = C_occ B^P C_vir^T                     (AO back-transform, Eqs. 32-34, 39)
 // evaluated as two "NT" contractions with K-contiguous operands:
 //   GEMM-1   HT[nu'][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]          nu' = spatial (Morton) position of AO nu
-//   GEMM-2   S^P[mu'][nu']  = Gamma^P_{mu nu} + Gamma^P_{nu mu}
-//                           = sum_i C_occ[mu][i] HT[nu'][(P,i)] + sum_i HT[mu'][(P,i)] C_occ[nu][i]
-//            only on tiles of 32 rows x 64 GATHERED columns of the spatially ordered AO index: per 32-row panel the
-//            columns that hold a surviving pair element (tile list + gathered-column list), written as dense
-//            tiles that ris_k_pack_sym gathers into the packed pair order.
+//   GEMM-2   X^P[mu'][nu']  = Gamma^P_{mu nu} = sum_i C_occ[mu][i] HT[nu'][(P,i)]   for the SURVIVING (mu, nu) only,
+//            one problem per AO column nu' with P as the dense N dimension:
+//                X_nu'[m][P] = sum_i C_occ[partner_m(nu')][i] HT[nu'][(P,i)],
+//            m over the GATHERED list of nu's surviving partners (no tile cover of a sparse matrix: the only padding
+//            is the tail of a partner list and of the P range), and the result is ADDED (red.global.add.f64), times
+//            the pair's symmetry factor, straight into the P-minor packed K tile of the class kernels:
+//                tile[element(mu,nu)][P] += f X^P[mu'][nu'];   every element receives exactly its two halves
+//            Gamma^P_{mu nu} and Gamma^P_{nu mu} (one for a diagonal element), so the sum is order-independent.
+//            (Round 1 computed S^P = Gamma^P + Gamma^P^T on 32 x 64 tiles covering the sparse pair matrix -- 1.7x the
+//            algorithmic flops -- into a block buffer that a second kernel transposed into the tiles.)
 //
 // One kernel serves both:  C[m][n] = sum_seg sum_k A_seg[row(m)][k] B_seg[n][k]  (up to two K segments; row(m)
-// optionally through an index list, which is how GEMM-1 emits HT in spatial order).
+// optionally through an index list, which is how GEMM-1 emits HT in spatial order and GEMM-2 gathers its partners).
 // tcgen05.mma has no FP64 kind, so the tensor path for FP64 on sm_100a is the warp-level mma.sync f64 (DMMA;
 // SASS DMMA.8x8x4, 16 cycles of the pipe per SM sub-partition each).  Operands are staged global -> shared with
 // cp.async (LDGSTS) through a multi-stage pipeline that is synchronised by mbarriers only (full[s]: the stage's
@@ -17,17 +22,13 @@
 // DMMA pipe (profiles/r01_v3_ncu.md -> r01_v4_gemm.md).  Fragments are read with 128-bit shared loads from a
 // 16-double row whose halves are swapped on odd rows (bank-conflict free, no padding).
 //   GEMM-1: CTA tile 64x128, K step 16, 8 warps as 2 x 4, warp tile 32x32, 3 stages, 2 CTAs/SM
-//   GEMM-2: CTA tile 32x64,  K step 16, 2 warps as 1 x 2, warp tile 32x32, 3 stages, 5 CTAs/SM
+//   GEMM-2: CTA tile 64x64 (partners x aux),  K step 16, 4 warps as 2 x 2, warp tile 32x32, 3 stages, 3 CTAs/SM
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 constexpr int RIS_GBK = 16, RIS_GLD = 16;   // K step; shared row stride in doubles (swizzled, see the kernel)
-constexpr int RIS_GTILE2 = 64;           // GEMM-2 tile width (gathered columns); also the AO block edge of the fit_K bands
-#ifndef RIS_GPANEL
-#define RIS_GPANEL 32
-#endif
-constexpr int RIS_GPANEL_ROWS = RIS_GPANEL;   // GEMM-2 row-panel height (rows of the spatial AO order per tile)
+constexpr int RIS_GTILE2 = 64;           // AO block edge of the fit_K bands (spatial AO order)
 
 struct RisGemmSeg {
     const double* A; long long lda, bsA;   // A operand rows m, K contiguous; bsA = batch (blockIdx.z) stride in doubles
@@ -48,6 +49,12 @@ struct RisGemmParams {
     const int* gcols;                      // nullable, with tiles: GATHERED columns -- column n of tile t is the B row
                                            // gcols[tiles[t].y + n] (< 0: padding, zero column); tiles[t].y is then an
                                            // offset into gcols, not a block index
+    // SCATTER mode (template SCAT; GEMM-2): tile t = blockIdx.x is (column problem nu = tiles[t].x, first entry m0 =
+    // tiles[t].y of its partner list); row m of the tile is A row srows[m0 + m] (< 0: padding); B of problem nu starts
+    // at seg[0].B + nu * seg[0].bsB; blockIdx.y = n-tile; the result row m is ADDED to
+    // C[(scode[m0 + m] >> 1) * ldc + n] times (scode & 1 ? 0.5 : 1).
+    const int* srows;
+    const int* scode;
 };
 
 template <bool VEC16>
@@ -74,7 +81,7 @@ struct RisGemmCfg {
 // VEC16: all operand rows are 16-byte aligned (even leading dimensions, aligned bases) -> 16-byte cp.async
 // GATH: gathered-column tiles (p.gcols); a warp whose WN-column strip is all padding issues no MMAs (skipping single
 // 8-column sub-tiles was measured slower: the predicates break the MMA schedule, 48.2 -> 49.8 ms on config 4).
-template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool VEC16, bool GATH = false>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool VEC16, bool GATH = false, bool SCAT = false>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_dmma(const RisGemmParams p)
 {
     using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
@@ -88,7 +95,12 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
     int m0, n0;
     double* Cout;
     long long ldc;
-    if (p.tiles) {
+    int snu = 0;                                       // SCAT: the column problem of this tile
+    if (SCAT) {
+        const int2 tl = p.tiles[blockIdx.x];
+        snu = tl.x; m0 = tl.y; n0 = blockIdx.y * BN;
+        Cout = p.C; ldc = p.ldc;
+    } else if (p.tiles) {
         const int2 tl = p.tiles[blockIdx.x];
         m0 = tl.x * BM; n0 = p.gcols ? tl.y : tl.y * BN;
         Cout = p.C + (long long)blockIdx.z * p.bsC + (long long)blockIdx.x * p.tile_stride;
@@ -123,10 +135,15 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
         const RisGemmSeg& sg = p.seg[sidx];
         segK = sg.K;
         const double* Ag = sg.A + (long long)blockIdx.z * sg.bsA;
-        const double* Bg = sg.B + (long long)blockIdx.z * sg.bsB;
+        const double* Bg = sg.B + (long long)(SCAT ? snu : blockIdx.z) * sg.bsB;
 #pragma unroll
         for (int j = 0; j < NA; ++j) {
             const int r = m0 + (tid / CH) + j * (THREADS / CH);
+            if (SCAT) {
+                const int row = p.srows[r];            // the partner lists are padded to whole tiles
+                pa[j] = row >= 0 ? Ag + (long long)row * sg.lda + kc : nullptr;
+                continue;
+            }
             long long row = r;
             if (sidx == 0 && p.rowsA != nullptr && r < p.M) row = p.rowsA[r];
             pa[j] = r < p.M ? Ag + row * sg.lda + kc : nullptr;
@@ -239,6 +256,26 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, MINB) ris_k_gemm_d
     }
 
     // ---- epilogue: c0,c1 -> (row g, cols 2t, 2t+1); c2,c3 -> row g + 8
+    if (SCAT) {
+        const int Nr = p.N - n0;
+#pragma unroll
+        for (int i = 0; i < MT; ++i)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int code = p.scode[m0 + wm0 + 16 * i + g + 8 * h];
+                if (code < 0) continue;
+                const double f = (code & 1) ? 0.5 : 1.0;
+                double* dst = Cout + (long long)(code >> 1) * ldc + n0;
+#pragma unroll
+                for (int j = 0; j < NT; ++j) {
+                    const int c = wn0 + 8 * j + 2 * t;
+                    // (PTX has no vector form of red.add.f64: two 8-byte reductions into one 16-byte piece of the row)
+                    if (c < Nr) atomicAdd(dst + c, f * acc[i][j][2 * h]);
+                    if (c + 1 < Nr) atomicAdd(dst + c + 1, f * acc[i][j][2 * h + 1]);
+                }
+            }
+        return;
+    }
     const int Mrem = p.M - m0, Nrem = p.N - n0;
     const bool full = p.tiles != nullptr;              // block output: always a full BM x BN tile (zero padded)
     const bool vec = ((ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(Cout) & 15) == 0) && p.cdiv <= 0;
@@ -277,26 +314,26 @@ inline bool ris_gemm_aligned16(const RisGemmParams& p)
     return true;
 }
 
-template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool GATH = false>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, bool GATH = false, bool SCAT = false>
 inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
 {
     using Cfg = RisGemmCfg<BM, BN, WM, WN, STAGES>;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    const bool vec16 = ris_gemm_aligned16(p);
+    if (Cfg::SMEM + 1024 > 48 * 1024) {     // (+ the static barriers) per device and context: set at every launch that needs
+                                            // it, no process-wide cache
+        const cudaError_t e = vec16 ? cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH, SCAT>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM)
+                                    : cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH, SCAT>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-        if (e != cudaSuccess) return e;
-        configured = true;
     }
     dim3 grid;
-    if (p.tiles) grid = dim3(ntiles, 1, batch);
+    if (SCAT) grid = dim3(ntiles, (p.N + BN - 1) / BN, 1);
+    else if (p.tiles) grid = dim3(ntiles, 1, batch);
     else grid = dim3((p.M + BM - 1) / BM, (p.N + BN - 1) / BN, batch);
     if (grid.x == 0 || grid.y == 0 || grid.z == 0) return cudaSuccess;
-    if (ris_gemm_aligned16(p)) ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
-    else ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    if (vec16) ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, true, GATH, SCAT><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
+    else ris_k_gemm_dmma<BM, BN, WM, WN, STAGES, MINB, false, GATH, SCAT><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -310,13 +347,14 @@ inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int b
 #endif
     return ris_gemm_launch_cfg<64, 128, 32, 32, RIS_G1_STAGES, 2>(st, p, batch, 0);
 }
-// GEMM-2: tile list of RIS_GTILE2 rows x RIS_GTILE2 gathered columns (p.gcols required)
-inline cudaError_t ris_gemm_blocks(cudaStream_t st, const RisGemmParams& p, int batch, int ntiles)
-{
-    // GATH = false: skipping the MMAs of all-padding strips measured slower than issuing them (48.2 vs 49.0 ms, config 4)
-#ifndef RIS_G2_STAGES
+// GEMM-2 (scatter mode): tiles of RIS_G2_BM gathered partner rows x RIS_G2_BN aux functions, K = nocc
+#ifndef RIS_G2_BM
+#define RIS_G2_BM 64            // measured on config 4 (r02): 64x64 / 3 CTAs 29.8 ms per step, 32x64 / 5 CTAs 30.2, / 6 CTAs
+#define RIS_G2_BN 64            // 30.3, 32x64 with 4 stages 32.5
 #define RIS_G2_STAGES 3
-#define RIS_G2_MINB (RIS_GPANEL_ROWS == 32 ? 5 : 3)   // measured on config 4: 5 -> 44.3 ms, 6 -> 45.4, 3 or 4 -> 47.1
+#define RIS_G2_MINB 3
 #endif
-    return ris_gemm_launch_cfg<RIS_GPANEL_ROWS, RIS_GTILE2, 32, 32, RIS_G2_STAGES, RIS_G2_MINB, false>(st, p, batch, ntiles);
+inline cudaError_t ris_gemm_scatter(cudaStream_t st, const RisGemmParams& p, int ntiles)
+{
+    return ris_gemm_launch_cfg<RIS_G2_BM, RIS_G2_BN, 32, 32, RIS_G2_STAGES, RIS_G2_MINB, false, true>(st, p, 1, ntiles);
 }

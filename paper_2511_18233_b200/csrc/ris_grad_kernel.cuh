@@ -1,19 +1,29 @@
 // ris_grad_kernel.cuh -- the fused class kernel: S1 Boys + S2 derivative-integral recurrence +
 // S3 contraction with the D / Gamma^P tile + S4 reduction, one instantiation per
-// (l_mu,l_nu) class.  Eq. 27 terms 1-2 for the integrals of Eq. 21
+// (l_mu,l_nu) class and contraction type.  Eq. 27 terms 1-2 for the integrals of Eq. 21
 // (PAPER.md:119).
 //
 // Mapping ("aux lanes"): the 32 lanes of a warp hold 32 different auxiliary functions P (blockIdx.y selects the
-// chunk of 32) and walk TOGETHER through the shell pairs of a warp task (a window of ~64 packed primitive pairs,
+// chunk of 32) and walk TOGETHER through the shell pairs of a warp task (a window of packed primitive pairs,
 // ris_internal.h).  Everything that belongs to the shell pair -- pair record, primitive-pair records, loop trip counts,
 // the host-centre phases, the D tile of the J term -- is therefore warp-uniform: it is staged once per task into the
 // warp's shared memory with coalesced 16-byte copies and read back as broadcasts, there is no divergence except the
 // Boys-function branch, and what varies per lane (aux centre / exponent, W - P, Boys values, the Gamma^P tile of the
-// K term, stored P-minor so a warp reads 256 contiguous bytes) is exactly the per-lane arithmetic.
+// K term, stored P-minor so a warp reads 256 contiguous bytes per element) is exactly the per-lane arithmetic.
+//
+// Tile staging (north_star: "shared-memory staging of D/Gamma tiles"): the pair's tile -- K: NEL rows of 32 aux values per
+// state, J: NEL values per state -- is copied global -> shared with cp.async (LDGSTS) at the START of the pair, state by
+// state into a ring of NS slots, and is waited for only when the contraction of that state begins: the DRAM / L2 latency
+// of the Gamma^P read runs under the primitive loop (profiles/r01_v9_ncu.md: the K kernels lost 10-15 % to
+// long_scoreboard stalls on these loads, (2,2) 78 %).
+//
+// Primitive loop: software-pipelined by hand -- the record load and the branch-free front of the prefactor chain
+// (rsqrt(p + alpha), T) of primitive k+1 are issued next to the wide recurrence of primitive k.
+//
 // The per-state gradient accumulators are per-lane shared-memory slots (conflict-free: lane-contiguous), which keeps the
-// register file for the recurrence and lets the light classes run 16 warps per SM:
+// register file for the recurrence:
 //   aux side   g[A_P] = -(dA + dB) summed over the pairs (translational invariance): the lane owns P, so this is one
-//              slot per (state, x) over ALL tasks of the warp; the four warps of a block (same P chunk) are summed
+//              slot per (state, x) over ALL tasks of the warp; the warps of a block (same P chunk) are summed
 //              in fixed order at the end, one atomic per (block, P, state, x).
 //   pair side  g[A_mu], g[A_nu]: slots across the consecutive shell pairs of one atom pair (the pairs of a class
 //              are sorted by atom pair), then a fixed-order sum over the lanes and one atomic per (atom pair, state,
@@ -24,38 +34,7 @@
 #include "ris_core.cuh"
 #include "ris_internal.h"
 
-// One host-centre phase of a contracted triplet: the primitive pairs q[0 .. nk) hosted on centre Z (host l = LH,
-// other l = LO), then HRR / derivative / tile contraction into the lane's accumulator slots.
-template <int LH, int LO, bool TR>
-RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
-                       double ZOz, double alpha, double auxfac, const double* __restrict__ boys,
-                       const double* __restrict__ tile, size_t estride, size_t sstride, int nb, const double* __restrict__ sc,
-                       double* __restrict__ slot)
-{
-    using K = RisClass<LH, LO>;
-    double acc[K::NACC];
-#pragma unroll
-    for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
-    for (int k = 0; k < nk; ++k, q += RIS_PRIM_FIELDS) {
-        const double2 r0 = *reinterpret_cast<const double2*>(q);
-        const double2 r1 = *reinterpret_cast<const double2*>(q + 2);
-        const double2 r2 = *reinterpret_cast<const double2*>(q + 4);
-        const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
-        ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
-                                 alpha, auxfac, boys, acc);
-    }
-    ris_hrrc<LH, LO, TR, 33, 32>(acc, ZOx, ZOy, ZOz, tile, estride, sstride, nb, sc, slot);
-}
-
-template <int NEL>
-RIS_DEV void ris_prefetch_tile(const double* t, size_t estride, size_t sstride, int nb, int lstride)
-{
-    const int rows = lstride ? NEL : (NEL + 15) / 16;
-    const size_t step = lstride ? estride : 16;
-    for (int s = 0; s < nb; ++s)
-        for (int e = 0; e < rows; ++e) asm volatile("prefetch.global.L1 [%0];" ::"l"(t + (size_t)s * sstride + (size_t)e * step));
-}
-
+// ------------------------------------------------------------------------------------------------ tuning
 // resident blocks per SM the register allocation aims at (light classes: latency-bound prefactor / Boys chains
 // want warps; heavy classes: the contracted targets want registers)
 #ifndef RIS_MB1
@@ -66,27 +45,173 @@ RIS_DEV void ris_prefetch_tile(const double* t, size_t estride, size_t sstride, 
 #endif
 // SPLIT: the heavy classes (l_mu + l_nu >= 4) run their two host-centre phases as two launches (PH = 1: primitive pairs
 // hosted on A, PH = 2: hosted on B; PH = 0: both in one kernel).  With both phases inlined the (2,2) kernel is 94 KB of
-// SASS and stalls on instruction fetch (profiles/r01_v5_ncu.md: no_instruction 7.1 cycles per issue); one phase is 47 KB.
+// SASS and stalls on instruction fetch; one phase is 47 KB.
 #ifndef RIS_SPLIT_L
 #define RIS_SPLIT_L 4
+#endif
+#ifndef RIS_PIPE_L
+#define RIS_PIPE_L -1           // software-pipelined primitive loop for l_mu + l_nu <= this.  Measured on config 4 (r02):
+#endif                          // slower for every class ((1,0) J 0.78 -> 0.92 ms): the extra live front spills at the
+                                // register caps below and the last front of a phase is wasted -- off
+#ifndef RIS_STAGE_BYTES
+#define RIS_STAGE_BYTES 4608    // shared-memory budget per warp for the K tile ring (at least 2 slots are always taken)
 #endif
 template <int LA, int LB> struct RisGradTune {
     static constexpr int MINB = (LA + LB <= 1) ? RIS_MB1 : (LA + LB == 2 ? RIS_MB2 : (LA + LB == 3 ? RIS_MB3 : RIS_MB4));
     static constexpr bool SPLIT = (LA + LB >= RIS_SPLIT_L);
+    static constexpr bool PIPE = (LA + LB <= RIS_PIPE_L);
+    static constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
+    // slots of the tile ring: K -- as many states as fit the budget, at least 2 (1 for the f classes, whose slot is 15-26 KB
+    // per warp), at most RIS_NB_MAX; J -- all states (a few doubles each)
+    static constexpr int NSK_LO = (NEL * 256 * 2 <= 20480) ? 2 : 1;
+    static constexpr int NSK = (RIS_STAGE_BYTES / (NEL * 256) < NSK_LO) ? NSK_LO
+                             : (RIS_STAGE_BYTES / (NEL * 256) > RIS_NB_MAX ? RIS_NB_MAX : RIS_STAGE_BYTES / (NEL * 256));
+};
+// doubles of a tile ring of ns slots: K -- slots of NEL rows of 32 aux values; J -- slots of NEL values
+template <int LA, int LB, bool KT> __host__ __device__ constexpr int ris_grad_tile_doubles(int ns)
+{
+    return KT ? ns * RisGradTune<LA, LB>::NEL * 32 : ((ns * RisGradTune<LA, LB>::NEL + 1) & ~1);
+}
+
+// ------------------------------------------------------------------------------------------------ tile ring
+__device__ __forceinline__ void ris_cp_async8(double* dst, const double* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void ris_cp_async16(double* dst, const double* src, int src_bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void ris_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void ris_cp_wait(int pending)       // pending = groups that may still be in flight (0..4)
+{
+    switch (pending) {
+    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
+    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
+    }
+}
+
+// The staged tile of ONE shell pair.  State s lives in slot s % NS; get(s) returns the lane's view of it
+// (element el at ptr[el * ES]) after its copy has landed, and refills the slot the previous state left.
+//   K (KT): slot = [NEL][32] doubles, one 256-byte row per element (the 32 aux of this warp's chunk): two rows per
+//           warp-wide 16-byte cp.async; rows of the last chunk are zero-filled beyond p1.
+//   J:      slot = [NEL] doubles (the same for every lane): one 8-byte cp.async per element.
+template <int NEL, int NS, bool KT>
+struct RisTileRing {
+    static constexpr int SLOT = KT ? NEL * 32 : NEL;
+    __device__ __forceinline__ constexpr size_t es() const { return KT ? 32 : 1; }
+    double* buf;               // this warp's ring
+    const double* g;           // K: tile + first element of the pair * estride + chunk offset; J: tile + first element
+    size_t estride, sstride;
+    int nb, ns, lane, nv;      // ns = min(nb, NS) slots in use; nv: valid aux functions of this warp's chunk (K)
+    int issued;                // states whose copy has been issued (and committed) since begin()
+
+    __device__ __forceinline__ int slot_of(int s) const { return s < ns ? s : (s - ns < ns ? s - ns : s % ns); }
+    __device__ __forceinline__ void issue(int s)
+    {
+        double* dst = buf + slot_of(s) * SLOT;
+        const double* src = g + (size_t)s * sstride;
+        if (KT) {
+            const int c2 = (lane & 15) * 2;
+            const int bytes = min(max(nv - c2, 0), 2) * 8;
+#pragma unroll
+            for (int r = 0; r < NEL; r += 2) {
+                const int row = r + (lane >> 4);
+                if ((NEL & 1) == 0 || row < NEL) ris_cp_async16(dst + row * 32 + c2, src + (size_t)row * estride + c2, bytes);
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < NEL; e += 32)
+                if (e + lane < NEL) ris_cp_async8(dst + e + lane, src + e + lane);
+        }
+        ris_cp_commit();
+    }
+    // start of a pair (or of its second host phase when the ring does not hold all states): every lane has finished
+    // reading the previous contents (the caller's __syncwarp)
+    __device__ __forceinline__ void begin()
+    {
+        issued = 0;
+        for (int s = 0; s < ns; ++s) issue(s);
+        issued = ns;
+    }
+    __device__ __forceinline__ const double* get(int s)
+    {
+        if (s > 0 && issued < nb) {      // issued == s - 1 + ns: the slot state s-1 leaves is the next one's, and it is
+            __syncwarp();                // free once every lane is done with state s-1
+            issue(issued);
+            ++issued;
+        }
+        ris_cp_wait(issued - 1 - s);
+        __syncwarp();
+        return buf + slot_of(s) * SLOT + (KT ? lane : 0);
+    }
+    __device__ __forceinline__ bool holds_all() const { return nb <= ns; }
 };
 
-template <int LA, int LB, int PH>
+// ------------------------------------------------------------------------------------------------ one host-centre phase
+// The primitive pairs q[0 .. nk) hosted on centre Z (host l = LH, other l = LO), then HRR / derivative / tile contraction
+// into the lane's accumulator slots.
+template <int LH, int LO, bool TR, bool PIPE, bool KT, class Ring>
+RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
+                       double ZOz, double alpha, double auxfac, const double* __restrict__ boys, Ring& ring, int nb,
+                       const double* __restrict__ sc, double* __restrict__ slot)
+{
+    using K = RisClass<LH, LO>;
+    constexpr int E = K::E;
+    double acc[K::NACC];
+#pragma unroll
+    for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
+    if (PIPE) {
+        // front of primitive k+1 (record load, rsqrt(p + alpha), T: branch-free) next to Boys + recurrence of primitive k
+        double2 r0 = *reinterpret_cast<const double2*>(q), r1 = *reinterpret_cast<const double2*>(q + 2);
+        double2 r2 = *reinterpret_cast<const double2*>(q + 4), r3 = *reinterpret_cast<const double2*>(q + 6);
+        RisPrimFront f;
+        ris_prim_front(r0.x, r0.y, r1.x, r1.y, r3.y, ZCx, ZCy, ZCz, alpha, auxfac, f);
+        for (int k = 0; k < nk; ++k) {
+            const double* __restrict__ qn = q + (size_t)(k + 1 < nk ? k + 1 : k) * RIS_PRIM_FIELDS;
+            const double2 n0 = *reinterpret_cast<const double2*>(qn), n1 = *reinterpret_cast<const double2*>(qn + 2);
+            const double2 n2 = *reinterpret_cast<const double2*>(qn + 4), n3 = *reinterpret_cast<const double2*>(qn + 6);
+            RisPrimFront fn;
+            ris_prim_front(n0.x, n0.y, n1.x, n1.y, n3.y, ZCx, ZCy, ZCz, alpha, auxfac, fn);
+            double F[E + 1];
+            ris_boys<E>(f.T, boys, F, f.kappa);
+            ris_vrr<LH, LO>(F, r0.y, r1.x, r1.y, -f.q * f.X0, -f.q * f.X1, -f.q * f.X2, r2.x, f.q, TR ? r3.x : r2.y,
+                            TR ? r2.y : r3.x, acc);
+            r0 = n0; r1 = n1; r2 = n2; r3 = n3; f = fn;
+        }
+    } else {
+        for (int k = 0; k < nk; ++k, q += RIS_PRIM_FIELDS) {
+            const double2 r0 = *reinterpret_cast<const double2*>(q);
+            const double2 r1 = *reinterpret_cast<const double2*>(q + 2);
+            const double2 r2 = *reinterpret_cast<const double2*>(q + 4);
+            const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
+            ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
+                                     alpha, auxfac, boys, acc);
+        }
+    }
+    ris_hrrc<LH, LO, TR, 33, KT ? 0 : 32>(acc, ZOx, ZOy, ZOz, ring, nb, sc, slot);
+}
+
+// KT: K-type contraction (Gamma^P tile, P-minor, one column per lane); else J-type (D tile shared by all lanes, scaled by
+// c_aux[s][P]).
+template <int LA, int LB, int PH, bool KT>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
 {
-    constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
+    using Tune = RisGradTune<LA, LB>;
+    constexpr int NEL = Tune::NEL;
+    constexpr int NS = KT ? Tune::NSK : RIS_NB_MAX;          // upper bound of the ring; prm.ring_ns slots are in use
     extern __shared__ __align__(16) unsigned char sm_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const RisClassPack& pk = prm.pk;
     const int nb = prm.nb;
-    const size_t wbytes = ris_grad_warp_smem(pk.kmax, nb);
+    const size_t wbytes = ris_grad_warp_smem(pk.task_prims, pk.kmax, nb, ris_grad_tile_doubles<LA, LB, KT>(prm.ring_ns));
     double* s_prim = reinterpret_cast<double*>(sm_raw + (size_t)warp * wbytes);
-    RisPairRec* s_pair = reinterpret_cast<RisPairRec*>(s_prim + (size_t)RIS_PRIM_FIELDS * (RIS_TASK_PRIMS + pk.kmax));
-    double* s_red = reinterpret_cast<double*>(s_pair + RIS_TASK_PRIMS);      // [6 nb][33]  pair side: A x,y,z, B x,y,z per state
+    RisPairRec* s_pair = reinterpret_cast<RisPairRec*>(s_prim + (size_t)RIS_PRIM_FIELDS * (pk.task_prims + pk.kmax));
+    double* s_tile = reinterpret_cast<double*>(s_pair + pk.task_prims);      // tile ring (16-byte aligned)
+    double* s_red = s_tile + ris_grad_tile_doubles<LA, LB, KT>(prm.ring_ns); // [6 nb][33]  pair side: A x,y,z, B x,y,z per state
     double* s_gaux = s_red + 6 * nb * 33;                                    // [3 nb][32]  aux side
     double* s_sc = s_gaux + 3 * nb * 32;                                     // [nb][32]    J: c_aux[s][P]; K: 1
     const size_t gaux_off = (size_t)(reinterpret_cast<unsigned char*>(s_gaux) - (sm_raw + (size_t)warp * wbytes));
@@ -98,11 +223,16 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
     const double* ax = prm.aux + 5 * (size_t)Pe;
     const double Cx = ax[0], Cy = ax[1], Cz = ax[2], alpha = ax[3];
     const double auxfac = live ? ax[4] : 0.0;          // a dead lane computes exact zeros
-    for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale ? prm.cscale[(size_t)s * prm.naux + Pe] : 1.0;
+    if (!KT)
+        for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale[(size_t)s * prm.naux + Pe];
     for (int i = 0; i < 6 * nb; ++i) s_red[i * 33 + lane] = 0.0;
     for (int i = 0; i < 3 * nb; ++i) s_gaux[i * 32 + lane] = 0.0;
-    const double* __restrict__ tile_lane = prm.tile + (size_t)(Pe - prm.p0) * prm.lstride;
-    const size_t estride = (size_t)prm.estride, sstride = (size_t)prm.sstride;
+    RisTileRing<NEL, NS, KT> ring;
+    ring.buf = s_tile;
+    ring.estride = (size_t)prm.estride; ring.sstride = (size_t)prm.sstride;
+    ring.nb = nb; ring.ns = prm.ring_ns; ring.lane = lane;
+    ring.nv = min(32, prm.p1 - prm.p0 - (int)blockIdx.y * 32);
+    const double* __restrict__ tile_chunk = prm.tile + (KT ? (size_t)blockIdx.y * 32 : 0);
     int curA = -1, curB = -1;
     __syncwarp();
 
@@ -155,20 +285,20 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
         for (int j = 0; j < ip1 - ip0; ++j) {
             const RisPairRec pr = s_pair[j];
             if (pr.atA != curA || pr.atB != curB) { flush(); curA = pr.atA; curB = pr.atB; }
-            const double* __restrict__ tile = tile_lane + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * estride;
+            const bool runA = PH != 2 && pr.nkA > 0, runB = PH != 1 && pr.nkB > 0;
+            ring.g = tile_chunk + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * ring.estride;
+            __syncwarp();                              // every lane is done with the previous pair's tile
+            if (runA || runB) ring.begin();
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
-#ifdef RIS_PREFETCH_TILE   // measured on config 4: no gain (7.6 -> 7.9 ms/step), kept for experiments
-            // the NEXT pair's tile rows start their way from HBM / L2 to L1 while this pair's primitives run
-            // (K: one 256-byte row per element and state across the warp; J: the pair's few contiguous lines)
-            if (ip0 + j + 1 < pk.npairs) ris_prefetch_tile<NEL>(tile + (size_t)NEL * estride, estride, sstride, nb, prm.lstride);
-#endif
-            if (PH != 2 && pr.nkA > 0)
-                ris_phase<LA, LB, false>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
-                                         estride, sstride, nb, s_sc + lane, s_red + lane);
+            if (runA)
+                ris_phase<LA, LB, false, Tune::PIPE, KT>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, ring,
+                                                     nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
-            if (PH != 1 && pr.nkB > 0)
-                ris_phase<LB, LA, true>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz, alpha,
-                                        auxfac, prm.boys, tile, estride, sstride, nb, s_sc + lane, s_red + lane);
+            if (runB) {
+                if (runA && !ring.holds_all()) { __syncwarp(); ring.begin(); }      // the ring has rolled past state 0
+                ris_phase<LB, LA, true, Tune::PIPE, KT>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
+                                                    alpha, auxfac, prm.boys, ring, nb, s_sc + lane, s_red + lane);
+            }
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
         if (prm.det != nullptr) {
@@ -186,7 +316,7 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
     }
     flush();
 
-    // aux side: the four warps of the block hold the same 32 aux functions
+    // aux side: the warps of the block hold the same 32 aux functions
     __syncthreads();
     if (warp == 0 && live) {
         for (int i = 0; i < 3 * nb; ++i) {
@@ -200,36 +330,52 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
     }
 }
 
-template <int LA, int LB, int PH>
-void ris_launch_grad_phase(const RisGradParams& p, cudaStream_t st)
+template <int LA, int LB, int PH, bool KT>
+cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
 {
-    const size_t smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.kmax, p.nb);
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(ris_grad_kernel<LA, LB, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = smem;
+    // ring slots: all states when they fit the class budget, fewer when the task records of a long contraction (kmax up
+    // to 576 primitive pairs) leave less than that of the 227 KB a block may use
+    RisGradParams p = p0_;
+    constexpr int NSMAX = KT ? RisGradTune<LA, LB>::NSK : RIS_NB_MAX;
+    p.ring_ns = p.nb < NSMAX ? p.nb : NSMAX;
+    size_t smem = 0;
+    for (;; --p.ring_ns) {
+        smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.task_prims, p.pk.kmax, p.nb, ris_grad_tile_doubles<LA, LB, KT>(p.ring_ns));
+        if (smem <= 227 * 1024 || p.ring_ns == 1) break;
+    }
+    // the opt-in is per device and context: set it at every launch that needs it (a host-side call of ~1 us) instead of
+    // caching it in process-wide state
+    if (smem > 48 * 1024) {
+        const cudaError_t e = cudaFuncSetAttribute(ris_grad_kernel<LA, LB, PH, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
     }
     // blockIdx.y: chunks of 32 aux functions; blockIdx.x: the blocks of a chunk, together one resident wave of
     // long-lived warps drawing tasks (few aux-side atomics, no wave quantisation)
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
-    static int nsm = 0;
-    if (nsm == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
-    const int nx = std::max(1, std::min(nbt, (nsm * RisGradTune<LA, LB>::MINB + ny - 1) / ny));
-    ris_grad_kernel<LA, LB, PH><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    const int nx = std::max(1, std::min(nbt, (p.nsm * RisGradTune<LA, LB>::MINB + ny - 1) / ny));
+    ris_grad_kernel<LA, LB, PH, KT><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    return cudaGetLastError();
 }
 
-// p.task_ctr holds two zeroed ticket arrays of ny counters each (one per phase launch)
-template <int LA, int LB>
-void ris_launch_grad(const RisGradParams& p, cudaStream_t st)
+// p.task_ctr holds two zeroed ticket arrays of ny counters each (one per phase launch); p.lstride selects the type
+template <int LA, int LB, bool KT>
+cudaError_t ris_launch_grad_t(const RisGradParams& p, cudaStream_t st)
 {
-    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
     if constexpr (RisGradTune<LA, LB>::SPLIT) {
         RisGradParams q = p;
-        ris_launch_grad_phase<LA, LB, 1>(q, st);
+        cudaError_t e = ris_launch_grad_phase<LA, LB, 1, KT>(q, st);
+        if (e != cudaSuccess) return e;
         q.task_ctr = p.task_ctr + (p.p1 - p.p0 + 31) / 32;
-        ris_launch_grad_phase<LA, LB, 2>(q, st);
+        return ris_launch_grad_phase<LA, LB, 2, KT>(q, st);
     } else {
-        ris_launch_grad_phase<LA, LB, 0>(p, st);
+        return ris_launch_grad_phase<LA, LB, 0, KT>(p, st);
     }
+}
+
+template <int LA, int LB>
+cudaError_t ris_launch_grad(const RisGradParams& p, cudaStream_t st)
+{
+    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
+    return p.lstride ? ris_launch_grad_t<LA, LB, true>(p, st) : ris_launch_grad_t<LA, LB, false>(p, st);
 }

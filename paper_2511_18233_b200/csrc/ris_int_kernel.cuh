@@ -118,19 +118,17 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
 }
 
 template <int LA, int LB, bool STORE>
-void ris_launch_int(const RisGradParams& p, cudaStream_t st)
+cudaError_t ris_launch_int(const RisGradParams& p, cudaStream_t st)
 {
-    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return;
+    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
     const size_t smem = RIS_GRAD_WARPS * ris_int_warp_smem(p.pk.kmax, p.nb);
-    static size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaFuncSetAttribute(ris_int_kernel<LA, LB, STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = smem;
+    if (smem > 48 * 1024) {          // per device and context: set at every launch that needs it, no process-wide cache
+        const cudaError_t e = cudaFuncSetAttribute(ris_int_kernel<LA, LB, STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
     }
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
-    static int nsm = 0;
-    if (nsm == 0) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
-    const int nx = std::max(1, std::min(nbt, (nsm * 3 + ny - 1) / ny));
+    const int nx = std::max(1, std::min(nbt, (p.nsm * 3 + ny - 1) / ny));
     ris_int_kernel<LA, LB, STORE><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    return cudaGetLastError();
 }

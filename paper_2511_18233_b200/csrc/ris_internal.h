@@ -16,7 +16,7 @@ constexpr int RIS_NB_MAX = 5;           // states per class-kernel launch (per-s
 __host__ __device__ inline int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
 __host__ __device__ inline int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
 // task window by class weight: a (d,d) primitive triplet costs ~10x an (s,s) one, and a task should stay ~10-20 us
-__host__ __device__ inline int ris_task_prims(int la, int lb) { return la + lb <= 2 ? 32 : (la + lb <= 3 ? 16 : 8); }
+__host__ __device__ inline int ris_task_prims(int la, int lb) { return la + lb <= 1 ? 24 : (la + lb <= 2 ? 32 : (la + lb <= 3 ? 16 : 8)); }
 
 // One packed shell pair (64 bytes, read by a whole warp as a broadcast).
 struct __align__(16) RisPairRec {
@@ -50,6 +50,7 @@ struct RisClassPack {
 struct RisGradParams {
     RisClassPack pk;
     int naux, natoms;
+    int nsm;                 // SMs of the context's device (grid sizing)
     const double* aux;       // [naux][5] Cx,Cy,Cz,alpha,auxfac
     const double* boys;      // table for M = E of this class
     // packed tiles: element el of state s for aux P sits at tile[s*sstride + el*estride + (P - p0)*lstride]
@@ -59,6 +60,7 @@ struct RisGradParams {
     int lstride;
     const double* cscale;    // J: c_aux[nb][naux]; K: nullptr
     int nb;
+    int ring_ns;             // slots of the shared-memory tile ring (set by the launcher)
     int p0, p1;              // aux range of this launch; blockIdx.y selects 32 of them, one per lane
     int* task_ctr;           // [chunks of 32 aux] zeroed ticket counters of this launch (dynamic task hand-out)
     double* grad;            // [nb][natoms][3], accumulated with atomics
@@ -81,13 +83,26 @@ __device__ __forceinline__ void ris_grad_add(const RisGradParams& prm, size_t id
     atomicAdd(prm.det + 2 * idx + 1, (unsigned long long)lo);
 }
 
-typedef void (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
+typedef cudaError_t (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
 extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];
 
-// dynamic shared memory of a class-kernel block (host + device agree through this)
-__host__ __device__ inline size_t ris_grad_warp_smem(int kmax, int nb)
+
+// Dynamic shared memory of one warp of a class-kernel block with a tile ring of `tile_doubles` (host + device agree
+// through this; ris_grad_kernel.cuh).
+__host__ __device__ inline size_t ris_grad_warp_smem(int window, int kmax, int nb, int tile_doubles)
 {
-    return (size_t)64 * (RIS_TASK_PRIMS + kmax)      // primitive-pair records of the task
-         + (size_t)64 * RIS_TASK_PRIMS               // pair records of the task
-         + (size_t)8 * (6 * nb * 33 + 3 * nb * 32 + nb * 32);   // pair-side slots [6 nb][33], aux-side slots, scales
+    return (size_t)64 * (window + kmax)              // primitive-pair records of the task (window = pk.task_prims)
+         + (size_t)64 * window                       // pair records of the task
+         + (size_t)8 * (6 * nb * 33 + 3 * nb * 32 + nb * 32)   // pair-side slots [6 nb][33], aux-side slots, scales
+         + (size_t)8 * tile_doubles;                 // tile ring
+}
+// Largest number of states per launch (<= RIS_NB_MAX) with which a block of class (la,lb) and its smallest tile ring (one
+// slot) stays within the 227 KB a block may use; 0 if not even one state fits.
+inline int ris_grad_nb_cap(int la, int lb, int kmax, bool ktype)
+{
+    const int nel = ris_ncart(la) * ris_ncart(lb);
+    for (int nb = RIS_NB_MAX; nb >= 1; --nb)
+        if (RIS_GRAD_WARPS * ris_grad_warp_smem(ris_task_prims(la, lb), kmax, nb, ktype ? nel * 32 : ((nel + 1) & ~1)) <= (size_t)227 * 1024)
+            return nb;
+    return 0;
 }

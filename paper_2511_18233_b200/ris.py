@@ -12,7 +12,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libris_b200.so")
+# RIS_B200_LIB: load a side-by-side variant build (paper_2511_18233_b200.build with RIS_BUILD_TAG) instead -- kernel tuning only
+LIB_PATH = os.environ.get("RIS_B200_LIB") or os.path.join(_HERE, "libris_b200.so")
 _lib = None
 
 EXPORTS = [

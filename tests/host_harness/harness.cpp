@@ -59,8 +59,8 @@ static void phase_t(int nk, const double* prim, bool hostA, const double* Z, con
     if (!used) return;
     // slots as in the class kernel: slot[(s*6 + c)*SL], c = 0..2 centre A, 3..5 centre B (stride SL = 1 here), unit scales
     std::vector<double> sc((size_t)nb, 1.0);
-    ris_hrrc<LH, LO, TR, 1, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], tile, (size_t)1, (size_t)(K::NCA * K::NCB), nb,
-                               sc.data(), out);
+    RisTilePlain ring{tile, (size_t)1, (size_t)(K::NCA * K::NCB)};
+    ris_hrrc<LH, LO, TR, 1, 1>(acc, Z[0] - ZO[0], Z[1] - ZO[1], Z[2] - ZO[2], ring, nb, sc.data(), out);
 }
 
 template <int LA, int LB>

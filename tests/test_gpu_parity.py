@@ -206,31 +206,25 @@ def test_invalid_arguments_are_reported():
 
 # ----------------------------------------------------------------- full-size configs, sampled outputs
 def _edge_atoms(ctx, mol, want):
-    """Atoms whose outputs exercise the seams of the pair-restricted Gamma^P GEMM-2 (ris_diag_gemm2_layout): atoms with
-    a SHELL that straddles a row-panel edge of the spatial AO order (its same-shell pair folds two elements onto one S
-    position -> overflow gather), atoms whose AOs straddle a panel edge or a column-tile edge, then evenly spaced ones."""
-    pos, rows, cols, ntiles, novf = ctx.gemm2_layout()
-    off = mol.ao_off
-    shell_edge, row_edge, col_edge = [], [], []
-    for a in range(mol.natoms):
-        sh = [s for s in range(mol.nshells) if mol.shell_atom[s] == a]
-        p_at = np.concatenate([pos[off[s]:off[s] + synth.ncart(int(mol.shell_l[s]))] for s in sh])
-        if any(pos[off[s]] // rows != pos[off[s] + synth.ncart(int(mol.shell_l[s])) - 1] // rows for s in sh):
-            shell_edge.append(a)
-        elif p_at.min() // rows != p_at.max() // rows:
-            row_edge.append(a)
-        elif p_at.min() // cols != p_at.max() // cols:
-            col_edge.append(a)
+    """Atoms whose outputs exercise the seams of the Gamma^P GEMM-2 (ris_diag_gemm2_layout: tiles of `rows` gathered
+    partners x `cols` aux functions): the aux functions (= atoms) on either side of every aux-tile edge and the last one
+    (ragged tail of the P range), the first and last atom in the SPATIAL AO order (shortest / edge partner lists), then
+    evenly spaced ones."""
+    pos, rows, cols, ntiles, nentries = ctx.gemm2_layout()
+    assert rows > 0 and cols > 0 and ntiles > 0 and nentries == 2 * ctx.npair_elements
     pick = []
-    for group, n in ((shell_edge, want // 3), (row_edge, want // 4), (col_edge, want // 4)):
-        step = max(1, len(group) // max(n, 1))
-        pick += group[::step][:n]
-    for a in np.linspace(0, mol.natoms - 1, want).astype(int):
+    for e in range(cols, mol.natoms, cols):
+        pick += [e - 1, e]
+    pick += [mol.natoms - 1]
+    ao_atom = np.repeat(mol.shell_atom, [synth.ncart(int(l)) for l in mol.shell_l])
+    pick += [int(ao_atom[np.argmin(pos)]), int(ao_atom[np.argmax(pos)])]
+    pick = list(dict.fromkeys(pick))[:want]
+    for a in np.linspace(0, mol.natoms - 1, 2 * want).astype(int):
         if len(pick) >= want:
             break
         if int(a) not in pick:
             pick.append(int(a))
-    return sorted(pick), dict(shell_edge=len(shell_edge), row_edge=len(row_edge), col_edge=len(col_edge), novf=novf)
+    return sorted(pick), dict(rows=rows, cols=cols, ntiles=ntiles)
 
 
 @pytest.mark.parametrize("cfg,natoms_sampled", [(3, 12), (5, 8), (4, 12)])
@@ -243,7 +237,7 @@ def test_full_size_sampled_atoms(cfg, natoms_sampled):
     atoms, info = _edge_atoms(ctx, wl.mol, natoms_sampled)
     assert len(atoms) == natoms_sampled
     if cfg == 4:
-        assert info["novf"] > 0 and info["shell_edge"] > 0       # the overflow path is exercised at full size
+        assert 63 in atoms and 64 in atoms and 299 in atoms      # both sides of an aux-tile edge, the ragged tail
     cut = 1e-22 if cfg == 4 else 0.0
     rJ, _ = orc.grad_J(wl.mol, wl.D, wl.c_aux, atoms=atoms, prim_cutoff=cut)
     assert_parity(gJ, rJ, f"config {cfg} J", literal=True)
