@@ -34,6 +34,14 @@ In the generated code "a" always means the host: a2 = 2 x host exponent, PA = P 
 AB = host centre - other centre, ga = d/d(host centre), gb = d/d(other centre).  TR selects the tile
 element order: false -> (c_host*n_other + c_other), true -> (c_other*n_host + c_host).
 
+Classes whose OTHER shell is an s function (lo = 0, host l = lh > = 0; the kernels run (l,0) pairs with the l shell as
+host for EVERY primitive pair) need no transfer at all: the integral is [a 0|, and the derivative with respect to the s
+centre is taken by one DIRECT Obara-Saika step on that centre instead of the HRR,
+    d/dB_i (a 0|P) = 2b [a, 1_i|,   [a,1_i|^(0) = PB_i [a]^(0) + WP_i [a]^(1) + a_i/(2p) ([a-1_i]^(0) - (rho/p) [a-1_i]^(1)),
+with PB = (a/p)(A - B) formed from the exponents (no cancellation for any exponent ratio).  One host phase per pair instead
+of two halves the per-pair work (HRR, tile contraction, slot updates) of the (s,s), (p,s), (d,s), (f,s) classes; targets:
+    acc2a[e] += 2a [e], e = lh+1;   accbd[a][i] += 2b [a,1_i|, a in comps(lh), i = x,y,z;   acc1[e] += [e], e = lh-1.
+
 Component order inside a shell of degree l: lx descending, then ly descending.
 """
 from __future__ import annotations
@@ -80,8 +88,9 @@ class ClassPlan:
     def __init__(self, la, lb):
         self.la, self.lb = la, lb
         self.E = la + lb + 1
+        self.direct_b = (lb == 0)          # d/dB by a direct OS step on the s centre (see the module docstring)
         self.r2a = list(range(la + 1, self.E + 1))
-        self.r2b = list(range(la, self.E + 1))
+        self.r2b = [] if self.direct_b else list(range(la, self.E + 1))
         lo = la - 1 if la >= 1 else la
         self.r1 = list(range(lo, self.E - 1)) if (la >= 1 or lb >= 1) else []
         self.off = {}
@@ -90,9 +99,15 @@ class ClassPlan:
             for e in rng:
                 self.off[(tag, e)] = n
                 n += nc(e)
+        if self.direct_b:
+            self.off_bd = n                # accbd[(component of la) * 3 + i]
+            n += 3 * nc(la)
         self.nacc = n
         self.fams = [("2a", self.r2a, "a2"), ("2b", self.r2b, "b2"), ("1", self.r1, None)]
         self.vrr_name = f"ris_vrr_{la}{lb}"
+
+    def acc_bd(self, a, i):
+        return f"acc[{self.off_bd + 3 * cidx(a) + i}]"
 
     def acc(self, tag, e, c):
         return f"acc[{self.off[(tag, e)] + cidx(c)}]"
@@ -126,9 +141,13 @@ def gen_vrr(pl: ClassPlan) -> str:
     out = []
     w = out.append
     w(f"// class ({la},{lb}): E={E}, {pl.nacc} contracted targets")
+    w("// ACC: the contracted targets -- a double[NACC] array (registers) or any type with operator[] (the class kernel parks")
+    w("// part of them in shared memory for the heavy classes)")
+    w("template <class ACC>")
+    direct = getattr(pl, "direct_b", False)
     w(f"RIS_DEV void {pl.vrr_name}(const double (&F)[{E + 1}], double PA0, double PA1, double PA2,")
     w("    double WP0, double WP1, double WP2, double oo2p, double q, double a2, double b2,")
-    w(f"    double (&acc)[{pl.nacc}])")
+    w("    ACC& acc" + (", double PB0, double PB1, double PB2)" if direct else ")"))
     w("{")
     PA = ["PA0", "PA1", "PA2"]
     WP = ["WP0", "WP1", "WP2"]
@@ -161,12 +180,23 @@ def gen_vrr(pl: ClassPlan) -> str:
     for e in range(emin_target, E + 1):
         for c in comps(e):
             want(e, c, 0)
+    if direct:                      # [a,1_i|^(0) needs [a]^(0), [a]^(1) and the brackets of [a-1_i]
+        for c in comps(la):
+            want(la, c, 0)
+            want(la, c, 1)
+            for i in range(3):
+                if c[i] >= 1:
+                    want(la - 1, lower(c, i), 0)
+                    want(la - 1, lower(c, i), 1)
 
     def v(e, c, m):
         return "F[%d]" % m if e == 0 else f"v{e}_{cidx(c)}_{m}"
 
     brackets = set()
-    kk = sorted({c[i] - 1 for (e, c, m) in need if e >= 2 for i in [pick_dir(c)] if c[i] >= 2})
+    kk = {c[i] - 1 for (e, c, m) in need if e >= 2 for i in [pick_dir(c)] if c[i] >= 2}
+    if direct:
+        kk |= {c[i] for c in comps(la) for i in range(3) if c[i] >= 1}
+    kk = sorted(kk)
     for k in kk:
         w(f"    const double k{k} = {float(k)} * oo2p;")
     for e in range(1, E + 1):
@@ -196,6 +226,19 @@ def gen_vrr(pl: ClassPlan) -> str:
                     w(f"    {pl.acc(tag, e, c)} = fma({scale}, {val}, {pl.acc(tag, e, c)});")
                 else:
                     w(f"    {pl.acc(tag, e, c)} += {val};")
+    if direct:
+        PB = ["PB0", "PB1", "PB2"]
+        for c in comps(la):
+            for i in range(3):
+                expr = f"fma({PB[i]}, {v(la, c, 0)}, {WP[i]} * {v(la, c, 1)})"
+                if c[i] >= 1:
+                    c1 = lower(c, i)
+                    bn = f"b{la - 1}_{cidx(c1)}_0"
+                    if bn not in brackets:
+                        brackets.add(bn)
+                        w(f"    const double {bn} = fma(-q, {v(la - 1, c1, 1)}, {v(la - 1, c1, 0)});")
+                    expr = f"fma(k{c[i]}, {bn}, {expr})"
+                w(f"    {pl.acc_bd(c, i)} = fma(b2, {expr}, {pl.acc_bd(c, i)});")
     w("}")
     return "\n".join(out)
 
@@ -237,13 +280,13 @@ def gen_hrrc(pl: ClassPlan) -> str:
     w("// (the host centre is B in the TR instantiations).  The tile comes from a provider: ring.get(s) returns the tile of")
     w("// state s (shared-memory ring of the class kernel, or plain memory), element (c_host,c_other) at t[el * ring.es()],")
     w("// el by TR (see gen_classes.py).")
-    w("template <bool TR, int SL, int SC, class Ring>")
-    w(f"RIS_DEV void ris_hrrc_{la}{lb}(const double (&acc)[{pl.nacc}], double AB0, double AB1, double AB2,")
+    w("template <bool TR, int SL, int SC, class Ring, class ACC>")
+    w(f"RIS_DEV void ris_hrrc_{la}{lb}(const ACC& acc, double AB0, double AB1, double AB2,")
     w("    Ring& ring, int nb, const double* __restrict__ sc, double* __restrict__ slot)")
     w("{")
     done = set()
     X2a = gen_hrr_chain(w, pl, "2a", la + 1, lb, "xa", done)
-    Y2b = gen_hrr_chain(w, pl, "2b", la, lb + 1, "yb", done)
+    Y2b = None if pl.direct_b else gen_hrr_chain(w, pl, "2b", la, lb + 1, "yb", done)
     X1m = gen_hrr_chain(w, pl, "1", la - 1, lb, "xm", done) if la >= 1 else None
     Y1m = gen_hrr_chain(w, pl, "1", la, lb - 1, "xm", done) if lb >= 1 else None
     nca, ncb = nc(la), nc(lb)
@@ -259,7 +302,8 @@ def gen_hrrc(pl: ClassPlan) -> str:
                 w(f"          ga{i} = fma(w, {X2a(raise_(a, i), b)}, ga{i});")
                 if a[i] >= 1:
                     w(f"          ga{i} = fma(-{float(a[i])} * w, {X1m(lower(a, i), b)}, ga{i});")
-                w(f"          gb{i} = fma(w, {Y2b(a, raise_(b, i))}, gb{i});")
+                gbv = pl.acc_bd(a, i) if pl.direct_b else Y2b(a, raise_(b, i))
+                w(f"          gb{i} = fma(w, {gbv}, gb{i});")
                 if b[i] >= 1:
                     w(f"          gb{i} = fma(-{float(b[i])} * w, {Y1m(a, lower(b, i))}, gb{i});")
             w("        }")

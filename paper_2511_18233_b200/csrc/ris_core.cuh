@@ -167,15 +167,22 @@ struct RisTilePlain {
     RIS_DEV const double* get(int s) const { return tile + (size_t)s * sstride; }
 };
 
-template <int LH, int LO>
+// ZO = Z - O (host centre minus other centre).  Classes with an s function on the other centre (LO = 0) take the derivative
+// with respect to it by a direct recurrence step there (gen_classes.py): P - O = (h/p)(Z - O), from the exponents.
+template <int LH, int LO, class ACC>
 RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, double oo2p, double h2, double o2,
                               double coef, double ZCx, double ZCy, double ZCz, double alpha, double auxfac,
-                              const double* __restrict__ boys_tab, double (&acc)[RisClass<LH, LO>::NACC])
+                              const double* __restrict__ boys_tab, ACC& acc, double ZOx, double ZOy, double ZOz)
 {
     constexpr int E = RisClass<LH, LO>::E;
     RisPrimHead<E> h;
     ris_prim_head<E>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
-    ris_vrr<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc);
+    if constexpr (LO == 0) {
+        const double hp = h2 * oo2p;
+        ris_vrr<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc, hp * ZOx, hp * ZOy, hp * ZOz);
+    } else {
+        ris_vrr<LH, LO>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc);
+    }
 }
 
 // Undifferentiated primitive triplet (v_P = sum D_{mu nu} (mu nu|P), Eq. 21):

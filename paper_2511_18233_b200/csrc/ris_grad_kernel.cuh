@@ -33,6 +33,7 @@
 #pragma once
 #include "ris_core.cuh"
 #include "ris_internal.h"
+#include <type_traits>
 
 // ------------------------------------------------------------------------------------------------ tuning
 // resident blocks per SM the register allocation aims at (light classes: latency-bound prefactor / Boys chains
@@ -66,11 +67,13 @@ template <int LA, int LB> struct RisGradTune {
     static constexpr int NSK_LO = (NEL * 256 * 2 <= 20480) ? 2 : 1;
     static constexpr int NSK = (RIS_STAGE_BYTES / (NEL * 256) < NSK_LO) ? NSK_LO
                              : (RIS_STAGE_BYTES / (NEL * 256) > RIS_NB_MAX ? RIS_NB_MAX : RIS_STAGE_BYTES / (NEL * 256));
+    static constexpr bool STAGE_K = ris_grad_stage_k(LA, LB);      // else the K tile is read straight from global memory
+    static constexpr int NW = RIS_GRAD_WARPS;                      // warps per block
 };
 // doubles of a tile ring of ns slots: K -- slots of NEL rows of 32 aux values; J -- slots of NEL values
 template <int LA, int LB, bool KT> __host__ __device__ constexpr int ris_grad_tile_doubles(int ns)
 {
-    return KT ? ns * RisGradTune<LA, LB>::NEL * 32 : ((ns * RisGradTune<LA, LB>::NEL + 1) & ~1);
+    return KT ? (RisGradTune<LA, LB>::STAGE_K ? ns * RisGradTune<LA, LB>::NEL * 32 : 0) : ((ns * RisGradTune<LA, LB>::NEL + 1) & ~1);
 }
 
 // ------------------------------------------------------------------------------------------------ tile ring
@@ -151,6 +154,18 @@ struct RisTileRing {
     __device__ __forceinline__ bool holds_all() const { return nb <= ns; }
 };
 
+// Unstaged K tile (the 60- and 100-element classes): the same interface on global memory, element el of state s of this
+// lane's aux function at g[s * sstride + el * estride].
+struct RisTileDirectK {
+    const double* g;           // tile + first element of the pair * estride + chunk offset (set per pair)
+    size_t estride, sstride;
+    int nb, ns, lane, nv, issued;
+    __device__ __forceinline__ size_t es() const { return estride; }
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ const double* get(int s) const { return g + (size_t)s * sstride + (lane < nv ? lane : 0); }
+    __device__ __forceinline__ bool holds_all() const { return true; }
+};
+
 // ------------------------------------------------------------------------------------------------ one host-centre phase
 // The primitive pairs q[0 .. nk) hosted on centre Z (host l = LH, other l = LO), then HRR / derivative / tile contraction
 // into the lane's accumulator slots.
@@ -178,8 +193,14 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
             ris_prim_front(n0.x, n0.y, n1.x, n1.y, n3.y, ZCx, ZCy, ZCz, alpha, auxfac, fn);
             double F[E + 1];
             ris_boys<E>(f.T, boys, F, f.kappa);
-            ris_vrr<LH, LO>(F, r0.y, r1.x, r1.y, -f.q * f.X0, -f.q * f.X1, -f.q * f.X2, r2.x, f.q, TR ? r3.x : r2.y,
-                            TR ? r2.y : r3.x, acc);
+            const double h2 = TR ? r3.x : r2.y, o2 = TR ? r2.y : r3.x;
+            if constexpr (LO == 0) {
+                const double hp = h2 * r2.x;
+                ris_vrr<LH, LO>(F, r0.y, r1.x, r1.y, -f.q * f.X0, -f.q * f.X1, -f.q * f.X2, r2.x, f.q, h2, o2, acc, hp * ZOx, hp * ZOy,
+                                hp * ZOz);
+            } else {
+                ris_vrr<LH, LO>(F, r0.y, r1.x, r1.y, -f.q * f.X0, -f.q * f.X1, -f.q * f.X2, r2.x, f.q, h2, o2, acc);
+            }
             r0 = n0; r1 = n1; r2 = n2; r3 = n3; f = fn;
         }
     } else {
@@ -189,7 +210,7 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
             const double2 r2 = *reinterpret_cast<const double2*>(q + 4);
             const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
             ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
-                                     alpha, auxfac, boys, acc);
+                                     alpha, auxfac, boys, acc, ZOx, ZOy, ZOz);
         }
     }
     ris_hrrc<LH, LO, TR, 33, KT ? 0 : 32>(acc, ZOx, ZOy, ZOz, ring, nb, sc, slot);
@@ -198,7 +219,7 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
 // KT: K-type contraction (Gamma^P tile, P-minor, one column per lane); else J-type (D tile shared by all lanes, scaled by
 // c_aux[s][P]).
 template <int LA, int LB, int PH, bool KT>
-__global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
+__global__ void __launch_bounds__(32 * RisGradTune<LA, LB>::NW, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
 {
     using Tune = RisGradTune<LA, LB>;
     constexpr int NEL = Tune::NEL;
@@ -213,7 +234,7 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
     double* s_tile = reinterpret_cast<double*>(s_pair + pk.task_prims);      // tile ring (16-byte aligned)
     double* s_red = s_tile + ris_grad_tile_doubles<LA, LB, KT>(prm.ring_ns); // [6 nb][33]  pair side: A x,y,z, B x,y,z per state
     double* s_gaux = s_red + 6 * nb * 33;                                    // [3 nb][32]  aux side
-    double* s_sc = s_gaux + 3 * nb * 32;                                     // [nb][32]    J: c_aux[s][P]; K: 1
+    double* s_sc = s_gaux + 3 * nb * 32;                                     // [nb][32]    J: c_aux[s][P]
     const size_t gaux_off = (size_t)(reinterpret_cast<unsigned char*>(s_gaux) - (sm_raw + (size_t)warp * wbytes));
 
     // this lane's auxiliary function
@@ -227,8 +248,9 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
         for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale[(size_t)s * prm.naux + Pe];
     for (int i = 0; i < 6 * nb; ++i) s_red[i * 33 + lane] = 0.0;
     for (int i = 0; i < 3 * nb; ++i) s_gaux[i * 32 + lane] = 0.0;
-    RisTileRing<NEL, NS, KT> ring;
-    ring.buf = s_tile;
+    constexpr bool STAGED = !KT || Tune::STAGE_K;
+    typename std::conditional<STAGED, RisTileRing<NEL, NS, KT>, RisTileDirectK>::type ring;
+    if constexpr (STAGED) ring.buf = s_tile;
     ring.estride = (size_t)prm.estride; ring.sstride = (size_t)prm.sstride;
     ring.nb = nb; ring.ns = prm.ring_ns; ring.lane = lane;
     ring.nv = min(32, prm.p1 - prm.p0 - (int)blockIdx.y * 32);
@@ -285,7 +307,7 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
         for (int j = 0; j < ip1 - ip0; ++j) {
             const RisPairRec pr = s_pair[j];
             if (pr.atA != curA || pr.atB != curB) { flush(); curA = pr.atA; curB = pr.atB; }
-            const bool runA = PH != 2 && pr.nkA > 0, runB = PH != 1 && pr.nkB > 0;
+            const bool runA = PH != 2 && pr.nkA > 0, runB = LB > 0 && PH != 1 && pr.nkB > 0;
             ring.g = tile_chunk + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * ring.estride;
             __syncwarp();                              // every lane is done with the previous pair's tile
             if (runA || runB) ring.begin();
@@ -294,10 +316,12 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
                 ris_phase<LA, LB, false, Tune::PIPE, KT>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, ring,
                                                      nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
-            if (runB) {
-                if (runA && !ring.holds_all()) { __syncwarp(); ring.begin(); }      // the ring has rolled past state 0
-                ris_phase<LB, LA, true, Tune::PIPE, KT>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
-                                                    alpha, auxfac, prm.boys, ring, nb, s_sc + lane, s_red + lane);
+            if constexpr (LB > 0) {        // (l,s) pairs are hosted on the l shell for every primitive pair: one phase
+                if (runB) {
+                    if (runA && !ring.holds_all()) { __syncwarp(); ring.begin(); }      // the ring has rolled past state 0
+                    ris_phase<LB, LA, true, Tune::PIPE, KT>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy,
+                                                            -pr.ABz, alpha, auxfac, prm.boys, ring, nb, s_sc + lane, s_red + lane);
+                }
             }
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
@@ -322,7 +346,7 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, RisGradTune<LA, LB>::MINB) r
         for (int i = 0; i < 3 * nb; ++i) {
             double v = 0.0;
 #pragma unroll
-            for (int w = 0; w < RIS_GRAD_WARPS; ++w)
+            for (int w = 0; w < Tune::NW; ++w)
                 v += reinterpret_cast<const double*>(sm_raw + (size_t)w * wbytes + gaux_off)[i * 32 + lane];
             const int s = i / 3, x = i - 3 * s;
             ris_grad_add(prm, ((size_t)s * prm.natoms + P) * 3 + x, v);
@@ -339,8 +363,9 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     constexpr int NSMAX = KT ? RisGradTune<LA, LB>::NSK : RIS_NB_MAX;
     p.ring_ns = p.nb < NSMAX ? p.nb : NSMAX;
     size_t smem = 0;
+    constexpr int NW = RisGradTune<LA, LB>::NW;
     for (;; --p.ring_ns) {
-        smem = RIS_GRAD_WARPS * ris_grad_warp_smem(p.pk.task_prims, p.pk.kmax, p.nb, ris_grad_tile_doubles<LA, LB, KT>(p.ring_ns));
+        smem = NW * ris_grad_warp_smem(p.pk.task_prims, p.pk.kmax, p.nb, ris_grad_tile_doubles<LA, LB, KT>(p.ring_ns));
         if (smem <= 227 * 1024 || p.ring_ns == 1) break;
     }
     // the opt-in is per device and context: set it at every launch that needs it (a host-side call of ~1 us) instead of
@@ -352,9 +377,11 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     // blockIdx.y: chunks of 32 aux functions; blockIdx.x: the blocks of a chunk, together one resident wave of
     // long-lived warps drawing tasks (few aux-side atomics, no wave quantisation)
     const int ny = (p.p1 - p.p0 + 31) / 32;
-    const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
-    const int nx = std::max(1, std::min(nbt, (p.nsm * RisGradTune<LA, LB>::MINB + ny - 1) / ny));
-    ris_grad_kernel<LA, LB, PH, KT><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    const int nbt = (p.pk.ntasks + NW - 1) / NW;
+    // resident blocks per SM: the register target, or what the shared memory of the block allows
+    const int resident = std::max(1, std::min<int>(RisGradTune<LA, LB>::MINB * RIS_GRAD_WARPS / NW, (int)((227 * 1024) / (smem + 1024))));
+    const int nx = std::max(1, std::min(nbt, (p.nsm * resident + ny - 1) / ny));
+    ris_grad_kernel<LA, LB, PH, KT><<<dim3(nx, ny), 32 * NW, smem, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -13,10 +13,10 @@ constexpr int RIS_TASK_PRIMS = 32;      // a warp task = the shell pairs whose f
                                         // fewer than window + kmax of them)
 constexpr int RIS_NB_MAX = 5;           // states per class-kernel launch (per-state gradient slots in shared memory)
 
-__host__ __device__ inline int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
-__host__ __device__ inline int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
+__host__ __device__ constexpr int ris_class_id(int la, int lb) { return la * (la + 1) / 2 + lb; }
+__host__ __device__ constexpr int ris_ncart(int l) { return (l + 1) * (l + 2) / 2; }
 // task window by class weight: a (d,d) primitive triplet costs ~10x an (s,s) one, and a task should stay ~10-20 us
-__host__ __device__ inline int ris_task_prims(int la, int lb) { return la + lb <= 1 ? 24 : (la + lb <= 2 ? 32 : (la + lb <= 3 ? 16 : 8)); }
+__host__ __device__ constexpr int ris_task_prims(int la, int lb) { return la + lb <= 1 ? 24 : (la + lb <= 2 ? 32 : (la + lb <= 3 ? 16 : 8)); }
 
 // One packed shell pair (64 bytes, read by a whole warp as a broadcast).
 struct __align__(16) RisPairRec {
@@ -87,6 +87,10 @@ typedef cudaError_t (*ris_grad_launcher)(const RisGradParams&, cudaStream_t);
 extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];
 
 
+// ---- per-class configuration of the class kernels, shared by host sizing code and the kernel templates ----------------
+// K tiles of the biggest classes (60 / 100 elements: 15-26 KB per state and warp) are read straight from global memory
+__host__ __device__ constexpr bool ris_grad_stage_k(int la, int lb) { return ris_ncart(la) * ris_ncart(lb) < 60; }
+
 // Dynamic shared memory of one warp of a class-kernel block with a tile ring of `tile_doubles` (host + device agree
 // through this; ris_grad_kernel.cuh).
 __host__ __device__ inline size_t ris_grad_warp_smem(int window, int kmax, int nb, int tile_doubles)
@@ -101,8 +105,9 @@ __host__ __device__ inline size_t ris_grad_warp_smem(int window, int kmax, int n
 inline int ris_grad_nb_cap(int la, int lb, int kmax, bool ktype)
 {
     const int nel = ris_ncart(la) * ris_ncart(lb);
+    const int ring = ktype ? (ris_grad_stage_k(la, lb) ? nel * 32 : 0) : ((nel + 1) & ~1);
     for (int nb = RIS_NB_MAX; nb >= 1; --nb)
-        if (RIS_GRAD_WARPS * ris_grad_warp_smem(ris_task_prims(la, lb), kmax, nb, ktype ? nel * 32 : ((nel + 1) & ~1)) <= (size_t)227 * 1024)
+        if (RIS_GRAD_WARPS * ris_grad_warp_smem(ris_task_prims(la, lb), kmax, nb, ring) <= (size_t)227 * 1024)
             return nb;
     return 0;
 }

@@ -57,8 +57,9 @@ __global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_pair_survey(RisMolDev m,
     const double* B = m.coords + 3 * m.shell_atom[nu];
     const double dx = A[0] - B[0], dy = A[1] - B[1], dz = A[2] - B[2];
     const double AB2 = dx * dx + dy * dy + dz * dz;
-    // (s,s) pairs have no angular momentum to transfer: every primitive pair is hosted on A (one phase per pair)
-    const bool ss = m.shell_l[mu] + m.shell_l[nu] == 0;
+    // (l,s) pairs are hosted on the l shell (mu) for every primitive pair: nothing is transferred by the HRR, the derivative
+    // with respect to the s centre is a direct recurrence step there (gen_classes.py) -- one phase per pair
+    const bool ss = m.shell_l[nu] == 0;
     int nA = 0, nB = 0;
     for (int ka = 0; ka < m.shell_nprim[mu]; ++ka)
         for (int kb = 0; kb < m.shell_nprim[nu]; ++kb) {
@@ -191,7 +192,7 @@ __global__ void ris_k_pair_pack(RisMolDev m, RisClassPack pk, const long long* l
     pk.ao[ip] = m.shell_ao[mu]; pk.ao[n + ip] = m.shell_ao[nu];
     pk.symf[ip] = (mu == nu) ? 0.5f : 1.0f;
     double* q = pk.prim + (size_t)pk.prim_off[ip] * RIS_PRIM_FIELDS;
-    const bool ss = pk.la + pk.lb == 0;
+    const bool ss = pk.lb == 0;
     int k = 0, kA = 0;
     for (int host = 0; host < 2; ++host) {
         for (int ka = 0; ka < m.shell_nprim[mu]; ++ka)

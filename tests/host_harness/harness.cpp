@@ -46,15 +46,18 @@ static void phase_t(int nk, const double* prim, bool hostA, const double* Z, con
                     double alpha, double auxfac, const double* tile, int nb, double* out)
 {
     using K = RisClass<LH, LO>;
+    // (l,s) pairs: every primitive pair is hosted on the l shell (ris_setup.cuh), whatever the exponents
+    constexpr bool lb0 = TR ? (LH == 0) : (LO == 0);
     double acc[K::NACC];
     for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
     int used = 0;
     for (int k = 0; k < nk; ++k) {
         const double* q = prim + 8 * k;
-        if ((q[5] >= q[6]) != hostA) continue;
+        if ((q[5] >= q[6] || lb0) != hostA) continue;
         ++used;
         ris_prim_triplet<LH, LO>(q[0], q[1], q[2], q[3], q[4], hostA ? q[5] : q[6], hostA ? q[6] : q[5], q[7],
-                                 Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac, tab(K::E), acc);
+                                 Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac, tab(K::E), acc, Z[0] - ZO[0], Z[1] - ZO[1],
+                                 Z[2] - ZO[2]);
     }
     if (!used) return;
     // slots as in the class kernel: slot[(s*6 + c)*SL], c = 0..2 centre A, 3..5 centre B (stride SL = 1 here), unit scales
@@ -88,12 +91,13 @@ static void phase0_t(int nk, const double* prim, bool hostA, const double* Z, co
                      double alpha, double auxfac, const double* tile, int nb, int nel, double* out)
 {
     using K = RisClass0<LH, LO>;
+    constexpr bool lb0 = TR ? (LH == 0) : (LO == 0);
     double acc[K::NACC];
     for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
     int used = 0;
     for (int k = 0; k < nk; ++k) {
         const double* q = prim + 8 * k;
-        if ((q[5] >= q[6]) != hostA) continue;
+        if ((q[5] >= q[6] || lb0) != hostA) continue;
         ++used;
         ris_prim_triplet0<LH, LO>(q[0], q[1], q[2], q[3], q[4], q[7], Z[0] - C[0], Z[1] - C[1], Z[2] - C[2], alpha, auxfac,
                                   tab(K::E), acc);

@@ -56,16 +56,20 @@ def test_device_boys_interpolation_vs_mpmath(harness, M):
 CLASSES = [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2), (3, 0), (3, 1), (3, 2), (3, 3)]
 
 
-@pytest.mark.parametrize("la,lb", CLASSES)
-def test_class_recurrence_vs_oracle(harness, la, lb):
-    """One contracted triplet per class: VRR + accumulation + HRR + derivative + contraction against the
-    oracle's McMurchie-Davidson result (a different algorithm), for near and far aux centres."""
+@pytest.mark.parametrize("la,lb,span", [(la, lb, "normal") for la, lb in CLASSES] +
+                         [(la, lb, "extreme") for la, lb in CLASSES])
+def test_class_recurrence_vs_oracle(harness, la, lb, span):
+    """One contracted triplet per class: VRR + accumulation + HRR (or the direct step on the s centre of an (l,s) pair) +
+    derivative + contraction against the oracle's McMurchie-Davidson result (a different algorithm), for near and far aux
+    centres.  span = "extreme": exponents log-uniform in [0.05, 300] (ratios up to 6000 inside one pair: the product
+    centre sits on top of either centre) -- what the two-host rule and the direct step exist for."""
     rng = np.random.default_rng(10 * la + lb)
+    lo, hi = (0.15, 4.0) if span == "normal" else (0.05, 300.0)
     for trial, dist in enumerate([1.5, 6.0, 40.0]):
         coords = np.array([[0.1, -0.2, 0.3], [1.1, 0.7, -0.6], [0, 0, 0]], dtype=float)
         v = rng.normal(size=3)
         coords[2] = coords[0] + dist * v / np.linalg.norm(v)
-        mol = synth.tiny_molecule(100 + trial, [[la], [lb], []], coords, lo=0.15, hi=4.0, nprim=3)
+        mol = synth.tiny_molecule(100 + trial, [[la], [lb], []], coords, lo=lo, hi=hi, nprim=3)
         nca, ncb = synth.ncart(la), synth.ncart(lb)
         nb = 2
         tile = rng.standard_normal((nb, nca, ncb))
@@ -80,7 +84,8 @@ def test_class_recurrence_vs_oracle(harness, la, lb):
             for kb in range(3):
                 a, b = mol.prim_exp[ka], mol.prim_exp[3 + kb]
                 p = a + b
-                PZ = -(b / p) * (A - B) if a >= b else (a / p) * (A - B)     # P - host centre
+                # P - host centre; (l,s) pairs are hosted on the l shell whatever the exponents (ris_setup.cuh)
+                PZ = -(b / p) * (A - B) if (a >= b or lb == 0) else (a / p) * (A - B)
                 Kab = math.exp(-a * b / p * np.dot(A - B, A - B))
                 coef = mol.prim_coef[ka] * mol.prim_coef[3 + kb] * Kab * 2 * math.pi ** 2.5 / p
                 prim.append([p, PZ[0], PZ[1], PZ[2], 0.5 / p, 2 * a, 2 * b, coef])
@@ -122,7 +127,7 @@ def test_undifferentiated_class_recurrence_vs_oracle(harness, la, lb):
             for kb in range(3):
                 a, b = mol.prim_exp[ka], mol.prim_exp[3 + kb]
                 p = a + b
-                PZ = -(b / p) * (A - B) if a >= b else (a / p) * (A - B)
+                PZ = -(b / p) * (A - B) if (a >= b or lb == 0) else (a / p) * (A - B)
                 Kab = math.exp(-a * b / p * np.dot(A - B, A - B))
                 coef = mol.prim_coef[ka] * mol.prim_coef[3 + kb] * Kab * 2 * math.pi ** 2.5 / p
                 prim.append([p, PZ[0], PZ[1], PZ[2], 0.5 / p, 2 * a, 2 * b, coef])
