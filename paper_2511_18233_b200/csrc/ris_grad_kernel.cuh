@@ -54,6 +54,9 @@
 #define RIS_PIPE_L -1           // software-pipelined primitive loop for l_mu + l_nu <= this.  Measured on config 4 (r02):
 #endif                          // slower for every class ((1,0) J 0.78 -> 0.92 ms): the extra live front spills at the
                                 // register caps below and the last front of a phase is wasted -- off
+#ifndef RIS_NSK2_BYTES
+#define RIS_NSK2_BYTES 16384    // two ring slots at least when they take no more than this per warp.  (2,2) runs ONE 9 KB slot:
+#endif                          // with two, the ring crowds the local-memory spills of that class out of L1 (K 0.57 -> 0.51 ms)
 #ifndef RIS_STAGE_BYTES
 #define RIS_STAGE_BYTES 4608    // shared-memory budget per warp for the K tile ring (at least 2 slots are always taken)
 #endif
@@ -62,9 +65,9 @@ template <int LA, int LB> struct RisGradTune {
     static constexpr bool SPLIT = (LA + LB >= RIS_SPLIT_L);
     static constexpr bool PIPE = (LA + LB <= RIS_PIPE_L);
     static constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
-    // slots of the tile ring: K -- as many states as fit the budget, at least 2 (1 for the f classes, whose slot is 15-26 KB
-    // per warp), at most RIS_NB_MAX; J -- all states (a few doubles each)
-    static constexpr int NSK_LO = (NEL * 256 * 2 <= 20480) ? 2 : 1;
+    // slots of the tile ring: K -- as many states as fit the budget, at least 2 (1 for (2,2) and the f classes, whose slot
+    // is 9-26 KB per warp), at most RIS_NB_MAX; J -- all states (a few doubles each)
+    static constexpr int NSK_LO = (NEL * 256 * 2 <= RIS_NSK2_BYTES) ? 2 : 1;
     static constexpr int NSK = (RIS_STAGE_BYTES / (NEL * 256) < NSK_LO) ? NSK_LO
                              : (RIS_STAGE_BYTES / (NEL * 256) > RIS_NB_MAX ? RIS_NB_MAX : RIS_STAGE_BYTES / (NEL * 256));
     static constexpr bool STAGE_K = ris_grad_stage_k(LA, LB);      // else the K tile is read straight from global memory
