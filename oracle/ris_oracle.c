@@ -27,6 +27,14 @@
  * finite differences, translational invariance, brute-force quadrature, far-aux limit.
  * Nothing in this file is "parity unpinned".
  *
+ * NEXT-2 ("a single GTO for each angular momentum component (up to l = 2) on each atom",
+ * PAPER.md:168 "s- and p-type for Coulomb, only s-type for exchange"): the J-fit auxiliary set may hold p-type functions.
+ * An auxiliary FUNCTION is (atom, l in {0,1}, Cartesian component i, exponent); the p function
+ *   chi_{P,i}(r) = N_p (r - C)_i exp(-alpha |r-C|^2),  N_p = (2 alpha/pi)^(3/4) 2 sqrt(alpha)   (normalised)
+ * is the centre derivative of the s primitive, (r-C)_i e^{..} = (1/2 alpha) d/dC_i e^{..}, so in the Hermite basis it only
+ * shifts the Coulomb tensor: [ab|p_i] = -(1/2 alpha) pref sum E_tuv R_{tuv + 1_i}.  mol->naux_fn = 0 selects the default
+ * set (one s function per atom, exponent aux_exponents[atom]).
+ *
  * Conventions: atomic units; row-major double arrays; Cartesian component order inside a
  * shell: lx descending, then ly descending (xx,xy,xz,yy,yz,zz; ...).  prim_coef is applied
  * as-is to UNnormalised primitives; the aux function carries N_P = (2 alpha/pi)^(3/4).
@@ -188,10 +196,25 @@ static real hsum(const real *Ex, int nx, const real *Ey, int ny, const real *Ez,
  *   d/dC_x[ab|P] = -pref sum E_tuv R^0_{t+1,u,v}              (explicit aux derivative)
  * out[0] = value, out[1..3] = d/dA, out[4..6] = d/dB, out[7..9] = d/dC.
  */
+void ris_oracle_prim3c_aux(const int la[3], const int lb[3], double a_, double b_, double alpha_,
+                           const double A[3], const double B[3], const double C[3], int aux_l, int aux_comp, double out[10]);
+
 void ris_oracle_prim3c(const int la[3], const int lb[3], double a_, double b_, double alpha_,
                        const double A[3], const double B[3], const double C[3], double out[10])
 {
+    ris_oracle_prim3c_aux(la, lb, a_, b_, alpha_, A, B, C, 0, 0, out);
+}
+
+/* The same for an unnormalised auxiliary primitive of type aux_l (0: s, 1: p with component aux_comp):
+ *   [ab|p_i] = (1/2 alpha) d/dC_i [ab|s] = -(1/2 alpha) pref sum E_tuv R_{tuv + 1_i}           (R depends on P - C)
+ * i.e. the Coulomb tensor is read with the shift sh = 1_i and the factor fP = -1/(2 alpha) (s: sh = 0, fP = 1);
+ * d/dC_d shifts once more and flips the sign. */
+void ris_oracle_prim3c_aux(const int la[3], const int lb[3], double a_, double b_, double alpha_,
+                           const double A[3], const double B[3], const double C[3], int aux_l, int aux_comp, double out[10])
+{
     real a = a_, b = b_, alpha = alpha_;
+    const int sh0 = (aux_l == 1 && aux_comp == 0), sh1 = (aux_l == 1 && aux_comp == 1), sh2 = (aux_l == 1 && aux_comp == 2);
+    const real fP = aux_l == 1 ? -1.0 / (2.0 * alpha) : 1.0;
     real p = a + b, rho = p * alpha / (p + alpha);
     real P[3], X[3];
     Etab E[3];
@@ -202,36 +225,36 @@ void ris_oracle_prim3c(const int la[3], const int lb[3], double a_, double b_, d
     }
     int L = la[0] + la[1] + la[2] + lb[0] + lb[1] + lb[2];
     Rtab *R = malloc(sizeof(Rtab));
-    hermite_R(L + 2, rho, X, *R);
-    real pref = 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
+    hermite_R(L + 2 + aux_l, rho, X, *R);
+    real pref = fP * 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
 #define EE(d, i, j) E[d][i][j], (i) + (j)
-    out[0] = pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R, 0, 0, 0);
+    out[0] = pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R, sh0, sh1, sh2);
     for (int d = 0; d < 3; ++d) {
         int ia[3] = {la[0], la[1], la[2]}, ib[3] = {lb[0], lb[1], lb[2]};
         real up, dn;
         /* bra centre A */
         ia[d] = la[d] + 1;
-        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, sh0, sh1, sh2);
         dn = 0.0;
         if (la[d] > 0) {
             ia[d] = la[d] - 1;
-            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, sh0, sh1, sh2);
         }
         out[1 + d] = pref * (2.0 * a * up - la[d] * dn);
         ia[d] = la[d];
         /* ket-side bra centre B */
         ib[d] = lb[d] + 1;
-        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+        up = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, sh0, sh1, sh2);
         dn = 0.0;
         if (lb[d] > 0) {
             ib[d] = lb[d] - 1;
-            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, 0, 0, 0);
+            dn = hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), *R, sh0, sh1, sh2);
         }
         out[4 + d] = pref * (2.0 * b * up - lb[d] * dn);
         ib[d] = lb[d];
         /* aux centre C, explicitly */
         out[7 + d] = -pref * hsum(EE(0, la[0], lb[0]), EE(1, la[1], lb[1]), EE(2, la[2], lb[2]), *R,
-                                  d == 0, d == 1, d == 2);
+                                  sh0 + (d == 0), sh1 + (d == 1), sh2 + (d == 2));
     }
 #undef EE
     free(R);
@@ -254,6 +277,29 @@ void ris_oracle_prim2c(double alpha_, double beta_, const double RP[3], const do
     for (int d = 0; d < 3; ++d) out[1 + d] = -2.0 * rho * X[d] * pref * F[1];
 }
 
+/* Two-centre integral between unnormalised auxiliary primitives of type (lP, iP) at RP and (lQ, iQ) at RQ (l in {0,1}):
+ * in the Hermite basis, with X = RP - RQ,
+ *   (Lambda_t^P | Lambda_u^Q) = (-1)^|u| kappa R_{t+u}(rho, X),  kappa = 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)),
+ * and p_i = Lambda_{1_i}/(2 exponent).  out[0] = value, out[1..3] = d/dR_P (= -d/dR_Q: a function of X only). */
+void ris_oracle_prim2c_lm(double alpha_, double beta_, int lP, int iP, int lQ, int iQ, const double RP[3], const double RQ[3],
+                          double out[4])
+{
+    real alpha = alpha_, beta = beta_;
+    real rho = alpha * beta / (alpha + beta);
+    real X[3] = {(real)RP[0] - RQ[0], (real)RP[1] - RQ[1], (real)RP[2] - RQ[2]};
+    Rtab *R = malloc(sizeof(Rtab));
+    hermite_R(lP + lQ + 1, rho, X, *R);
+    int sh[3] = {0, 0, 0};
+    if (lP == 1) sh[iP] += 1;
+    if (lQ == 1) sh[iQ] += 1;
+    real g = 2.0 * pow(PI, (real)2.5) / (alpha * beta * sqrt(alpha + beta));
+    if (lP == 1) g /= 2.0 * alpha;
+    if (lQ == 1) g /= -2.0 * beta;          /* (-1)^|u| */
+    out[0] = (double)(g * (*R)[sh[0]][sh[1]][sh[2]]);
+    for (int d = 0; d < 3; ++d) out[1 + d] = (double)(g * (*R)[sh[0] + (d == 0)][sh[1] + (d == 1)][sh[2] + (d == 2)]);
+    free(R);
+}
+
 /* ---------------------------------------------------------------- molecule description */
 typedef struct {
     int natoms;
@@ -261,8 +307,18 @@ typedef struct {
     int nshells;
     const int32_t *shell_atom, *shell_l, *shell_nprim, *shell_prim_off;
     const double *prim_exp, *prim_coef;
-    const double *aux_exponents;   /* [natoms] */
+    const double *aux_exponents;   /* [natoms]: the default set, one s function per atom */
+    /* optional explicit auxiliary FUNCTION list (NEXT-2, the J-fit set); naux_fn = 0: the default set above */
+    int naux_fn;
+    const int32_t *aux_atom, *aux_l, *aux_comp;    /* [naux_fn] */
+    const double *aux_exp;                         /* [naux_fn] */
 } ris_oracle_mol;
+
+static int aux_count(const ris_oracle_mol *m) { return m->naux_fn > 0 ? m->naux_fn : m->natoms; }
+static int aux_atom_of(const ris_oracle_mol *m, int P) { return m->naux_fn > 0 ? m->aux_atom[P] : P; }
+static int aux_l_of(const ris_oracle_mol *m, int P) { return m->naux_fn > 0 ? m->aux_l[P] : 0; }
+static int aux_comp_of(const ris_oracle_mol *m, int P) { return m->naux_fn > 0 ? m->aux_comp[P] : 0; }
+static double aux_exp_of(const ris_oracle_mol *m, int P) { return m->naux_fn > 0 ? m->aux_exp[P] : m->aux_exponents[P]; }
 
 static int ncart(int l) { return (l + 1) * (l + 2) / 2; }
 
@@ -276,6 +332,8 @@ static void cart_components(int l, int comp[][3])
 }
 
 static real aux_norm(real alpha) { return pow(2.0 * alpha / PI, (real)0.75); }
+/* normalised Cartesian p: N_p = (2 alpha/pi)^(3/4) (4 alpha)^(1/2) */
+static real aux_norm_l(real alpha, int l) { return l == 1 ? aux_norm(alpha) * 2.0 * sqrt(alpha) : aux_norm(alpha); }
 
 /* ---------------------------------------------------------------- O6: contraction for one aux P
  * For aux function P (on atom P) and nmat dense matrices G_s[nao][nao] with scale factors
@@ -301,10 +359,13 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
         ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
     }
     int nao = ao_off[nsh];
-    real alpha = mol->aux_exponents[P];
-    real NP = aux_norm(alpha);
-    const double *C = mol->coords + 3 * P;
-    int Pmasked = atom_mask ? atom_mask[P] : 1;
+    real alpha = aux_exp_of(mol, P);
+    const int lP = aux_l_of(mol, P), iP = aux_comp_of(mol, P), atP = aux_atom_of(mol, P);
+    /* s: Coulomb tensor as it is; p_i: shifted by 1_i, factor -1/(2 alpha) (see ris_oracle_prim3c_aux) */
+    const int sh0 = (lP == 1 && iP == 0), sh1 = (lP == 1 && iP == 1), sh2 = (lP == 1 && iP == 2);
+    real NP = lP == 1 ? aux_norm_l(alpha, 1) * (-1.0 / (2.0 * alpha)) : aux_norm(alpha);
+    const double *C = mol->coords + 3 * atP;
+    int Pmasked = atom_mask ? atom_mask[atP] : 1;
     size_t ng = (size_t)nmat * natoms * 3;
 
 #pragma omp parallel
@@ -349,35 +410,35 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
                             hermite_E(la + 1, lb + 1, a, b, (real)A[d] - Bc[d], E[d]);
                         }
                         Rtab R;
-                        hermite_R(la + lb + 2, rho, X, R);
+                        hermite_R(la + lb + 2 + lP, rho, X, R);
                         real pref = NP * da * db * 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
                         for (int ca = 0; ca < na; ++ca)
                             for (int cb = 0; cb < nb; ++cb) {
                                 const int *ia = compa[ca], *ib = compb[cb];
                                 real *o = buf + (ca * 10 + cb) * 10;
 #define EE(d, i, j) E[d][i][j], (i) + (j)
-                                o[0] += pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R, 0, 0, 0);
+                                o[0] += pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R, sh0, sh1, sh2);
                                 for (int d = 0; d < 3; ++d) {
                                     int ja[3] = {ia[0], ia[1], ia[2]}, jb[3] = {ib[0], ib[1], ib[2]};
                                     real up, dn = 0.0;
                                     ja[d] = ia[d] + 1;
-                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, sh0, sh1, sh2);
                                     if (ia[d] > 0) {
                                         ja[d] = ia[d] - 1;
-                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, sh0, sh1, sh2);
                                     }
                                     o[1 + d] += pref * (2.0 * a * up - ia[d] * dn);
                                     ja[d] = ia[d];
                                     jb[d] = ib[d] + 1;
-                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                    up = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, sh0, sh1, sh2);
                                     dn = 0.0;
                                     if (ib[d] > 0) {
                                         jb[d] = ib[d] - 1;
-                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, 0, 0, 0);
+                                        dn = hsum(EE(0, ja[0], jb[0]), EE(1, ja[1], jb[1]), EE(2, ja[2], jb[2]), R, sh0, sh1, sh2);
                                     }
                                     o[4 + d] += pref * (2.0 * b * up - ib[d] * dn);
                                     o[7 + d] += -pref * hsum(EE(0, ia[0], ib[0]), EE(1, ia[1], ib[1]), EE(2, ia[2], ib[2]), R,
-                                                             d == 0, d == 1, d == 2);
+                                                             sh0 + (d == 0), sh1 + (d == 1), sh2 + (d == 2));
                                 }
 #undef EE
                             }
@@ -395,7 +456,7 @@ int ris_oracle_contract_P(const ris_oracle_mol *mol, int P, int nmat, const doub
                             for (int d = 0; d < 3; ++d) {
                                 g[at_a * 3 + d] += w * o[1 + d];
                                 g[at_b * 3 + d] += w * o[4 + d];
-                                g[P * 3 + d] += w * o[7 + d];
+                                g[atP * 3 + d] += w * o[7 + d];
                             }
                         }
                 }
@@ -426,9 +487,11 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
         ao_off[s + 1] = ao_off[s] + ncart(mol->shell_l[s]);
     }
     int nao = ao_off[nsh];
-    real alpha = mol->aux_exponents[P];
-    real NP = aux_norm(alpha);
-    const double *C = mol->coords + 3 * P;
+    real alpha = aux_exp_of(mol, P);
+    const int lP = aux_l_of(mol, P), iP = aux_comp_of(mol, P);
+    const int sh0 = (lP == 1 && iP == 0), sh1 = (lP == 1 && iP == 1), sh2 = (lP == 1 && iP == 2);
+    real NP = lP == 1 ? aux_norm_l(alpha, 1) * (-1.0 / (2.0 * alpha)) : aux_norm(alpha);
+    const double *C = mol->coords + 3 * aux_atom_of(mol, P);
 #pragma omp parallel for schedule(dynamic, 1)
     for (int sa = 0; sa < nsh; ++sa) {
         int la = mol->shell_l[sa], na = ncart(la);
@@ -461,13 +524,13 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
                         hermite_E(la, lb, a, b, (real)A[d] - Bc[d], E[d]);
                     }
                     Rtab R;
-                    hermite_R(la + lb, rho, X, R);
+                    hermite_R(la + lb + lP, rho, X, R);
                     real pref = NP * da * db * 2.0 * pow(PI, (real)2.5) / (p * alpha * sqrt(p + alpha));
                     for (int ca = 0; ca < na; ++ca)
                         for (int cb = 0; cb < nb; ++cb) {
                             const int *ia = compa[ca], *ib = compb[cb];
                             buf[ca * 10 + cb] += pref * hsum(E[0][ia[0]][ib[0]], ia[0] + ib[0], E[1][ia[1]][ib[1]], ia[1] + ib[1],
-                                                             E[2][ia[2]][ib[2]], ia[2] + ib[2], R, 0, 0, 0);
+                                                             E[2][ia[2]][ib[2]], ia[2] + ib[2], R, sh0, sh1, sh2);
                         }
                 }
             }
@@ -487,19 +550,22 @@ int ris_oracle_int3c_P(const ris_oracle_mol *mol, int P, double prim_cutoff, dou
 int ris_oracle_grad_PQ(const ris_oracle_mol *mol, int nbatch, const double *c, const double *dq,
                        long double *gacc, long double *eacc)
 {
-    int n = mol->natoms;
+    int n = aux_count(mol), nat = mol->natoms;
     for (int s = 0; s < nbatch; ++s)
         for (int P = 0; P < n; ++P)
             for (int Q = 0; Q < n; ++Q) {
                 double o[4];
-                double aP = mol->aux_exponents[P], aQ = mol->aux_exponents[Q];
-                ris_oracle_prim2c(aP, aQ, mol->coords + 3 * P, mol->coords + 3 * Q, o);
-                long double w = (long double)c[s * n + P] * dq[s * n + Q] * (double)aux_norm(aP) * (double)aux_norm(aQ);
+                double aP = aux_exp_of(mol, P), aQ = aux_exp_of(mol, Q);
+                int lP = aux_l_of(mol, P), lQ = aux_l_of(mol, Q), atP = aux_atom_of(mol, P), atQ = aux_atom_of(mol, Q);
+                if (lP == 0 && lQ == 0) ris_oracle_prim2c(aP, aQ, mol->coords + 3 * atP, mol->coords + 3 * atQ, o);
+                else ris_oracle_prim2c_lm(aP, aQ, lP, aux_comp_of(mol, P), lQ, aux_comp_of(mol, Q), mol->coords + 3 * atP,
+                                          mol->coords + 3 * atQ, o);
+                long double w = (long double)c[s * n + P] * dq[s * n + Q] * (double)aux_norm_l(aP, lP) * (double)aux_norm_l(aQ, lQ);
                 eacc[s] += w * o[0];
-                if (P == Q) continue;
+                if (atP == atQ) continue;          /* both functions move together: the integral depends on R_P - R_Q only */
                 for (int d = 0; d < 3; ++d) {
-                    gacc[((size_t)s * n + P) * 3 + d] += w * o[1 + d];
-                    gacc[((size_t)s * n + Q) * 3 + d] -= w * o[1 + d];
+                    gacc[((size_t)s * nat + atP) * 3 + d] += w * o[1 + d];
+                    gacc[((size_t)s * nat + atQ) * 3 + d] -= w * o[1 + d];
                 }
             }
     return 0;

@@ -51,7 +51,10 @@ class _Mol(C.Structure):
     _fields_ = [("natoms", C.c_int), ("coords", C.c_void_p), ("nshells", C.c_int),
                 ("shell_atom", C.c_void_p), ("shell_l", C.c_void_p), ("shell_nprim", C.c_void_p),
                 ("shell_prim_off", C.c_void_p), ("prim_exp", C.c_void_p), ("prim_coef", C.c_void_p),
-                ("aux_exponents", C.c_void_p)]
+                ("aux_exponents", C.c_void_p),
+                # explicit auxiliary function list (NEXT-2: the J-fit set with p functions); naux_fn = 0: default set
+                ("naux_fn", C.c_int), ("aux_atom", C.c_void_p), ("aux_l", C.c_void_p), ("aux_comp", C.c_void_p),
+                ("aux_exp", C.c_void_p)]
 
 
 class extended_precision:
@@ -82,6 +85,10 @@ def _load(so):
         _lib.ris_oracle_prim3c.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double,
                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.ris_oracle_prim2c.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.ris_oracle_prim3c_aux.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double,
+                                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        _lib.ris_oracle_prim2c_lm.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                              C.c_void_p, C.c_void_p]
         _lib.ris_oracle_contract_P.argtypes = [C.POINTER(_Mol), C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
         _lib.ris_oracle_contract_P.restype = C.c_int
@@ -104,10 +111,28 @@ def _i32(x):
     return np.ascontiguousarray(x, dtype=np.int32)
 
 
-class _Held:
-    """Keeps the numpy buffers alive next to the C struct."""
+def jfit_functions(mol):
+    """The J-fit auxiliary FUNCTIONS of `mol` as arrays (atom, l, component, exponent), or None when the molecule carries
+    no explicit J-fit set (then J and K share the default set: one s function per atom).  mol.jfit = (atom[], l[], exp[])
+    lists auxiliary SHELLS with l in {0, 1}; a p shell expands into its x, y, z components, in that order."""
+    jf = getattr(mol, "jfit", None)
+    if jf is None:
+        return None
+    at, ll, ex = (np.asarray(x) for x in jf)
+    fa, fl, fc, fe = [], [], [], []
+    for a, l, e in zip(at, ll, ex):
+        assert int(l) in (0, 1), "auxiliary shells are s or p"
+        for comp in range(1 if int(l) == 0 else 3):
+            fa.append(int(a)); fl.append(int(l)); fc.append(comp); fe.append(float(e))
+    return _i32(fa), _i32(fl), _i32(fc), _f64(fe)
 
-    def __init__(self, mol):
+
+class _Held:
+    """Keeps the numpy buffers alive next to the C struct.  jfit=True: the J-type calls see the molecule's J-fit auxiliary
+    set (if it has one); the K-type calls always see the default set."""
+
+    def __init__(self, mol, jfit=False):
+        self.aux = jfit_functions(mol) if jfit else None
         self.arrs = dict(coords=_f64(mol.coords), shell_atom=_i32(mol.shell_atom), shell_l=_i32(mol.shell_l),
                          shell_nprim=_i32(mol.shell_nprim), shell_prim_off=_i32(mol.shell_prim_off),
                          prim_exp=_f64(mol.prim_exp), prim_coef=_f64(mol.prim_coef),
@@ -119,7 +144,14 @@ class _Held:
                                        for at, l in zip(a["shell_atom"], a["shell_l"])]).astype(np.int64)
         self.c = _Mol(self.natoms, a["coords"].ctypes.data, a["shell_l"].shape[0], a["shell_atom"].ctypes.data,
                       a["shell_l"].ctypes.data, a["shell_nprim"].ctypes.data, a["shell_prim_off"].ctypes.data,
-                      a["prim_exp"].ctypes.data, a["prim_coef"].ctypes.data, a["aux_exponents"].ctypes.data)
+                      a["prim_exp"].ctypes.data, a["prim_coef"].ctypes.data, a["aux_exponents"].ctypes.data,
+                      0, None, None, None, None)
+        self.naux = self.natoms
+        if self.aux is not None:
+            fa, fl, fc, fe = self.aux
+            self.naux = int(fa.shape[0])
+            self.c.naux_fn = self.naux
+            self.c.aux_atom, self.c.aux_l, self.c.aux_comp, self.c.aux_exp = (x.ctypes.data for x in (fa, fl, fc, fe))
 
 
 def boys(mmax: int, T: float) -> np.ndarray:
@@ -135,6 +167,24 @@ def prim3c(la, lb, a, b, alpha, A, B, Cc) -> np.ndarray:
     out = np.zeros(10)
     lib().ris_oracle_prim3c(la.ctypes.data, lb.ctypes.data, a, b, alpha, A.ctypes.data, B.ctypes.data,
                             Cc.ctypes.data, out.ctypes.data)
+    return out
+
+
+def prim3c_aux(la, lb, a, b, alpha, A, B, Cc, aux_l, aux_comp) -> np.ndarray:
+    """As prim3c for an unnormalised auxiliary primitive of type aux_l (0: s; 1: p, component aux_comp)."""
+    la, lb = _i32(la), _i32(lb)
+    A, B, Cc = _f64(A), _f64(B), _f64(Cc)
+    out = np.zeros(10)
+    lib().ris_oracle_prim3c_aux(la.ctypes.data, lb.ctypes.data, a, b, alpha, A.ctypes.data, B.ctypes.data,
+                                Cc.ctypes.data, int(aux_l), int(aux_comp), out.ctypes.data)
+    return out
+
+
+def prim2c_lm(alpha, beta, lP, iP, lQ, iQ, RP, RQ) -> np.ndarray:
+    """[value, d/dR_P(3)] of the two-centre integral between unnormalised s / p auxiliary primitives."""
+    RP, RQ = _f64(RP), _f64(RQ)
+    out = np.zeros(4)
+    lib().ris_oracle_prim2c_lm(alpha, beta, int(lP), int(iP), int(lQ), int(iQ), RP.ctypes.data, RQ.ctypes.data, out.ctypes.data)
     return out
 
 
@@ -164,14 +214,14 @@ def _finish(g, e, mask):
 
 def grad_J(mol, D, c_aux, *, atoms=None, prim_cutoff=0.0, aux=None):
     """G_J and E_J = sum D_{mu nu} c_P (mu nu|P).  D [nbatch][nao][nao] (any symmetry), c [nbatch][naux]."""
-    h = _Held(mol)
+    h = _Held(mol, jfit=True)
     D = _f64(D).reshape(-1, h.nao, h.nao)
-    c_aux = _f64(c_aux).reshape(D.shape[0], h.natoms)
+    c_aux = _f64(c_aux).reshape(D.shape[0], h.naux)
     nb = D.shape[0]
     mask = _mask(h.natoms, atoms)
     g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
     e = np.zeros(nb, dtype=np.longdouble)
-    for P in (range(h.natoms) if aux is None else aux):
+    for P in (range(h.naux) if aux is None else aux):
         sc = _f64(c_aux[:, P])
         rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, sc.ctypes.data,
                                          mask.ctypes.data if mask is not None else None, prim_cutoff,
@@ -215,9 +265,9 @@ def grad_K(mol, C_occ, C_vir, B, *, atoms=None, prim_cutoff=0.0, aux=None):
 
 def grad_PQ(mol, c_aux, d_aux):
     """G_PQ and E_PQ = sum_{PQ} c_P d_Q (P|Q) (positive sign; Eq. 27's minus is the caller's)."""
-    h = _Held(mol)
-    c_aux = _f64(c_aux).reshape(-1, h.natoms)
-    d_aux = _f64(d_aux).reshape(-1, h.natoms)
+    h = _Held(mol, jfit=True)
+    c_aux = _f64(c_aux).reshape(-1, h.naux)
+    d_aux = _f64(d_aux).reshape(-1, h.naux)
     nb = c_aux.shape[0]
     g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
     e = np.zeros(nb, dtype=np.longdouble)
@@ -235,13 +285,13 @@ def grad_PQ(mol, c_aux, d_aux):
 # and, for fixed symmetric-or-not D, Eq. 27 gives
 #   dE_RIJ/dxi = sum_P c_P v_P^xi - 1/2 c^T M^xi c = G_J(D, c) - 1/2 G_PQ(c, c).
 def vec_J(mol, D, *, prim_cutoff=0.0):
-    """v[s][P] = sum_{mu nu} D^s_{mu nu} (mu nu|P) over all ordered (mu, nu)."""
-    h = _Held(mol)
+    """v[s][P] = sum_{mu nu} D^s_{mu nu} (mu nu|P) over all ordered (mu, nu); P runs over the J-fit set."""
+    h = _Held(mol, jfit=True)
     D = _f64(D).reshape(-1, h.nao, h.nao)
     nb = D.shape[0]
     one = np.ones(nb)
-    v = np.zeros((nb, h.natoms))
-    for P in range(h.natoms):
+    v = np.zeros((nb, h.naux))
+    for P in range(h.naux):
         g = np.zeros((nb, h.natoms, 3), dtype=np.longdouble)
         e = np.zeros(nb, dtype=np.longdouble)
         rc = lib().ris_oracle_contract_P(C.byref(h.c), P, nb, D.ctypes.data, one.ctypes.data, None, prim_cutoff,
@@ -264,10 +314,27 @@ def metric(mol):
     return M
 
 
+def metric_J(mol):
+    """The metric of the J-fit set: M[f][g] = N_f N_g (f|g) over s and p functions (Eq. 22; the set of
+    PAPER.md:125 / 168).  Without an explicit J-fit set this is metric(mol)."""
+    fn = jfit_functions(mol)
+    if fn is None:
+        return metric(mol)
+    fa, fl, fc, fe = fn
+    R = _f64(mol.coords)
+    n = fa.shape[0]
+    N = (2.0 * fe / np.pi) ** 0.75 * np.where(fl == 1, 2.0 * np.sqrt(fe), 1.0)
+    M = np.zeros((n, n))
+    for P in range(n):
+        for Q in range(n):
+            M[P, Q] = N[P] * N[Q] * prim2c_lm(fe[P], fe[Q], fl[P], fc[P], fl[Q], fc[Q], R[fa[P]], R[fa[Q]])[0]
+    return M
+
+
 def fit_J(mol, D, *, prim_cutoff=0.0):
-    """(v, c, E_RIJ): c = M^-1 v, E_RIJ[s] = 1/2 v[s].c[s]."""
+    """(v, c, E_RIJ): c = M^-1 v, E_RIJ[s] = 1/2 v[s].c[s]; M = the J-fit metric."""
     v = vec_J(mol, D, prim_cutoff=prim_cutoff)
-    c = np.linalg.solve(metric(mol), v.T).T
+    c = np.linalg.solve(metric_J(mol), v.T).T
     return v, c, 0.5 * np.einsum("sp,sp->s", v, c)
 
 
