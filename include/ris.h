@@ -8,8 +8,10 @@
  *       [sum_AB (pq|A) M^-1_AB (B|sr)]^xi = sum (pq|A)^xi M^-1 (B|sr) + sum (pq|A) M^-1 (B|sr)^xi
  *                                           - sum (pq|A) M^-1 M^xi M^-1 (B|sr),
  *   with the three-centre integrals (pq|A) and the metric M_AB = (A|B) of Eqs. 21-22
- *   over the minimal auxiliary basis of ONE s-type Gaussian per atom, contracted
- *   with everything that is not an integral derivative:
+ *   over the minimal auxiliary basis (one GTO per angular-momentum component and atom; the paper's
+ *   runs use s AND p functions for the Coulomb term and s functions only for exchange) -- the default set
+ *   here is ONE s-type Gaussian per atom for both terms, ris_set_jfit gives the J-type calls an s + p set of their own --
+ *   contracted with everything that is not an integral derivative:
  *
  *   ris_grad_J :  G[s][A][x] = sum_{mu nu} sum_P D^s_{mu nu} c^s_P  d(mu nu|P)/dR_{A,x}       (terms 1-2, Coulomb)
  *   ris_grad_K :  G[s][A][x] = sum_P sum_{mu nu} Gamma^{s,P}_{mu nu} d(mu nu|P)/dR_{A,x},
@@ -90,7 +92,7 @@ int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, cons
               const ris_options* opt, void* cuda_stream);
 
 /* J-type contraction.  D device [nbatch][nao][nao] (symmetric or not: only D + D^T contributes),
- * c_aux device [nbatch][naux], grad device [nbatch][natoms][3]. */
+ * c_aux device [nbatch][naux_J] (naux_J = naux unless ris_set_jfit was called), grad device [nbatch][natoms][3]. */
 int ris_grad_J(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, double* grad);
 
 /* K-type contraction.  C_occ device [nao][nocc], C_vir device [nao][nvir] ("occ"/"vir" are just the
@@ -98,7 +100,7 @@ int ris_grad_J(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, d
 int ris_grad_K(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                const double* B, double* grad);
 
-/* Two-centre term.  c_aux, d_aux device [nbatch][naux], grad device [nbatch][natoms][3]. */
+/* Two-centre term.  c_aux, d_aux device [nbatch][naux_J], grad device [nbatch][natoms][3]. */
 int ris_grad_PQ(ris_ctx* ctx, int nbatch, const double* c_aux, const double* d_aux, double* grad);
 
 /* ---- Fitting step, J type (Eqs. 21-22) --------------------------------
@@ -139,6 +141,19 @@ int ris_grad_PQ_host(ris_ctx* ctx, int nbatch, const double* c_aux, const double
 int ris_grad_host(ris_ctx* ctx, int nbatch_J, const double* D, const double* c_aux, const double* d_aux, int nbatch_K,
                   int nocc, int nvir, const double* C_occ, const double* C_vir, const double* B, double* grad_J,
                   double* grad_K, double* grad_PQ);
+
+/* ---- J-fit auxiliary set with p functions -----------------------------------
+ * ris_set_jfit replaces, for the J-TYPE calls only (ris_grad_J, ris_fit_J, ris_grad_PQ and their *_host forms, ris_metric_J),
+ * the default set by nshell_aux auxiliary SHELLS: shell k sits on atom aux_atom[k], has l = aux_l[k] in {0, 1} and exponent
+ * aux_exp[k] (host arrays, copied).  The set's FUNCTIONS are the shells in input order, a p shell expanding into x, y, z:
+ *     s:  N exp(-alpha |r-C|^2),            N = (2 alpha/pi)^(3/4)
+ *     p:  N (r-C)_i exp(-alpha |r-C|^2),    N = (2 alpha/pi)^(3/4) 2 sqrt(alpha)      (unit self-overlap, as the s function)
+ * c_aux / d_aux / v / c then have ris_naux_J() entries per state in that order.  The K-type calls (ris_grad_K, ris_fit_K,
+ * ris_metric, ris_grad_PQ_full) keep the default s set, as in the paper's runs.  May be called again (new set);
+ * RIS_EINVAL for l > 1, an atom out of range or a non-positive exponent.  ris_metric_J: M_out device [naux_J][naux_J]. */
+int ris_set_jfit(ris_ctx* ctx, int nshell_aux, const int32_t* aux_atom, const int32_t* aux_l, const double* aux_exp);
+int ris_naux_J(const ris_ctx* ctx);
+int ris_metric_J(ris_ctx* ctx, double* M_out);
 
 int ris_destroy(ris_ctx* ctx);
 const char* ris_strerror(int status);

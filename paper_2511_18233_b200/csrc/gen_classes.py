@@ -363,6 +363,106 @@ def gen_hrr0w(pl: ClassPlan0) -> str:
     return "\n".join(out)
 
 
+
+# --------------------------------------------------------------------------- p-type auxiliary functions (NEXT-2)
+# PAPER.md:125 ("a single GTO for each angular momentum component (up to l = 2) on each atom"), PAPER.md:168 ("s- and
+# p-type for Coulomb").  The aux function is (r-C)_i exp(-alpha |r-C|^2); one more Obara-Saika step, on the aux centre,
+#   [a b|p_i]^(m) = WC_i [a b|s]^(m+1) + a_i/(2(p+alpha)) [a-1_i b|s]^(m+1) + b_i/(2(p+alpha)) [a b-1_i|s]^(m+1),
+#   WC = W - C = (1 - rho/p)(P - C),
+# turns the s-aux integrals of one Boys order higher into the targets; the bra HRR and the contraction code are the ones
+# of the s-aux class (same target layout).  Emission is a memoised recursion over ([a], b in {0, 1_j}, ket in {s, p_i}, m).
+
+class Emitter:
+    def __init__(self, w, direct_names):
+        self.w = w
+        self.memo = {}
+        self.dn = direct_names     # argument names: PA, WP, PB lists, WC scalar name, ...
+
+    def k(self, n):                # n / (2p)
+        return f"k{n}"
+
+    def get(self, a, b, ket, m):
+        """name of [a b|ket]^(m); a: bra triple on the host; b: None or direction j of a p function on the other (s) centre;
+        ket: None (s aux) or direction i (p aux)."""
+        key = (a, b, ket, m)
+        if key in self.memo:
+            return self.memo[key]
+        w = self.w
+        if ket is not None:
+            i = ket
+            terms = [f"WC * {self.get(a, b, None, m + 1)}"]
+            if a[i] >= 1:
+                terms.append(f"{float(a[i])} * oo2pa * {self.get(lower(a, i), b, None, m + 1)}")
+            if b == i:
+                terms.append(f"oo2pa * {self.get(a, None, None, m + 1)}")
+            name = f"t{sum(a)}_{cidx(a)}_{'n' if b is None else b}_{m}"
+            w(f"    const double {name} = " + " + ".join(terms) + ";")
+        elif b is not None:
+            j = b
+            expr = f"fma(PB{j}, {self.get(a, None, None, m)}, WP{j} * {self.get(a, None, None, m + 1)})"
+            if a[j] >= 1:
+                expr = f"fma({self.k(a[j])}, {self.bracket(lower(a, j), m)}, {expr})"
+            name = f"u{sum(a)}_{cidx(a)}_{j}_{m}"
+            w(f"    const double {name} = {expr};")
+        elif sum(a) == 0:
+            name = f"F[{m}]"
+        else:
+            ones = [d for d in range(3) if a[d] == 1]
+            d = ones[0] if ones else min((x for x in range(3) if a[x] > 0), key=lambda x: a[x])
+            a1 = lower(a, d)
+            expr = f"fma(PA{d}, {self.get(a1, None, None, m)}, WP{d} * {self.get(a1, None, None, m + 1)})"
+            if a[d] >= 2:
+                expr = f"fma({self.k(a[d] - 1)}, {self.bracket(lower(a, d, 2), m)}, {expr})"
+            name = f"v{sum(a)}_{cidx(a)}_{m}"
+            w(f"    const double {name} = {expr};")
+        self.memo[key] = name
+        return name
+
+    def bracket(self, a, m):
+        key = ("br", a, m)
+        if key not in self.memo:
+            name = f"b{sum(a)}_{cidx(a)}_{m}"
+            self.w(f"    const double {name} = fma(-q, {self.get(a, None, None, m + 1)}, {self.get(a, None, None, m)});")
+            self.memo[key] = name
+        return self.memo[key]
+
+
+def gen_vrr_p(pl, i: int) -> str:
+    """VRR + accumulation of the targets [e0|p_i] (and, for the direct classes, 2b [a,1_j|p_i]) of plan `pl` (ClassPlan or
+    ClassPlan0) for the p aux component i.  F holds kappa F_m, m = 0 .. E+1."""
+    la, lb, E = pl.la, pl.lb, pl.E
+    direct = getattr(pl, "direct_b", False)
+    out = []
+    w = out.append
+    w(f"// class ({la},{lb}), p-type aux component {i}: {pl.nacc} contracted targets")
+    w("template <class ACC>")
+    w(f"RIS_DEV void {pl.vrr_name.replace('ris_vrr', 'ris_vrrp')}_{i}(const double (&F)[{E + 2}], double PA0, double PA1, double PA2,")
+    w("    double WP0, double WP1, double WP2, double oo2p, double q, double a2, double b2,")
+    w("    ACC& acc, double WC, double oo2pa" + (", double PB0, double PB1, double PB2)" if direct else ")"))
+    w("{")
+    for n in range(1, E + 2):
+        w(f"    const double k{n} = {float(n)} * oo2p;")
+    em = Emitter(w, None)
+    for e in range(0, E + 1):
+        for c in comps(e):
+            val = None
+            for tag, rng, scale in pl.fams:
+                if e not in rng:
+                    continue
+                if val is None:
+                    val = em.get(c, None, i, 0)
+                if scale:
+                    w(f"    {pl.acc(tag, e, c)} = fma({scale}, {val}, {pl.acc(tag, e, c)});")
+                else:
+                    w(f"    {pl.acc(tag, e, c)} += {val};")
+    if direct:
+        for c in comps(la):
+            for j in range(3):
+                w(f"    {pl.acc_bd(c, j)} = fma(b2, {em.get(c, j, i, 0)}, {pl.acc_bd(c, j)});")
+    w("}")
+    return "\n".join(out)
+
+
 def generate() -> str:
     parts = ["// GENERATED by gen_classes.py -- do not edit.  See that file for the recurrences.",
              "#pragma once", ""]
@@ -389,6 +489,11 @@ def generate() -> str:
         parts.append("")
         parts.append(gen_hrr0w(p0))
         parts.append("")
+        for i in range(3):
+            parts.append(gen_vrr_p(pl, i))
+            parts.append("")
+            parts.append(gen_vrr_p(p0, i))
+            parts.append("")
     # dispatch helpers
     parts.append("template <int LA, int LB, class... A> RIS_DEV void ris_vrr(A&&... a) {")
     for la, lb in classes:
@@ -398,6 +503,12 @@ def generate() -> str:
     for la, lb in classes:
         parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_vrr0_{la}{lb}(static_cast<A&&>(a)...);")
     parts.append("}")
+    for nm in ("ris_vrrp", "ris_vrrp0"):
+        parts.append(f"template <int LA, int LB, int DIR, class... A> RIS_DEV void {nm}(A&&... a) {{")
+        for la, lb in classes:
+            for i in range(3):
+                parts.append(f"    if constexpr (LA == {la} && LB == {lb} && DIR == {i}) {nm}_{la}{lb}_{i}(static_cast<A&&>(a)...);")
+        parts.append("}")
     parts.append("template <int LA, int LB, bool TR, int SL, class... A> RIS_DEV void ris_hrr0c(A&&... a) {")
     for la, lb in classes:
         parts.append(f"    if constexpr (LA == {la} && LB == {lb}) ris_hrr0c_{la}{lb}<TR, SL>(static_cast<A&&>(a)...);")

@@ -53,13 +53,23 @@ struct ris_ctx {
     ris_options opt{};
     int natoms = 0, nshells = 0, nao = 0, naux = 0;
     double* d_coords = nullptr;
-    double* d_aux = nullptr;           // [naux][5]
+    double* d_aux = nullptr;           // [naux][RIS_AUX_FIELDS] the default set: one s function per atom (K type; J type too
+                                       // unless ris_set_jfit gave the J term a set of its own)
+    // J-fit set (NEXT-2): s and p functions.  Without ris_set_jfit these alias the default set.
+    bool jfit = false;
+    int naux_J = 0;                    // functions of the J-fit set
+    double* d_jfn = nullptr;           // [naux_J][RIS_AUX_FIELDS] records in FUNCTION order (two-centre kernels)
+    double* d_jlist[4] = {nullptr};    // the same records grouped by type: s, p_x, p_y, p_z (class kernels: one launch each)
+    int jcnt[4] = {0, 0, 0, 0};
+    int *d_atom_fn_off = nullptr, *d_atom_fn = nullptr;   // CSR atom -> functions of the J-fit set
+    double* d_chol_J = nullptr;        // Cholesky factor of the J-fit metric (explicit set only; else d_chol)
     int *d_shell_atom = nullptr, *d_shell_l = nullptr, *d_shell_nprim = nullptr, *d_shell_poff = nullptr, *d_shell_ao = nullptr;
     double *d_pexp = nullptr, *d_pcoef = nullptr;
     RisClassPack cls[RIS_NCLASS]{};
     std::vector<void*> owned;          // every device allocation of the packed data
+    std::vector<double> h_coords;      // host copy of the geometry (ris_set_jfit places its functions on the atoms)
     long long nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
-    double* d_boys[8] = {nullptr};
+    double* d_boys[9] = {nullptr};     // Boys tables of top order M = 0..8 (M = 8: d/dR of (ff|p))
     double* d_minv = nullptr;          // [naux][nauxp] inverse metric (built by the first ris_fit_K)
     // band of the spatially ordered AO index per 64-row block (from the GEMM-2 block list): columns
     // [rb_jlo*64, (rb_jlo*64 + rb_kw)) hold every surviving partner of the block's rows
@@ -198,7 +208,7 @@ static const char* const kGradNames[RIS_NCLASS] = {
     "ris_grad_kernel<2,2>", "ris_grad_kernel<3,0>", "ris_grad_kernel<3,1>", "ris_grad_kernel<3,2>", "ris_grad_kernel<3,3>"};
 // Algorithmic FP64 flops per primitive triplet by E = la + lb + 1 (SURVEY.md 8(d) model: setup ~45, Boys ~30 + 4E,
 // 7 flops per OS-VRR intermediate, scaled accumulation), plus 12 nca ncb flops per contracted triplet and state.
-static const double kModelFlopsByE[8] = {90.0, 140.0, 250.0, 450.0, 750.0, 1250.0, 2000.0, 3100.0};
+static const double kModelFlopsByE[9] = {90.0, 140.0, 250.0, 450.0, 750.0, 1250.0, 2000.0, 3100.0, 4600.0};
 // heaviest class first (flops per primitive triplet), so the tail is made of light kernels
 static const int kClassOrder[RIS_NCLASS] = {9, 8, 7, 5, 6, 4, 3, 2, 1, 0};
 
@@ -282,6 +292,17 @@ static unsigned long long morton3(const double* r, const double* lo)
     return code;
 }
 
+// One auxiliary-function record: centre, exponent, N/alpha, then (atom, function index), (l, component) as int pairs.
+//   s: N = (2 alpha/pi)^(3/4);   p_i: N (r - C)_i exp(-alpha |r-C|^2) with N = (2 alpha/pi)^(3/4) 2 sqrt(alpha)
+static void aux_record(double* r, const double* xyz, double al, int l, int comp, int atom, int fn)
+{
+    const double N = std::pow(2.0 * al / M_PI, 0.75) * (l == 1 ? 2.0 * std::sqrt(al) : 1.0);
+    r[0] = xyz[0]; r[1] = xyz[1]; r[2] = xyz[2]; r[3] = al; r[4] = N / al;
+    const int ids[4] = {atom, fn, l, comp};
+    std::memcpy(r + 5, ids, sizeof ids);
+    r[7] = 0.0;
+}
+
 extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int nshells, const int32_t* shell_atom,
                          const int32_t* shell_l, const int32_t* shell_nprim, const int32_t* shell_prim_off,
                          const double* prim_exp, const double* prim_coef, const double* aux_exponents,
@@ -332,24 +353,24 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     if ((rc = dev_upload(c, &c->d_pexp, prim_exp, (size_t)nprim_tot))) return rc;
     if ((rc = dev_upload(c, &c->d_pcoef, prim_coef, (size_t)nprim_tot))) return rc;
 
-    // aux records {Cx,Cy,Cz,alpha,N_P/alpha} and the potential maximum used by the screening bound
-    std::vector<double> aux((size_t)5 * natoms);
+    // aux records (ris_internal.h: RisGradParams::aux) and the potential maximum used by the screening bound
+    std::vector<double> aux((size_t)RIS_AUX_FIELDS * natoms);
     double vmax = 0.0;
     for (int P = 0; P < natoms; ++P) {
-        const double al = aux_exponents[P], N = std::pow(2.0 * al / M_PI, 0.75);
-        aux[5 * P + 0] = coords[3 * P]; aux[5 * P + 1] = coords[3 * P + 1]; aux[5 * P + 2] = coords[3 * P + 2];
-        aux[5 * P + 3] = al; aux[5 * P + 4] = N / al;
-        vmax = std::max(vmax, N * 2.0 * M_PI / al);
+        aux_record(&aux[(size_t)RIS_AUX_FIELDS * P], coords + 3 * P, aux_exponents[P], 0, 0, P, P);
+        vmax = std::max(vmax, std::pow(2.0 * aux_exponents[P] / M_PI, 0.75) * 2.0 * M_PI / aux_exponents[P]);
     }
     if ((rc = dev_upload(c, &c->d_aux, aux.data(), aux.size()))) return rc;
+    c->h_coords.assign(coords, coords + 3 * (size_t)natoms);
+    c->naux_J = natoms; c->d_jfn = c->d_aux; c->d_jlist[0] = c->d_aux; c->jcnt[0] = natoms;
 
-    // Boys tables, one per top order M = 0..7 (M = 0: the undifferentiated (ss|P) of the fitting step)
+    // Boys tables, one per top order M = 0..8 (M = 0: the undifferentiated (ss|P) of the fitting step)
     // (geometry-independent: the host tables are built once per process, in long double, and kept)
     {
-        static std::vector<double> tabs[8];
+        static std::vector<double> tabs[9];
         static std::mutex tabs_mu;
         std::lock_guard<std::mutex> lk(tabs_mu);
-        for (int M = 0; M <= 7; ++M) {
+        for (int M = 0; M <= 8; ++M) {
             if (tabs[M].empty()) ris_build_boys_table(M, RIS_BOYS_NGRID, RIS_BOYS_PER_UNIT, tabs[M]);
             if ((rc = dev_upload(c, &c->d_boys[M], tabs[M].data(), tabs[M].size()))) return rc;
         }
@@ -585,9 +606,14 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
 }
 
 // One launch per class, heaviest class first.  tile / sstride / estride / lstride: see RisGradParams.
+// aux / aux_type / naux_row: the list of auxiliary functions of this pass (records, type 0 = s, 1..3 = p_x..p_z) and the row
+// length of cscale; [p0, p1) = range of list positions.
 static int launch_classes(ris_ctx* c, const double* tile, long long sstride, long long estride, int lstride,
-                          const double* cscale, int nb, int p0, int p1, double* grad, unsigned long long* det)
+                          const double* cscale, int nb, int p0, int p1, double* grad, unsigned long long* det,
+                          const double* aux = nullptr, int aux_type = 0, int naux_row = 0)
 {
+    if (!aux) { aux = c->d_aux; naux_row = c->naux; }
+    const int eb = aux_type ? 2 : 1;       // Boys order above la + lb: the derivative, and the step on a p aux centre
     const int ny = (p1 - p0 + 31) / 32;
     int* ctr;
     // two ticket arrays per class: the heavy classes run their host-centre phases as two launches
@@ -618,13 +644,14 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         if (side) CU(cudaStreamWaitEvent(st, c->fork_ev, 0));
         RisGradParams p{};
         p.task_ctr = ctr + (size_t)2 * k * ny;
-        p.pk = pk; p.naux = c->naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb + 1];
+        p.pk = pk; p.naux = naux_row; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = aux; p.aux_type = aux_type;
+        p.boys = c->d_boys[pk.la + pk.lb + eb];
         p.tile = tile; p.sstride = sstride; p.estride = estride; p.lstride = lstride; p.cscale = cscale; p.nb = nb;
         p.p0 = p0; p.p1 = p1;
         p.grad = grad; p.det = det; p.det_flag = det ? (int*)c->ws[WS_DET] : nullptr;
         const double np_ = (double)(p1 - p0), nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
         {
-            ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + 1] + 12.0 * nel * pk.npairs * nb),
+            ProfScope ps(c, kGradNames[k], np_ * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + eb] + 12.0 * nel * pk.npairs * nb),
                          8.0 * (lstride ? np_ : 1.0) * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS, st, false);
             CU(ris_grad_launchers[k](p, st));
         }
@@ -704,9 +731,12 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
         int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile);
         if (rc) return rc;
         if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
-        if ((rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux, nb, 0, c->naux,
-                                 grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
-            return rc;
+        for (int t = 0; t < 4; ++t)         // one pass per type of auxiliary function: s, p_x, p_y, p_z
+            if (c->jcnt[t] > 0 &&
+                (rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux_J, nb, 0, c->jcnt[t],
+                                     grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr,
+                                     c->d_jlist[t], t, c->naux_J)))
+                return rc;
     }
     return det_end(c, nbatch, det, grad);
 }
@@ -718,12 +748,12 @@ __global__ void ris_k_metric(int n, const double* __restrict__ aux, const double
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)n * n) return;
     const int P = (int)(t / n), Q = (int)(t - (long long)P * n);
-    const double X0 = aux[5 * P] - aux[5 * Q], X1 = aux[5 * P + 1] - aux[5 * Q + 1], X2 = aux[5 * P + 2] - aux[5 * Q + 2];
-    const double al = aux[5 * P + 3], be = aux[5 * Q + 3];
+    const double X0 = aux[RIS_AUX_FIELDS * P] - aux[RIS_AUX_FIELDS * Q], X1 = aux[RIS_AUX_FIELDS * P + 1] - aux[RIS_AUX_FIELDS * Q + 1], X2 = aux[RIS_AUX_FIELDS * P + 2] - aux[RIS_AUX_FIELDS * Q + 2];
+    const double al = aux[RIS_AUX_FIELDS * P + 3], be = aux[RIS_AUX_FIELDS * Q + 3];
     const double sI = ris_rsqrt(al + be);
     double F[1];
     ris_boys<0>(al * be * sI * sI * (X0 * X0 + X1 * X1 + X2 * X2), boys0, F);
-    M[t] = aux[5 * P + 4] * aux[5 * Q + 4] * (2.0 * 17.493418327624862846) * sI * F[0];
+    M[t] = aux[RIS_AUX_FIELDS * P + 4] * aux[RIS_AUX_FIELDS * Q + 4] * (2.0 * 17.493418327624862846) * sI * F[0];
 }
 
 // In-place Cholesky factor M = L L^T (lower triangle) by ONE block, right-looking, column by column: naux = natoms is a
@@ -783,10 +813,144 @@ __global__ void __launch_bounds__(256) ris_k_chol_solve(int n, const double* __r
     for (int i = threadIdx.x; i < n; i += blockDim.x) cout[(size_t)s * n + i] = y[i];
 }
 
-static int metric_factor(ris_ctx* c)
+// ---- two-centre integrals over the s and p functions of an explicit J-fit set (NEXT-2; Eq. 22) ----
+// p_i(r; C, alpha) = (r - C)_i exp(-alpha |r-C|^2) = (1/2 alpha) d/dC_i of the s primitive, so with R = C_f - C_g and
+// V(R) = F_0(rho R^2):  (f|g) = N_f N_g 2 pi^{5/2}/(alpha beta sqrt(alpha+beta)) (1/2 alpha)^{l_f} (-1/2 beta)^{l_g} d_i^{l_f} d_j^{l_g} V,
+// and d/dC_f adds one more d_k.  Cartesian derivatives of V, with G_n = (-2 rho)^n F_n(rho R^2):
+//   d_a V = X_a G_1;  d_a d_b V = X_a X_b G_2 + delta_ab G_1;
+//   d_a d_b d_c V = X_a X_b X_c G_3 + (delta_ab X_c + delta_ac X_b + delta_bc X_a) G_2.
+RIS_DEV double ris_dV(int n, const int* d, const double* X, const double* G)
 {
-    if (c->d_chol) return RIS_OK;
-    const int n = c->naux;
+    if (n == 0) return G[0];
+    if (n == 1) return X[d[0]] * G[1];
+    if (n == 2) return fma(X[d[0]] * X[d[1]], G[2], d[0] == d[1] ? G[1] : 0.0);
+    const double t = (d[0] == d[1] ? X[d[2]] : 0.0) + (d[0] == d[2] ? X[d[1]] : 0.0) + (d[1] == d[2] ? X[d[0]] : 0.0);
+    return fma(X[d[0]] * X[d[1]] * X[d[2]], G[3], t * G[2]);
+}
+
+struct RisAuxFn { double C[3], al, fac; int atom, fn, l, comp; };
+RIS_DEV RisAuxFn ris_aux_fn(const double* __restrict__ rec, int f)
+{
+    const double* r = rec + (size_t)RIS_AUX_FIELDS * f;
+    RisAuxFn a;
+    a.C[0] = r[0]; a.C[1] = r[1]; a.C[2] = r[2]; a.al = r[3]; a.fac = r[4];
+    const int2 i0 = *reinterpret_cast<const int2*>(r + 5), i1 = *reinterpret_cast<const int2*>(r + 6);
+    a.atom = i0.x; a.fn = i0.y; a.l = i1.x; a.comp = i1.y;
+    return a;
+}
+
+// common factor and direction list of the pair (f, g); returns the number of directions
+RIS_DEV int ris_pair_fg(const RisAuxFn& f, const RisAuxFn& g, double* X, int* d, double& pref, double& rho)
+{
+    X[0] = f.C[0] - g.C[0]; X[1] = f.C[1] - g.C[1]; X[2] = f.C[2] - g.C[2];
+    const double sI = ris_rsqrt(f.al + g.al);
+    rho = f.al * g.al * sI * sI;
+    pref = f.fac * g.fac * (2.0 * 17.493418327624862846) * sI;
+    int n = 0;
+    if (f.l) { d[n++] = f.comp; pref *= 0.5 / f.al; }
+    if (g.l) { d[n++] = g.comp; pref *= -0.5 / g.al; }
+    return n;
+}
+
+__global__ void ris_k_metric_fn(int n, const double* __restrict__ rec, const double* __restrict__ boys2, double* __restrict__ M)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n * n) return;
+    const RisAuxFn f = ris_aux_fn(rec, (int)(t / n)), g = ris_aux_fn(rec, (int)(t % n));
+    double X[3], pref, rho, F[3];
+    int d[3];
+    const int nd = ris_pair_fg(f, g, X, d, pref, rho);
+    ris_boys<2>(rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]), boys2, F);
+    const double G[3] = {F[0], -2.0 * rho * F[1], 4.0 * rho * rho * F[2]};
+    M[t] = pref * ris_dV(nd, d, X, G);
+}
+
+// g[s][A] = sum_{f on A} sum_{g not on A} (c_f d_g + c_g d_f) d(f|g)/dC_f: one block per (atom, state), the atom's functions
+// in list order, threads over g, fixed-order block reduction (deterministic).  Pairs on one atom move together: no term.
+__global__ void __launch_bounds__(128) ris_k_grad_pq_fn(int n, const double* __restrict__ rec, const int* __restrict__ afo,
+                                                        const int* __restrict__ afn, const double* __restrict__ boys3,
+                                                        const double* __restrict__ cv, const double* __restrict__ dv,
+                                                        double* __restrict__ grad)
+{
+    const int A = blockIdx.x, s = blockIdx.y;
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (int k = afo[A]; k < afo[A + 1]; ++k) {
+        const RisAuxFn f = ris_aux_fn(rec, afn[k]);
+        const double cf = cv[(size_t)s * n + f.fn], df = dv[(size_t)s * n + f.fn];
+        for (int q = threadIdx.x; q < n; q += blockDim.x) {
+            const RisAuxFn g = ris_aux_fn(rec, q);
+            if (g.atom == A) continue;
+            double X[3], pref, rho, F[4];
+            int d[3];
+            const int nd = ris_pair_fg(f, g, X, d, pref, rho);
+            ris_boys<3>(rho * (X[0] * X[0] + X[1] * X[1] + X[2] * X[2]), boys3, F);
+            const double m2r = -2.0 * rho;
+            const double G[4] = {F[0], m2r * F[1], m2r * m2r * F[2], m2r * m2r * m2r * F[3]};
+            const double w = (cf * dv[(size_t)s * n + q] + cv[(size_t)s * n + q] * df) * pref;
+            for (int x = 0; x < 3; ++x) {
+                d[nd] = x;
+                acc[x] = fma(w, ris_dV(nd + 1, d, X, G), acc[x]);
+            }
+        }
+    }
+    __shared__ double red[3][128];
+    for (int x = 0; x < 3; ++x) red[x][threadIdx.x] = acc[x];
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if (threadIdx.x < o)
+            for (int x = 0; x < 3; ++x) red[x][threadIdx.x] += red[x][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) grad[((size_t)s * gridDim.x + A) * 3 + threadIdx.x] = red[threadIdx.x][0];
+}
+
+extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom, const int32_t* aux_l, const double* aux_exp)
+{
+    if (!c || nshell_aux < 1 || !aux_atom || !aux_l || !aux_exp) return RIS_EINVAL;
+    int nfn = 0;
+    for (int i = 0; i < nshell_aux; ++i) {
+        if (aux_atom[i] < 0 || aux_atom[i] >= c->natoms || aux_l[i] < 0 || aux_l[i] > 1 || !std::isfinite(aux_exp[i]) || !(aux_exp[i] > 0.0))
+            return RIS_EINVAL;
+        nfn += aux_l[i] ? 3 : 1;
+    }
+    CU(cudaSetDevice(c->device));
+    std::vector<double> fn((size_t)RIS_AUX_FIELDS * nfn), lists[4];
+    std::vector<std::vector<int>> on_atom(c->natoms);
+    int f = 0;
+    for (int i = 0; i < nshell_aux; ++i)
+        for (int comp = 0; comp < (aux_l[i] ? 3 : 1); ++comp, ++f) {
+            double* r = &fn[(size_t)RIS_AUX_FIELDS * f];
+            aux_record(r, &c->h_coords[3 * (size_t)aux_atom[i]], aux_exp[i], aux_l[i], comp, aux_atom[i], f);
+            std::vector<double>& L = lists[aux_l[i] ? 1 + comp : 0];
+            L.insert(L.end(), r, r + RIS_AUX_FIELDS);
+            on_atom[aux_atom[i]].push_back(f);
+        }
+    std::vector<int> off(c->natoms + 1, 0), idx;
+    for (int a = 0; a < c->natoms; ++a) { idx.insert(idx.end(), on_atom[a].begin(), on_atom[a].end()); off[a + 1] = (int)idx.size(); }
+    int rc;
+    CU(cudaStreamSynchronize(c->stream));           // the host vectors below are read by async copies: finish them here
+    if ((rc = dev_upload(c, &c->d_jfn, fn.data(), fn.size()))) return rc;
+    for (int t = 0; t < 4; ++t) {
+        c->jcnt[t] = (int)(lists[t].size() / RIS_AUX_FIELDS);
+        c->d_jlist[t] = nullptr;
+        if (c->jcnt[t] && (rc = dev_upload(c, &c->d_jlist[t], lists[t].data(), lists[t].size()))) return rc;
+    }
+    if ((rc = dev_upload(c, &c->d_atom_fn_off, off.data(), off.size()))) return rc;
+    if ((rc = dev_upload(c, &c->d_atom_fn, idx.data(), idx.size()))) return rc;
+    CU(cudaStreamSynchronize(c->stream));
+    c->jfit = true; c->naux_J = nfn; c->d_chol_J = nullptr;
+    return RIS_OK;
+}
+
+extern "C" int ris_naux_J(const ris_ctx* c) { return c ? c->naux_J : RIS_EINVAL; }
+
+// jset: the metric of the J-fit set (the default set when ris_set_jfit was never called)
+static int metric_factor(ris_ctx* c, bool jset = false)
+{
+    const bool own = jset && c->jfit;
+    double*& chol = own ? c->d_chol_J : c->d_chol;
+    if (chol) return RIS_OK;
+    const int n = own ? c->naux_J : c->naux;
     int rc;
     double* L;
     int* flag;
@@ -794,7 +958,8 @@ static int metric_factor(ris_ctx* c)
     if ((rc = dev_alloc(c, &flag, 1, true))) return rc;
     {
         ProfScope ps(c, "ris_k_metric", 40.0 * n * (double)n, 8.0 * n * (double)n);
-        ris_k_metric<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_aux, c->d_boys[0], L);
+        if (own) ris_k_metric_fn<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_jfn, c->d_boys[2], L);
+        else ris_k_metric<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_aux, c->d_boys[0], L);
     }
     {
         ProfScope ps(c, "ris_k_cholesky", (double)n * n * n / 3.0, 8.0 * n * (double)n);
@@ -804,7 +969,18 @@ static int metric_factor(ris_ctx* c)
     CU(cudaMemcpyAsync(&hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (hflag) return RIS_EINVAL;          // metric not positive definite (coincident aux centres)
-    c->d_chol = L;
+    chol = L;
+    return RIS_OK;
+}
+
+extern "C" int ris_metric_J(ris_ctx* c, double* M)
+{
+    if (!c || !M) return RIS_EINVAL;
+    if (!c->jfit) return ris_metric(c, M);
+    CU(cudaSetDevice(c->device));
+    const int n = c->naux_J;
+    ris_k_metric_fn<<<(unsigned)(((long long)n * n + 255) / 256), 256, 0, c->stream>>>(n, c->d_jfn, c->d_boys[2], M);
+    CU(cudaGetLastError());
     return RIS_OK;
 }
 
@@ -821,43 +997,48 @@ extern "C" int ris_metric(ris_ctx* c, double* M)
 extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out, double* c_out)
 {
     if (!c || nbatch < 1 || !D || !c_out) return RIS_EINVAL;
-    if ((size_t)c->naux * sizeof(double) > 48 * 1024) return RIS_EINVAL;     // substitution vector in static-size shared memory
+    if ((size_t)c->naux_J * sizeof(double) > 48 * 1024) return RIS_EINVAL;     // substitution vector in static-size shared memory
     CU(cudaSetDevice(c->device));
     int rc;
-    if ((rc = metric_factor(c))) return rc;
+    if ((rc = metric_factor(c, true))) return rc;
     const long long nao2 = (long long)c->nao * c->nao;
-    const int naux = c->naux;
+    const int naux = c->naux_J;
     double* v = v_out;
     if (!v && (rc = ws_get(c, WS_OUT, sizeof(double) * (size_t)nbatch * naux, (void**)&v))) return rc;
     CU(cudaMemsetAsync(v, 0, sizeof(double) * (size_t)nbatch * naux, c->stream));
-    const int ny = (naux + 31) / 32;
     for (int s0 = 0, nb; s0 < nbatch; s0 += nb) {
         nb = next_nb(nbatch - s0, RIS_NB_MAX);
         double* tile;
         if ((rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile))) return rc;
         if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
-        int* ctr;
-        if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr))) return rc;
-        CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
-        for (int oi = 0; oi < RIS_NCLASS; ++oi) {
-            const int k = kClassOrder[oi];
-            const RisClassPack& pk = c->cls[k];
-            if (pk.npairs == 0) continue;
-            RisGradParams p{};
-            p.task_ctr = ctr + (size_t)2 * k * ny;
-            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
-            p.tile = tile; p.sstride = c->nelem_real; p.estride = 1; p.lstride = 0; p.nb = nb;
-            p.p0 = 0; p.p1 = naux; p.grad = v + (size_t)s0 * naux;
-            const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
-            ProfScope ps(c, kIntNames[k], (double)naux * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb] + 2.0 * nel * pk.npairs * nb),
-                         8.0 * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
-            CU(ris_int_launchers[k](p, c->stream));
+        for (int t = 0; t < 4; ++t) {       // one pass per type of auxiliary function: s, p_x, p_y, p_z
+            const int nl = c->jcnt[t];
+            if (nl == 0) continue;
+            const int ny = (nl + 31) / 32;
+            int* ctr;
+            if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr))) return rc;
+            CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
+            for (int oi = 0; oi < RIS_NCLASS; ++oi) {
+                const int k = kClassOrder[oi];
+                const RisClassPack& pk = c->cls[k];
+                if (pk.npairs == 0) continue;
+                RisGradParams p{};
+                p.task_ctr = ctr + (size_t)2 * k * ny;
+                p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_jlist[t]; p.aux_type = t;
+                p.boys = c->d_boys[pk.la + pk.lb + (t ? 1 : 0)];
+                p.tile = tile; p.sstride = c->nelem_real; p.estride = 1; p.lstride = 0; p.nb = nb;
+                p.p0 = 0; p.p1 = nl; p.grad = v + (size_t)s0 * naux;
+                const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
+                ProfScope ps(c, kIntNames[k], (double)nl * ((double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + (t ? 1 : 0)] + 2.0 * nel * pk.npairs * nb),
+                             8.0 * nel * pk.npairs * nb + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
+                CU(ris_int_launchers[k](p, c->stream));
+            }
+            CU(cudaGetLastError());
         }
-        CU(cudaGetLastError());
     }
     {
         ProfScope ps(c, "ris_k_chol_solve", 2.0 * naux * (double)naux * nbatch, 8.0 * naux * (double)naux * nbatch);
-        ris_k_chol_solve<<<nbatch, 256, sizeof(double) * naux, c->stream>>>(naux, c->d_chol, v, c_out);
+        ris_k_chol_solve<<<nbatch, 256, sizeof(double) * naux, c->stream>>>(naux, c->jfit ? c->d_chol_J : c->d_chol, v, c_out);
     }
     CU(cudaGetLastError());
     return RIS_OK;
@@ -1060,12 +1241,12 @@ __global__ void __launch_bounds__(128) ris_k_grad_pq_full(int naux, const double
 {
     const int P = blockIdx.x, s = blockIdx.y;
     const double* Gs = G + (size_t)s * naux * naux;
-    const double Px = aux[5 * P], Py = aux[5 * P + 1], Pz = aux[5 * P + 2], al = aux[5 * P + 3], fP = aux[5 * P + 4];
+    const double Px = aux[RIS_AUX_FIELDS * P], Py = aux[RIS_AUX_FIELDS * P + 1], Pz = aux[RIS_AUX_FIELDS * P + 2], al = aux[RIS_AUX_FIELDS * P + 3], fP = aux[RIS_AUX_FIELDS * P + 4];
     double g0 = 0.0, g1 = 0.0, g2 = 0.0;
     for (int Q = threadIdx.x; Q < naux; Q += blockDim.x) {
         if (Q == P) continue;
-        const double X0 = Px - aux[5 * Q], X1 = Py - aux[5 * Q + 1], X2 = Pz - aux[5 * Q + 2];
-        const double be = aux[5 * Q + 3], fQ = aux[5 * Q + 4];
+        const double X0 = Px - aux[RIS_AUX_FIELDS * Q], X1 = Py - aux[RIS_AUX_FIELDS * Q + 1], X2 = Pz - aux[RIS_AUX_FIELDS * Q + 2];
+        const double be = aux[RIS_AUX_FIELDS * Q + 3], fQ = aux[RIS_AUX_FIELDS * Q + 4];
         const double sI = ris_rsqrt(al + be);
         const double rho = al * be * sI * sI;
         double F[2];
@@ -1213,13 +1394,13 @@ __global__ void __launch_bounds__(128) ris_k_grad_pq(int naux, int nb, const dou
                                                      const double* __restrict__ dv, double* __restrict__ grad)
 {
     const int P = blockIdx.x, s = blockIdx.y;
-    const double Px = aux[5 * P], Py = aux[5 * P + 1], Pz = aux[5 * P + 2], al = aux[5 * P + 3], fP = aux[5 * P + 4];
+    const double Px = aux[RIS_AUX_FIELDS * P], Py = aux[RIS_AUX_FIELDS * P + 1], Pz = aux[RIS_AUX_FIELDS * P + 2], al = aux[RIS_AUX_FIELDS * P + 3], fP = aux[RIS_AUX_FIELDS * P + 4];
     const double cP = cv[(size_t)s * naux + P], dP = dv[(size_t)s * naux + P];
     double g0 = 0.0, g1 = 0.0, g2 = 0.0;
     for (int Q = threadIdx.x; Q < naux; Q += blockDim.x) {
         if (Q == P) continue;
-        const double X0 = Px - aux[5 * Q], X1 = Py - aux[5 * Q + 1], X2 = Pz - aux[5 * Q + 2];
-        const double be = aux[5 * Q + 3], fQ = aux[5 * Q + 4];
+        const double X0 = Px - aux[RIS_AUX_FIELDS * Q], X1 = Py - aux[RIS_AUX_FIELDS * Q + 1], X2 = Pz - aux[RIS_AUX_FIELDS * Q + 2];
+        const double be = aux[RIS_AUX_FIELDS * Q + 3], fQ = aux[RIS_AUX_FIELDS * Q + 4];
         const double sI = ris_rsqrt(al + be);
         const double rho = al * be * sI * sI;
         double F[2];
@@ -1244,8 +1425,12 @@ extern "C" int ris_grad_PQ(ris_ctx* c, int nbatch, const double* c_aux, const do
 {
     if (!c || nbatch < 1 || !c_aux || !d_aux || !grad) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
-    ProfScope ps(c, "ris_k_grad_pq", 60.0 * c->naux * (double)c->naux * nbatch, 0.0);
-    ris_k_grad_pq<<<dim3(c->naux, nbatch), 128, 0, c->stream>>>(c->naux, nbatch, c->d_aux, c->d_boys[1], c_aux, d_aux, grad);
+    ProfScope ps(c, "ris_k_grad_pq", 60.0 * c->naux_J * (double)c->naux_J * nbatch, 0.0);
+    if (c->jfit)
+        ris_k_grad_pq_fn<<<dim3(c->natoms, nbatch), 128, 0, c->stream>>>(c->naux_J, c->d_jfn, c->d_atom_fn_off, c->d_atom_fn, c->d_boys[3],
+                                                                       c_aux, d_aux, grad);
+    else
+        ris_k_grad_pq<<<dim3(c->naux, nbatch), 128, 0, c->stream>>>(c->naux, nbatch, c->d_aux, c->d_boys[1], c_aux, d_aux, grad);
     CU(cudaGetLastError());
     return RIS_OK;
 }
@@ -1274,7 +1459,7 @@ extern "C" int ris_grad_J_host(ris_ctx* c, int nbatch, const double* D, const do
     int rc;
     const size_t ng = (size_t)nbatch * c->natoms * 3;
     if ((rc = h2d(c, WS_IN0, D, (size_t)nbatch * c->nao * c->nao, &dD))) return rc;
-    if ((rc = h2d(c, WS_IN1, c_aux, (size_t)nbatch * c->naux, &dc))) return rc;
+    if ((rc = h2d(c, WS_IN1, c_aux, (size_t)nbatch * c->naux_J, &dc))) return rc;
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = ris_grad_J(c, nbatch, dD, dc, dg))) return rc;
     return d2h_grad(c, dg, grad, ng);
@@ -1346,8 +1531,8 @@ extern "C" int ris_grad_PQ_host(ris_ctx* c, int nbatch, const double* c_aux, con
     double *dc, *dd, *dg;
     int rc;
     const size_t ng = (size_t)nbatch * c->natoms * 3;
-    if ((rc = h2d(c, WS_IN0, c_aux, (size_t)nbatch * c->naux, &dc))) return rc;
-    if ((rc = h2d(c, WS_IN1, d_aux, (size_t)nbatch * c->naux, &dd))) return rc;
+    if ((rc = h2d(c, WS_IN0, c_aux, (size_t)nbatch * c->naux_J, &dc))) return rc;
+    if ((rc = h2d(c, WS_IN1, d_aux, (size_t)nbatch * c->naux_J, &dd))) return rc;
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = ris_grad_PQ(c, nbatch, dc, dd, dg))) return rc;
     return d2h_grad(c, dg, grad, ng);
@@ -1366,8 +1551,8 @@ extern "C" int ris_grad_host(ris_ctx* c, int nbJ, const double* D, const double*
     int rc;
     double *dc, *dd, *dCo, *dCv, *dD, *dB, *dg;
     const size_t nJ = (size_t)nbJ * c->natoms * 3, nK = (size_t)nbK * c->natoms * 3;
-    if ((rc = h2d(c, WS_HC, c_aux, (size_t)nbJ * c->naux, &dc))) return rc;
-    if ((rc = h2d(c, WS_HDQ, d_aux, (size_t)nbJ * c->naux, &dd))) return rc;
+    if ((rc = h2d(c, WS_HC, c_aux, (size_t)nbJ * c->naux_J, &dc))) return rc;
+    if ((rc = h2d(c, WS_HDQ, d_aux, (size_t)nbJ * c->naux_J, &dd))) return rc;
     if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
     if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
     const size_t nD = (size_t)nbJ * c->nao * c->nao;

@@ -185,6 +185,39 @@ RIS_DEV void ris_prim_triplet(double p, double PZx, double PZy, double PZz, doub
     }
 }
 
+// p-type auxiliary function, component DIR (NEXT-2): the s-aux ladder one Boys order higher, then one
+// recurrence step on the aux centre (gen_classes.py "p-type auxiliary functions"): WC = (W - C)_DIR = (1 - rho/p)(P - C)_DIR,
+// 1/(2(p + alpha)) = (rho/p)/(2 alpha).  boys_tab: the table of order E + 1.
+template <int LH, int LO, int DIR, class ACC>
+RIS_DEV void ris_prim_triplet_p(double p, double PZx, double PZy, double PZz, double oo2p, double h2, double o2,
+                                double coef, double ZCx, double ZCy, double ZCz, double alpha, double auxfac,
+                                const double* __restrict__ boys_tab, ACC& acc, double ZOx, double ZOy, double ZOz)
+{
+    constexpr int E = RisClass<LH, LO>::E;
+    RisPrimHead<E + 1> h;
+    ris_prim_head<E + 1>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
+    const double X = DIR == 0 ? ZCx + PZx : (DIR == 1 ? ZCy + PZy : ZCz + PZz);
+    const double WC = (1.0 - h.q) * X, oo2pa = 0.5 * h.q / alpha;
+    if constexpr (LO == 0) {
+        const double hp = h2 * oo2p;
+        ris_vrrp<LH, LO, DIR>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc, WC, oo2pa, hp * ZOx, hp * ZOy, hp * ZOz);
+    } else {
+        ris_vrrp<LH, LO, DIR>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, h2, o2, acc, WC, oo2pa);
+    }
+}
+
+template <int LH, int LO, int DIR>
+RIS_DEV void ris_prim_triplet0_p(double p, double PZx, double PZy, double PZz, double oo2p, double coef, double ZCx,
+                                 double ZCy, double ZCz, double alpha, double auxfac, const double* __restrict__ boys_tab,
+                                 double (&acc)[RisClass0<LH, LO>::NACC])
+{
+    constexpr int E = RisClass0<LH, LO>::E;
+    RisPrimHead<E + 1> h;
+    ris_prim_head<E + 1>(p, PZx, PZy, PZz, coef, ZCx, ZCy, ZCz, alpha, auxfac, boys_tab, h);
+    const double X = DIR == 0 ? ZCx + PZx : (DIR == 1 ? ZCy + PZy : ZCz + PZz);
+    ris_vrrp0<LH, LO, DIR>(h.F, PZx, PZy, PZz, h.W0, h.W1, h.W2, oo2p, h.q, 0.0, 0.0, acc, (1.0 - h.q) * X, 0.5 * h.q / alpha);
+}
+
 // Undifferentiated primitive triplet (v_P = sum D_{mu nu} (mu nu|P), Eq. 21):
 // the same head, the VRR up to e = lh + lo, unscaled accumulation of [e0|s].
 template <int LH, int LO>

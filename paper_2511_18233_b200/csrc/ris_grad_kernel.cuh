@@ -172,7 +172,7 @@ struct RisTileDirectK {
 // ------------------------------------------------------------------------------------------------ one host-centre phase
 // The primitive pairs q[0 .. nk) hosted on centre Z (host l = LH, other l = LO), then HRR / derivative / tile contraction
 // into the lane's accumulator slots.
-template <int LH, int LO, bool TR, bool PIPE, bool KT, class Ring>
+template <int LH, int LO, bool TR, bool PIPE, bool KT, int AUX, class Ring>
 RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
                        double ZOz, double alpha, double auxfac, const double* __restrict__ boys, Ring& ring, int nb,
                        const double* __restrict__ sc, double* __restrict__ slot)
@@ -182,7 +182,7 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
     double acc[K::NACC];
 #pragma unroll
     for (int i = 0; i < K::NACC; ++i) acc[i] = 0.0;
-    if (PIPE) {
+    if (PIPE && AUX == 0) {
         // front of primitive k+1 (record load, rsqrt(p + alpha), T: branch-free) next to Boys + recurrence of primitive k
         double2 r0 = *reinterpret_cast<const double2*>(q), r1 = *reinterpret_cast<const double2*>(q + 2);
         double2 r2 = *reinterpret_cast<const double2*>(q + 4), r3 = *reinterpret_cast<const double2*>(q + 6);
@@ -212,16 +212,20 @@ RIS_DEV void ris_phase(int nk, const double* __restrict__ q, double ZCx, double 
             const double2 r1 = *reinterpret_cast<const double2*>(q + 2);
             const double2 r2 = *reinterpret_cast<const double2*>(q + 4);
             const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
-            ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
-                                     alpha, auxfac, boys, acc, ZOx, ZOy, ZOz);
+            if constexpr (AUX == 0)
+                ris_prim_triplet<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy, ZCz,
+                                         alpha, auxfac, boys, acc, ZOx, ZOy, ZOz);
+            else
+                ris_prim_triplet_p<LH, LO, AUX - 1>(r0.x, r0.y, r1.x, r1.y, r2.x, TR ? r3.x : r2.y, TR ? r2.y : r3.x, r3.y, ZCx, ZCy,
+                                                    ZCz, alpha, auxfac, boys, acc, ZOx, ZOy, ZOz);
         }
     }
     ris_hrrc<LH, LO, TR, 33, KT ? 0 : 32>(acc, ZOx, ZOy, ZOz, ring, nb, sc, slot);
 }
 
 // KT: K-type contraction (Gamma^P tile, P-minor, one column per lane); else J-type (D tile shared by all lanes, scaled by
-// c_aux[s][P]).
-template <int LA, int LB, int PH, bool KT>
+// c_aux[s][function]).  AUX: type of the auxiliary functions of this launch's list -- 0: s; 1, 2, 3: p_x, p_y, p_z (J only).
+template <int LA, int LB, int PH, bool KT, int AUX = 0>
 __global__ void __launch_bounds__(32 * RisGradTune<LA, LB>::NW, RisGradTune<LA, LB>::MINB) ris_grad_kernel(const RisGradParams prm)
 {
     using Tune = RisGradTune<LA, LB>;
@@ -240,15 +244,17 @@ __global__ void __launch_bounds__(32 * RisGradTune<LA, LB>::NW, RisGradTune<LA, 
     double* s_sc = s_gaux + 3 * nb * 32;                                     // [nb][32]    J: c_aux[s][P]
     const size_t gaux_off = (size_t)(reinterpret_cast<unsigned char*>(s_gaux) - (sm_raw + (size_t)warp * wbytes));
 
-    // this lane's auxiliary function
-    const int P = prm.p0 + blockIdx.y * 32 + lane;
-    const bool live = P < prm.p1;
-    const int Pe = live ? P : prm.p1 - 1;
-    const double* ax = prm.aux + 5 * (size_t)Pe;
+    // this lane's auxiliary function: position in the launch's list -> record (centre, exponent, N/alpha, atom, function index)
+    const int pos = prm.p0 + blockIdx.y * 32 + lane;
+    const bool live = pos < prm.p1;
+    const int Pe = live ? pos : prm.p1 - 1;
+    const double* ax = prm.aux + RIS_AUX_FIELDS * (size_t)Pe;
     const double Cx = ax[0], Cy = ax[1], Cz = ax[2], alpha = ax[3];
     const double auxfac = live ? ax[4] : 0.0;          // a dead lane computes exact zeros
+    const int2 ids = *reinterpret_cast<const int2*>(ax + 5);
+    const int P = ids.x;                               // the atom the function sits on: its gradient row
     if (!KT)
-        for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale[(size_t)s * prm.naux + Pe];
+        for (int s = 0; s < nb; ++s) s_sc[s * 32 + lane] = prm.cscale[(size_t)s * prm.naux + ids.y];
     for (int i = 0; i < 6 * nb; ++i) s_red[i * 33 + lane] = 0.0;
     for (int i = 0; i < 3 * nb; ++i) s_gaux[i * 32 + lane] = 0.0;
     constexpr bool STAGED = !KT || Tune::STAGE_K;
@@ -316,13 +322,13 @@ __global__ void __launch_bounds__(32 * RisGradTune<LA, LB>::NW, RisGradTune<LA, 
             if (runA || runB) ring.begin();
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
             if (runA)
-                ris_phase<LA, LB, false, Tune::PIPE, KT>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, ring,
+                ris_phase<LA, LB, false, Tune::PIPE, KT, AUX>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, ring,
                                                      nb, s_sc + lane, s_red + lane);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
             if constexpr (LB > 0) {        // (l,s) pairs are hosted on the l shell for every primitive pair: one phase
                 if (runB) {
                     if (runA && !ring.holds_all()) { __syncwarp(); ring.begin(); }      // the ring has rolled past state 0
-                    ris_phase<LB, LA, true, Tune::PIPE, KT>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy,
+                    ris_phase<LB, LA, true, Tune::PIPE, KT, AUX>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy,
                                                             -pr.ABz, alpha, auxfac, prm.boys, ring, nb, s_sc + lane, s_red + lane);
                 }
             }
@@ -357,7 +363,7 @@ __global__ void __launch_bounds__(32 * RisGradTune<LA, LB>::NW, RisGradTune<LA, 
     }
 }
 
-template <int LA, int LB, int PH, bool KT>
+template <int LA, int LB, int PH, bool KT, int AUX>
 cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
 {
     // ring slots: all states when they fit the class budget, fewer when the task records of a long contraction (kmax up
@@ -374,7 +380,7 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     // the opt-in is per device and context: set it at every launch that needs it (a host-side call of ~1 us) instead of
     // caching it in process-wide state
     if (smem > 48 * 1024) {
-        const cudaError_t e = cudaFuncSetAttribute(ris_grad_kernel<LA, LB, PH, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const cudaError_t e = cudaFuncSetAttribute(ris_grad_kernel<LA, LB, PH, KT, AUX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     // blockIdx.y: chunks of 32 aux functions; blockIdx.x: the blocks of a chunk, together one resident wave of
@@ -384,28 +390,36 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     // resident blocks per SM: the register target, or what the shared memory of the block allows
     const int resident = std::max(1, std::min<int>(RisGradTune<LA, LB>::MINB * RIS_GRAD_WARPS / NW, (int)((227 * 1024) / (smem + 1024))));
     const int nx = std::max(1, std::min(nbt, (p.nsm * resident + ny - 1) / ny));
-    ris_grad_kernel<LA, LB, PH, KT><<<dim3(nx, ny), 32 * NW, smem, st>>>(p);
+    ris_grad_kernel<LA, LB, PH, KT, AUX><<<dim3(nx, ny), 32 * NW, smem, st>>>(p);
     return cudaGetLastError();
 }
 
-// p.task_ctr holds two zeroed ticket arrays of ny counters each (one per phase launch); p.lstride selects the type
-template <int LA, int LB, bool KT>
+// p.task_ctr holds two zeroed ticket arrays of ny counters each (one per phase launch)
+template <int LA, int LB, bool KT, int AUX>
 cudaError_t ris_launch_grad_t(const RisGradParams& p, cudaStream_t st)
 {
     if constexpr (RisGradTune<LA, LB>::SPLIT) {
         RisGradParams q = p;
-        cudaError_t e = ris_launch_grad_phase<LA, LB, 1, KT>(q, st);
+        cudaError_t e = ris_launch_grad_phase<LA, LB, 1, KT, AUX>(q, st);
         if (e != cudaSuccess) return e;
         q.task_ctr = p.task_ctr + (p.p1 - p.p0 + 31) / 32;
-        return ris_launch_grad_phase<LA, LB, 2, KT>(q, st);
+        return ris_launch_grad_phase<LA, LB, 2, KT, AUX>(q, st);
     } else {
-        return ris_launch_grad_phase<LA, LB, 0, KT>(p, st);
+        return ris_launch_grad_phase<LA, LB, 0, KT, AUX>(p, st);
     }
 }
 
+// p.lstride selects the contraction type (K: P-minor tile), p.aux_type the auxiliary function type of the list (J only)
 template <int LA, int LB>
 cudaError_t ris_launch_grad(const RisGradParams& p, cudaStream_t st)
 {
     if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
-    return p.lstride ? ris_launch_grad_t<LA, LB, true>(p, st) : ris_launch_grad_t<LA, LB, false>(p, st);
+    if (p.lstride) return p.aux_type == 0 ? ris_launch_grad_t<LA, LB, true, 0>(p, st) : cudaErrorInvalidValue;
+    switch (p.aux_type) {
+    case 0: return ris_launch_grad_t<LA, LB, false, 0>(p, st);
+    case 1: return ris_launch_grad_t<LA, LB, false, 1>(p, st);
+    case 2: return ris_launch_grad_t<LA, LB, false, 2>(p, st);
+    case 3: return ris_launch_grad_t<LA, LB, false, 3>(p, st);
+    default: return cudaErrorInvalidValue;
+    }
 }

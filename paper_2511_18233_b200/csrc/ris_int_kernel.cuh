@@ -12,7 +12,7 @@
 
 // STORE: instead of the dot with a tile, the contracted integrals themselves are added to out[el * ostride] (the
 // P-minor integral buffer of ris_fit_K); tile / slot are unused then.
-template <int LH, int LO, bool TR, bool STORE>
+template <int LH, int LO, bool TR, bool STORE, int AUX>
 RIS_DEV void ris_phase0(int nk, const double* __restrict__ q, double ZCx, double ZCy, double ZCz, double ZOx, double ZOy,
                         double ZOz, double alpha, double auxfac, const double* __restrict__ boys,
                         const double* __restrict__ tile, size_t sstride, int nb, double* __restrict__ slot,
@@ -27,7 +27,8 @@ RIS_DEV void ris_phase0(int nk, const double* __restrict__ q, double ZCx, double
         const double2 r1 = *reinterpret_cast<const double2*>(q + 2);
         const double2 r2 = *reinterpret_cast<const double2*>(q + 4);
         const double2 r3 = *reinterpret_cast<const double2*>(q + 6);
-        ris_prim_triplet0<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, r3.y, ZCx, ZCy, ZCz, alpha, auxfac, boys, acc);
+        if constexpr (AUX == 0) ris_prim_triplet0<LH, LO>(r0.x, r0.y, r1.x, r1.y, r2.x, r3.y, ZCx, ZCy, ZCz, alpha, auxfac, boys, acc);
+        else ris_prim_triplet0_p<LH, LO, AUX - 1>(r0.x, r0.y, r1.x, r1.y, r2.x, r3.y, ZCx, ZCy, ZCz, alpha, auxfac, boys, acc);
     }
     if constexpr (STORE) ris_hrr0w<LH, LO, TR>(acc, ZOx, ZOy, ZOz, out, ostride);
     else ris_hrr0c<LH, LO, TR, 32>(acc, ZOx, ZOy, ZOz, tile, (size_t)1, sstride, nb, slot);
@@ -42,7 +43,7 @@ __host__ __device__ inline size_t ris_int_warp_smem(int kmax, int nb)
 // prm.tile: J tile [nb][packed elements] (estride 1); prm.grad: v [nb][naux] (zeroed by the caller).
 // STORE: prm.grad is the integral buffer [packed elements][estride] (P-minor, zeroed by the caller), element el of aux P
 // at grad[el * estride + (P - p0)]; nb is 0.
-template <int LA, int LB, bool STORE>
+template <int LA, int LB, bool STORE, int AUX = 0>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisGradParams prm)
 {
     constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
@@ -56,12 +57,13 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
     double* s_v = reinterpret_cast<double*>(s_pair + RIS_TASK_PRIMS);       // [nb][32]
     const size_t v_off = (size_t)(reinterpret_cast<unsigned char*>(s_v) - (sm_raw + (size_t)warp * wbytes));
 
-    const int P = prm.p0 + blockIdx.y * 32 + lane;
-    const bool live = P < prm.p1;
-    const int Pe = live ? P : prm.p1 - 1;
-    const double* ax = prm.aux + 5 * (size_t)Pe;
+    const int pos = prm.p0 + blockIdx.y * 32 + lane;       // position in the launch's list of auxiliary functions
+    const bool live = pos < prm.p1;
+    const int Pe = live ? pos : prm.p1 - 1;
+    const double* ax = prm.aux + RIS_AUX_FIELDS * (size_t)Pe;
     const double Cx = ax[0], Cy = ax[1], Cz = ax[2], alpha = ax[3];
     const double auxfac = live ? ax[4] : 0.0;
+    const int fn = reinterpret_cast<const int2*>(ax + 5)->y;  // index of the function: its entry of v
     for (int s = 0; s < nb; ++s) s_v[s * 32 + lane] = 0.0;
     const size_t sstride = (size_t)prm.sstride;
     __syncwarp();
@@ -95,11 +97,11 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
                                             : nullptr;
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
             if (pr.nkA > 0 && (!STORE || live))
-                ris_phase0<LA, LB, false, STORE>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
+                ris_phase0<LA, LB, false, STORE, AUX>(pr.nkA, q, ACx, ACy, ACz, pr.ABx, pr.ABy, pr.ABz, alpha, auxfac, prm.boys, tile,
                                                  sstride, nb, s_v + lane, out, (size_t)prm.estride);
             q += (size_t)pr.nkA * RIS_PRIM_FIELDS;
             if (pr.nkB > 0 && (!STORE || live))
-                ris_phase0<LB, LA, true, STORE>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
+                ris_phase0<LB, LA, true, STORE, AUX>(pr.nkB, q, ACx - pr.ABx, ACy - pr.ABy, ACz - pr.ABz, -pr.ABx, -pr.ABy, -pr.ABz,
                                                 alpha, auxfac, prm.boys, tile, sstride, nb, s_v + lane, out, (size_t)prm.estride);
             q += (size_t)pr.nkB * RIS_PRIM_FIELDS;
         }
@@ -112,23 +114,40 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
 #pragma unroll
             for (int w = 0; w < RIS_GRAD_WARPS; ++w)
                 v += reinterpret_cast<const double*>(sm_raw + (size_t)w * wbytes + v_off)[s * 32 + lane];
-            atomicAdd(prm.grad + (size_t)s * prm.naux + P, v);
+            atomicAdd(prm.grad + (size_t)s * prm.naux + fn, v);
         }
     }
 }
 
-template <int LA, int LB, bool STORE>
-cudaError_t ris_launch_int(const RisGradParams& p, cudaStream_t st)
+template <int LA, int LB, bool STORE, int AUX>
+cudaError_t ris_launch_int_t(const RisGradParams& p, cudaStream_t st)
 {
-    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
     const size_t smem = RIS_GRAD_WARPS * ris_int_warp_smem(p.pk.kmax, p.nb);
     if (smem > 48 * 1024) {          // per device and context: set at every launch that needs it, no process-wide cache
-        const cudaError_t e = cudaFuncSetAttribute(ris_int_kernel<LA, LB, STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const cudaError_t e = cudaFuncSetAttribute(ris_int_kernel<LA, LB, STORE, AUX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS;
     const int nx = std::max(1, std::min(nbt, (p.nsm * 3 + ny - 1) / ny));
-    ris_int_kernel<LA, LB, STORE><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
+    ris_int_kernel<LA, LB, STORE, AUX><<<dim3(nx, ny), RIS_GRAD_THREADS, smem, st>>>(p);
     return cudaGetLastError();
+}
+
+// p.aux_type: type of the auxiliary functions of the launch's list (p functions: the dot-product form only)
+template <int LA, int LB, bool STORE>
+cudaError_t ris_launch_int(const RisGradParams& p, cudaStream_t st)
+{
+    if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
+    if constexpr (STORE) {
+        return p.aux_type == 0 ? ris_launch_int_t<LA, LB, true, 0>(p, st) : cudaErrorInvalidValue;
+    } else {
+        switch (p.aux_type) {
+        case 0: return ris_launch_int_t<LA, LB, false, 0>(p, st);
+        case 1: return ris_launch_int_t<LA, LB, false, 1>(p, st);
+        case 2: return ris_launch_int_t<LA, LB, false, 2>(p, st);
+        case 3: return ris_launch_int_t<LA, LB, false, 3>(p, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
 }

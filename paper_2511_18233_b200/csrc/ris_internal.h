@@ -5,6 +5,7 @@
 
 constexpr int RIS_LMAX = 3;
 constexpr int RIS_NCLASS = 10;          // (la,lb), la >= lb, la <= 3
+constexpr int RIS_AUX_FIELDS = 8;       // doubles per aux record (RisGradParams::aux)
 constexpr int RIS_PRIM_FIELDS = 8;      // p, (P-Z)x, (P-Z)y, (P-Z)z, 1/(2p), 2a, 2b, coef   (Z = host centre); one 64-byte record
 constexpr int RIS_GRAD_WARPS = 4;       // warps per class-kernel block
 constexpr int RIS_GRAD_THREADS = 32 * RIS_GRAD_WARPS;
@@ -49,9 +50,14 @@ struct RisClassPack {
 // Launch description of one class kernel (by value to the kernel).
 struct RisGradParams {
     RisClassPack pk;
-    int naux, natoms;
+    int naux, natoms;        // naux: functions in the coefficient vector (row length of cscale / v)
     int nsm;                 // SMs of the context's device (grid sizing)
-    const double* aux;       // [naux][5] Cx,Cy,Cz,alpha,auxfac
+    // aux records of this launch's LIST of auxiliary functions, 8 doubles each: Cx, Cy, Cz, alpha, N/alpha, then two ints
+    // (atom of the function -> gradient row, index of the function -> column of cscale / v), one double of padding.
+    // K type and the default J set: the list is all naux s functions (atom = index).  A J-fit set with p functions (NEXT-2)
+    // is run as four lists -- s, p_x, p_y, p_z -- with aux_type 0..3 selecting the kernel specialisation.
+    const double* aux;
+    int aux_type;
     const double* boys;      // table for M = E of this class
     // packed tiles: element el of state s for aux P sits at tile[s*sstride + el*estride + (P - p0)*lstride]
     //   J: estride 1, lstride 0 (D tile, the same for every P);  K: estride = padded P-batch, lstride 1 (Gamma^P)
@@ -61,7 +67,7 @@ struct RisGradParams {
     const double* cscale;    // J: c_aux[nb][naux]; K: nullptr
     int nb;
     int ring_ns;             // slots of the shared-memory tile ring (set by the launcher)
-    int p0, p1;              // aux range of this launch; blockIdx.y selects 32 of them, one per lane
+    int p0, p1;              // range of list positions of this launch; blockIdx.y selects 32 of them, one per lane
     int* task_ctr;           // [chunks of 32 aux] zeroed ticket counters of this launch (dynamic task hand-out)
     double* grad;            // [nb][natoms][3], accumulated with atomics
     unsigned long long* det; // deterministic mode: [nb][natoms][3][2] fixed-point accumulators (hi, lo), else nullptr

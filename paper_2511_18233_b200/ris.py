@@ -18,7 +18,7 @@ _lib = None
 
 EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host", "ris_grad_host",
-    "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full",
+    "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full", "ris_set_jfit", "ris_naux_J", "ris_metric_J",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
     "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
@@ -51,6 +51,8 @@ def load_library():
     lib.ris_grad_PQ.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_fit_J.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_metric.argtypes = [vp, vp]
+    lib.ris_metric_J.argtypes = [vp, vp]
+    lib.ris_set_jfit.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_fit_K.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ_full.argtypes = [vp, ci, vp, vp]
     lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
@@ -60,7 +62,7 @@ def load_library():
     lib.ris_destroy.argtypes = [vp]
     lib.ris_strerror.argtypes = [ci]
     lib.ris_strerror.restype = C.c_char_p
-    for name in ("ris_nao", "ris_naux", "ris_natoms", "ris_p_batch", "ris_profile_reset", "ris_profile_count"):
+    for name in ("ris_nao", "ris_naux", "ris_naux_J", "ris_natoms", "ris_p_batch", "ris_profile_reset", "ris_profile_count"):
         getattr(lib, name).argtypes = [vp]
     for name in ("ris_npairs", "ris_nprimpairs"):
         getattr(lib, name).argtypes = [vp, ci, ci]
@@ -131,6 +133,19 @@ class RisContext:
         self.nao = self._lib.ris_nao(h)
         self.naux = self._lib.ris_naux(h)
         self.natoms = self._lib.ris_natoms(h)
+        self.naux_J = self._lib.ris_naux_J(h)
+        if getattr(mol, "jfit", None) is not None:
+            self.set_jfit(*mol.jfit)
+
+    def set_jfit(self, aux_atom, aux_l, aux_exp):
+        """J-fit auxiliary set with p functions (ris_set_jfit): shells (atom, l in {0, 1}, exponent); the J-type calls then
+        take naux_J coefficients per state."""
+        at, ll, ex = _np(aux_atom, np.int32), _np(aux_l, np.int32), _np(aux_exp, np.float64)
+        if not (at.shape == ll.shape == ex.shape and at.ndim == 1):
+            raise RisError("set_jfit: aux_atom, aux_l, aux_exp must be 1-D arrays of one length")
+        with self._ordered():
+            _check(self._lib.ris_set_jfit(self._h, at.shape[0], at.ctypes.data, ll.ctypes.data, ex.ctypes.data))
+        self.naux_J = self._lib.ris_naux_J(self._h)
 
     # ---- stream ordering: the library enqueues on the stream given at setup.  When the caller's CURRENT torch stream
     # is a different one (where its inputs were produced and where it will read the outputs), the setup stream first
@@ -194,7 +209,7 @@ class RisContext:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
         with self._ordered():
             _check(self._lib.ris_grad_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)),
-                                        self._dev(c_aux, (nb, self.naux)), self._dev(out, (nb, self.natoms, 3))))
+                                        self._dev(c_aux, (nb, self.naux_J)), self._dev(out, (nb, self.natoms, 3))))
         return out
 
     def grad_K(self, C_occ, C_vir, B, out=None):
@@ -212,19 +227,19 @@ class RisContext:
         if out is None:
             out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
         with self._ordered():
-            _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux)), self._dev(d_aux, (nb, self.naux)),
+            _check(self._lib.ris_grad_PQ(self._h, nb, self._dev(c_aux, (nb, self.naux_J)), self._dev(d_aux, (nb, self.naux_J)),
                                          self._dev(out, (nb, self.natoms, 3))))
         return out
 
     # ---- fitting step, J type (argument marshalling only)
     def fit_J(self, D):
-        """(v, c): v[s][P] = sum D^s_{mu nu} (mu nu|P), c = M^-1 v; both [nbatch][naux] on the device."""
+        """(v, c): v[s][P] = sum D^s_{mu nu} (mu nu|P), c = M^-1 v; both [nbatch][naux_J] on the device."""
         nb = D.shape[0]
-        v = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
-        c = self._torch.empty((nb, self.naux), dtype=self._torch.float64, device=self.device)
+        v = self._torch.empty((nb, self.naux_J), dtype=self._torch.float64, device=self.device)
+        c = self._torch.empty((nb, self.naux_J), dtype=self._torch.float64, device=self.device)
         with self._ordered():
-            _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux)),
-                                       self._dev(c, (nb, self.naux))))
+            _check(self._lib.ris_fit_J(self._h, nb, self._dev(D, (nb, self.nao, self.nao)), self._dev(v, (nb, self.naux_J)),
+                                       self._dev(c, (nb, self.naux_J))))
         return v, c
 
     def fit_K(self, C_occ, C_vir):
@@ -250,6 +265,13 @@ class RisContext:
         M = self._torch.empty((self.naux, self.naux), dtype=self._torch.float64, device=self.device)
         with self._ordered():
             _check(self._lib.ris_metric(self._h, self._dev(M, (self.naux, self.naux))))
+        return M
+
+    def metric_J(self):
+        n = self.naux_J
+        M = self._torch.empty((n, n), dtype=self._torch.float64, device=self.device)
+        with self._ordered():
+            _check(self._lib.ris_metric_J(self._h, self._dev(M, (n, n))))
         return M
 
     # ---- host-buffer calls (numpy arrays or CPU tensors, float64, C-contiguous; copies happen inside the C call)

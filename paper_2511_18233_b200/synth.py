@@ -44,6 +44,9 @@ class Molecule:
     prim_exp: np.ndarray        # [nprim_total] bohr^-2
     prim_coef: np.ndarray       # [nprim_total], applied as-is to unnormalised primitives
     aux_exponents: np.ndarray   # [natoms] bohr^-2; aux P sits on atom P
+    # optional J-fit auxiliary set with p functions (NEXT-2): SHELLS (atom[], l[] in {0, 1}, exponent[]);
+    # None: the J term uses the default set above
+    jfit: tuple | None = None
 
     @property
     def natoms(self) -> int:
@@ -267,6 +270,30 @@ def make_workload(config: int, *, nbatch_override: int | None = None,
                     C_occ, C_vir, B, 1e-13,
                     {"config": config, "seed": config - 1, "nao": nao, "naux": naux,
                      "nbatch_J": nbJ, "nbatch_K": nbK})
+
+
+def with_jfit(mol: Molecule, seed: int, p_on=None) -> Molecule:
+    """A copy of `mol` carrying a J-fit set of one s shell (the default exponent) and one p shell per atom -- the set the
+    paper's calculations use for the Coulomb term.  The paper's fitted exponents (Ref. 87) are
+    not available: the p exponent is the atom's s exponent times a seeded factor in [0.8, 2.0].  p_on: atoms that get the
+    p shell (default all)."""
+    import copy
+    rng = np.random.default_rng(seed)
+    fac = rng.uniform(0.8, 2.0, size=mol.natoms)
+    at, ll, ex = [], [], []
+    for A in range(mol.natoms):
+        at.append(A); ll.append(0); ex.append(float(mol.aux_exponents[A]))
+        if p_on is None or A in p_on:
+            at.append(A); ll.append(1); ex.append(float(mol.aux_exponents[A] * fac[A]))
+    out = copy.copy(mol)
+    out.jfit = (np.array(at, dtype=np.int32), np.array(ll, dtype=np.int32), np.array(ex, dtype=np.float64))
+    return out
+
+
+def naux_jfit(mol: Molecule) -> int:
+    if mol.jfit is None:
+        return mol.natoms
+    return int(sum(3 if l else 1 for l in mol.jfit[1]))
 
 
 def tiny_molecule(seed: int, ls_per_atom, coords_bohr, lo=0.2, hi=3.0, nprim=2) -> Molecule:

@@ -34,10 +34,13 @@ def harness():
     lib.harness_triplet.argtypes = [C.c_int, C.c_int, C.c_int] + [C.c_void_p] * 4 + [C.c_double, C.c_double,
                                                                                     C.c_void_p, C.c_int, C.c_void_p]
     lib.harness_triplet0.argtypes = lib.harness_triplet.argtypes
+    lib.harness_triplet_aux.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int] + [C.c_void_p] * 4 + [C.c_double, C.c_double,
+                                                                                                 C.c_void_p, C.c_int, C.c_void_p]
+    lib.harness_triplet0_aux.argtypes = lib.harness_triplet_aux.argtypes
     return lib
 
 
-@pytest.mark.parametrize("M", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("M", [0, 1, 2, 3, 4, 5, 6, 7, 8])
 def test_device_boys_interpolation_vs_mpmath(harness, M):
     mpmath.mp.dps = 40
     rng = np.random.default_rng(M)
@@ -141,3 +144,59 @@ def test_undifferentiated_class_recurrence_vs_oracle(harness, la, lb):
                                       alpha, auxfac, np.ascontiguousarray(tile).ctypes.data, nb, out.ctypes.data)
         assert rc == 0
         np.testing.assert_allclose(out, ref, rtol=0, atol=2e-13 * max(np.abs(ref).max(), 1e-3))
+
+
+def _prim_records(mol, A, B, lb):
+    """primitive-pair records exactly as ris_setup packs them (3 primitives per shell)"""
+    prim = []
+    for ka in range(3):
+        for kb in range(3):
+            a, b = mol.prim_exp[ka], mol.prim_exp[3 + kb]
+            p = a + b
+            PZ = -(b / p) * (A - B) if (a >= b or lb == 0) else (a / p) * (A - B)
+            Kab = math.exp(-a * b / p * np.dot(A - B, A - B))
+            coef = mol.prim_coef[ka] * mol.prim_coef[3 + kb] * Kab * 2 * math.pi ** 2.5 / p
+            prim.append([p, PZ[0], PZ[1], PZ[2], 0.5 / p, 2 * a, 2 * b, coef])
+    return np.ascontiguousarray(prim)
+
+
+@pytest.mark.parametrize("la,lb", CLASSES)
+def test_p_aux_class_recurrence_vs_oracle(harness, la, lb):
+    """NEXT-2: a p-type auxiliary shell on the third centre.  Derivative and undifferentiated contracted
+    triplets of every class, each p component, against the oracle's Hermite-shift evaluation (a different algorithm: the
+    CUDA path takes one Obara-Saika step on the aux centre)."""
+    rng = np.random.default_rng(300 + 10 * la + lb)
+    for trial, dist in enumerate([1.3, 5.0, 35.0]):
+        coords = np.array([[0.1, -0.2, 0.3], [1.1, 0.7, -0.6], [0, 0, 0]], dtype=float)
+        v = rng.normal(size=3)
+        coords[2] = coords[0] + dist * v / np.linalg.norm(v)
+        mol = synth.tiny_molecule(400 + trial, [[la], [lb], []], coords, lo=0.15, hi=6.0, nprim=3)
+        alpha = float(rng.uniform(0.1, 1.5))
+        mol.jfit = (np.array([2]), np.array([1]), np.array([alpha]))
+        nca, ncb = synth.ncart(la), synth.ncart(lb)
+        nb = 2
+        tile = rng.standard_normal((nb, nca, ncb))
+        G = np.zeros((nb, mol.nao, mol.nao))
+        G[:, :nca, nca:] = tile
+        A, B = coords[0], coords[1]
+        prim = _prim_records(mol, A, B, lb)
+        auxfac = (2 * alpha / math.pi) ** 0.75 * 2.0 * math.sqrt(alpha) / alpha
+        AB = A - B
+        Cc = np.ascontiguousarray(coords[2])
+        v_ref = orc.vec_J(mol, G)                        # [nb][3]
+        for comp in range(3):
+            g, _ = orc.grad_J(mol, G, np.eye(3)[comp][None].repeat(nb, 0))
+            out = np.zeros((nb, 6))
+            rc = harness.harness_triplet_aux(la, lb, comp + 1, 9, prim.ctypes.data, A.ctypes.data, AB.ctypes.data, Cc.ctypes.data,
+                                             alpha, auxfac, np.ascontiguousarray(tile).ctypes.data, nb, out.ctypes.data)
+            assert rc == 0
+            ref = np.concatenate([g[:, 0, :], g[:, 1, :]], axis=1)
+            scale = np.abs(g).max()
+            np.testing.assert_allclose(out, ref, rtol=0, atol=2e-13 * scale)
+            np.testing.assert_allclose(-(out[:, :3] + out[:, 3:]), g[:, 2, :], rtol=0, atol=2e-13 * scale)
+            out0 = np.zeros(nb)
+            rc = harness.harness_triplet0_aux(la, lb, comp + 1, 9, prim.ctypes.data, A.ctypes.data, AB.ctypes.data,
+                                              Cc.ctypes.data, alpha, auxfac, np.ascontiguousarray(tile).ctypes.data, nb,
+                                              out0.ctypes.data)
+            assert rc == 0
+            np.testing.assert_allclose(out0, v_ref[:, comp], rtol=0, atol=2e-13 * max(np.abs(v_ref).max(), 1e-3))
