@@ -458,3 +458,51 @@ def ris_pair_gradient(mol, D1, D2, c_x):
     G = np.stack([sum(Minv[A, B] * (X1[B] + X2[B]) for B in range(n)) for A in range(n)])
     gK = grad_dense_K(mol, G) - grad_PQ_full(mol, N[None])[0]
     return gJ - c_x * gK
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3 / NEXT-4c: products of the ris coupling matrix with trial vectors -- the excitation-energy stage
+# (Casida / TDA, Eqs. 1-5 with the ris integrals of Eqs. 20-22) and the ris-approximated
+# (A + B) of the Z-vector equation (Eq. 19; Sec. 4.2).  With i, j occupied and a, b virtual,
+# Eqs. 2-5 and 20-21 give (the orbital-energy diagonal of A is the caller's)
+#   K_{ai,bj} = g^ris_{ai,jb} = (ai|jb)^ris - c_x (ab|ji)^ris        (coupling part of A, Eq. 2)
+#   K_{ai,jb} = g^ris_{ai,bj} = (ai|bj)^ris - c_x (aj|bi)^ris        (B, Eq. 3)
+#   (pq|sr)^ris = sum_AB (pq|A) M^-1_AB (B|sr)                        (Eq. 21; Coulomb term with the J-fit set and its metric,
+#                                                                      exchange terms with the default s set)
+# so every product the solvers need is one linear combination
+#   sigma_ia = sum_jb [ cJ (ia|jb)^ris - cKA (ij|ab)^ris - cKB (ib|ja)^ris ] X_jb :
+#   A-coupling: (1, c_x, 0);  B: (1, 0, c_x);  A + B: (2, c_x, c_x);  A - B: (0, c_x, -c_x)
+# (spin-adaptation factors, e.g. cJ = 2 for closed-shell singlets, are the caller's: reading R-sign).
+# Tiny molecules only: dense AO tensors, the four-index matrix written out.
+def int3c_J(mol, f, *, prim_cutoff=0.0):
+    """(mu nu|f) for function f of the J-fit set (the default set when the molecule has none)."""
+    h = _Held(mol, jfit=True)
+    out = np.zeros((h.nao, h.nao))
+    rc = lib().ris_oracle_int3c_P(C.byref(h.c), int(f), prim_cutoff, out.ctypes.data)
+    assert rc == 0
+    return out
+
+
+def mo_tensor(I, C_left, C_right):
+    """T[P][l][r] = sum_{mu nu} C_left[mu,l] I[P][mu][nu] C_right[nu,r]"""
+    return np.einsum("ml,pmn,nr->plr", _f64(C_left), I, _f64(C_right))
+
+
+def coupling_ris(mol, C_occ, C_vir, cJ, cKA, cKB):
+    """The matrix K[i,a,j,b] = cJ (ia|jb)^ris - cKA (ij|ab)^ris - cKB (ib|ja)^ris."""
+    nK = np.asarray(mol.coords).shape[0]
+    IK = np.stack([int3c(mol, P) for P in range(nK)])
+    MJ = metric_J(mol)
+    IJ = np.stack([int3c_J(mol, f) for f in range(MJ.shape[0])])
+    MJinv, MKinv = np.linalg.inv(MJ), np.linalg.inv(metric(mol))
+    Tov_J = mo_tensor(IJ, C_occ, C_vir)
+    Too, Tov, Tvv = mo_tensor(IK, C_occ, C_occ), mo_tensor(IK, C_occ, C_vir), mo_tensor(IK, C_vir, C_vir)
+    K = cJ * np.einsum("Aia,AB,Bjb->iajb", Tov_J, MJinv, Tov_J)
+    K -= cKA * np.einsum("Aij,AB,Bab->iajb", Too, MKinv, Tvv)
+    K -= cKB * np.einsum("Aib,AB,Bja->iajb", Tov, MKinv, Tov)
+    return K
+
+
+def matvec_ris(mol, C_occ, C_vir, X, cJ, cKA, cKB):
+    """sigma[v][i][a] = sum_jb K[i,a,j,b] X[v][j][b]"""
+    return np.einsum("iajb,vjb->via", coupling_ris(mol, C_occ, C_vir, cJ, cKA, cKB), _f64(X))
