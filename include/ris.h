@@ -155,6 +155,26 @@ int ris_set_jfit(ris_ctx* ctx, int nshell_aux, const int32_t* aux_atom, const in
 int ris_naux_J(const ris_ctx* ctx);
 int ris_metric_J(ris_ctx* ctx, double* M_out);
 
+/* ---- Products of the ris coupling matrix with trial vectors (SURVEY.md 8(f) NEXT-3 and NEXT-4c) ------------------------
+ * The excitation-energy stage (Casida / TDA: Eqs. 1-5 with the ris integrals of Eqs. 20-22; the
+ * stored "reduced-size MO basis" tensors of PAPER.md:160) and the ris-approximated (A + B) of the Z-vector equation (Eq. 19,
+ * PAPER.md:107; Sec. 4.2).  With i, j over the nocc columns of C_occ and a, b over the nvir columns of C_vir,
+ *     sigma[v][i][a] = sum_jb [ cJ (ia|jb) - cKA (ij|ab) - cKB (ib|ja) ]^ris X[v][j][b],
+ *     (pq|sr)^ris = sum_AB (pq|A) M^-1_AB (B|sr)   (Eq. 21; the Coulomb term over the J-fit set and its metric -- see
+ *                                                   ris_set_jfit -- the two exchange terms over the default s set)
+ *   coupling part of A (Eq. 2): (cJ, cKA, cKB) = (1, c_x, 0);  B (Eq. 3): (1, 0, c_x);  A + B: (2, c_x, c_x);  A - B: (0, c_x, -c_x).
+ *   The orbital-energy diagonal of A and spin-adaptation factors (cJ = 2 for closed-shell singlets) are the caller's.
+ * ris_resp_setup: C_occ device [nao][nocc], C_vir device [nao][nvir]; builds and keeps (ctx-owned, about
+ *   8 (naux_J nocc nvir + naux (nvir^2 + 2 nocc nvir + nocc^2)) bytes) the MO-basis tensors (ia|f), (ab|P), M^-1 (ij|P),
+ *   (ia|P), M^-1 (ia|P) in the layouts the products read; call it again after the orbitals change.  RIS_EINVAL when a metric
+ *   is not positive definite or an auxiliary set has more than 6144 functions; RIS_ENOMEM when the tensors do not fit.
+ * ris_resp_matvec: X, sigma device [nvec][nocc][nvir]; sigma is overwritten.  A zero coefficient skips its term.
+ *   RIS_EINVAL before ris_resp_setup.  Deterministic (fixed summation order).
+ * ris_resp_free releases the stored tensors (ris_destroy and ris_set_jfit do it too). */
+int ris_resp_setup(ris_ctx* ctx, int nocc, int nvir, const double* C_occ, const double* C_vir);
+int ris_resp_matvec(ris_ctx* ctx, int nvec, double cJ, double cKA, double cKB, const double* X, double* sigma);
+int ris_resp_free(ris_ctx* ctx);
+
 int ris_destroy(ris_ctx* ctx);
 const char* ris_strerror(int status);
 

@@ -46,6 +46,16 @@ extern "C" const char* ris_strerror(int status)
 // --------------------------------------------------------------------------------------- context
 struct ProfRec { const char* name; cudaEvent_t e0, e1; double flops, bytes; };
 
+// Stored MO-basis tensors and scratch of the coupling-matrix products (ris_resp.cuh)
+struct RisResp {
+    bool ready = false;
+    int no = 0, nv = 0, nop = 0, nvp = 0;      // nocc, nvir and their even paddings
+    int nz = 0, pc = 0, nKp = 0;               // split of the (P, j) contraction: nz ranges of pc aux functions, nKp = nz pc
+    double *TJ = nullptr, *Tvv = nullptr, *BooT = nullptr, *Bov = nullptr, *TovT = nullptr;
+    double *Xp = nullptr, *Y = nullptr, *part = nullptr, *uw = nullptr;
+    int vc = 0, nchunk = 0;                    // vectors per pass the scratch is sized for; chunks of the Coulomb reduction
+};
+
 struct ris_ctx {
     int device = 0;
     int nsm = 0;                       // SMs of `device` (grid sizing of the class kernels)
@@ -71,6 +81,7 @@ struct ris_ctx {
     long long nelem_real = 0, npairs_total = 0, nprim_surv = 0, nprim_total = 0;
     double* d_boys[9] = {nullptr};     // Boys tables of top order M = 0..8 (M = 8: d/dR of (ff|p))
     double* d_minv = nullptr;          // [naux][nauxp] inverse metric (built by the first ris_fit_K)
+    double* d_minv_J = nullptr;        // the same for an explicit J-fit set
     // band of the spatially ordered AO index per 64-row block (from the GEMM-2 block list): columns
     // [rb_jlo*64, (rb_jlo*64 + rb_kw)) hold every surviving partner of the block's rows
     std::vector<int> rb_jlo, rb_kw;
@@ -95,15 +106,16 @@ struct ris_ctx {
     cudaEvent_t join_ev[RIS_NCLASS] = {nullptr}, fork_ev = nullptr;
     cudaEvent_t copy_extra = nullptr;             // the extra payload of upload_B_chunked has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
-    void* ws[20] = {nullptr};
-    size_t ws_bytes[20] = {0};
+    void* ws[22] = {nullptr};
+    size_t ws_bytes[22] = {0};
+    RisResp resp;
     int last_pbatch = 0;
     std::vector<ProfRec> prof;
     std::vector<cudaEvent_t> ev_pool;
 };
 
 enum { WS_TILE = 0, WS_H = 1, WS_UNUSED2 = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
-       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_N = 20 };
+       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_RESP_T = 20, WS_RESP_B = 21, WS_N = 22 };
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -541,6 +553,7 @@ extern "C" int ris_destroy(ris_ctx* c)
 {
     if (!c) return RIS_EINVAL;
     cudaStreamSynchronize(c->stream);
+    ris_resp_free(c);
     for (void* p : c->owned) cudaFree(p);
     for (int i = 0; i < WS_N; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
     for (cudaEvent_t e : c->copy_ev) cudaEventDestroy(e);
@@ -938,7 +951,8 @@ extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom,
     if ((rc = dev_upload(c, &c->d_atom_fn_off, off.data(), off.size()))) return rc;
     if ((rc = dev_upload(c, &c->d_atom_fn, idx.data(), idx.size()))) return rc;
     CU(cudaStreamSynchronize(c->stream));
-    c->jfit = true; c->naux_J = nfn; c->d_chol_J = nullptr;
+    c->jfit = true; c->naux_J = nfn; c->d_chol_J = nullptr; c->d_minv_J = nullptr;
+    ris_resp_free(c);                       // stored Coulomb tensors belong to the previous set
     return RIS_OK;
 }
 
@@ -1120,62 +1134,73 @@ __global__ void ris_k_pad2d(int rows, int cols, int ld, const double* __restrict
     out[i] = cidx < cols ? in[(size_t)r * cols + cidx] : 0.0;
 }
 
-static int metric_inverse(ris_ctx* c)
+static int metric_inverse(ris_ctx* c, bool jset = false)
 {
-    if (c->d_minv) return RIS_OK;
+    const bool own = jset && c->jfit;
+    double*& slot = own ? c->d_minv_J : c->d_minv;
+    if (slot) return RIS_OK;
     int rc;
-    if ((rc = metric_factor(c))) return rc;
-    const int n = c->naux, np_ = (n + 1) & ~1;
+    if ((rc = metric_factor(c, jset))) return rc;
+    const int n = own ? c->naux_J : c->naux, np_ = (n + 1) & ~1;
     double *eye, *inv, *minv;
     if ((rc = dev_alloc(c, &eye, (size_t)n * n, false))) return rc;
     if ((rc = dev_alloc(c, &inv, (size_t)n * n, false))) return rc;
     if ((rc = dev_alloc(c, &minv, (size_t)n * np_, false))) return rc;
     const unsigned nb1 = (unsigned)(((long long)n * n + 255) / 256), nb2 = (unsigned)(((long long)n * np_ + 255) / 256);
     ris_k_eye<<<nb1, 256, 0, c->stream>>>(n, eye);
-    ris_k_chol_solve<<<n, 256, sizeof(double) * n, c->stream>>>(n, c->d_chol, eye, inv);
+    ris_k_chol_solve<<<n, 256, sizeof(double) * n, c->stream>>>(n, own ? c->d_chol_J : c->d_chol, eye, inv);
     ris_k_pad2d<<<nb2, 256, 0, c->stream>>>(n, n, np_, inv, minv);
     CU(cudaGetLastError());
-    c->d_minv = minv;
+    slot = minv;
     return RIS_OK;
 }
 
-extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir, double* T_out, double* B_out)
+// The MO-basis three-index tensor over either auxiliary set, for any two coefficient matrices:
+//   T[P][l][r] = sum_{mu nu} C_left[mu,l] (mu nu|P) C_right[nu,r]   (row length ldr >= nr, padding zero),  B = M^-1 T.
+// jset: P runs over the J-fit set (its functions in input order) and M is its metric.  B_out may be null (no fit).
+static int fit_mo(ris_ctx* c, bool jset, int nocc, int nvir, int ldr, const double* C_occ, const double* C_vir, double* T_out,
+                  double* B_out)
 {
-    if (!c || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B_out) return RIS_EINVAL;
-    if ((size_t)c->naux * sizeof(double) > 48 * 1024) return RIS_EINVAL;
+    const bool own = jset && c->jfit;
+    const int nao = c->nao, naux = own ? c->naux_J : c->naux;
+    if ((size_t)naux * sizeof(double) > 48 * 1024 || ldr < nvir) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
     int rc;
-    if ((rc = metric_inverse(c))) return rc;
-    const int nao = c->nao, naux = c->naux;
+    if (B_out && (rc = metric_inverse(c, jset))) return rc;
     const int naop = (nao + 1) & ~1, nauxp = (naux + 1) & ~1, pbp = (naux + 3) & ~3;
-    const long long nia = (long long)nocc * nvir;
-    double *I, *slab, *Ut, *T, *Tt, *CvT, *CoT;
+    const long long nia = (long long)nocc * ldr;
+    double *I, *slab, *Ut, *T, *Tt = nullptr, *CvT, *CoT;
     if ((rc = ws_get(c, WS_FIT_I, sizeof(double) * (size_t)std::max<long long>(c->nelem_real, 1) * pbp, (void**)&I))) return rc;
     if ((rc = ws_get(c, WS_FIT_SLAB, sizeof(double) * (size_t)naux * c->slab_stride, (void**)&slab))) return rc;
     if ((rc = ws_get(c, WS_FIT_UT, sizeof(double) * (size_t)naux * nvir * naop, (void**)&Ut))) return rc;
-    if ((rc = ws_get(c, WS_FIT_TT, sizeof(double) * (size_t)nia * nauxp, (void**)&Tt))) return rc;
+    if (B_out && (rc = ws_get(c, WS_FIT_TT, sizeof(double) * (size_t)nia * nauxp, (void**)&Tt))) return rc;
     if ((rc = ws_get(c, WS_FIT_CV, sizeof(double) * (size_t)nvir * naop, (void**)&CvT))) return rc;
     if ((rc = ws_get(c, WS_FIT_CO, sizeof(double) * (size_t)nocc * naop, (void**)&CoT))) return rc;
     T = T_out;
     if (!T && (rc = ws_get(c, WS_FIT_T, sizeof(double) * (size_t)naux * nia, (void**)&T))) return rc;
     CU(cudaMemsetAsync(I, 0, sizeof(double) * (size_t)std::max<long long>(c->nelem_real, 1) * pbp, c->stream));
     CU(cudaMemsetAsync(slab, 0, sizeof(double) * (size_t)naux * c->slab_stride, c->stream));
+    if (ldr != nvir) CU(cudaMemsetAsync(T, 0, sizeof(double) * (size_t)naux * nia, c->stream));
     const int ny = (naux + 31) / 32;
-    {   // 1. integrals
+    for (int t = 0; t < (own ? 4 : 1); ++t) {   // 1. integrals, one pass per type of auxiliary function
+        const int nl = own ? c->jcnt[t] : naux;
+        if (nl == 0) continue;
+        const int nyl = (nl + 31) / 32;
         int* ctr;
-        if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, (void**)&ctr))) return rc;
-        CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * ny, c->stream));
+        if ((rc = ws_get(c, WS_CTR, sizeof(int) * (size_t)2 * RIS_NCLASS * nyl, (void**)&ctr))) return rc;
+        CU(cudaMemsetAsync(ctr, 0, sizeof(int) * (size_t)2 * RIS_NCLASS * nyl, c->stream));
         for (int oi = 0; oi < RIS_NCLASS; ++oi) {
             const int k = kClassOrder[oi];
             const RisClassPack& pk = c->cls[k];
             if (pk.npairs == 0) continue;
             RisGradParams p{};
-            p.task_ctr = ctr + (size_t)2 * k * ny;
-            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = c->d_aux; p.boys = c->d_boys[pk.la + pk.lb];
-            p.estride = pbp; p.nb = 0; p.p0 = 0; p.p1 = naux; p.grad = I;
+            p.task_ctr = ctr + (size_t)2 * k * nyl;
+            p.pk = pk; p.naux = naux; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = own ? c->d_jlist[t] : c->d_aux; p.aux_type = t;
+            p.boys = c->d_boys[pk.la + pk.lb + (t ? 1 : 0)];
+            p.estride = pbp; p.nb = 0; p.p0 = 0; p.p1 = nl; p.grad = I;
             const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb);
-            ProfScope ps(c, kIntNames[k], (double)naux * (double)pk.nprim * kModelFlopsByE[pk.la + pk.lb],
-                         8.0 * nel * pk.npairs * naux + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
+            ProfScope ps(c, kIntNames[k], (double)nl * (double)pk.nprim * kModelFlopsByE[pk.la + pk.lb + (t ? 1 : 0)],
+                         8.0 * nel * pk.npairs * nl + 8.0 * (double)pk.nprim * RIS_PRIM_FIELDS);
             CU(ris_ints_launchers[k](p, c->stream));
         }
         CU(cudaGetLastError());
@@ -1214,11 +1239,12 @@ extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, co
     {   // 4. GEMM-B: T[P][i][a]
         RisGemmParams g{};
         g.seg[0] = RisGemmSeg{CoT, naop, 0, Ut, naop, (long long)nvir * naop, nao};
-        g.nseg = 1; g.M = nocc; g.N = nvir; g.C = T; g.ldc = nvir; g.bsC = nia;
+        g.nseg = 1; g.M = nocc; g.N = nvir; g.C = T; g.ldc = ldr; g.bsC = nia;
         ProfScope ps(c, "ris_gemm_dmma(T=CoccT*Ut^T)", 2.0 * naux * (double)nocc * nvir * nao,
                      8.0 * ((double)naux * nvir * nao + (double)naux * nia));
         CU(ris_gemm_dense(c->stream, g, naux));
     }
+    if (!B_out) return RIS_OK;
     {   // 5. Tt[(i,a)][Q], then B[P][(i,a)] = sum_Q Minv[P][Q] Tt[(i,a)][Q]
         ProfScope ps(c, "ris_k_transpose", 0.0, 16.0 * naux * (double)nia);
         ris_k_transpose<<<dim3((unsigned)((nia + 31) / 32), (nauxp + 31) / 32), dim3(32, 8), 0, c->stream>>>(naux, nia, nauxp, T, Tt);
@@ -1226,14 +1252,22 @@ extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, co
     }
     {
         RisGemmParams g{};
-        g.seg[0] = RisGemmSeg{Tt, nauxp, 0, c->d_minv, nauxp, 0, naux};
+        g.seg[0] = RisGemmSeg{Tt, nauxp, 0, own ? c->d_minv_J : c->d_minv, nauxp, 0, naux};
         g.nseg = 1; g.M = (int)nia; g.N = naux; g.C = B_out; g.ldc = 1; g.bsC = 0;
-        g.cdiv = 1; g.cpad = (int)nia;
+        g.cdiv = 1; g.cpad = nia;
         ProfScope ps(c, "ris_gemm_dmma(B=Minv*T)", 2.0 * naux * (double)naux * nia, 16.0 * naux * (double)nia);
         CU(ris_gemm_dense(c->stream, g, 1));
     }
     return RIS_OK;
 }
+
+extern "C" int ris_fit_K(ris_ctx* c, int nocc, int nvir, const double* C_occ, const double* C_vir, double* T_out, double* B_out)
+{
+    if (!c || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B_out) return RIS_EINVAL;
+    return fit_mo(c, false, nocc, nvir, nvir, C_occ, C_vir, T_out, B_out);
+}
+
+#include "ris_resp.cuh"
 
 // Metric term of Eq. 27 with a FULL matrix: g[s][A] = sum_{PQ} G[s][P][Q] d(P|Q)/dR_A, positive sign.
 __global__ void __launch_bounds__(128) ris_k_grad_pq_full(int naux, const double* __restrict__ aux, const double* __restrict__ boys1,

@@ -42,7 +42,7 @@ struct RisGemmParams {
     int M, N;
     const int* rowsA;                      // nullable: A row of output row m is rowsA[m] (segment 0 only)
     double* C; long long ldc, bsC;         // dense output: C[z*bsC + m*ldc + col(n)]
-    int cdiv, cpad;                        // cdiv > 0: col(n) = (n / cdiv) * cpad + n % cdiv (padded sub-blocks); else col(n) = n
+    int cdiv; long long cpad;              // cdiv > 0: col(n) = (n / cdiv) * cpad + n % cdiv (padded sub-blocks); else col(n) = n
     const int2* tiles;                     // nullptr: grid.x = m-tile, grid.y = n-tile (dense).  Otherwise tile t =
     long long tile_stride;                 // blockIdx.x covers rows tiles[t].x*BM.., cols tiles[t].y*BN.. and is
                                            // written as a dense BM x BN block at C + z*bsC + t*tile_stride (ld BN)

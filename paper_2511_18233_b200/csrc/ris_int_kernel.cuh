@@ -41,8 +41,8 @@ __host__ __device__ inline size_t ris_int_warp_smem(int kmax, int nb)
 }
 
 // prm.tile: J tile [nb][packed elements] (estride 1); prm.grad: v [nb][naux] (zeroed by the caller).
-// STORE: prm.grad is the integral buffer [packed elements][estride] (P-minor, zeroed by the caller), element el of aux P
-// at grad[el * estride + (P - p0)]; nb is 0.
+// STORE: prm.grad is the integral buffer [packed elements][estride] (function-minor, zeroed by the caller), element el of
+// the auxiliary function with index fn (its record's id) at grad[el * estride + fn]; nb is 0.
 template <int LA, int LB, bool STORE, int AUX = 0>
 __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisGradParams prm)
 {
@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(RIS_GRAD_THREADS, 3) ris_int_kernel(const RisG
             const RisPairRec pr = s_pair[j];
             const double* __restrict__ tile = STORE ? nullptr : prm.tile + (size_t)pk.elem_off + (size_t)(ip0 + j) * NEL;
             // a dead lane (P beyond the range) must not write: the phases below are skipped for it
-            double* __restrict__ out = STORE ? prm.grad + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * (size_t)prm.estride + (Pe - prm.p0)
+            double* __restrict__ out = STORE ? prm.grad + ((size_t)pk.elem_off + (size_t)(ip0 + j) * NEL) * (size_t)prm.estride + fn
                                             : nullptr;
             const double ACx = pr.Ax - Cx, ACy = pr.Ay - Cy, ACz = pr.Az - Cz;
             if (pr.nkA > 0 && (!STORE || live))
@@ -134,13 +134,19 @@ cudaError_t ris_launch_int_t(const RisGradParams& p, cudaStream_t st)
     return cudaGetLastError();
 }
 
-// p.aux_type: type of the auxiliary functions of the launch's list (p functions: the dot-product form only)
+// p.aux_type: type of the auxiliary functions of the launch's list
 template <int LA, int LB, bool STORE>
 cudaError_t ris_launch_int(const RisGradParams& p, cudaStream_t st)
 {
     if (p.pk.npairs <= 0 || p.pk.ntasks <= 0 || p.p1 <= p.p0) return cudaSuccess;
     if constexpr (STORE) {
-        return p.aux_type == 0 ? ris_launch_int_t<LA, LB, true, 0>(p, st) : cudaErrorInvalidValue;
+        switch (p.aux_type) {
+        case 0: return ris_launch_int_t<LA, LB, true, 0>(p, st);
+        case 1: return ris_launch_int_t<LA, LB, true, 1>(p, st);
+        case 2: return ris_launch_int_t<LA, LB, true, 2>(p, st);
+        case 3: return ris_launch_int_t<LA, LB, true, 3>(p, st);
+        default: return cudaErrorInvalidValue;
+        }
     } else {
         switch (p.aux_type) {
         case 0: return ris_launch_int_t<LA, LB, false, 0>(p, st);

@@ -19,6 +19,7 @@ _lib = None
 EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host", "ris_grad_host",
     "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full", "ris_set_jfit", "ris_naux_J", "ris_metric_J",
+    "ris_resp_setup", "ris_resp_matvec", "ris_resp_free",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
     "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
@@ -53,6 +54,9 @@ def load_library():
     lib.ris_metric.argtypes = [vp, vp]
     lib.ris_metric_J.argtypes = [vp, vp]
     lib.ris_set_jfit.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_resp_setup.argtypes = [vp, ci, ci, vp, vp]
+    lib.ris_resp_matvec.argtypes = [vp, ci, cd, cd, cd, vp, vp]
+    lib.ris_resp_free.argtypes = [vp]
     lib.ris_fit_K.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ_full.argtypes = [vp, ci, vp, vp]
     lib.ris_grad_J_host.argtypes = [vp, ci, vp, vp, vp]
@@ -273,6 +277,30 @@ class RisContext:
         with self._ordered():
             _check(self._lib.ris_metric_J(self._h, self._dev(M, (n, n))))
         return M
+
+    # ---- coupling-matrix products (excitation-energy stage, ris Z-vector)
+    def resp_setup(self, C_occ, C_vir):
+        nocc, nvir = C_occ.shape[1], C_vir.shape[1]
+        with self._ordered():
+            _check(self._lib.ris_resp_setup(self._h, nocc, nvir, self._dev(C_occ, (self.nao, nocc)), self._dev(C_vir, (self.nao, nvir))))
+        self._resp_shape = (nocc, nvir)
+
+    def resp_matvec(self, X, cJ, cKA, cKB, out=None):
+        """sigma[v][i][a] = sum_jb [cJ (ia|jb) - cKA (ij|ab) - cKB (ib|ja)]^ris X[v][j][b]"""
+        shape = getattr(self, "_resp_shape", None)
+        if shape is None:
+            raise RisError("resp_matvec before resp_setup")
+        nvec = X.shape[0]
+        if out is None:
+            out = self._torch.empty((nvec,) + shape, dtype=self._torch.float64, device=self.device)
+        with self._ordered():
+            _check(self._lib.ris_resp_matvec(self._h, nvec, float(cJ), float(cKA), float(cKB), self._dev(X, (nvec,) + shape),
+                                             self._dev(out, (nvec,) + shape)))
+        return out
+
+    def resp_free(self):
+        _check(self._lib.ris_resp_free(self._h))
+        self._resp_shape = None
 
     # ---- host-buffer calls (numpy arrays or CPU tensors, float64, C-contiguous; copies happen inside the C call)
     @staticmethod
