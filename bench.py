@@ -9,8 +9,11 @@ the metric string (3c2e-derivative primitive triplets/s, % FP64 peak) in the sam
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
-N > 1 (torchrun): the path shards over independent states: every rank runs the same
-molecule with its own batch of states, no data-path collective; value = time / (N * nbatch)  ("scaling": "weak").
+N > 1 (torchrun), default `--shard aux`: ONE batch of states sharded over the auxiliary index (DESIGN.md
+"Multi-GPU"): rank r holds B[:, P_r] only and evaluates ris_grad_J_range / ris_grad_K_range on its block of aux functions,
+one NCCL all-reduce of (nbatch_J + nbatch_K) natoms 3 doubles completes the gradients on every rank; total work is fixed,
+value = time / nbatch ("scaling": "strong").  `--shard states`: every rank runs the same molecule with its own batch of
+states (independent problems), no data-path collective; value = time / (N * nbatch)  ("scaling": "weak").
 """
 from __future__ import annotations
 
@@ -50,6 +53,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = the largest")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--shard", default="aux", choices=["aux", "states"], help="N > 1: what the ranks split (see the module docstring)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-baseline-full", action="store_true",
@@ -220,8 +224,16 @@ def run_ours(args):
         torch.cuda.synchronize()
         setup_ms = min(setup_ms, (time.perf_counter() - t0) * 1e3)
 
+    sharded = world > 1 and args.shard == "aux"
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k))).pin_memory()
-            for k in ("D", "c_aux", "d_aux", "C_occ", "C_vir", "B")}
+            for k in ("D", "c_aux", "d_aux", "C_occ", "C_vir")}
+    if sharded:
+        from paper_2511_18233_b200 import shard
+        my_aux = shard.aux_range(ctx.naux, rank, world)
+        host["B"] = torch.from_numpy(np.ascontiguousarray(wl.B[:, my_aux.start:my_aux.stop])).pin_memory()   # this rank's slice only
+        gJK = torch.empty((nbJ + nbK, mol.natoms, 3), dtype=torch.float64, device=dev)
+    else:
+        host["B"] = torch.from_numpy(np.ascontiguousarray(wl.B)).pin_memory()
     d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
     gJ = torch.empty((nbJ, mol.natoms, 3), dtype=torch.float64, device=dev)
     gK = torch.empty((nbK, mol.natoms, 3), dtype=torch.float64, device=dev)
@@ -234,10 +246,15 @@ def run_ours(args):
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if timed else None
         if timed:
             ev[0].record()
-        ctx.grad_J(d["D"], d["c_aux"], out=gJ)
-        if timed:
-            ev[1].record()
-        ctx.grad_K(d["C_occ"], d["C_vir"], d["B"], out=gK)
+        if sharded:         # J and K shares + the all-reduce (charged to the K interval below)
+            if timed:
+                ev[1].record()
+            shard.grad_JK_sharded(ctx, d["D"], d["c_aux"], d["C_occ"], d["C_vir"], d["B"], out=gJK)
+        else:
+            ctx.grad_J(d["D"], d["c_aux"], out=gJ)
+            if timed:
+                ev[1].record()
+            ctx.grad_K(d["C_occ"], d["C_vir"], d["B"], out=gK)
         if timed:
             ev[2].record()
         ctx.grad_PQ(d["c_aux"], d["d_aux"], out=gQ)
@@ -281,9 +298,11 @@ def run_ours(args):
     # ms per state: every term divided by ITS OWN number of states (config 2 runs 2 J/PQ states and 1 K state); the
     # remainder of the step (launch gaps between the calls) is charged to the larger batch.  Equal batches: ms_step/nbatch.
     gap = max(ms_total - (ms_J + ms_K + ms_Q), 0.0)
-    value = (ms_J / nbJ + ms_K / nbK + ms_Q / nbJ + gap / nstates) / args.steps / world
+    value = (ms_J / nbJ + ms_K / nbK + ms_Q / nbJ + gap / nstates) / args.steps / (1 if sharded else world)
     per_term = {"J_ms_per_state": round(ms_J / nbJ / args.steps, 4), "K_ms_per_state": round(ms_K / nbK / args.steps, 4),
                 "PQ_ms_per_state": round(ms_Q / nbJ / args.steps, 4), "nbatch_J": nbJ, "nbatch_K": nbK}
+    if sharded:
+        per_term["note"] = "aux-sharded: K_ms_per_state holds this step's J share + K share + the all-reduce (max over ranks)"
 
     # ---- per-kernel accounting from the CUDA events the library records around every launch (same stream)
     groups = {}
@@ -332,7 +351,13 @@ def run_ours(args):
         hJ = np.empty((nbJ, mol.natoms, 3)); hK = np.empty((nbK, mol.natoms, 3)); hQ = np.empty((nbJ, mol.natoms, 3))
 
         def step_host():
-            ctx.grad_host(host["D"], host["c_aux"], host["d_aux"], host["C_occ"], host["C_vir"], host["B"], out=(hJ, hK, hQ))
+            if sharded:     # this rank's inputs up, its shares + the all-reduce, the gradients down
+                t = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+                a, b = shard.grad_JK_sharded(ctx, t["D"], t["c_aux"], t["C_occ"], t["C_vir"], t["B"], out=gJK)
+                q = ctx.grad_PQ(t["c_aux"], t["d_aux"], out=gQ)
+                hJ[...] = a.cpu().numpy(); hK[...] = b.cpu().numpy(); hQ[...] = q.cpu().numpy()
+            else:
+                ctx.grad_host(host["D"], host["c_aux"], host["d_aux"], host["C_occ"], host["C_vir"], host["B"], out=(hJ, hK, hQ))
 
         step_host()
         barrier()
@@ -349,6 +374,8 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             t_e2e = float(t.item())
         # the end-to-end result is the resident-input result (same kernels, other copy schedule)
+        if sharded:
+            gJ, gK = gJK[:nbJ], gJK[nbJ:]
         e2e_err = max(float(np.abs(h - g.cpu().numpy()).max() / max(1e-300, float(g.abs().max())))
                       for h, g in ((hJ, gJ), (hK, gK), (hQ, gQ)))
         if not e2e_err <= 5e-14:
@@ -356,11 +383,13 @@ def run_ours(args):
         h2d = 8 * (host["D"].numel() + host["c_aux"].numel() + host["d_aux"].numel() + host["C_occ"].numel()
                    + host["C_vir"].numel() + host["B"].numel())
         d2h = 8 * (hJ.size + hK.size + hQ.size)
-        e2e = {"value": round(t_e2e / (world * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        e2e = {"value": round(t_e2e / ((1 if sharded else world) * nstates), 4), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": n_e2e, "e2e_checked": True, "e2e_max_dev_of_scale": e2e_err, "ms_per_step_each": [round(r, 2) for r in reps],
-               "median_ms_per_state": round(sorted(reps)[len(reps) // 2] / (world * nstates), 4),
-               "how": "ris_grad_host (J + K + PQ in one call) on pinned host buffers; host wall clock around the call, which returns "
-                      "after the D2H copy of the gradients; B goes up in P chunks on a copy stream under the J kernels and the GEMMs"}
+               "median_ms_per_state": round(sorted(reps)[len(reps) // 2] / ((1 if sharded else world) * nstates), 4),
+               "how": ("aux-sharded: per rank, its inputs (B[:, P_r] only) from pinned host memory, ris_grad_J_range + ris_grad_K_range, "
+                       "the NCCL all-reduce, ris_grad_PQ, gradients back to the host; host wall clock, max over ranks; bytes are per rank") if sharded else
+                      ("ris_grad_host (J + K + PQ in one call) on pinned host buffers; host wall clock around the call, which returns "
+                       "after the D2H copy of the gradients; B goes up in P chunks on a copy stream under the J kernels and the GEMMs")}
 
     # ---- NEXT-1 (reported beside the metric, outside the timed step): the J-type fitting step on the same workload
     ctx.fit_J(d["D"])                                       # builds the metric's Cholesky factor (one-off per geometry)
@@ -388,22 +417,66 @@ def run_ours(args):
     for g in fit["ris_fit_K_kernels"].values():
         g["tflops"] = round(g["tflops"] / (g["ms"] * 1e-3) * 1e-12, 2) if g["ms"] > 0 else None
 
+    # ---- NEXT-3 / NEXT-4c (reported beside the metric): the ris coupling-matrix products for a block of 8 trial vectors
+    resp = None
+    try:
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        ctx.resp_setup(d["C_occ"], d["C_vir"])
+        r1.record()
+        torch.cuda.synchronize()
+        resp = {"ris_resp_setup_ms": round(r0.elapsed_time(r1), 2), "nvec": 8,
+                "what": "sigma = sum_jb [cJ (ia|jb) - cKA (ij|ab) - cKB (ib|ja)]^ris X_jb, 8 vectors per call"}
+        Xv = torch.randn((8, wl.nocc, wl.nvir), dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        sg = torch.empty_like(Xv)
+        for label, coef in (("tda_A_ms", (2.0, 0.25, 0.0)), ("z_vector_ApB_ms", (4.0, 0.25, 0.25))):
+            ctx.resp_matvec(Xv, *coef, out=sg)
+            torch.cuda.synchronize()
+            ctx.profile_reset()
+            r0.record()
+            for _ in range(3):
+                ctx.resp_matvec(Xv, *coef, out=sg)
+            r1.record()
+            torch.cuda.synchronize()
+            resp[label] = round(r0.elapsed_time(r1) / 3, 3)
+            kk = {}
+            for name, ms, fl, by in ctx.profile():
+                g = kk.setdefault(name, {"ms": 0.0, "tflops": 0.0, "gbs": 0.0})
+                g["ms"] += ms / 3; g["tflops"] += fl / 3; g["gbs"] += by / 3
+            for g in kk.values():
+                t = g["ms"] * 1e-3
+                g["tflops"] = round(g["tflops"] / t * 1e-12, 2) if t > 0 else None
+                g["gbs"] = round(g["gbs"] / t * 1e-9, 1) if t > 0 else None
+                g["ms"] = round(g["ms"], 3)
+            resp[label.replace("_ms", "_kernels")] = kk
+            gm = [g for n, g in kk.items() if n.startswith("ris_gemm")]
+            if gm:
+                tot = sum(g["ms"] for g in gm)
+                resp[label.replace("_ms", "_gemm_frac_of_dmma_peak")] = round(sum(g["tflops"] * g["ms"] for g in gm) / tot / mma_peak, 4)
+        ctx.resp_free()
+    except Exception as exc:                  # the block is an extra: a failure here must not lose the metric line
+        resp = {"error": repr(exc)}
+
     line = {
         "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": False,
+        "scaling": "strong" if sharded else "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl.name, "natoms": mol.natoms, "nao": mol.nao, "naux": mol.natoms, "nocc": wl.nocc,
                    "nvir": wl.nvir, "nbatch_J": nbJ, "nbatch_K": nbK, "schwarz_tol": wl.schwarz_tol,
                    "p_batch": ctx.p_batch, "l2": "inputs larger than L2 (B alone is %.2f GB)" % (host["B"].numel() * 8e-9)
                    if host["B"].numel() * 8 > 200e6 else "inputs smaller than L2; no flush (latency-bound case)",
-                   "step": "ris_grad_J + ris_grad_K + ris_grad_PQ, all states; ris_setup excluded (one-off per geometry)"},
+                   "step": "ris_grad_J + ris_grad_K + ris_grad_PQ, all states; ris_setup excluded (one-off per geometry)",
+                   "parallelism": ("aux%d: one batch of states, aux index split over %d ranks, one all-reduce" % (world, world)) if sharded
+                                  else ("replicas%d: every rank its own batch of states" % world if world > 1 else "single GPU")},
         "per_term": per_term,
         "setup_ms": round(setup_ms, 2), "setup_first_ms": round(setup_first_ms, 2), "e2e": e2e, "gpu_launches": len(prof),
         "roofline": roofline, "integral_kernels": integrals,
         "gamma_gemm": {"ms_per_step": round(gemm_ms / args.steps, 4),
                        "tflops": round(gemm_fl / (gemm_ms * 1e-3) * 1e-12, 3) if gemm_ms else None,
                        "fp64_mma_peak_tflops": round(mma_peak, 2)},
-        "kernels": kernels, "fit_step": fit, "clocks": clocks,
+        "kernels": kernels, "fit_step": fit, "resp_step": resp, "clocks": clocks,
     }
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:

@@ -142,6 +142,19 @@ int ris_grad_host(ris_ctx* ctx, int nbatch_J, const double* D, const double* c_a
                   int nocc, int nvir, const double* C_occ, const double* C_vir, const double* B, double* grad_J,
                   double* grad_K, double* grad_PQ);
 
+/* ---- Sharding over the auxiliary index (NEXT-4a) ------------------------------------------------------
+ * Both three-centre contractions are sums over the auxiliary index, so the work of ONE state splits over GPUs by ranges of
+ * it; the partial gradients add up to the full one (one all-reduce of nbatch natoms 3 doubles, done by the caller, e.g.
+ * paper_2511_18233_b200/shard.py over NCCL).
+ * ris_grad_K_range: the K-type contraction restricted to aux functions P in [p_lo, p_hi); B_local device
+ *   [nbatch][p_hi - p_lo][nocc][nvir] holds ONLY this range (each GPU keeps its own slice of B); grad is overwritten with the
+ *   partial result.  An empty range gives zeros.
+ * ris_grad_J_range: the J-type contraction restricted to J-fit functions f in [f_lo, f_hi); c_aux keeps its full row
+ *   length [nbatch][naux_J]. */
+int ris_grad_K_range(ris_ctx* ctx, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                     const double* B_local, int p_lo, int p_hi, double* grad);
+int ris_grad_J_range(ris_ctx* ctx, int nbatch, const double* D, const double* c_aux, int f_lo, int f_hi, double* grad);
+
 /* ---- J-fit auxiliary set with p functions -----------------------------------
  * ris_set_jfit replaces, for the J-TYPE calls only (ris_grad_J, ris_fit_J, ris_grad_PQ and their *_host forms, ris_metric_J),
  * the default set by nshell_aux auxiliary SHELLS: shell k sits on atom aux_atom[k], has l = aux_l[k] in {0, 1} and exponent

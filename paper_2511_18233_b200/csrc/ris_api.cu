@@ -71,6 +71,7 @@ struct ris_ctx {
     double* d_jfn = nullptr;           // [naux_J][RIS_AUX_FIELDS] records in FUNCTION order (two-centre kernels)
     double* d_jlist[4] = {nullptr};    // the same records grouped by type: s, p_x, p_y, p_z (class kernels: one launch each)
     int jcnt[4] = {0, 0, 0, 0};
+    std::vector<int> h_jlist_fn[4];    // function index of every list entry (ascending): ranges of functions -> list positions
     int *d_atom_fn_off = nullptr, *d_atom_fn = nullptr;   // CSR atom -> functions of the J-fit set
     double* d_chol_J = nullptr;        // Cholesky factor of the J-fit metric (explicit set only; else d_chol)
     int *d_shell_atom = nullptr, *d_shell_l = nullptr, *d_shell_nprim = nullptr, *d_shell_poff = nullptr, *d_shell_ao = nullptr;
@@ -728,9 +729,20 @@ static int det_end(ris_ctx* c, int nbatch, const unsigned long long* acc, double
 }
 
 // --------------------------------------------------------------------------------------- J
+static int grad_J_impl(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad, int f_lo, int f_hi);
 extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad)
 {
-    if (!c || nbatch < 1 || !D || !c_aux || !grad) return RIS_EINVAL;
+    return c ? grad_J_impl(c, nbatch, D, c_aux, grad, 0, c->naux_J) : RIS_EINVAL;
+}
+extern "C" int ris_grad_J_range(ris_ctx* c, int nbatch, const double* D, const double* c_aux, int f_lo, int f_hi, double* grad)
+{
+    return c ? grad_J_impl(c, nbatch, D, c_aux, grad, f_lo, f_hi) : RIS_EINVAL;
+}
+
+// [f_lo, f_hi): the J-fit FUNCTIONS this call sums over (c_aux keeps its full row length)
+static int grad_J_impl(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad, int f_lo, int f_hi)
+{
+    if (!c || nbatch < 1 || !D || !c_aux || !grad || f_lo < 0 || f_hi > c->naux_J || f_lo > f_hi) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     const long long nao2 = (long long)c->nao * c->nao;
@@ -744,12 +756,22 @@ extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double*
         int rc = ws_get(c, WS_TILE, sizeof(double) * (size_t)nb * c->nelem_real, (void**)&tile);
         if (rc) return rc;
         if ((rc = pack_tiles(c, D + (size_t)s0 * nao2, nao2, nb, tile, c->nelem_real))) return rc;
-        for (int t = 0; t < 4; ++t)         // one pass per type of auxiliary function: s, p_x, p_y, p_z
-            if (c->jcnt[t] > 0 &&
-                (rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux_J, nb, 0, c->jcnt[t],
+        for (int t = 0; t < 4; ++t) {       // one pass per type of auxiliary function: s, p_x, p_y, p_z
+            // list positions whose function index lies in [f_lo, f_hi): the lists are in ascending function order
+            int q0 = 0, q1 = c->jcnt[t];
+            if (c->jfit) {
+                const std::vector<int>& fn = c->h_jlist_fn[t];
+                q0 = (int)(std::lower_bound(fn.begin(), fn.end(), f_lo) - fn.begin());
+                q1 = (int)(std::lower_bound(fn.begin(), fn.end(), f_hi) - fn.begin());
+            } else {
+                q0 = f_lo; q1 = f_hi;
+            }
+            if (q1 > q0 &&
+                (rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux_J, nb, q0, q1,
                                      grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr,
                                      c->d_jlist[t], t, c->naux_J)))
                 return rc;
+        }
     }
     return det_end(c, nbatch, det, grad);
 }
@@ -928,6 +950,7 @@ extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom,
     }
     CU(cudaSetDevice(c->device));
     std::vector<double> fn((size_t)RIS_AUX_FIELDS * nfn), lists[4];
+    std::vector<int> lfn[4];
     std::vector<std::vector<int>> on_atom(c->natoms);
     int f = 0;
     for (int i = 0; i < nshell_aux; ++i)
@@ -936,6 +959,7 @@ extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom,
             aux_record(r, &c->h_coords[3 * (size_t)aux_atom[i]], aux_exp[i], aux_l[i], comp, aux_atom[i], f);
             std::vector<double>& L = lists[aux_l[i] ? 1 + comp : 0];
             L.insert(L.end(), r, r + RIS_AUX_FIELDS);
+            lfn[aux_l[i] ? 1 + comp : 0].push_back(f);
             on_atom[aux_atom[i]].push_back(f);
         }
     std::vector<int> off(c->natoms + 1, 0), idx;
@@ -945,6 +969,7 @@ extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom,
     if ((rc = dev_upload(c, &c->d_jfn, fn.data(), fn.size()))) return rc;
     for (int t = 0; t < 4; ++t) {
         c->jcnt[t] = (int)(lists[t].size() / RIS_AUX_FIELDS);
+        c->h_jlist_fn[t] = lfn[t];
         c->d_jlist[t] = nullptr;
         if (c->jcnt[t] && (rc = dev_upload(c, &c->d_jlist[t], lists[t].data(), lists[t].size()))) return rc;
     }
@@ -1325,14 +1350,20 @@ __global__ void ris_k_pad_rows(int rows, int cols, int ld, const int* __restrict
 // B of state s is resident; the compute stream waits for it right before that chunk's GEMM-1, so the H2D copy runs
 // ahead of the GEMMs instead of in front of them.
 constexpr int RIS_COPY_CHUNKS = 8;     // *_host: B of a state goes up in this many P ranges, GEMM-1 follows chunk by chunk
+// [p_lo, p_hi): the aux functions this call sums over (all of them, or one rank's share when the K term is sharded over P);
+// B then holds only those: [nbatch][p_hi - p_lo][nocc][nvir].
 static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
-                       const double* B, double* grad, const cudaEvent_t* b_ready)
+                       const double* B, double* grad, const cudaEvent_t* b_ready, int p_lo = 0, int p_hi = -1)
 {
-    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !B || !grad) return RIS_EINVAL;
+    if (!c || nbatch < 1 || nocc < 1 || nvir < 1 || !C_occ || !C_vir || !grad) return RIS_EINVAL;
+    if (p_hi < 0) p_hi = c->naux;
+    if (p_lo < 0 || p_hi > c->naux || p_lo > p_hi) return RIS_EINVAL;
+    const int nloc = p_hi - p_lo;
+    if (!B && nloc > 0) return RIS_EINVAL;              // an empty share has no B
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
-    if (c->nelem_real == 0) return RIS_OK;                // every shell pair screened out: the gradient is exactly zero
-    const int nao = c->nao, naux = c->naux;
+    if (c->nelem_real == 0 || nloc == 0) return RIS_OK;   // every shell pair screened out / empty share: exactly zero
+    const int nao = c->nao, naux = nloc;
     const int cap = nb_cap(c, true);
     if (cap < 1) return RIS_ENOMEM;
     const int nbmax = next_nb(nbatch, cap);
@@ -1373,7 +1404,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
                 CU(cudaMemsetAsync(tile, 0, sizeof(double) * (size_t)nb * pbp * c->nelem_real, c->stream));
             }
             for (int s = 0; s < nb; ++s) {
-                const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;
+                const double* Bs = B + (((size_t)(s0 + s) * naux + p0) * nocc) * nvir;      // p0: offset within the share
                 // GEMM-1: HT[nu][(P,i)] = sum_a C_vir[nu][a] B[P][i][a]; with b_ready, in RIS_COPY_CHUNKS column chunks
                 // (ranges of P), each waiting only for its own slice of B
                 const int nch = (b_ready && p0 == 0 && np == naux) ? RIS_COPY_CHUNKS : 1;
@@ -1405,7 +1436,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
                     CU(ris_gemm_scatter(c->stream, g, c->ntiles));
                 }
             }
-            if ((rc = launch_classes(c, tile, (long long)pbp * c->nelem_real, pbp, 1, nullptr, nb, p0, p0 + np,
+            if ((rc = launch_classes(c, tile, (long long)pbp * c->nelem_real, pbp, 1, nullptr, nb, p_lo + p0, p_lo + p0 + np,
                                      grad + (size_t)s0 * c->natoms * 3, det ? det + (size_t)2 * s0 * c->natoms * 3 : nullptr)))
                 return rc;
         }
@@ -1417,6 +1448,13 @@ extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const doub
                           const double* B, double* grad)
 {
     return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B, grad, nullptr);
+}
+
+extern "C" int ris_grad_K_range(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
+                                const double* B_local, int p_lo, int p_hi, double* grad)
+{
+    if (!c || p_lo < 0 || p_hi < p_lo) return RIS_EINVAL;
+    return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B_local, grad, nullptr, p_lo, p_hi);
 }
 
 // --------------------------------------------------------------------------------------- PQ (S5)

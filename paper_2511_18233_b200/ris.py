@@ -19,7 +19,7 @@ _lib = None
 EXPORTS = [
     "ris_setup", "ris_grad_J", "ris_grad_K", "ris_grad_PQ", "ris_grad_J_host", "ris_grad_K_host", "ris_grad_PQ_host", "ris_grad_host",
     "ris_fit_J", "ris_metric", "ris_fit_K", "ris_grad_PQ_full", "ris_set_jfit", "ris_naux_J", "ris_metric_J",
-    "ris_resp_setup", "ris_resp_matvec", "ris_resp_free",
+    "ris_resp_setup", "ris_resp_matvec", "ris_resp_free", "ris_grad_K_range", "ris_grad_J_range",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
     "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
@@ -50,6 +50,8 @@ def load_library():
     lib.ris_grad_J.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_grad_K.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
     lib.ris_grad_PQ.argtypes = [vp, ci, vp, vp, vp]
+    lib.ris_grad_K_range.argtypes = [vp, ci, ci, ci, vp, vp, vp, ci, ci, vp]
+    lib.ris_grad_J_range.argtypes = [vp, ci, vp, vp, ci, ci, vp]
     lib.ris_fit_J.argtypes = [vp, ci, vp, vp, vp]
     lib.ris_metric.argtypes = [vp, vp]
     lib.ris_metric_J.argtypes = [vp, vp]
@@ -224,6 +226,29 @@ class RisContext:
             _check(self._lib.ris_grad_K(self._h, nb, nocc, nvir, self._dev(C_occ, (self.nao, nocc)),
                                         self._dev(C_vir, (self.nao, nvir)), self._dev(B, (nb, self.naux, nocc, nvir)),
                                         self._dev(out, (nb, self.natoms, 3))))
+        return out
+
+    def grad_K_range(self, C_occ, C_vir, B_local, p_lo, p_hi, out=None):
+        """Partial K-type gradient over aux functions [p_lo, p_hi); B_local holds only that range."""
+        nb, nocc, nvir = B_local.shape[0], C_occ.shape[1], C_vir.shape[1]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        with self._ordered():
+            _check(self._lib.ris_grad_K_range(self._h, nb, nocc, nvir, self._dev(C_occ, (self.nao, nocc)),
+                                              self._dev(C_vir, (self.nao, nvir)),
+                                              self._dev(B_local, (nb, p_hi - p_lo, nocc, nvir)), int(p_lo), int(p_hi),
+                                              self._dev(out, (nb, self.natoms, 3))))
+        return out
+
+    def grad_J_range(self, D, c_aux, f_lo, f_hi, out=None):
+        """Partial J-type gradient over J-fit functions [f_lo, f_hi)."""
+        nb = D.shape[0]
+        if out is None:
+            out = self._torch.empty((nb, self.natoms, 3), dtype=self._torch.float64, device=self.device)
+        with self._ordered():
+            _check(self._lib.ris_grad_J_range(self._h, nb, self._dev(D, (nb, self.nao, self.nao)),
+                                              self._dev(c_aux, (nb, self.naux_J)), int(f_lo), int(f_hi),
+                                              self._dev(out, (nb, self.natoms, 3))))
         return out
 
     def grad_PQ(self, c_aux, d_aux, out=None):
