@@ -56,6 +56,8 @@ def parse_args():
     ap.add_argument("--shard", default="aux", choices=["aux", "states"], help="N > 1: what the ranks split (see the module docstring)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the fit_step / resp_step blocks reported beside the metric "
+                    "(profiler runs: the launch list then holds the setup, the peak probes and the steps only)")
     ap.add_argument("--cpu-baseline-full", action="store_true",
                     help="time the oracle over the WHOLE workload (minutes on config 3; not for config 4) and single-threaded")
     ap.add_argument("--oracle-aux", type=int, default=0, help="aux functions in the oracle's timed sample (0 = auto)")
@@ -391,35 +393,39 @@ def run_ours(args):
                       ("ris_grad_host (J + K + PQ in one call) on pinned host buffers; host wall clock around the call, which returns "
                        "after the D2H copy of the gradients; B goes up in P chunks on a copy stream under the J kernels and the GEMMs")}
 
-    # ---- NEXT-1 (reported beside the metric, outside the timed step): the J-type fitting step on the same workload
-    ctx.fit_J(d["D"])                                       # builds the metric's Cholesky factor (one-off per geometry)
-    torch.cuda.synchronize()
-    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    f0.record()
-    for _ in range(3):
-        ctx.fit_J(d["D"])
-    f1.record()
-    torch.cuda.synchronize()
-    fit = {"ris_fit_J_ms_per_state": round(f0.elapsed_time(f1) / 3 / nbJ, 4), "nbatch": nbJ,
-           "what": "v_P = sum D (mu nu|P) on the undifferentiated class kernels + Cholesky solve c = M^-1 v"}
-    ctx.fit_K(d["C_occ"], d["C_vir"])                       # builds M^-1, sizes the scratch
-    torch.cuda.synchronize()
-    ctx.profile_reset()
-    f0.record()
-    ctx.fit_K(d["C_occ"], d["C_vir"])
-    f1.record()
-    torch.cuda.synchronize()
-    fit["ris_fit_K_ms"] = round(f0.elapsed_time(f1), 3)
-    fit["ris_fit_K_kernels"] = {}
-    for name, ms, fl, by in ctx.profile():
-        g = fit["ris_fit_K_kernels"].setdefault(name, {"ms": 0.0, "tflops": 0.0})
-        g["ms"] = round(g["ms"] + ms, 3); g["tflops"] += fl
-    for g in fit["ris_fit_K_kernels"].values():
-        g["tflops"] = round(g["tflops"] / (g["ms"] * 1e-3) * 1e-12, 2) if g["ms"] > 0 else None
+    fit = None
+    if not args.no_extras and not sharded:
+        # ---- NEXT-1 (reported beside the metric, outside the timed step): the J-type fitting step on the same workload
+        ctx.fit_J(d["D"])                                       # builds the metric's Cholesky factor (one-off per geometry)
+        torch.cuda.synchronize()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(3):
+            ctx.fit_J(d["D"])
+        f1.record()
+        torch.cuda.synchronize()
+        fit = {"ris_fit_J_ms_per_state": round(f0.elapsed_time(f1) / 3 / nbJ, 4), "nbatch": nbJ,
+               "what": "v_P = sum D (mu nu|P) on the undifferentiated class kernels + Cholesky solve c = M^-1 v"}
+        ctx.fit_K(d["C_occ"], d["C_vir"])                       # builds M^-1, sizes the scratch
+        torch.cuda.synchronize()
+        ctx.profile_reset()
+        f0.record()
+        ctx.fit_K(d["C_occ"], d["C_vir"])
+        f1.record()
+        torch.cuda.synchronize()
+        fit["ris_fit_K_ms"] = round(f0.elapsed_time(f1), 3)
+        fit["ris_fit_K_kernels"] = {}
+        for name, ms, fl, by in ctx.profile():
+            g = fit["ris_fit_K_kernels"].setdefault(name, {"ms": 0.0, "tflops": 0.0})
+            g["ms"] = round(g["ms"] + ms, 3); g["tflops"] += fl
+        for g in fit["ris_fit_K_kernels"].values():
+            g["tflops"] = round(g["tflops"] / (g["ms"] * 1e-3) * 1e-12, 2) if g["ms"] > 0 else None
 
     # ---- NEXT-3 / NEXT-4c (reported beside the metric): the ris coupling-matrix products for a block of 8 trial vectors
     resp = None
     try:
+        if args.no_extras or sharded:
+            raise StopIteration
         torch.cuda.synchronize()
         r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         r0.record()
@@ -455,6 +461,8 @@ def run_ours(args):
                 tot = sum(g["ms"] for g in gm)
                 resp[label.replace("_ms", "_gemm_frac_of_dmma_peak")] = round(sum(g["tflops"] * g["ms"] for g in gm) / tot / mma_peak, 4)
         ctx.resp_free()
+    except StopIteration:
+        resp = None
     except Exception as exc:                  # the block is an extra: a failure here must not lose the metric line
         resp = {"error": repr(exc)}
 
