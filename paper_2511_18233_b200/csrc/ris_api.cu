@@ -763,8 +763,10 @@ static int grad_J_impl(ris_ctx* c, int nbatch, const double* D, const double* c_
                 const std::vector<int>& fn = c->h_jlist_fn[t];
                 q0 = (int)(std::lower_bound(fn.begin(), fn.end(), f_lo) - fn.begin());
                 q1 = (int)(std::lower_bound(fn.begin(), fn.end(), f_hi) - fn.begin());
-            } else {
+            } else if (t == 0) {            // default set: the s list IS the function order; there are no p lists
                 q0 = f_lo; q1 = f_hi;
+            } else {
+                q0 = q1 = 0;
             }
             if (q1 > q0 &&
                 (rc = launch_classes(c, tile, c->nelem_real, 1, 0, c_aux + (size_t)s0 * c->naux_J, nb, q0, q1,
