@@ -506,3 +506,86 @@ def coupling_ris(mol, C_occ, C_vir, cJ, cKA, cKB):
 def matvec_ris(mol, C_occ, C_vir, X, cJ, cKA, cKB):
     """sigma[v][i][a] = sum_jb K[i,a,j,b] X[v][j][b]"""
     return np.einsum("iajb,vjb->via", coupling_ris(mol, C_occ, C_vir, cJ, cKA, cKB), _f64(X))
+
+
+# --------------------------------------------------------------------------- spherical-harmonic shells (NEXT-4b)
+# PAPER.md:170 runs def2-TZVP, a spherical-harmonic basis; SURVEY.md 8(f) NEXT-4 lists the shells, DESIGN.md reading R-sph
+# fixes the convention: a spherical shell of degree l holds the 2l+1 functions
+#     chi_{lm}(r) = S_lm(r - A) sum_k d_k exp(-a_k |r - A|^2),     m = -l .. l  (in this order),
+# S_lm the REAL regular solid harmonic in Racah normalisation, S_lm = sqrt(4 pi/(2l+1)) r^l Y_lm^{real}
+# (S_00 = 1, S_1m = y, z, x, S_20 = z^2 - (x^2 + y^2)/2, ...).  Its expansion in Cartesian monomials is written out
+# from the closed formula (Helgaker, Jorgensen, Olsen, "Molecular Electronic-Structure Theory", Eqs. 6.4.47-6.4.50):
+#     S_lm = N_lm sum_{t=0}^{[(l-|m|)/2]} sum_{u=0}^{t} sum_{v} C^{lm}_{tuv} x^{2t+|m|-2(u+v)} y^{2(u+v)} z^{l-2t-|m|},
+#     v = v_m, v_m + 1, ..., [|m|/2 - v_m] + v_m,   v_m = 0 (m >= 0) or 1/2 (m < 0),
+#     C^{lm}_{tuv} = (-1)^{t+v-v_m} (1/4)^t binom(l,t) binom(l-t,|m|+t) binom(t,u) binom(|m|,2v),
+#     N_lm = 1/(2^{|m|} l!) sqrt(2 (l+|m|)! (l-|m|)! / 2^{delta_{m0}}).
+# Every integral over spherical functions is the same linear combination of the Cartesian ones, so the contractions in the
+# spherical AO basis are the Cartesian ones with D_cart = U^T D_sph U, C_cart = U^T C_sph (U block diagonal).
+
+def _cart_comps(l):
+    return [(lx, ly, l - lx - ly) for lx in range(l, -1, -1) for ly in range(l - lx, -1, -1)]
+
+
+def solid_harmonic_cart(l: int) -> np.ndarray:
+    """T[m + l][c]: coefficient of the Cartesian monomial c (order lx descending, then ly descending) in S_lm."""
+    from math import comb, factorial, sqrt
+    comps = _cart_comps(l)
+    T = np.zeros((2 * l + 1, len(comps)))
+    for m in range(-l, l + 1):
+        am = abs(m)
+        N = sqrt(2.0 * factorial(l + am) * factorial(l - am) / (2.0 if m == 0 else 1.0)) / (2.0 ** am * factorial(l))
+        twovm = 0 if m >= 0 else 1                    # 2 v_m
+        for t in range((l - am) // 2 + 1):
+            for u in range(t + 1):
+                # v = v_m + k, k = 0 .. floor(|m|/2 - v_m)
+                kmax = (am - twovm) // 2
+                for k in range(kmax + 1):
+                    twov = twovm + 2 * k              # 2 v  (an odd number for m < 0)
+                    sign = (-1) ** (t + k)            # t + v - v_m = t + k
+                    Cc = sign * 0.25 ** t * comb(l, t) * comb(l - t, am + t) * comb(t, u) * comb(am, twov)
+                    ex = 2 * t + am - 2 * u - twov    # 2t + |m| - 2(u + v)
+                    ey = 2 * u + twov                 # 2(u + v)
+                    ez = l - 2 * t - am
+                    T[m + l, comps.index((ex, ey, ez))] += N * Cc
+    return T
+
+
+def nao_sph(mol) -> int:
+    return int(sum(2 * int(l) + 1 for l in mol.shell_l))
+
+
+def sph_matrix(mol) -> np.ndarray:
+    """U[nao_sph][nao_cart], block diagonal over the shells: chi^sph = U chi^cart."""
+    ls = [int(l) for l in mol.shell_l]
+    U = np.zeros((sum(2 * l + 1 for l in ls), sum((l + 1) * (l + 2) // 2 for l in ls)))
+    r = c = 0
+    for l in ls:
+        T = solid_harmonic_cart(l)
+        U[r:r + T.shape[0], c:c + T.shape[1]] = T
+        r += T.shape[0]; c += T.shape[1]
+    return U
+
+
+def density_sph_to_cart(mol, D_sph):
+    """D_cart = U^T D_sph U for [nbatch][nao_sph][nao_sph] (or one matrix)."""
+    U = sph_matrix(mol)
+    return np.einsum("mc,...mn,nd->...cd", U, _f64(D_sph), U)
+
+
+def coef_sph_to_cart(mol, C_sph):
+    """C_cart = U^T C_sph for [nao_sph][n]."""
+    return sph_matrix(mol).T @ _f64(C_sph)
+
+
+def grad_J_sph(mol, D_sph, c_aux, **kw):
+    return grad_J(mol, density_sph_to_cart(mol, D_sph), c_aux, **kw)
+
+
+def grad_K_sph(mol, C_occ_sph, C_vir_sph, B, **kw):
+    return grad_K(mol, coef_sph_to_cart(mol, C_occ_sph), coef_sph_to_cart(mol, C_vir_sph), B, **kw)
+
+
+def int3c_sph(mol, P, **kw):
+    """(mu nu|P) over the spherical functions of the molecule, [nao_sph][nao_sph]."""
+    U = sph_matrix(mol)
+    return U @ int3c(mol, P, **kw) @ U.T
