@@ -78,6 +78,13 @@ typedef struct ris_options {
                              differences at the 1e-16 relative level of the summation order. */
     int p_batch;          /* aux functions per Gamma^P batch in ris_grad_K; 0 = choose from free memory */
     int profile;          /* nonzero: record CUDA events around every kernel (see ris_profile_*) */
+    int spherical;        /* nonzero: the caller's AO basis is spherical-harmonic (def2-TZVP):
+                             shell s holds the 2l+1 functions S_lm(r - A) sum_k d_k exp(-a_k |r - A|^2), m = -l..l in this
+                             order, S_lm = sqrt(4 pi/(2l+1)) r^l Y_lm^real the real regular solid harmonics in Racah
+                             normalisation (S_1m = y, z, x; S_20 = zz - (xx + yy)/2; ...; the same prim_coef as the Cartesian
+                             shell).  ris_nao() and every AO dimension of D, C_occ, C_vir then count sum (2l+1) functions; the
+                             transformation to the Cartesian components the kernels run on happens on the device inside
+                             each call.  Default 0: Cartesian shells. */
 } ris_options;
 
 /* Build the context: copies the molecule to the device and runs shell-pair screening, sorting by

@@ -569,7 +569,7 @@ def sph_matrix(mol) -> np.ndarray:
 def density_sph_to_cart(mol, D_sph):
     """D_cart = U^T D_sph U for [nbatch][nao_sph][nao_sph] (or one matrix)."""
     U = sph_matrix(mol)
-    return np.einsum("mc,...mn,nd->...cd", U, _f64(D_sph), U)
+    return U.T @ _f64(D_sph) @ U          # matmul broadcasts over the leading state index
 
 
 def coef_sph_to_cart(mol, C_sph):

@@ -8,6 +8,7 @@
 #include "ris_gemm.cuh"
 #include "ris_internal.h"
 #include "ris_setup.cuh"
+#include "ris_sph.cuh"
 
 constexpr int RIS_NPRIM_MAX = 24;        // primitives per shell (kmax <= 576: the class-kernel task fits in shared memory)
 
@@ -61,7 +62,9 @@ struct ris_ctx {
     int nsm = 0;                       // SMs of `device` (grid sizing of the class kernels)
     cudaStream_t stream = nullptr;
     ris_options opt{};
-    int natoms = 0, nshells = 0, nao = 0, naux = 0;
+    int natoms = 0, nshells = 0, nao = 0, naux = 0;   // nao: Cartesian AOs (what the kernels run on)
+    int nao_in = 0;                    // AOs of the caller's basis: nao, or sum (2l+1) with opt.spherical (ris_sph.cuh)
+    int *d_sph0 = nullptr, *d_sph_lc = nullptr;   // spherical mode: per Cartesian AO the first spherical AO of its shell, 16 l + component
     double* d_coords = nullptr;
     double* d_aux = nullptr;           // [naux][RIS_AUX_FIELDS] the default set: one s function per atom (K type; J type too
                                        // unless ris_set_jfit gave the J term a set of its own)
@@ -107,8 +110,8 @@ struct ris_ctx {
     cudaEvent_t join_ev[RIS_NCLASS] = {nullptr}, fork_ev = nullptr;
     cudaEvent_t copy_extra = nullptr;             // the extra payload of upload_B_chunked has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
-    void* ws[22] = {nullptr};
-    size_t ws_bytes[22] = {0};
+    void* ws[32] = {nullptr};
+    size_t ws_bytes[32] = {0};
     RisResp resp;
     int last_pbatch = 0;
     std::vector<ProfRec> prof;
@@ -116,7 +119,8 @@ struct ris_ctx {
 };
 
 enum { WS_TILE = 0, WS_H = 1, WS_UNUSED2 = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5, WS_OUT = 6, WS_COCC = 7, WS_DET = 8, WS_CTR = 9,
-       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_RESP_T = 20, WS_RESP_B = 21, WS_N = 22 };
+       WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_RESP_T = 20, WS_RESP_B = 21, WS_SPH_A = 22, WS_SPH_B = 23, WS_N = 24 };
+static_assert(WS_N <= 32, "ris_ctx::ws holds 32 workspace slots");
 
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
@@ -355,8 +359,20 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     c->opt.schwarz_tol = 1e-13;
     if (opt) c->opt = *opt;
     c->natoms = natoms; c->nshells = nshells; c->nao = nao; c->naux = natoms;
+    c->nao_in = nao;
 
     int rc;
+    if (c->opt.spherical) {
+        std::vector<int> sph0((size_t)nao), lc((size_t)nao);
+        int ns = 0;
+        for (int s = 0; s < nshells; ++s) {
+            for (int k = 0; k < ris_ncart(shell_l[s]); ++k) { sph0[shell_ao[s] + k] = ns; lc[shell_ao[s] + k] = 16 * shell_l[s] + k; }
+            ns += 2 * shell_l[s] + 1;
+        }
+        c->nao_in = ns;
+        if ((rc = dev_upload(c, &c->d_sph0, sph0.data(), sph0.size()))) return rc;
+        if ((rc = dev_upload(c, &c->d_sph_lc, lc.data(), lc.size()))) return rc;
+    }
     if ((rc = dev_upload(c, &c->d_coords, coords, (size_t)3 * natoms))) return rc;
     if ((rc = dev_upload(c, &c->d_shell_atom, shell_atom, (size_t)nshells))) return rc;
     if ((rc = dev_upload(c, &c->d_shell_l, shell_l, (size_t)nshells))) return rc;
@@ -571,7 +587,7 @@ extern "C" int ris_destroy(ris_ctx* c)
     return RIS_OK;
 }
 
-extern "C" int ris_nao(const ris_ctx* c) { return c ? c->nao : RIS_EINVAL; }
+extern "C" int ris_nao(const ris_ctx* c) { return c ? c->nao_in : RIS_EINVAL; }
 extern "C" int ris_naux(const ris_ctx* c) { return c ? c->naux : RIS_EINVAL; }
 extern "C" int ris_natoms(const ris_ctx* c) { return c ? c->natoms : RIS_EINVAL; }
 extern "C" long long ris_npairs(const ris_ctx* c, int la, int lb)
@@ -589,6 +605,25 @@ extern "C" long long ris_ntriplets(const ris_ctx* c) { return c ? c->nprim_surv 
 extern "C" long long ris_ntriplets_unscreened(const ris_ctx* c) { return c ? c->nprim_total * c->naux : RIS_EINVAL; }
 extern "C" long long ris_npair_elements(const ris_ctx* c) { return c ? c->nelem_real : RIS_EINVAL; }
 extern "C" int ris_p_batch(const ris_ctx* c) { return c ? c->last_pbatch : RIS_EINVAL; }
+
+// Spherical mode (ris_sph.cuh): the caller's coefficient matrix [nao_in][ncol] expanded to Cartesian rows [nao][ncol] in a
+// ctx-owned buffer; Cartesian mode hands the pointer through.
+static int sph_coef(ris_ctx* c, int slot, const double* C, int ncol, const double** out)
+{
+    *out = C;
+    if (!c->opt.spherical) return RIS_OK;
+    double* w;
+    int rc = ws_get(c, slot, sizeof(double) * (size_t)c->nao * ncol, (void**)&w);
+    if (rc) return rc;
+    const long long n = (long long)c->nao * ncol;
+    {
+        ProfScope ps(c, "ris_k_sph_coef", 2.0 * n, 16.0 * n);
+        ris_k_sph_coef<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->nao, ncol, c->d_sph0, c->d_sph_lc, C, w);
+    }
+    CU(cudaGetLastError());
+    *out = w;
+    return RIS_OK;
+}
 
 // --------------------------------------------------------------------------------------- tile packing
 // J tiles: out[slab][elem_off + ip*nel + e] = symf[ip] * (G[slab][mu0+ca][nu0+cb] + G[slab][nu0+cb][mu0+ca]),  e = ca*ncb + cb.
@@ -613,7 +648,10 @@ static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab,
         const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
         ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel * nslab, 24.0 * nel * nslab);
         dim3 grid((unsigned)(((long long)nel + 255) / 256), 1, nslab);
-        ris_k_pack_tiles<<<grid, 256, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
+        if (c->opt.spherical)
+            ris_k_pack_tiles_sph<<<grid, 256, 0, c->stream>>>(pk, c->nao_in, c->d_sph0, G, gstride, out, ostride);
+        else
+            ris_k_pack_tiles<<<grid, 256, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
     }
     CU(cudaGetLastError());
     return RIS_OK;
@@ -745,7 +783,7 @@ static int grad_J_impl(ris_ctx* c, int nbatch, const double* D, const double* c_
     if (!c || nbatch < 1 || !D || !c_aux || !grad || f_lo < 0 || f_hi > c->naux_J || f_lo > f_hi) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
-    const long long nao2 = (long long)c->nao * c->nao;
+    const long long nao2 = (long long)c->nao_in * c->nao_in;
     unsigned long long* det;
     { int rc = det_begin(c, nbatch, &det); if (rc) return rc; }
     const int cap = nb_cap(c, false);
@@ -1042,7 +1080,7 @@ extern "C" int ris_fit_J(ris_ctx* c, int nbatch, const double* D, double* v_out,
     CU(cudaSetDevice(c->device));
     int rc;
     if ((rc = metric_factor(c, true))) return rc;
-    const long long nao2 = (long long)c->nao * c->nao;
+    const long long nao2 = (long long)c->nao_in * c->nao_in;
     const int naux = c->naux_J;
     double* v = v_out;
     if (!v && (rc = ws_get(c, WS_OUT, sizeof(double) * (size_t)nbatch * naux, (void**)&v))) return rc;
@@ -1193,6 +1231,12 @@ static int fit_mo(ris_ctx* c, bool jset, int nocc, int nvir, int ldr, const doub
     if ((size_t)naux * sizeof(double) > 48 * 1024 || ldr < nvir) return RIS_EINVAL;
     CU(cudaSetDevice(c->device));
     int rc;
+    {   // spherical mode: Cartesian rows of the two coefficient matrices (one expansion when they are the same matrix)
+        const bool same = C_occ == C_vir && nocc == nvir;
+        if ((rc = sph_coef(c, WS_SPH_A, C_occ, nocc, &C_occ))) return rc;
+        if (same) C_vir = C_occ;
+        else if ((rc = sph_coef(c, WS_SPH_B, C_vir, nvir, &C_vir))) return rc;
+    }
     if (B_out && (rc = metric_inverse(c, jset))) return rc;
     const int naop = (nao + 1) & ~1, nauxp = (naux + 1) & ~1, pbp = (naux + 3) & ~3;
     const long long nia = (long long)nocc * ldr;
@@ -1366,6 +1410,7 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     CU(cudaMemsetAsync(grad, 0, sizeof(double) * (size_t)nbatch * c->natoms * 3, c->stream));
     if (c->nelem_real == 0 || nloc == 0) return RIS_OK;   // every shell pair screened out / empty share: exactly zero
     const int nao = c->nao, naux = nloc;
+    { int rc0; if ((rc0 = sph_coef(c, WS_SPH_A, C_occ, nocc, &C_occ)) || (rc0 = sph_coef(c, WS_SPH_B, C_vir, nvir, &C_vir))) return rc0; }
     const int cap = nb_cap(c, true);
     if (cap < 1) return RIS_ENOMEM;
     const int nbmax = next_nb(nbatch, cap);
@@ -1532,7 +1577,7 @@ extern "C" int ris_grad_J_host(ris_ctx* c, int nbatch, const double* D, const do
     double *dD, *dc, *dg;
     int rc;
     const size_t ng = (size_t)nbatch * c->natoms * 3;
-    if ((rc = h2d(c, WS_IN0, D, (size_t)nbatch * c->nao * c->nao, &dD))) return rc;
+    if ((rc = h2d(c, WS_IN0, D, (size_t)nbatch * c->nao_in * c->nao_in, &dD))) return rc;
     if ((rc = h2d(c, WS_IN1, c_aux, (size_t)nbatch * c->naux_J, &dc))) return rc;
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = ris_grad_J(c, nbatch, dD, dc, dg))) return rc;
@@ -1587,8 +1632,8 @@ extern "C" int ris_grad_K_host(ris_ctx* c, int nbatch, int nocc, int nvir, const
     // B (the bulk of the input: naux*nocc*nvir doubles per state) goes up state by state on a second stream, each
     // state's GEMMs waiting only for their own slice: the PCIe transfer of state s+1 hides behind the GEMMs of state s.
     // The small operands go first: the H2D copy engine serves transfers in issue order across streams.
-    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
-    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
+    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao_in * nocc, &dCo))) return rc;
+    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao_in * nvir, &dCv))) return rc;
     if ((rc = upload_B_chunked(c, nbatch, nocc, nvir, B, &dB))) return rc;
     if ((rc = ws_get(c, WS_OUT, ng * sizeof(double), (void**)&dg))) return rc;
     if ((rc = grad_K_impl(c, nbatch, nocc, nvir, dCo, dCv, dB, dg, c->copy_ev.data()))) {
@@ -1627,9 +1672,9 @@ extern "C" int ris_grad_host(ris_ctx* c, int nbJ, const double* D, const double*
     const size_t nJ = (size_t)nbJ * c->natoms * 3, nK = (size_t)nbK * c->natoms * 3;
     if ((rc = h2d(c, WS_HC, c_aux, (size_t)nbJ * c->naux_J, &dc))) return rc;
     if ((rc = h2d(c, WS_HDQ, d_aux, (size_t)nbJ * c->naux_J, &dd))) return rc;
-    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao * nocc, &dCo))) return rc;
-    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao * nvir, &dCv))) return rc;
-    const size_t nD = (size_t)nbJ * c->nao * c->nao;
+    if ((rc = h2d(c, WS_IN1, C_occ, (size_t)c->nao_in * nocc, &dCo))) return rc;
+    if ((rc = h2d(c, WS_IN2, C_vir, (size_t)c->nao_in * nvir, &dCv))) return rc;
+    const size_t nD = (size_t)nbJ * c->nao_in * c->nao_in;
     if ((rc = ws_get(c, WS_HD, nD * sizeof(double), (void**)&dD))) return rc;
     if ((rc = upload_B_chunked(c, nbK, nocc, nvir, B, &dB, D, dD, nD))) return rc;
     if ((rc = ws_get(c, WS_OUT, (2 * nJ + nK) * sizeof(double), (void**)&dg))) return rc;

@@ -33,7 +33,8 @@ class RisError(RuntimeError):
 
 
 class RisOptions(C.Structure):
-    _fields_ = [("schwarz_tol", C.c_double), ("deterministic", C.c_int), ("p_batch", C.c_int), ("profile", C.c_int)]
+    _fields_ = [("schwarz_tol", C.c_double), ("deterministic", C.c_int), ("p_batch", C.c_int), ("profile", C.c_int),
+                ("spherical", C.c_int)]
 
 
 def load_library():
@@ -118,7 +119,7 @@ class RisContext:
     """ris_setup(coords, shells, aux_exponents) -> context with ris_grad_J / ris_grad_K / ris_grad_PQ."""
 
     def __init__(self, mol, *, schwarz_tol: float = 1e-13, deterministic: bool = False, p_batch: int = 0,
-                 profile: bool = False, stream=None):
+                 profile: bool = False, spherical: bool = False, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RisError("no CUDA device: the ris library has no CPU fallback")
@@ -129,14 +130,15 @@ class RisContext:
         arrs = (_np(mol.coords, np.float64), _np(mol.shell_atom, np.int32), _np(mol.shell_l, np.int32),
                 _np(mol.shell_nprim, np.int32), _np(mol.shell_prim_off, np.int32), _np(mol.prim_exp, np.float64),
                 _np(mol.prim_coef, np.float64), _np(mol.aux_exponents, np.float64))
-        opt = RisOptions(schwarz_tol, int(deterministic), int(p_batch), int(profile))
+        opt = RisOptions(schwarz_tol, int(deterministic), int(p_batch), int(profile), int(spherical))
         h = C.c_void_p()
         _check(self._lib.ris_setup(C.byref(h), arrs[0].shape[0], arrs[0].ctypes.data, arrs[1].shape[0],
                                    arrs[1].ctypes.data, arrs[2].ctypes.data, arrs[3].ctypes.data, arrs[4].ctypes.data,
                                    arrs[5].ctypes.data, arrs[6].ctypes.data, arrs[7].ctypes.data, C.byref(opt),
                                    C.c_void_p(self.stream.cuda_stream)))
         self._h = h
-        self.nao = self._lib.ris_nao(h)
+        self.nao = self._lib.ris_nao(h)            # AOs of the caller's basis (spherical: sum of 2l+1)
+        self.nao_cart = int(sum((int(l) + 1) * (int(l) + 2) // 2 for l in arrs[2]))
         self.naux = self._lib.ris_naux(h)
         self.natoms = self._lib.ris_natoms(h)
         self.naux_J = self._lib.ris_naux_J(h)
@@ -393,7 +395,7 @@ class RisContext:
     # ---- measurement / diagnostics (include/ris_bench.h)
     def gemm2_layout(self):
         """(ao_pos[nao], panel_rows, tile_cols, ntiles, novf) of the pair-restricted Gamma^P GEMM-2."""
-        pos = np.empty(self.nao, dtype=np.int32)
+        pos = np.empty(self.nao_cart, dtype=np.int32)
         r, c, nt, nv = C.c_int(), C.c_int(), C.c_int(), C.c_int()
         _check(self._lib.ris_diag_gemm2_layout(self._h, pos.ctypes.data, C.byref(r), C.byref(c), C.byref(nt), C.byref(nv)))
         return pos, r.value, c.value, nt.value, nv.value
