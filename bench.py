@@ -273,10 +273,12 @@ def run_ours(args):
     fp64_peak = probe_fp64_peak()            # DFMA chains, TFLOP/s (MEASURED_PEAKS.json has no FP64 figure)
     mma_peak = probe_fp64_mma_peak()         # mma.sync f64 chains, TFLOP/s
 
+    # The timed region runs WITHOUT the library's per-launch events (two event records per launch are a tenth of a
+    # small molecule's step); the per-kernel table comes from a second, profiled pass of the same steps below.
+    ctx.profile_enable(False)
     for _ in range(max(args.warmup, 0)):
         step()
     barrier()
-    ctx.profile_reset()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -288,7 +290,15 @@ def run_ours(args):
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
+    ctx.profile_enable(True)
+    step()
+    barrier()
+    ctx.profile_reset()
+    for _ in range(args.steps):
+        step()
+    barrier()
     prof = ctx.profile()
+    ctx.profile_enable(False)                # the end-to-end loop below is timed without it as well
     ms_J = sum(ev[0].elapsed_time(ev[1]) for ev in marks)
     ms_K = sum(ev[1].elapsed_time(ev[2]) for ev in marks)
     ms_Q = sum(ev[2].elapsed_time(ev[3]) for ev in marks)

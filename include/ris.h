@@ -214,6 +214,7 @@ int ris_p_batch(const ris_ctx* ctx);                           /* Gamma^P batch 
  * kernel launches recorded since the last ris_profile_reset; ris_profile_get returns launch i's kernel
  * name (static string) and device time in milliseconds. */
 int ris_profile_reset(ris_ctx* ctx);
+int ris_profile_enable(ris_ctx* ctx, int on);                   /* switch the recording on / off for the calls that follow */
 int ris_profile_count(ris_ctx* ctx);
 int ris_profile_get(ris_ctx* ctx, int i, const char** name, float* ms);
 /* ALGORITHMIC work of launch i (what the method must compute / move, not what the kernel happens to do):

@@ -137,8 +137,10 @@ static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 
 template <class T> static int dev_alloc(ris_ctx* c, T** p, size_t n, bool zero)
 {
+    // stream-ordered allocation from the device's default memory pool: a context built after another one was destroyed
+    // (a new geometry in a running process) gets its ~50 buffers back from the pool instead of from the driver
     void* q = nullptr;
-    cudaError_t e = cudaMalloc(&q, std::max<size_t>(n, 1) * sizeof(T));
+    cudaError_t e = cudaMallocAsync(&q, std::max<size_t>(n, 1) * sizeof(T), c->stream);
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return RIS_ENOMEM; }
     CU(e);
     c->owned.push_back(q);
@@ -187,6 +189,13 @@ extern "C" int ris_profile_get(ris_ctx* c, int i, const char** name, float* ms)
     CU(cudaEventSynchronize(c->prof[i].e1));
     CU(cudaEventElapsedTime(ms, c->prof[i].e0, c->prof[i].e1));
     *name = c->prof[i].name;
+    return RIS_OK;
+}
+
+extern "C" int ris_profile_enable(ris_ctx* c, int on)
+{
+    if (!c) return RIS_EINVAL;
+    c->opt.profile = on ? 1 : 0;
     return RIS_OK;
 }
 
@@ -355,6 +364,14 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
     struct Guard { ris_ctx* c; bool ok = false; ~Guard() { if (!ok) ris_destroy(c); } } guard{c};
     CU(cudaGetDevice(&c->device));
     CU(cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device));
+    {   // keep up to 1 GiB of freed packed-pair buffers in the default pool between contexts (the default gives
+        // everything back to the driver at the next synchronisation)
+        cudaMemPool_t pool;
+        CU(cudaDeviceGetDefaultMemPool(&pool, c->device));
+        unsigned long long keep = 1ull << 30, cur = 0;
+        CU(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &cur));
+        if (cur < keep) CU(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    }
     c->stream = (cudaStream_t)cuda_stream;
     c->opt.schwarz_tol = 1e-13;
     if (opt) c->opt = *opt;
@@ -446,7 +463,7 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         ProfScope ps(c, "ris_k_radix_pass");
         long long* lout = d_list[pass & 1];
         ris_k_radix_hist<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_key, shifts[pass], d_hist);
-        ris_k_radix_scan<<<1, 32, 0, c->stream>>>(nblk, d_hist, d_base, d_meta, d_meta + RIS_NBIN);
+        ris_k_radix_scan<<<1, 32 * RIS_NBIN, 0, c->stream>>>(nblk, d_hist, d_base, d_meta, d_meta + RIS_NBIN);
         ris_k_radix_scatter<<<nblk, RIS_SCAN_BLOCK, 0, c->stream>>>(ntot, lin, d_key, shifts[pass], d_base, d_meta + RIS_NBIN, lout);
         lin = lout;
     }
@@ -571,7 +588,8 @@ extern "C" int ris_destroy(ris_ctx* c)
     if (!c) return RIS_EINVAL;
     cudaStreamSynchronize(c->stream);
     ris_resp_free(c);
-    for (void* p : c->owned) cudaFree(p);
+    for (void* p : c->owned) cudaFreeAsync(p, c->stream);
+    cudaStreamSynchronize(c->stream);
     for (int i = 0; i < WS_N; ++i) if (c->ws[i]) cudaFree(c->ws[i]);
     for (cudaEvent_t e : c->copy_ev) cudaEventDestroy(e);
     if (c->copy_gate) cudaEventDestroy(c->copy_gate);

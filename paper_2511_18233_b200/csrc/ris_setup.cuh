@@ -95,18 +95,31 @@ __global__ void __launch_bounds__(RIS_SCAN_BLOCK) ris_k_radix_hist(long long n, 
 }
 
 // Exclusive scan over blocks for each bin -> base[blk][bin]; totals[bin]; start[bin] (bin-major order).
-__global__ void ris_k_radix_scan(int nblk, const int* hist, int* base, int* totals, int* start)
+// One block of RIS_NBIN warps, warp c = bin c: every lane sums a contiguous run of blocks (independent loads), the lane sums
+// are scanned with shuffles, a second pass writes the bases.  (One thread per bin walking all blocks took 0.27 ms per pass
+// at config 4 -- 3562 blocks, 7 passes: two thirds of the kernel time of ris_setup.)
+__global__ void __launch_bounds__(32 * RIS_NBIN) ris_k_radix_scan(int nblk, const int* hist, int* base, int* totals, int* start)
 {
-    const int c = threadIdx.x;
-    if (c < RIS_NBIN) {
-        int run = 0;
-        for (int b = 0; b < nblk; ++b) { base[b * RIS_NBIN + c] = run; run += hist[b * RIS_NBIN + c]; }
-        totals[c] = run;
+    __shared__ int tot[RIS_NBIN];
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int per = (nblk + 31) / 32;
+    const int b0 = min(lane * per, nblk), b1 = min(b0 + per, nblk);
+    int sum = 0;
+#pragma unroll 4
+    for (int b = b0; b < b1; ++b) sum += hist[b * RIS_NBIN + c];
+    int incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
     }
+    int run = incl - sum;
+    for (int b = b0; b < b1; ++b) { base[b * RIS_NBIN + c] = run; run += hist[b * RIS_NBIN + c]; }
+    if (lane == 31) { totals[c] = incl; tot[c] = incl; }
     __syncthreads();
-    if (c == 0) {
-        int run = 0;
-        for (int k = 0; k < RIS_NBIN; ++k) { start[k] = run; run += totals[k]; }
+    if (threadIdx.x == 0) {
+        int r = 0;
+        for (int k = 0; k < RIS_NBIN; ++k) { start[k] = r; r += tot[k]; }
     }
 }
 

@@ -22,7 +22,7 @@ EXPORTS = [
     "ris_resp_setup", "ris_resp_matvec", "ris_resp_free", "ris_grad_K_range", "ris_grad_J_range",
     "ris_destroy", "ris_strerror", "ris_nao", "ris_naux", "ris_natoms", "ris_npairs", "ris_npairs_total",
     "ris_nprimpairs", "ris_ntriplets", "ris_ntriplets_unscreened", "ris_npair_elements", "ris_p_batch",
-    "ris_profile_reset", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
+    "ris_profile_reset", "ris_profile_enable", "ris_profile_count", "ris_profile_get", "ris_profile_get_work",
     # include/ris_bench.h: measurement / diagnostics, not the product boundary
     "ris_probe_fp64_peak", "ris_probe_fp64_mma_peak", "ris_diag_gemm2_layout",
 ]
@@ -71,6 +71,7 @@ def load_library():
     lib.ris_strerror.restype = C.c_char_p
     for name in ("ris_nao", "ris_naux", "ris_naux_J", "ris_natoms", "ris_p_batch", "ris_profile_reset", "ris_profile_count"):
         getattr(lib, name).argtypes = [vp]
+    lib.ris_profile_enable.argtypes = [vp, ci]
     for name in ("ris_npairs", "ris_nprimpairs"):
         getattr(lib, name).argtypes = [vp, ci, ci]
         getattr(lib, name).restype = C.c_longlong
@@ -403,6 +404,9 @@ class RisContext:
     # ---- profiling
     def profile_reset(self):
         _check(self._lib.ris_profile_reset(self._h))
+
+    def profile_enable(self, on: bool):
+        _check(self._lib.ris_profile_enable(self._h, int(bool(on))))
 
     def profile(self):
         """[(kernel name, ms, algorithmic flops, algorithmic bytes)] for every launch since the last reset
