@@ -67,7 +67,10 @@ typedef struct ris_options {
                                    < tau / (naux sqrt(n_unique_shell_pairs)),
                              (the bound on |(ab|P)| for s-type primitives -- the aux potential peaks at
                              N_P 2 pi/alpha_P -- times a factor for polynomial / derivative growth, with the
-                             random-sign accumulation over naux x pairs folded into the threshold);
+                             random-sign accumulation over naux x pairs folded into the threshold).  For l > 0 the
+                             criterion is HEURISTIC: the polynomial prefactors |P-A|^la |P-B|^lb are not bounded
+                             rigorously by the factor; it is validated empirically -- at tau = 1e-13 the results equal
+                             the unscreened ones to 5e-15 of the gradient scale on configs 2-3 (tests/test_gpu_parity.py);
                              a shell pair is dropped when all its primitive pairs are.  There is no screening on
                              the aux index (the Coulomb tail is 1/R). */
     int deterministic;    /* nonzero: bitwise run-to-run reproducible results.  Every in-block sum already has a fixed

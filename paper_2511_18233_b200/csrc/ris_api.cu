@@ -107,6 +107,8 @@ struct ris_ctx {
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
     cudaStream_t side[RIS_NCLASS] = {nullptr};    // class kernels of small molecules run concurrently on these
+    cudaStream_t side2[RIS_NCLASS] = {nullptr};   // ... and the second host-phase launch of a split (heavy) class on these
+    cudaEvent_t join2_ev[RIS_NCLASS] = {nullptr};
     cudaEvent_t join_ev[RIS_NCLASS] = {nullptr}, fork_ev = nullptr;
     cudaEvent_t copy_extra = nullptr;             // the extra payload of upload_B_chunked has landed
     cudaEvent_t copy_gate = nullptr;              // compute stream -> copy stream: the staging buffer is free
@@ -598,6 +600,8 @@ extern "C" int ris_destroy(ris_ctx* c)
     for (int k = 0; k < RIS_NCLASS; ++k) {
         if (c->join_ev[k]) cudaEventDestroy(c->join_ev[k]);
         if (c->side[k]) cudaStreamDestroy(c->side[k]);
+        if (c->join2_ev[k]) cudaEventDestroy(c->join2_ev[k]);
+        if (c->side2[k]) cudaStreamDestroy(c->side2[k]);
     }
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     ris_profile_reset(c);
@@ -703,6 +707,8 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
             if (!c->side[k]) {
                 CU(cudaStreamCreateWithFlags(&c->side[k], cudaStreamNonBlocking));
                 CU(cudaEventCreateWithFlags(&c->join_ev[k], cudaEventDisableTiming));
+                CU(cudaStreamCreateWithFlags(&c->side2[k], cudaStreamNonBlocking));
+                CU(cudaEventCreateWithFlags(&c->join2_ev[k], cudaEventDisableTiming));
             }
         CU(cudaEventRecord(c->fork_ev, c->stream));
     }
@@ -711,8 +717,11 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
         const cudaStream_t st = side ? c->side[k] : c->stream;
+        const bool two = side && ris_grad_split(pk.la, pk.lb);     // the second host phase of a split class on its own stream
         if (side) CU(cudaStreamWaitEvent(st, c->fork_ev, 0));
+        if (two) CU(cudaStreamWaitEvent(c->side2[k], c->fork_ev, 0));
         RisGradParams p{};
+        p.phase2_stream = two ? c->side2[k] : nullptr;
         p.task_ctr = ctr + (size_t)2 * k * ny;
         p.pk = pk; p.naux = naux_row; p.natoms = c->natoms; p.nsm = c->nsm; p.aux = aux; p.aux_type = aux_type;
         p.boys = c->d_boys[pk.la + pk.lb + eb];
@@ -728,6 +737,10 @@ static int launch_classes(ris_ctx* c, const double* tile, long long sstride, lon
         if (side) {
             CU(cudaEventRecord(c->join_ev[k], st));
             CU(cudaStreamWaitEvent(c->stream, c->join_ev[k], 0));
+        }
+        if (two) {
+            CU(cudaEventRecord(c->join2_ev[k], c->side2[k]));
+            CU(cudaStreamWaitEvent(c->stream, c->join2_ev[k], 0));
         }
     }
     CU(cudaGetLastError());

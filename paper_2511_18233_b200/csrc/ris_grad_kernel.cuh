@@ -47,9 +47,6 @@
 // SPLIT: the heavy classes (l_mu + l_nu >= 4) run their two host-centre phases as two launches (PH = 1: primitive pairs
 // hosted on A, PH = 2: hosted on B; PH = 0: both in one kernel).  With both phases inlined the (2,2) kernel is 94 KB of
 // SASS and stalls on instruction fetch; one phase is 47 KB.
-#ifndef RIS_SPLIT_L
-#define RIS_SPLIT_L 4
-#endif
 #ifndef RIS_PIPE_L
 #define RIS_PIPE_L -1           // software-pipelined primitive loop for l_mu + l_nu <= this.  Measured on config 4 (r02):
 #endif                          // slower for every class ((1,0) J 0.78 -> 0.92 ms): the extra live front spills at the
@@ -62,7 +59,7 @@
 #endif
 template <int LA, int LB> struct RisGradTune {
     static constexpr int MINB = (LA + LB <= 1) ? RIS_MB1 : (LA + LB == 2 ? RIS_MB2 : (LA + LB == 3 ? RIS_MB3 : RIS_MB4));
-    static constexpr bool SPLIT = (LA + LB >= RIS_SPLIT_L);
+    static constexpr bool SPLIT = ris_grad_split(LA, LB);
     static constexpr bool PIPE = (LA + LB <= RIS_PIPE_L);
     static constexpr int NEL = RisClass<LA, LB>::NCA * RisClass<LA, LB>::NCB;
     // slots of the tile ring: K -- as many states as fit the budget, at least 2 (1 for (2,2) and the f classes, whose slot
@@ -403,7 +400,7 @@ cudaError_t ris_launch_grad_t(const RisGradParams& p, cudaStream_t st)
         cudaError_t e = ris_launch_grad_phase<LA, LB, 1, KT, AUX>(q, st);
         if (e != cudaSuccess) return e;
         q.task_ctr = p.task_ctr + (p.p1 - p.p0 + 31) / 32;
-        return ris_launch_grad_phase<LA, LB, 2, KT, AUX>(q, st);
+        return ris_launch_grad_phase<LA, LB, 2, KT, AUX>(q, p.phase2_stream ? p.phase2_stream : st);
     } else {
         return ris_launch_grad_phase<LA, LB, 0, KT, AUX>(p, st);
     }

@@ -72,6 +72,8 @@ struct RisGradParams {
     double* grad;            // [nb][natoms][3], accumulated with atomics
     unsigned long long* det; // deterministic mode: [nb][natoms][3][2] fixed-point accumulators (hi, lo), else nullptr
     int* det_flag;           // set to 1 when a contribution leaves the fixed-point range
+    cudaStream_t phase2_stream;   // host side only: when set, the second host-phase launch of a split class goes here
+                                  // (small molecules: the two phases run side by side); nullptr = the launch stream
 };
 
 // Deterministic reduction (ris_options.deterministic): a contribution x is added as the integer pair
@@ -94,6 +96,11 @@ extern ris_grad_launcher ris_grad_launchers[RIS_NCLASS];
 
 
 // ---- per-class configuration of the class kernels, shared by host sizing code and the kernel templates ----------------
+// the heavy classes (l_mu + l_nu >= RIS_SPLIT_L) run their two host-centre phases as two launches (ris_grad_kernel.cuh)
+#ifndef RIS_SPLIT_L
+#define RIS_SPLIT_L 4
+#endif
+__host__ __device__ constexpr bool ris_grad_split(int la, int lb) { return la + lb >= RIS_SPLIT_L; }
 // K tiles of the biggest classes (60 / 100 elements: 15-26 KB per state and warp) are read straight from global memory
 __host__ __device__ constexpr bool ris_grad_stage_k(int la, int lb) { return ris_ncart(la) * ris_ncart(lb) < 60; }
 

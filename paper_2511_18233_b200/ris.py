@@ -346,6 +346,12 @@ class RisContext:
                            f"c_contiguous={a.flags.c_contiguous}")
         return C.c_void_p(a.ctypes.data), a.shape, a
 
+    @staticmethod
+    def _shape(p, shape, what):
+        """Host buffers carry no size across the C ABI: a wrong shape would be read (or written) out of bounds."""
+        if tuple(p[1]) != tuple(shape):
+            raise RisError(f"{what}: shape {tuple(p[1])} != expected {tuple(shape)}")
+
     def _host_out(self, out, shape):
         if out is None:
             out = np.empty(shape)
@@ -357,6 +363,7 @@ class RisContext:
     def grad_J_host(self, D, c_aux, out=None):
         pD, pc = self._host(D, "D"), self._host(c_aux, "c_aux")
         nb = pD[1][0]
+        self._shape(pD, (nb, self.nao, self.nao), "D"); self._shape(pc, (nb, self.naux_J), "c_aux")
         out, po = self._host_out(out, (nb, self.natoms, 3))
         with self._ordered():
             _check(self._lib.ris_grad_J_host(self._h, nb, pD[0], pc[0], po[0]))
@@ -365,6 +372,8 @@ class RisContext:
     def grad_K_host(self, C_occ, C_vir, B, out=None):
         po, pv, pB = self._host(C_occ, "C_occ"), self._host(C_vir, "C_vir"), self._host(B, "B")
         nb, nocc, nvir = pB[1][0], po[1][1], pv[1][1]
+        self._shape(po, (self.nao, nocc), "C_occ"); self._shape(pv, (self.nao, nvir), "C_vir")
+        self._shape(pB, (nb, self.naux, nocc, nvir), "B")
         out, pg = self._host_out(out, (nb, self.natoms, 3))
         with self._ordered():
             _check(self._lib.ris_grad_K_host(self._h, nb, nocc, nvir, po[0], pv[0], pB[0], pg[0]))
@@ -373,6 +382,7 @@ class RisContext:
     def grad_PQ_host(self, c_aux, d_aux, out=None):
         pc, pd = self._host(c_aux, "c_aux"), self._host(d_aux, "d_aux")
         nb = pc[1][0]
+        self._shape(pc, (nb, self.naux_J), "c_aux"); self._shape(pd, (nb, self.naux_J), "d_aux")
         out, pg = self._host_out(out, (nb, self.natoms, 3))
         with self._ordered():
             _check(self._lib.ris_grad_PQ_host(self._h, nb, pc[0], pd[0], pg[0]))
@@ -383,6 +393,9 @@ class RisContext:
         pD, pc, pd = self._host(D, "D"), self._host(c_aux, "c_aux"), self._host(d_aux, "d_aux")
         po, pv, pB = self._host(C_occ, "C_occ"), self._host(C_vir, "C_vir"), self._host(B, "B")
         nbJ, nbK, nocc, nvir = pD[1][0], pB[1][0], po[1][1], pv[1][1]
+        self._shape(pD, (nbJ, self.nao, self.nao), "D"); self._shape(pc, (nbJ, self.naux_J), "c_aux")
+        self._shape(pd, (nbJ, self.naux_J), "d_aux"); self._shape(po, (self.nao, nocc), "C_occ")
+        self._shape(pv, (self.nao, nvir), "C_vir"); self._shape(pB, (nbK, self.naux, nocc, nvir), "B")
         if out is None:
             out = (None, None, None)
         oJ, pJ = self._host_out(out[0], (nbJ, self.natoms, 3))
