@@ -16,6 +16,7 @@ constexpr int RIS_NPRIM_MAX = 24;        // primitives per shell (kmax <= 576: t
 #include <utility>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -107,6 +108,13 @@ struct ris_ctx {
     cudaStream_t copy_stream = nullptr;           // *_host entry points: H2D of B, one state ahead of the GEMMs
     std::vector<cudaEvent_t> copy_ev;             // [state] B of that state has landed
     cudaStream_t side[RIS_NCLASS] = {nullptr};    // class kernels of small molecules run concurrently on these
+    // Small molecules (the class kernels run side by side, see launch_classes): a device-pointer call whose arguments repeat
+    // is captured into a CUDA graph the second time and replayed from then on (run_graphed).
+    struct GraphSlot { std::vector<unsigned long long> key; cudaGraphExec_t exec = nullptr; };
+    GraphSlot gslot[2];                           // ris_grad_J(_range), ris_grad_K(_range)
+    cudaStream_t cap_stream = nullptr;            // the capture runs on a stream of our own (the caller's may be the legacy
+                                                  // default stream, which cannot be captured); the graph is launched into the caller's
+    bool small = false;                           // set by ris_setup: no class fills the GPU with its one resident wave
     cudaStream_t side2[RIS_NCLASS] = {nullptr};   // ... and the second host-phase launch of a split (heavy) class on these
     cudaEvent_t join2_ev[RIS_NCLASS] = {nullptr};
     cudaEvent_t join_ev[RIS_NCLASS] = {nullptr}, fork_ev = nullptr;
@@ -124,9 +132,20 @@ enum { WS_TILE = 0, WS_H = 1, WS_UNUSED2 = 2, WS_IN0 = 3, WS_IN1 = 4, WS_IN2 = 5
        WS_FIT_I = 10, WS_FIT_SLAB = 11, WS_FIT_UT = 12, WS_FIT_T = 13, WS_FIT_TT = 14, WS_FIT_CV = 15, WS_FIT_CO = 16, WS_HC = 17, WS_HDQ = 18, WS_HD = 19, WS_RESP_T = 20, WS_RESP_B = 21, WS_SPH_A = 22, WS_SPH_B = 23, WS_N = 24 };
 static_assert(WS_N <= 32, "ris_ctx::ws holds 32 workspace slots");
 
+// The captured graphs hold workspace and list pointers: drop them whenever one of those may have changed.
+static void graphs_invalidate(ris_ctx* c)
+{
+    for (auto& g : c->gslot) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        g.exec = nullptr;
+        g.key.clear();
+    }
+}
+
 static int ws_get(ris_ctx* c, int slot, size_t bytes, void** out)
 {
     if (c->ws_bytes[slot] < bytes) {
+        graphs_invalidate(c);
         if (c->ws[slot]) { CU(cudaStreamSynchronize(c->stream)); CU(cudaFree(c->ws[slot])); c->ws[slot] = nullptr; c->ws_bytes[slot] = 0; }
         cudaError_t e = cudaMalloc(&c->ws[slot], bytes);
         if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return RIS_ENOMEM; }
@@ -506,6 +525,13 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         }
     c->nelem_real = off;
     CU(cudaGetLastError());
+    {   // "small": no class fills the GPU with its one resident wave (the criterion of launch_classes for the default set)
+        long long most = 0;
+        const int ny = (natoms + 31) / 32;
+        for (int k = 0; k < RIS_NCLASS; ++k)
+            if (c->cls[k].npairs > 0) most = std::max(most, (long long)((c->cls[k].ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS) * ny);
+        c->small = most <= (long long)2 * c->nsm && !std::getenv("RIS_NO_GRAPH");    // (the variable: A/B measurements)
+    }
     // spatial AO order + block list for the pair-restricted Gamma^P GEMM-2
     {
         double lo[3] = {coords[0], coords[1], coords[2]};
@@ -589,6 +615,7 @@ extern "C" int ris_destroy(ris_ctx* c)
 {
     if (!c) return RIS_EINVAL;
     cudaStreamSynchronize(c->stream);
+    graphs_invalidate(c);
     ris_resp_free(c);
     for (void* p : c->owned) cudaFreeAsync(p, c->stream);
     cudaStreamSynchronize(c->stream);
@@ -604,6 +631,7 @@ extern "C" int ris_destroy(ris_ctx* c)
         if (c->side2[k]) cudaStreamDestroy(c->side2[k]);
     }
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     ris_profile_reset(c);
     delete c;
     return RIS_OK;
@@ -650,31 +678,45 @@ static int sph_coef(ris_ctx* c, int slot, const double* C, int ncol, const doubl
 // --------------------------------------------------------------------------------------- tile packing
 // J tiles: out[slab][elem_off + ip*nel + e] = symf[ip] * (G[slab][mu0+ca][nu0+cb] + G[slab][nu0+cb][mu0+ca]),  e = ca*ncb + cb.
 // Folds D + D^T onto the unique shell pairs.
-__global__ void ris_k_pack_tiles(RisClassPack pk, int nao, const double* __restrict__ G, long long gstride,
+// One launch for all classes: blockIdx.y selects the class (sph0 != nullptr: spherical mode, ris_sph.cuh).
+struct RisPackAll { RisClassPack pk[RIS_NCLASS]; int ncls; };
+__global__ void ris_k_pack_tiles(RisPackAll pa, int nao, const int* __restrict__ sph0, const double* __restrict__ G, long long gstride,
                                  double* __restrict__ out, long long ostride)
 {
-    const int nel = ris_ncart(pk.la) * ris_ncart(pk.lb), ncb = ris_ncart(pk.lb);
+    const RisClassPack& pk = pa.pk[blockIdx.y];
+    const int nca = ris_ncart(pk.la), ncb = ris_ncart(pk.lb), nel = nca * ncb;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)pk.npairs * nel) return;
     const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
-    const size_t r = (size_t)pk.ao[ip] + ca, q = (size_t)pk.ao[(size_t)pk.npairs + ip] + cb;
     const double* g = G + (size_t)blockIdx.z * gstride;
-    out[(size_t)blockIdx.z * ostride + pk.elem_off + idx] = (double)pk.symf[ip] * (g[r * nao + q] + g[q * nao + r]);
+    double v;
+    if (sph0 == nullptr) {
+        const size_t r = (size_t)pk.ao[ip] + ca, q = (size_t)pk.ao[(size_t)pk.npairs + ip] + cb;
+        v = g[r * nao + q] + g[q * nao + r];
+    } else {
+        v = ris_sph_pair_element(pk.la, pk.lb, ca, cb, (size_t)sph0[pk.ao[ip]], (size_t)sph0[pk.ao[(size_t)pk.npairs + ip]], nao, g);
+    }
+    out[(size_t)blockIdx.z * ostride + pk.elem_off + idx] = (double)pk.symf[ip] * v;
 }
 
 static int pack_tiles(ris_ctx* c, const double* G, long long gstride, int nslab, double* out, long long ostride)
 {
+    RisPackAll pa{};
+    long long most = 0;
+    double nel = 0.0;
     for (int k = 0; k < RIS_NCLASS; ++k) {
         const RisClassPack& pk = c->cls[k];
         if (pk.npairs == 0) continue;
-        const double nel = (double)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
-        ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel * nslab, 24.0 * nel * nslab);
-        dim3 grid((unsigned)(((long long)nel + 255) / 256), 1, nslab);
-        if (c->opt.spherical)
-            ris_k_pack_tiles_sph<<<grid, 256, 0, c->stream>>>(pk, c->nao_in, c->d_sph0, G, gstride, out, ostride);
-        else
-            ris_k_pack_tiles<<<grid, 256, 0, c->stream>>>(pk, c->nao, G, gstride, out, ostride);
+        pa.pk[pa.ncls++] = pk;
+        const long long n = (long long)ris_ncart(pk.la) * ris_ncart(pk.lb) * pk.npairs;
+        most = std::max(most, n);
+        nel += (double)n;
     }
+    if (pa.ncls == 0) return RIS_OK;
+    ProfScope ps(c, "ris_k_pack_tiles", 2.0 * nel * nslab, 24.0 * nel * nslab);
+    dim3 grid((unsigned)((most + 255) / 256), pa.ncls, nslab);
+    ris_k_pack_tiles<<<grid, 256, 0, c->stream>>>(pa, c->opt.spherical ? c->nao_in : c->nao, c->opt.spherical ? c->d_sph0 : nullptr, G,
+                                                  gstride, out, ostride);
     CU(cudaGetLastError());
     return RIS_OK;
 }
@@ -798,14 +840,63 @@ static int det_end(ris_ctx* c, int nbatch, const unsigned long long* acc, double
 }
 
 // --------------------------------------------------------------------------------------- J
+// Small molecules are bound by launch and cross-stream dependency latency (config 2: ~25 launches on up to 17 streams for
+// 0.15 ms of kernels).  A device-pointer call whose signature (arguments and sizes) repeats is therefore captured into a CUDA
+// graph on its second occurrence -- the ordinary launch sequence, recorded instead of run -- and replayed afterwards; a call
+// with a new signature runs directly and replaces the remembered one.  Not used while profiling, inside a capture of the
+// caller's own, or for molecules that fill the GPU (nothing to gain there).
+template <class F>
+static int run_graphed(ris_ctx* c, int slot, const std::vector<unsigned long long>& key, F&& body)
+{
+    if (!c->small || c->opt.profile) return body();
+    ris_ctx::GraphSlot& g = c->gslot[slot];
+    if (g.exec && g.key == key) { CU(cudaGraphLaunch(g.exec, c->stream)); return RIS_OK; }
+    if (g.key != key) {                               // first sight of this signature: run it, remember it
+        if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+        const int rc = body();
+        if (rc == RIS_OK) g.key = key; else g.key.clear();
+        return rc;
+    }
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    CU(cudaSetDevice(c->device));
+    if (cudaStreamIsCapturing(c->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return body(); }
+    if (!c->cap_stream) CU(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+    const cudaStream_t user = c->stream;
+    c->stream = c->cap_stream;                        // the launch sequence below is recorded on our stream ...
+    cudaError_t e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { cudaGetLastError(); c->stream = user; g.key.clear(); return body(); }
+    const int rc = body();
+    cudaGraph_t graph = nullptr;
+    e = cudaStreamEndCapture(c->stream, &graph);
+    c->stream = user;                                 // ... and replayed in the caller's
+    if (rc != RIS_OK || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        g.key.clear();
+        return rc != RIS_OK ? rc : body();            // capture refused: run directly
+    }
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) { cudaGetLastError(); g.exec = nullptr; g.key.clear(); return body(); }
+    CU(cudaGraphLaunch(g.exec, c->stream));
+    return RIS_OK;
+}
+static inline unsigned long long key_of(const void* p) { return (unsigned long long)(uintptr_t)p; }
+
 static int grad_J_impl(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad, int f_lo, int f_hi);
+static int grad_J_graphed(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad, int f_lo, int f_hi)
+{
+    const std::vector<unsigned long long> key = {1ull, (unsigned long long)nbatch, key_of(D), key_of(c_aux), key_of(grad),
+                                                 (unsigned long long)f_lo, (unsigned long long)f_hi};
+    return run_graphed(c, 0, key, [&]() { return grad_J_impl(c, nbatch, D, c_aux, grad, f_lo, f_hi); });
+}
 extern "C" int ris_grad_J(ris_ctx* c, int nbatch, const double* D, const double* c_aux, double* grad)
 {
-    return c ? grad_J_impl(c, nbatch, D, c_aux, grad, 0, c->naux_J) : RIS_EINVAL;
+    return c ? grad_J_graphed(c, nbatch, D, c_aux, grad, 0, c->naux_J) : RIS_EINVAL;
 }
 extern "C" int ris_grad_J_range(ris_ctx* c, int nbatch, const double* D, const double* c_aux, int f_lo, int f_hi, double* grad)
 {
-    return c ? grad_J_impl(c, nbatch, D, c_aux, grad, f_lo, f_hi) : RIS_EINVAL;
+    return c ? grad_J_graphed(c, nbatch, D, c_aux, grad, f_lo, f_hi) : RIS_EINVAL;
 }
 
 // [f_lo, f_hi): the J-fit FUNCTIONS this call sums over (c_aux keeps its full row length)
@@ -1047,6 +1138,7 @@ extern "C" int ris_set_jfit(ris_ctx* c, int nshell_aux, const int32_t* aux_atom,
     if ((rc = dev_upload(c, &c->d_atom_fn_off, off.data(), off.size()))) return rc;
     if ((rc = dev_upload(c, &c->d_atom_fn, idx.data(), idx.size()))) return rc;
     CU(cudaStreamSynchronize(c->stream));
+    graphs_invalidate(c);
     c->jfit = true; c->naux_J = nfn; c->d_chol_J = nullptr; c->d_minv_J = nullptr;
     ris_resp_free(c);                       // stored Coulomb tensors belong to the previous set
     return RIS_OK;
@@ -1522,17 +1614,26 @@ static int grad_K_impl(ris_ctx* c, int nbatch, int nocc, int nvir, const double*
     return det_end(c, nbatch, det, grad);
 }
 
+static int grad_K_graphed(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir, const double* B,
+                          double* grad, int p_lo, int p_hi)
+{
+    const std::vector<unsigned long long> key = {2ull, (unsigned long long)nbatch, (unsigned long long)nocc, (unsigned long long)nvir,
+                                                 key_of(C_occ), key_of(C_vir), key_of(B), key_of(grad),
+                                                 (unsigned long long)(long long)p_lo, (unsigned long long)(long long)p_hi};
+    return run_graphed(c, 1, key, [&]() { return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B, grad, nullptr, p_lo, p_hi); });
+}
 extern "C" int ris_grad_K(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                           const double* B, double* grad)
 {
-    return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B, grad, nullptr);
+    if (!c) return RIS_EINVAL;
+    return grad_K_graphed(c, nbatch, nocc, nvir, C_occ, C_vir, B, grad, 0, -1);
 }
 
 extern "C" int ris_grad_K_range(ris_ctx* c, int nbatch, int nocc, int nvir, const double* C_occ, const double* C_vir,
                                 const double* B_local, int p_lo, int p_hi, double* grad)
 {
     if (!c || p_lo < 0 || p_hi < p_lo) return RIS_EINVAL;
-    return grad_K_impl(c, nbatch, nocc, nvir, C_occ, C_vir, B_local, grad, nullptr, p_lo, p_hi);
+    return grad_K_graphed(c, nbatch, nocc, nvir, C_occ, C_vir, B_local, grad, p_lo, p_hi);
 }
 
 // --------------------------------------------------------------------------------------- PQ (S5)

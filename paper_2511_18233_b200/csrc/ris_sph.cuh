@@ -47,32 +47,27 @@ __device__ const double RIS_SPH_T[110] = {
 };
 __host__ __device__ constexpr int ris_sph_off(int l) { return l == 0 ? 0 : (l == 1 ? 1 : (l == 2 ? 10 : 40)); }
 
-// J tiles from a density in the spherical basis: the tile element (ca, cb) of pair ip is
-//   symf sum_{m m'} T_la[m][ca] T_lb[m'][cb] (G[mu0 + m][nu0 + m'] + G[nu0 + m'][mu0 + m]),
-// mu0 / nu0 = first spherical AO of the two shells (sph0[first Cartesian AO of the shell]).
-__global__ void ris_k_pack_tiles_sph(RisClassPack pk, int nao_s, const int* __restrict__ sph0, const double* __restrict__ G,
-                                     long long gstride, double* __restrict__ out, long long ostride)
+// J tiles from a density in the spherical basis (ris_k_pack_tiles): the tile element (ca, cb) of a pair is
+//   sum_{m m'} T_la[m][ca] T_lb[m'][cb] (G[mu0 + m][nu0 + m'] + G[nu0 + m'][mu0 + m]),
+// r0 / q0 = first spherical AO of the two shells, nao_s the spherical AO count.
+__device__ __forceinline__ double ris_sph_pair_element(int la, int lb, int ca, int cb, size_t r0, size_t q0, int nao_s,
+                                                       const double* __restrict__ g)
 {
-    const int nca = ris_ncart(pk.la), ncb = ris_ncart(pk.lb), nel = nca * ncb;
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (long long)pk.npairs * nel) return;
-    const int ip = (int)(idx / nel), e = (int)(idx - (long long)ip * nel), ca = e / ncb, cb = e - ca * ncb;
-    const size_t r0 = (size_t)sph0[pk.ao[ip]], q0 = (size_t)sph0[pk.ao[(size_t)pk.npairs + ip]];
-    const double* g = G + (size_t)blockIdx.z * gstride;
-    const double* Ta = RIS_SPH_T + ris_sph_off(pk.la) + ca;
-    const double* Tb = RIS_SPH_T + ris_sph_off(pk.lb) + cb;
+    const int nca = ris_ncart(la), ncb = ris_ncart(lb);
+    const double* Ta = RIS_SPH_T + ris_sph_off(la) + ca;
+    const double* Tb = RIS_SPH_T + ris_sph_off(lb) + cb;
     double v = 0.0;
-    for (int m = 0; m < 2 * pk.la + 1; ++m) {
+    for (int m = 0; m < 2 * la + 1; ++m) {
         const double ta = Ta[m * nca];
         if (ta == 0.0) continue;
         double w = 0.0;
-        for (int n = 0; n < 2 * pk.lb + 1; ++n) {
+        for (int n = 0; n < 2 * lb + 1; ++n) {
             const double tb = Tb[n * ncb];
             if (tb != 0.0) w = fma(tb, g[(r0 + m) * nao_s + q0 + n] + g[(q0 + n) * nao_s + r0 + m], w);
         }
         v = fma(ta, w, v);
     }
-    out[(size_t)blockIdx.z * ostride + pk.elem_off + idx] = (double)pk.symf[ip] * v;
+    return v;
 }
 
 // Coefficient matrix to Cartesian rows: out[r][j] = sum_m T_l[m][comp(r)] C[sph0(r) + m][j], r over the Cartesian AOs;

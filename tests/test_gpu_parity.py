@@ -388,3 +388,43 @@ def test_runs_on_a_caller_stream():
     assert_parity(v.cpu().numpy(), orc.vec_J(wl.mol, wl.D), "v on stream")
     assert_parity(T.cpu().numpy(), orc.tensor_K(wl.mol, wl.C_occ, wl.C_vir), "T on stream")
     ctx.close()
+
+
+def test_repeated_calls_replay_a_cuda_graph_with_current_data():
+    """Small molecules: a device-pointer call whose signature repeats is captured into a CUDA graph the second time and replayed
+    afterwards (ris_api.cu: run_graphed).  The replay must read the CURRENT contents of the buffers, a new signature must
+    run directly, and in deterministic mode all of them agree bitwise."""
+    wl = synth.make_workload(2)
+    ctx = ris_setup(wl.mol, deterministic=True)
+    D, c = dev(wl.D), dev(wl.c_aux)
+    Co, Cv, B = dev(wl.C_occ), dev(wl.C_vir), dev(wl.B)
+    outJ = torch.empty((wl.D.shape[0], wl.mol.natoms, 3), dtype=torch.float64, device="cuda")
+    outK = torch.empty((wl.B.shape[0], wl.mol.natoms, 3), dtype=torch.float64, device="cuda")
+    gJ = [ctx.grad_J(D, c, out=outJ).clone() for _ in range(4)]           # direct, capture + launch, replay, replay
+    gK = [ctx.grad_K(Co, Cv, B, out=outK).clone() for _ in range(4)]
+    for g in gJ[1:]:
+        assert torch.equal(g, gJ[0])
+    for g in gK[1:]:
+        assert torch.equal(g, gK[0])
+    assert_parity(gJ[0].cpu().numpy(), orc.grad_J(wl.mol, wl.D, wl.c_aux)[0], "J", literal=True)
+    assert_parity(gK[0].cpu().numpy(), orc.grad_K(wl.mol, wl.C_occ, wl.C_vir, wl.B)[0], "K")
+    # same pointers, new contents: the replay sees them
+    D.mul_(2.0); B.mul_(-0.5)
+    g2 = ctx.grad_J(D, c, out=outJ).clone()
+    k2 = ctx.grad_K(Co, Cv, B, out=outK).clone()
+    assert (g2 - 2.0 * gJ[0]).abs().max() <= 1e-14 * gJ[0].abs().max()
+    assert (k2 + 0.5 * gK[0]).abs().max() <= 1e-14 * gK[0].abs().max()
+    # a new signature (other buffers) runs directly and displaces the remembered one; then the old one again
+    D3 = dev(wl.D)
+    g3 = ctx.grad_J(D3, c)
+    assert torch.equal(g3, gJ[0])
+    g4 = ctx.grad_J(D, c, out=outJ)
+    assert torch.equal(g4, g2)
+    # an s + p J-fit set replaces the lists the J graph points to
+    m1 = synth.with_jfit(wl.mol, 3)
+    ctx.set_jfit(*m1.jfit)
+    c1 = dev(np.random.default_rng(0).standard_normal((wl.D.shape[0], synth.naux_jfit(m1))))
+    g5 = [ctx.grad_J(D3, c1).clone() for _ in range(3)]
+    assert torch.equal(g5[1], g5[0]) and torch.equal(g5[2], g5[0])
+    assert_parity(g5[0].cpu().numpy(), orc.grad_J(m1, wl.D, c1.cpu().numpy())[0], "J s+p")
+    ctx.close()
