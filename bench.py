@@ -374,7 +374,7 @@ def run_ours(args):
         for _ in range(max(1, min(args.warmup, 3))):    # (small molecules: the J part is captured into a CUDA graph on its second call)
             step_host()
         barrier()
-        n_e2e = max(1, min(args.steps, 5))
+        n_e2e = max(1, min(args.steps, 5 if ms_step > 20.0 else 50))      # sub-millisecond steps: more repetitions (host jitter)
         reps = []
         for _ in range(n_e2e):
             t0 = time.perf_counter()

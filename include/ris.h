@@ -37,6 +37,9 @@
  *     and scratch and frees them in ris_destroy.  Outputs are OVERWRITTEN, not accumulated.
  *   - Asynchrony: device-pointer calls enqueue work on the stream given at ris_setup and return; the
  *     caller synchronises that stream.  *_host calls return after the result is in host memory.
+ *     For small molecules (no angular-momentum class fills the GPU) a device-pointer call of ris_grad_J / ris_grad_K whose
+ *     arguments repeat is captured into a CUDA graph on its second occurrence and replayed from then on: the same kernels in
+ *     the same stream order, reading the buffers' current contents.
  *   - Errors: 0 on success, a negative ris_status otherwise; nothing aborts or throws across the ABI.
  *     There is no CPU fallback: without a usable CUDA device every call fails with RIS_ECUDA.
  */

@@ -356,5 +356,8 @@ inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int b
 #endif
 inline cudaError_t ris_gemm_scatter(cudaStream_t st, const RisGemmParams& p, int ntiles)
 {
+    // up to 32 auxiliary functions (molecules of a few tens of atoms): one 32-column tile, 2 warps per CTA -- half the padded
+    // MMA work and shared memory of the 64-column tile
+    if (p.N <= 32) return ris_gemm_launch_cfg<RIS_G2_BM, 32, 32, 32, RIS_G2_STAGES, 6, false, true>(st, p, 1, ntiles);
     return ris_gemm_launch_cfg<RIS_G2_BM, RIS_G2_BN, 32, 32, RIS_G2_STAGES, RIS_G2_MINB, false, true>(st, p, 1, ntiles);
 }
