@@ -359,5 +359,12 @@ inline cudaError_t ris_gemm_scatter(cudaStream_t st, const RisGemmParams& p, int
     // up to 32 auxiliary functions (molecules of a few tens of atoms): one 32-column tile, 2 warps per CTA -- half the padded
     // MMA work and shared memory of the 64-column tile
     if (p.N <= 32) return ris_gemm_launch_cfg<RIS_G2_BM, 32, 32, 32, RIS_G2_STAGES, 6, false, true>(st, p, 1, ntiles);
+    // the aux index is the N dimension and is padded to whole tiles: take the tile width (64, 96 or 112 columns; 2 x 2 warps
+    // of 32 x 32 / 48 / 56) that pads least -- 100 functions: 112 instead of 128, 84: 96, 300: 320 (ties: the 64-column tile)
+    const int pad64 = (p.N + 63) / 64 * 64, pad96 = (p.N + 95) / 96 * 96, pad112 = (p.N + 111) / 112 * 112;
+    if (pad112 < pad64 && pad112 <= pad96)
+        return ris_gemm_launch_cfg<RIS_G2_BM, 112, 32, 56, RIS_G2_STAGES, RIS_G2_MINB, false, true>(st, p, 1, ntiles);
+    if (pad96 < pad64)
+        return ris_gemm_launch_cfg<RIS_G2_BM, 96, 32, 48, RIS_G2_STAGES, RIS_G2_MINB, false, true>(st, p, 1, ntiles);
     return ris_gemm_launch_cfg<RIS_G2_BM, RIS_G2_BN, 32, 32, RIS_G2_STAGES, RIS_G2_MINB, false, true>(st, p, 1, ntiles);
 }
