@@ -55,7 +55,8 @@
 #define RIS_NSK2_BYTES 16384    // two ring slots at least when they take no more than this per warp.  (2,2) runs ONE 9 KB slot:
 #endif                          // with two, the ring crowds the local-memory spills of that class out of L1 (K 0.57 -> 0.51 ms)
 #ifndef RIS_STAGE_BYTES
-#define RIS_STAGE_BYTES 4608    // shared-memory budget per warp for the K tile ring (at least 2 slots are always taken)
+#define RIS_STAGE_BYTES 13824   // shared-memory budget per warp for the K tile ring: three states of the (2,1) class (18 rows of
+                                // 256 bytes each), so that the usual batch of <= 3 states has a slot per state (fast path of get)
 #endif
 template <int LA, int LB> struct RisGradTune {
     static constexpr int MINB = (LA + LB <= 1) ? RIS_MB1 : (LA + LB == 2 ? RIS_MB2 : (LA + LB == 3 ? RIS_MB3 : RIS_MB4));
@@ -113,9 +114,10 @@ struct RisTileRing {
     int issued;                // states whose copy has been issued (and committed) since begin()
 
     __device__ __forceinline__ int slot_of(int s) const { return s < ns ? s : (s - ns < ns ? s - ns : s % ns); }
-    __device__ __forceinline__ void issue(int s)
+    __device__ __forceinline__ void issue(int s) { issue_to(s, slot_of(s)); }
+    __device__ __forceinline__ void issue_to(int s, int slot)
     {
-        double* dst = buf + slot_of(s) * SLOT;
+        double* dst = buf + slot * SLOT;
         const double* src = g + (size_t)s * sstride;
         if (KT) {
             const int c2 = (lane & 15) * 2;
@@ -137,11 +139,22 @@ struct RisTileRing {
     __device__ __forceinline__ void begin()
     {
         issued = 0;
-        for (int s = 0; s < ns; ++s) issue(s);
+        for (int s = 0; s < ns; ++s) issue_to(s, s);
         issued = ns;
     }
     __device__ __forceinline__ const double* get(int s)
     {
+        if (nb <= ns) {
+            // every state has a slot of its own (the usual case): the copies were issued at the start of the pair, a whole
+            // primitive loop ago -- ONE wait for all of them at the first state, no refill, slot = state.  (The general path
+            // below costs ~100 integer / branch instructions per state: slot arithmetic with a modulo, a jump table for the
+            // immediate of cp.async.wait_group, the refill test; profiles/r02_v1_ncu.md: (0,0) ran 2.5 instructions per FP64 one.)
+            if (s == 0) {
+                asm volatile("cp.async.wait_all;" ::: "memory");
+                __syncwarp();
+            }
+            return buf + s * SLOT + (KT ? lane : 0);
+        }
         if (s > 0 && issued < nb) {      // issued == s - 1 + ns: the slot state s-1 leaves is the next one's, and it is
             __syncwarp();                // free once every lane is done with state s-1
             issue(issued);
@@ -367,11 +380,19 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     // to 576 primitive pairs) leave less than that of the 227 KB a block may use
     RisGradParams p = p0_;
     constexpr int NSMAX = KT ? RisGradTune<LA, LB>::NSK : RIS_NB_MAX;
-    p.ring_ns = p.nb < NSMAX ? p.nb : NSMAX;
-    size_t smem = 0;
     constexpr int NW = RisGradTune<LA, LB>::NW;
+    auto smem_of = [&](int ns) { return NW * ris_grad_warp_smem(p.pk.task_prims, p.pk.kmax, p.nb, ris_grad_tile_doubles<LA, LB, KT>(ns)); };
+    auto resident_of = [&](size_t bytes) {
+        return std::max(1, std::min<int>(RisGradTune<LA, LB>::MINB * RIS_GRAD_WARPS / NW, (int)((227 * 1024) / (bytes + 1024))));
+    };
+    // A slot per state (the fast path of the ring) when that costs no resident block; otherwise the smallest ring (K: one or
+    // two slots, refilled state by state) -- a half-sized ring gives neither.
+    const int ns_full = p.nb < NSMAX ? p.nb : NSMAX;
+    const int ns_lo = KT ? std::min(p.nb, RisGradTune<LA, LB>::NSK_LO) : ns_full;
+    p.ring_ns = (smem_of(ns_full) <= (size_t)227 * 1024 && resident_of(smem_of(ns_full)) >= resident_of(smem_of(ns_lo))) ? ns_full : ns_lo;
+    size_t smem = 0;
     for (;; --p.ring_ns) {
-        smem = NW * ris_grad_warp_smem(p.pk.task_prims, p.pk.kmax, p.nb, ris_grad_tile_doubles<LA, LB, KT>(p.ring_ns));
+        smem = smem_of(p.ring_ns);
         if (smem <= 227 * 1024 || p.ring_ns == 1) break;
     }
     // the opt-in is per device and context: set it at every launch that needs it (a host-side call of ~1 us) instead of
@@ -385,7 +406,7 @@ cudaError_t ris_launch_grad_phase(const RisGradParams& p0_, cudaStream_t st)
     const int ny = (p.p1 - p.p0 + 31) / 32;
     const int nbt = (p.pk.ntasks + NW - 1) / NW;
     // resident blocks per SM: the register target, or what the shared memory of the block allows
-    const int resident = std::max(1, std::min<int>(RisGradTune<LA, LB>::MINB * RIS_GRAD_WARPS / NW, (int)((227 * 1024) / (smem + 1024))));
+    const int resident = resident_of(smem);
     const int nx = std::max(1, std::min(nbt, (p.nsm * resident + ny - 1) / ny));
     ris_grad_kernel<LA, LB, PH, KT, AUX><<<dim3(nx, ny), 32 * NW, smem, st>>>(p);
     return cudaGetLastError();
