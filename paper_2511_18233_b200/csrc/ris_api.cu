@@ -530,7 +530,11 @@ extern "C" int ris_setup(ris_ctx** out, int natoms, const double* coords, int ns
         const int ny = (natoms + 31) / 32;
         for (int k = 0; k < RIS_NCLASS; ++k)
             if (c->cls[k].npairs > 0) most = std::max(most, (long long)((c->cls[k].ntasks + RIS_GRAD_WARPS - 1) / RIS_GRAD_WARPS) * ny);
-        c->small = most <= (long long)2 * c->nsm && !std::getenv("RIS_NO_GRAPH");    // (the variable: A/B measurements)
+        // ... AND little work altogether (under 1e7 primitive triplets: a call of well under a millisecond, where launch and
+        // dependency latency is what is being paid).  Config 5 (40 atoms with f shells, 5 ms per call) has few tasks per class
+        // but nothing to gain from a graph; its end-to-end call was measured slower and erratic with one (6.0 -> 6.7-11 ms).
+        c->small = most <= (long long)2 * c->nsm && c->nprim_surv * (long long)natoms < 10000000ll &&
+                   !std::getenv("RIS_NO_GRAPH");                                  // (the variable: A/B measurements)
     }
     // spatial AO order + block list for the pair-restricted Gamma^P GEMM-2
     {
