@@ -105,6 +105,28 @@ def test_spherical_fitting_step_and_matvec():
     ctx.close()
 
 
+def test_spherical_combined_host_call_and_aux_ranges():
+    """ris_grad_host (J + K + PQ from host buffers in one call) and the aux-range calls of the multi-GPU split with spherical
+    inputs: the same boundary transformation serves every entry point."""
+    wl = synth.make_workload(2)
+    mol = wl.mol
+    x = _inputs(mol, 77, 2, wl.nocc, wl.nvir)
+    d_aux = np.random.default_rng(78).standard_normal((2, mol.natoms))
+    ctx = ris_setup(mol, spherical=True)
+    gJ = ctx.grad_J(dev(x["D"]), dev(x["c"])).cpu().numpy()
+    gK = ctx.grad_K(dev(x["Co"]), dev(x["Cv"]), dev(x["B"])).cpu().numpy()
+    gQ = ctx.grad_PQ(dev(x["c"]), dev(d_aux)).cpu().numpy()
+    hJ, hK, hQ = ctx.grad_host(x["D"], x["c"], d_aux, x["Co"], x["Cv"], x["B"])
+    for h, g in ((hJ, gJ), (hK, gK), (hQ, gQ)):
+        assert np.abs(h - g).max() <= 5e-14 * np.abs(g).max()
+    partJ = ctx.grad_J_range(dev(x["D"]), dev(x["c"]), 0, 13).cpu().numpy() + ctx.grad_J_range(dev(x["D"]), dev(x["c"]), 13, mol.natoms).cpu().numpy()
+    partK = (ctx.grad_K_range(dev(x["Co"]), dev(x["Cv"]), dev(np.ascontiguousarray(x["B"][:, :13])), 0, 13).cpu().numpy()
+             + ctx.grad_K_range(dev(x["Co"]), dev(x["Cv"]), dev(np.ascontiguousarray(x["B"][:, 13:])), 13, mol.natoms).cpu().numpy())
+    assert np.abs(partJ - gJ).max() <= 5e-14 * np.abs(gJ).max()
+    assert np.abs(partK - gK).max() <= 5e-14 * np.abs(gK).max()
+    ctx.close()
+
+
 def test_spherical_shapes_are_checked():
     mol = synth.tiny_molecule(4, [[0, 2], [1]], [[0, 0, 0], [1.7, 0.2, 0.4]])
     ctx = ris_setup(mol, spherical=True)
