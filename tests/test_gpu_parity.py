@@ -256,6 +256,17 @@ def test_full_size_sampled_atoms(cfg, natoms_sampled):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg", [3, 5])
+def test_full_size_every_component(cfg):
+    """Configs 3 (100 atoms, 5 states) and 5 (f shells) at full size, EVERY gradient component of J and K against the
+    unscreened oracle (about 40 s of oracle each on 16 threads) -- not a sample."""
+    wl = synth.make_workload(cfg)
+    ctx, gJ, gK, _ = run_all(wl, schwarz_tol=wl.schwarz_tol)
+    ctx.close()
+    assert_parity(gJ, orc.grad_J(wl.mol, wl.D, wl.c_aux)[0], f"config {cfg} J, all atoms", literal=True)
+    assert_parity(gK, orc.grad_K(wl.mol, wl.C_occ, wl.C_vir, wl.B)[0], f"config {cfg} K, all atoms")
+
+
 def test_deterministic_mode_is_bitwise_reproducible_and_at_parity():
     """ris_options.deterministic (S4): fixed-order sums inside a block, 64-bit integer atomics of a
     fixed-point split across blocks -> two runs agree bit for bit, and the result still matches the oracle."""
