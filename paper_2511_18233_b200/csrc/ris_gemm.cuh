@@ -19,7 +19,7 @@
 // SASS DMMA.8x8x4, 16 cycles of the pipe per SM sub-partition each).  Operands are staged global -> shared with
 // cp.async (LDGSTS) through a multi-stage pipeline that is synchronised by mbarriers only (full[s]: the stage's
 // cp.async have landed; empty[s]: every warp has read its fragments) -- a CTA-wide barrier per K step cost 15 % of the
-// DMMA pipe (profiles/r01_v3_ncu.md -> r01_v4_gemm.md).  Fragments are read with 128-bit shared loads from a
+// DMMA pipe (measured in round 1).  Fragments are read with 128-bit shared loads from a
 // 16-double row whose halves are swapped on odd rows (bank-conflict free, no padding).
 //   GEMM-1: CTA tile 64x128, K step 16, 8 warps as 2 x 4, warp tile 32x32, 3 stages, 2 CTAs/SM
 //   GEMM-2: CTA tile 64x64 (partners x aux),  K step 16, 4 warps as 2 x 2, warp tile 32x32, 3 stages, 3 CTAs/SM
@@ -338,7 +338,7 @@ inline cudaError_t ris_gemm_launch_cfg(cudaStream_t st, const RisGemmParams& p, 
 }
 
 // GEMM-1: dense, CTA tile 64x128, 8 warps (2 x 4, warp tile 32x32), 3 stages, 2 CTAs/SM.  Measured on B200 (config 4,
-// profiles/r01_v4_gemm.md): 33.2 TFLOP/s = 90 % of the mma.sync f64 peak; 128x128 tiles with 8 or 16 warps on one
+// round 1; now profiles/r02_v1_ncu.md): 33.2 TFLOP/s = 90 % of the mma.sync f64 peak; 128x128 tiles with 8 or 16 warps on one
 // CTA/SM reach 31.3-31.6, 128x64 x 2 CTAs 31.9, the same tile with 4 stages 32.4.
 inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int batch)
 {
