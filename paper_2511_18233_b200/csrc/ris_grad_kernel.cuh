@@ -112,9 +112,8 @@ struct RisTileRing {
     size_t estride, sstride;
     int nb, ns, lane, nv;      // ns = min(nb, NS) slots in use; nv: valid aux functions of this warp's chunk (K)
     int issued;                // states whose copy has been issued (and committed) since begin()
+    int rd;                    // slot of the state get() returned last
 
-    __device__ __forceinline__ int slot_of(int s) const { return s < ns ? s : (s - ns < ns ? s - ns : s % ns); }
-    __device__ __forceinline__ void issue(int s) { issue_to(s, slot_of(s)); }
     __device__ __forceinline__ void issue_to(int s, int slot)
     {
         double* dst = buf + slot * SLOT;
@@ -155,14 +154,19 @@ struct RisTileRing {
             }
             return buf + s * SLOT + (KT ? lane : 0);
         }
-        if (s > 0 && issued < nb) {      // issued == s - 1 + ns: the slot state s-1 leaves is the next one's, and it is
-            __syncwarp();                // free once every lane is done with state s-1
-            issue(issued);
-            ++issued;
+        // states are asked for in order: rd = slot of state s, kept incrementally (s % ns without the division)
+        if (s == 0) rd = 0;
+        else {
+            if (issued < nb) {           // issued == s - 1 + ns: the slot state s-1 leaves (rd) is the next one's, and it is
+                __syncwarp();            // free once every lane is done with state s-1
+                issue_to(issued, rd);
+                ++issued;
+            }
+            rd = rd + 1 == ns ? 0 : rd + 1;
         }
         ris_cp_wait(issued - 1 - s);
         __syncwarp();
-        return buf + slot_of(s) * SLOT + (KT ? lane : 0);
+        return buf + rd * SLOT + (KT ? lane : 0);
     }
     __device__ __forceinline__ bool holds_all() const { return nb <= ns; }
 };
