@@ -350,6 +350,7 @@ inline cudaError_t ris_gemm_dense(cudaStream_t st, const RisGemmParams& p, int b
 // GEMM-2 (scatter mode): tiles of RIS_G2_BM gathered partner rows x RIS_G2_BN aux functions, K = nocc
 #ifndef RIS_G2_BM
 #define RIS_G2_BM 64            // measured on config 4 (r02): 64x64 / 3 CTAs 29.8 ms per step, 32x64 / 5 CTAs 30.2, / 6 CTAs
+                                // (skipping the MMAs of a warp whose 32-row strip is all padding: 30.9 -- left out)
 #define RIS_G2_BN 64            // 30.3, 32x64 with 4 stages 32.5
 #define RIS_G2_STAGES 3
 #define RIS_G2_MINB 3
